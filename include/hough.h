@@ -1,0 +1,218 @@
+/*
+ * hough.h -- C ABI of the B200-native Hough-transform track finder (libhough_b200.so).
+ *
+ * The operation is the data-parallel hot path of the fast tracking algorithm of
+ * arXiv:1305.4855: "each hit maps to a curve in the track-parameter space, the curves of
+ * all hits are accumulated, local maxima of the accumulator are the track candidates"
+ * (section 7; Fig. 3; section 8 for the curved
+ * 2-parameter case; "accumulator and peak detection reside in GPU memory").
+ * BASELINE.json north_star fixes its concrete form (restated as SURVEY.md section 8(c)
+ * A1..A7, which DESIGN.md section 2 adopts):
+ *
+ *   - parameters (phi0, d0, kappa); for every hit (x, y, layer), every phi0 bin centre i
+ *     and every d0 bin centre j:  s = -x sin(phi0_i) + y cos(phi0_i),
+ *       kappa = 2 (s - d0_j) / (r^2 - 2 d0_j s + d0_j^2),      r^2 = x^2 + y^2;
+ *     if kappa_min <= kappa < kappa_max the hit's layer bit is OR-ed into the uint32
+ *     mask of bin (i, j, k), k = the kappa bin;
+ *   - a bin is a peak iff popcount(mask) >= L_min and it beats all (up to 26)
+ *     neighbours, ties going to the lower linear index; phi0 may wrap;
+ *   - every peak is emitted, in ascending linear index, with its mask and the ascending
+ *     list of the hits that voted into exactly that bin.
+ *   All arithmetic is IEEE-754 binary32, round-to-nearest-even, unfused, in a fixed
+ *   order, so results are bit-identical to the CPU oracle.
+ *
+ * Conventions
+ *   - Pointers marked [device] are CUDA device pointers on the handle's device; [host]
+ *     are ordinary host pointers (pinned memory makes the async copies truly async).
+ *   - The library never allocates device memory: the caller hands in one workspace
+ *     (e.g. a torch tensor) and the output arrays, and keeps them alive.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Calls that take a stream only ENQUEUE work and return without synchronising,
+ *     unless stated otherwise.  One handle is used from one stream at a time.
+ *   - Every int-returning call returns HOUGH_OK (0) or a negative HOUGH_E* code; nothing
+ *     throws across the boundary; there is no global state.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns
+ *     HOUGH_ECUDA.
+ *   - Accumulator layout: bin (i, j, k) at linear index lin = (i*n_d0 + j)*n_kappa + k
+ *     (kappa fastest).
+ */
+#ifndef HOUGH_B200_H
+#define HOUGH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HOUGH_OK 0
+#define HOUGH_EINVAL (-1) /* bad argument / configuration */
+#define HOUGH_ENOMEM (-2) /* workspace or capacity too small */
+#define HOUGH_ECUDA (-3)  /* a CUDA runtime call failed (or no device) */
+#define HOUGH_ESTATE (-4) /* call order violated (e.g. hough_peaks before hough_vote) */
+
+/* hough_counts.flags */
+#define HOUGH_TRUNCATED_PEAKS 1u /* n_peaks > cap_peaks: only the first cap_peaks (in lin order) were written */
+#define HOUGH_TRUNCATED_HITS 2u  /* n_hit_entries > cap_hits: hit_index holds the first cap_hits entries */
+
+/* hough_config.options */
+#define HOUGH_OPT_NO_CULL 1u /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
+
+typedef struct hough_handle hough_handle; /* opaque */
+
+/*
+ * Grid and detector description (BASELINE.json north_star: "hough_create(layer radii,
+ * grid ranges/bins, L_min)").  Bin centres: phi0_i = phi_min + (i + 0.5)(phi_max - phi_min)/n_phi,
+ * d0_j likewise; kappa bins are the n_kappa equal half-open intervals of
+ * [kappa_min, kappa_max).  n_d0 = 1 with d0_min = d0_max = 0 is the 2-parameter transform
+ * through the interaction point.
+ */
+typedef struct hough_config {
+    int32_t n_layers;              /* 1..32; hit layer l sets mask bit l */
+    const double *layer_radius_cm; /* [host] n_layers radii, > 0; metadata only: the vote uses the hit's own x^2+y^2 */
+    double phi_min, phi_max;       /* phi_max > phi_min */
+    double d0_min, d0_max;         /* d0_max >= d0_min (equal only if n_d0 == 1) */
+    double kappa_min, kappa_max;   /* kappa_max > kappa_min */
+    int32_t n_phi, n_d0, n_kappa;  /* >= 1; n_kappa a multiple of 32; n_phi*n_d0*n_kappa < 2^32 */
+    int32_t L_min;                 /* 1..n_layers */
+    int32_t phi_wrap;              /* 1: phi0 is periodic in the peak test (needs n_phi >= 3); 0: not */
+    uint32_t max_hits;             /* largest n accepted by hough_vote / hough_process_host */
+    uint32_t cap_peaks;            /* capacity of the caller's peak arrays (>= 1) */
+    uint64_t cap_hits;             /* capacity of the caller's hit_index array (>= 1) */
+    int32_t tile_phi, tile_d0;     /* accumulator tile owned by one CTA, in cells; 0 = choose automatically */
+    uint32_t options;              /* HOUGH_OPT_* */
+    int32_t device;                /* CUDA device ordinal */
+} hough_config;
+
+/* Counters of one event, 32 bytes, same layout on host and device. */
+typedef struct hough_counts {
+    uint64_t n_votes;       /* votes cast (in-range solutions over all hit x cell pairs) */
+    uint64_t n_hit_entries; /* TRUE total length of the hit lists of the reported peaks */
+    uint32_t n_peaks;       /* TRUE number of peaks (may exceed cap_peaks) */
+    uint32_t n_bad_hits;    /* hits with layer outside [0, n_layers): cast no vote */
+    uint32_t flags;         /* HOUGH_TRUNCATED_* */
+    uint32_t reserved;
+} hough_counts;
+
+/*
+ * Output arrays of hough_peaks, all [device], caller-owned.  Peaks are in ascending lin.
+ * Peak p (p < min(n_peaks, cap_peaks)): bin[p] = lin, mask[p] = its layer mask, and its
+ * hits are hit_index[hit_offset[p] .. hit_offset[p+1]) in ascending hit index.
+ * hit_offset[min(n_peaks, cap_peaks)] = n_hit_entries.  Entries at positions >= cap_hits
+ * are not written (lists are complete while they fit).
+ */
+typedef struct hough_peaks_out {
+    uint32_t *bin;        /* [device] cap_peaks */
+    uint32_t *mask;       /* [device] cap_peaks */
+    uint64_t *hit_offset; /* [device] cap_peaks + 1 */
+    uint32_t *hit_index;  /* [device] cap_hits */
+    hough_counts *counts; /* [device] 1 */
+} hough_peaks_out;
+
+/* Host mirror of hough_peaks_out for hough_process_host ([host] pointers, same capacities). */
+typedef struct hough_host_out {
+    uint32_t *bin;
+    uint32_t *mask;
+    uint64_t *hit_offset;
+    uint32_t *hit_index; /* may be NULL: hit lists are then computed but not copied back */
+    hough_counts *counts;
+} hough_host_out;
+
+/* Bytes of device workspace hough_create needs for cfg (0 if cfg is invalid). */
+size_t hough_workspace_bytes(const hough_config *cfg);
+
+/*
+ * Validate cfg, build the bin-centre tables on the host in fp64 and round them once to
+ * fp32 (sin/cos of phi0_i, d0_j, 2 d0_j, d0_j^2, kappa_min, kappa_max, n_kappa/(kappa_max-kappa_min)),
+ * upload them and carve the accumulator and scratch out of `workspace` ([device], 256-byte
+ * aligned, >= hough_workspace_bytes(cfg)).  Synchronises the device once.  The library
+ * owns *out (free with hough_destroy); the caller owns the workspace.
+ * Errors: HOUGH_EINVAL (bad cfg / NULL), HOUGH_ENOMEM (workspace too small), HOUGH_ECUDA.
+ */
+int hough_create(const hough_config *cfg, void *workspace, size_t workspace_bytes, hough_handle **out);
+
+/* Free the handle and its table memory.  NULL is a no-op.  Never frees caller memory. */
+void hough_destroy(hough_handle *h);
+
+/*
+ * Process ONE event's hits (BASELINE.json north_star: "hough_vote(hits, n, stream)"):
+ * x, y [device] fp32[n] transverse coordinates in cm, layer [device] int32[n].  The
+ * accumulator is defined from scratch by this call (no accumulation across calls):
+ * hit preparation (r^2, layer bit), per-tile hit staging, shared-memory tile voting,
+ * tile write-out and the vote count are enqueued on the stream.  n = 0 is legal (all-zero
+ * accumulator).  Hits with a layer outside [0, n_layers) or non-finite coordinates cast no vote.
+ * The hit arrays must stay valid until the stream has passed this call's work AND the
+ * following hough_peaks (the hit lists re-read them).
+ * Errors: HOUGH_EINVAL (NULL handle, n > max_hits, NULL arrays with n > 0), HOUGH_ECUDA.
+ */
+int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
+               void *cuda_stream);
+
+/*
+ * Peak finding, compaction and hit lists of the event last given to hough_vote
+ * (north_star: "hough_peaks(out)"), enqueued on the stream; results go to the caller's
+ * device arrays, including out->counts, so that many events can be processed
+ * back-to-back without a host synchronisation.
+ * Errors: HOUGH_EINVAL, HOUGH_ESTATE (no hough_vote before), HOUGH_ECUDA.
+ */
+int hough_peaks(hough_handle *h, const hough_peaks_out *out, void *cuda_stream);
+
+/* [device] pointer to the n_phi*n_d0*n_kappa uint32 masks (lin order), valid after
+ * hough_vote's work has completed and until the next hough_vote.  NULL for a NULL handle. */
+const uint32_t *hough_accumulator(const hough_handle *h);
+
+/*
+ * Whole path for one event with HOST buffers: copies x, y, layer host->device (async on
+ * the stream), runs hough_vote + hough_peaks into `dev` (device arrays as for
+ * hough_peaks), copies counts, the peak arrays and (if host->hit_index != NULL) the hit
+ * lists back to `host`, and SYNCHRONISES the stream before returning.  Only the filled
+ * prefixes are copied back (a second small synchronisation on counts is used for that).
+ */
+int hough_process_host(hough_handle *h, const float *x, const float *y, const int32_t *layer,
+                       uint32_t n, const hough_peaks_out *dev, const hough_host_out *host,
+                       void *cuda_stream);
+
+/*
+ * Stand-alone accumulator kernels, used for the
+ * HBM-roofline measurements and as cross-checks:
+ *   hough_clear       zero the global accumulator (pure HBM write);
+ *   hough_peak_sweep  run only the peak-flag sweep over the current accumulator (reads
+ *                     4 B/bin once, writes 1 bit/bin) and leave the result in the workspace.
+ */
+int hough_clear(hough_handle *h, void *cuda_stream);
+int hough_peak_sweep(hough_handle *h, void *cuda_stream);
+
+/* Overwrite the accumulator from a [device] array of n_bins masks (test hook for the peak
+ * rule: lets a test run hough_peak_sweep / hough_peaks_only on a hand-made accumulator). */
+int hough_set_accumulator(hough_handle *h, const uint32_t *acc_dev, void *cuda_stream);
+/* Peak flags + compaction only (no hit lists: hit_offset/hit_index untouched, n_hit_entries = 0). */
+int hough_peaks_only(hough_handle *h, const hough_peaks_out *out, void *cuda_stream);
+
+/*
+ * Shared-memory atomic micro-benchmark that defines the "shared-atomic roofline" on the
+ * box: every SM runs `ctas_per_sm` CTAs of `threads` threads,
+ * each thread issues `iters` no-return 32-bit OR operations into the CTA's shared-memory table.
+ * mode 0: atomicOr, conflict-free (32 lanes -> 32 banks, distinct addresses);
+ * mode 1: atomicOr, pseudo-random addresses (bank conflicts as they fall);
+ * mode 2: plain load/OR/store on the same conflict-free addresses (no atomic), for comparison.
+ * Enqueues on the stream; *lane_ops (host) receives the number of lane-operations one
+ * launch performs.  Time it with CUDA events around the call.
+ */
+int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters,
+                          void *cuda_stream, uint64_t *lane_ops);
+
+/* Geometry the library chose (for reporting): tile_phi, tile_d0, n_tiles, threads per CTA,
+ * dynamic shared memory bytes of the vote kernel, number of SMs.  Any pointer may be NULL. */
+int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,
+                int32_t *threads, int32_t *smem_bytes, int32_t *n_sms);
+
+/* Number of kernel launches enqueued by this handle since creation (for bench accounting). */
+uint64_t hough_launch_count(const hough_handle *h);
+
+const char *hough_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOUGH_B200_H */

@@ -1,0 +1,559 @@
+// hough_api.cu -- the C ABI of include/hough.h: configuration checks, the bin-centre
+// tables (A1), the workspace carve-up, hit preparation (a1) and the call sequences of
+// hough_vote / hough_peaks.  No torch types, no exceptions, no global state.
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "hough_internal.cuh"
+
+// ------------------------------------------------------------------ a1: hit preparation
+// r2 = x*x + y*y (three roundings, A2), layer bit, bad-hit count; entries n..n_pad are
+// non-voting padding so that the staged chunks are always whole.
+__global__ void __launch_bounds__(256) k_prep(const float *__restrict__ x, const float *__restrict__ y,
+                                              const int32_t *__restrict__ layer, uint32_t n,
+                                              uint32_t n_pad, int n_layers, float *__restrict__ hx,
+                                              float *__restrict__ hy, float *__restrict__ hr2,
+                                              uint32_t *__restrict__ hbit, DevCounters *counters)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool bad = false;
+    if (i < n) {
+        float xv = x[i], yv = y[i];
+        float pp = __fmul_rn(xv, xv);
+        float qq = __fmul_rn(yv, yv);
+        int l = layer[i];
+        bad = (l < 0) || (l >= n_layers);
+        hx[i] = xv;
+        hy[i] = yv;
+        hr2[i] = __fadd_rn(pp, qq);
+        hbit[i] = bad ? 0u : (1u << l);
+    } else if (i < n_pad) {
+        hx[i] = 0.f;
+        hy[i] = 0.f;
+        hr2[i] = __int_as_float(0x7fc00000);
+        hbit[i] = 0u;
+    }
+    unsigned b = __ballot_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && b)
+        atomicAdd(&counters->n_bad_hits, (unsigned int)__popc(b));
+}
+
+cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
+                        cudaStream_t st)
+{
+    uint32_t n_pad = ((n + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
+    if (n_pad == 0)
+        return cudaSuccess;
+    k_prep<<<(n_pad + 255) / 256, 256, 0, st>>>(x, y, layer, n, n_pad, h->cfg.n_layers, h->hx, h->hy, h->hr2,
+                                                h->hbit, h->counters);
+    h->launches += 1;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ configuration
+static int cfg_valid(const hough_config *c)
+{
+    if (!c || !c->layer_radius_cm)
+        return 0;
+    if (c->n_layers < 1 || c->n_layers > 32)
+        return 0;
+    for (int l = 0; l < c->n_layers; ++l)
+        if (!(c->layer_radius_cm[l] > 0.0))
+            return 0;
+    if (c->n_phi < 1 || c->n_d0 < 1 || c->n_kappa < 32 || (c->n_kappa % 32) != 0)
+        return 0;
+    if (!(c->phi_max > c->phi_min) || !(c->kappa_max > c->kappa_min))
+        return 0;
+    if (c->n_d0 == 1 ? !(c->d0_max >= c->d0_min) : !(c->d0_max > c->d0_min))
+        return 0;
+    if (!isfinite(c->phi_min) || !isfinite(c->phi_max) || !isfinite(c->d0_min) || !isfinite(c->d0_max) ||
+        !isfinite(c->kappa_min) || !isfinite(c->kappa_max))
+        return 0;
+    double bins = (double)c->n_phi * (double)c->n_d0 * (double)c->n_kappa;
+    if (bins >= 4294967296.0)
+        return 0;
+    if (c->L_min < 1 || c->L_min > c->n_layers)
+        return 0;
+    if (c->phi_wrap != 0 && c->phi_wrap != 1)
+        return 0;
+    if (c->phi_wrap && c->n_phi < 3)
+        return 0;
+    if (c->cap_peaks < 1 || c->cap_hits < 1)
+        return 0;
+    if (c->tile_phi < 0 || c->tile_d0 < 0)
+        return 0;
+    if (c->n_kappa > 16384)
+        return 0; // one cell row must fit a shared-memory tile
+    return 1;
+}
+
+struct Carve {
+    size_t off;
+    unsigned char *base;
+    void *take(size_t bytes)
+    {
+        off = (off + 255) & ~(size_t)255;
+        void *p = base ? base + off : nullptr;
+        off += bytes;
+        return p;
+    }
+};
+
+static uint32_t pad_hits(uint32_t n)
+{
+    uint32_t p = ((n + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
+    return p ? p : HOUGH_CHUNK;
+}
+
+// Lays the workspace out; with base == NULL only the size is computed.
+static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_handle *h)
+{
+    Carve cv{0, base};
+    size_t n_bins = (size_t)c->n_phi * c->n_d0 * c->n_kappa;
+    size_t n_rows = (size_t)c->n_phi * c->n_d0;
+    uint32_t hp = pad_hits(c->max_hits);
+    uint32_t sb = (uint32_t)((n_rows + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
+    uint32_t sb2 = (uint32_t)(((size_t)c->cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
+    if (sb2 > sb)
+        sb = sb2;
+    sb += 1;
+    void *acc = cv.take(n_bins * 4);
+    void *t_sn = cv.take((size_t)c->n_phi * 4), *t_cs = cv.take((size_t)c->n_phi * 4);
+    void *t_d0c = cv.take((size_t)c->n_d0 * 4), *t_twod0 = cv.take((size_t)c->n_d0 * 4);
+    void *t_d0sq = cv.take((size_t)c->n_d0 * 4);
+    void *hx = cv.take((size_t)hp * 4), *hy = cv.take((size_t)hp * 4), *hr2 = cv.take((size_t)hp * 4);
+    void *hbit = cv.take((size_t)hp * 4);
+    void *rx = cv.take((size_t)hp * 4), *ry = cv.take((size_t)hp * 4), *rl = cv.take((size_t)hp * 4);
+    void *flags = cv.take(n_bins / 8);
+    void *row_base = cv.take((n_rows + 1) * 4);
+    void *list_len = cv.take((size_t)c->cap_peaks * 4);
+    // reset region: counters | tickets | status words (kept contiguous for one memset)
+    void *counters = cv.take(256 + (size_t)2 * sb * 8);
+    if (h) {
+        h->acc = (uint32_t *)acc;
+        h->t_sn = (float *)t_sn;
+        h->t_cs = (float *)t_cs;
+        h->t_d0c = (float *)t_d0c;
+        h->t_twod0 = (float *)t_twod0;
+        h->t_d0sq = (float *)t_d0sq;
+        h->hx = (float *)hx;
+        h->hy = (float *)hy;
+        h->hr2 = (float *)hr2;
+        h->hbit = (uint32_t *)hbit;
+        h->raw_x = (float *)rx;
+        h->raw_y = (float *)ry;
+        h->raw_layer = (int32_t *)rl;
+        h->max_hits_pad = hp;
+        h->flags = (uint32_t *)flags;
+        h->row_base = (uint32_t *)row_base;
+        h->list_len = (uint32_t *)list_len;
+        h->counters = (DevCounters *)counters;
+        h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
+        h->scan_status = (unsigned long long *)((unsigned char *)counters + 256);
+        h->scan_blocks_max = sb;
+    }
+    return (cv.off + 255) & ~(size_t)255;
+}
+
+size_t hough_workspace_bytes(const hough_config *cfg)
+{
+    if (!cfg_valid(cfg))
+        return 0;
+    return carve_workspace(cfg, nullptr, nullptr);
+}
+
+static int env_int(const char *name, int dflt)
+{
+    const char *s = getenv(name);
+    if (!s || !*s)
+        return dflt;
+    return atoi(s);
+}
+
+// Tile shapes.  Defaults aim at two resident CTAs per SM (<= ~113 KB of shared memory
+// each); cfg.tile_phi / tile_d0 or the HOUGH_TILE_* environment variables override.
+static int choose_geometry(hough_handle *h)
+{
+    const hough_config &c = h->cfg;
+    const int nk = c.n_kappa;
+    const int budget = env_int("HOUGH_SMEM_BUDGET", 113 * 1024);
+    const int staging = 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 8) * 16 + 256;
+    // vote
+    {
+        int cell_bytes = nk * 4 / h->g.pack;
+        int D = c.tile_d0 > 0 ? c.tile_d0 : env_int("HOUGH_TILE_D0", c.n_d0 < 8 ? c.n_d0 : 8);
+        if (D > c.n_d0)
+            D = c.n_d0;
+        int P = c.tile_phi > 0 ? c.tile_phi : env_int("HOUGH_TILE_PHI", 0);
+        if (P <= 0) {
+            int cells = (budget - staging) / cell_bytes;
+            P = cells / D;
+            if (P > 32)
+                P = 32;
+            if (P >= 16)
+                P = (P / 8) * 8;
+        }
+        if (P < 1)
+            P = 1;
+        if (P > c.n_phi)
+            P = c.n_phi;
+        int groups = (P * D + 31) / 32;
+        int split = env_int("HOUGH_VOTE_SPLIT", 0);
+        if (split <= 0) {
+            split = 512 / (32 * groups);
+            if (split < 1)
+                split = 1;
+            if (split > 8)
+                split = 8;
+        }
+        while (split > 1 && 32 * groups * split > 1024)
+            --split;
+        if (!sweep_geom_init(h, &h->vote_geom, P, D, split, 8 / h->g.pack, 0)) {
+            // fall back to the smallest tile
+            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 8 / h->g.pack, 0))
+                return 0;
+        }
+    }
+    // hit lists: u16 slot per bin + a u32 cursor per possible peak of the tile
+    {
+        int D = env_int("HOUGH_LIST_TILE_D0", c.n_d0 < 8 ? c.n_d0 : 8);
+        if (D > c.n_d0)
+            D = c.n_d0;
+        if (D > 1 && (D & 1))
+            --D;
+        int P = env_int("HOUGH_LIST_TILE_PHI", 0);
+        if (P <= 0) {
+            // bytes per cell ~ 2 nk (slots) + nk/2 (cursors) + 12
+            int per_cell = 2 * nk + nk / 2 + 16;
+            int cells = (budget - staging) / per_cell;
+            P = cells / D;
+            if (P > 32)
+                P = 32;
+            if (P >= 16)
+                P = (P / 8) * 8;
+        }
+        if (P < 1)
+            P = 1;
+        if (P > c.n_phi)
+            P = c.n_phi;
+        if (P > 1 && (P & 1))
+            --P;
+        int groups = (P * D + 31) / 32;
+        int split = env_int("HOUGH_LIST_SPLIT", 0);
+        if (split <= 0) {
+            split = 512 / (32 * groups);
+            if (split < 1)
+                split = 1;
+            if (split > 8)
+                split = 8;
+        }
+        while (split > 1 && 32 * groups * split > 1024)
+            --split;
+        if (!sweep_geom_init(h, &h->list_geom, P, D, split, 4, 1)) {
+            if (!sweep_geom_init(h, &h->list_geom, 1, 1, 4, 4, 1))
+                return 0;
+        }
+    }
+    // peak sweep
+    {
+        int Tj = env_int("HOUGH_PEAK_TJ", 14);
+        if (Tj > c.n_d0)
+            Tj = c.n_d0;
+        int Li = env_int("HOUGH_PEAK_LI", 16);
+        if (Li > c.n_phi)
+            Li = c.n_phi;
+        for (;;) {
+            size_t smem = (size_t)9 * (Tj + 2) * (nk / 4 + 2) * 4;
+            if (smem <= (size_t)200 * 1024 || Tj == 1) {
+                h->pk_smem = (int)smem;
+                break;
+            }
+            Tj = Tj > 2 ? Tj / 2 : 1;
+        }
+        if (h->pk_smem > 227 * 1024)
+            return 0;
+        h->pk_Tj = Tj;
+        h->pk_Li = Li;
+        h->pk_threads = env_int("HOUGH_PEAK_THREADS", 512);
+    }
+    return 1;
+}
+
+int hough_create(const hough_config *cfg, void *workspace, size_t workspace_bytes, hough_handle **out)
+{
+    if (!out)
+        return HOUGH_EINVAL;
+    *out = nullptr;
+    if (!cfg_valid(cfg) || !workspace)
+        return HOUGH_EINVAL;
+    if (((uintptr_t)workspace & 255) != 0)
+        return HOUGH_EINVAL;
+    size_t need = carve_workspace(cfg, nullptr, nullptr);
+    if (workspace_bytes < need)
+        return HOUGH_ENOMEM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) {
+        cudaGetLastError();
+        return HOUGH_ECUDA;
+    }
+    if (cudaSetDevice(cfg->device) != cudaSuccess)
+        return HOUGH_ECUDA;
+    hough_handle *h = new (std::nothrow) hough_handle();
+    if (!h)
+        return HOUGH_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    h->cfg = *cfg;
+    h->radii = (double *)malloc(sizeof(double) * cfg->n_layers);
+    memcpy(h->radii, cfg->layer_radius_cm, sizeof(double) * cfg->n_layers);
+    h->cfg.layer_radius_cm = h->radii;
+    h->device = cfg->device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) {
+        hough_destroy(h);
+        return HOUGH_ECUDA;
+    }
+    h->n_sms = prop.multiProcessorCount;
+    carve_workspace(cfg, (unsigned char *)workspace, h);
+
+    // A1: bin centres in fp64, one rounding to fp32
+    const int np = cfg->n_phi, nd = cfg->n_d0;
+    float *sn = (float *)malloc(sizeof(float) * np), *cs = (float *)malloc(sizeof(float) * np);
+    float *d0c = (float *)malloc(sizeof(float) * nd), *twod0 = (float *)malloc(sizeof(float) * nd);
+    float *d0sq = (float *)malloc(sizeof(float) * nd);
+    for (int i = 0; i < np; ++i) {
+        double phic = cfg->phi_min + ((double)i + 0.5) * (cfg->phi_max - cfg->phi_min) / (double)np;
+        sn[i] = (float)sin(phic);
+        cs[i] = (float)cos(phic);
+    }
+    float d0abs = 0.f;
+    for (int j = 0; j < nd; ++j) {
+        volatile float c0 = (float)(cfg->d0_min + ((double)j + 0.5) * (cfg->d0_max - cfg->d0_min) / (double)nd);
+        volatile float two = 2.0f * c0;
+        volatile float sq = c0 * c0; // one binary32 multiply (volatile: no contraction, no excess precision)
+        d0c[j] = c0;
+        twod0[j] = two;
+        d0sq[j] = sq;
+        if (fabsf(c0) > d0abs)
+            d0abs = fabsf(c0);
+    }
+    GridDev &g = h->g;
+    g.n_phi = np;
+    g.n_d0 = nd;
+    g.n_kappa = cfg->n_kappa;
+    g.L_min = cfg->L_min;
+    g.phi_wrap = cfg->phi_wrap;
+    g.pack = cfg->n_layers <= 16 ? 2 : 1;
+    if (env_int("HOUGH_FORCE_PACK1", 0))
+        g.pack = 1;
+    g.klo = (float)cfg->kappa_min;
+    g.khi = (float)cfg->kappa_max;
+    g.inv_dk = (float)((double)cfg->n_kappa / (cfg->kappa_max - cfg->kappa_min));
+    g.kabs = fmaxf(fabsf(g.klo), fabsf(g.khi));
+    g.d0_absmax = d0abs;
+    g.sn = h->t_sn;
+    g.cs = h->t_cs;
+    g.d0c = h->t_d0c;
+    g.twod0 = h->t_twod0;
+    g.d0sq = h->t_d0sq;
+    int ok = 1;
+    ok &= cudaMemcpy(h->t_sn, sn, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_cs, cs, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_d0c, d0c, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_twod0, twod0, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_d0sq, d0sq, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemset(h->counters, 0, 256 + (size_t)2 * h->scan_blocks_max * 8) == cudaSuccess;
+    free(sn);
+    free(cs);
+    free(d0c);
+    free(twod0);
+    free(d0sq);
+    if (!ok) {
+        cudaGetLastError();
+        hough_destroy(h);
+        return HOUGH_ECUDA;
+    }
+    if (!choose_geometry(h)) {
+        hough_destroy(h);
+        return HOUGH_EINVAL;
+    }
+    if (cudaDeviceSynchronize() != cudaSuccess) {
+        hough_destroy(h);
+        return HOUGH_ECUDA;
+    }
+    *out = h;
+    return HOUGH_OK;
+}
+
+void hough_destroy(hough_handle *h)
+{
+    if (!h)
+        return;
+    free(h->radii);
+    delete h;
+}
+
+#define CK(expr)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            cudaGetLastError();                                                                    \
+            return HOUGH_ECUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
+               void *cuda_stream)
+{
+    if (!h)
+        return HOUGH_EINVAL;
+    if (n > h->cfg.max_hits)
+        return HOUGH_EINVAL;
+    if (n > 0 && (!x || !y || !layer))
+        return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    h->n_hits = n;
+    CK(cudaMemsetAsync(h->counters, 0, 64, st));
+    CK(launch_prep(h, x, y, layer, n, st));
+    CK(launch_vote(h, st));
+    h->voted = 1;
+    return HOUGH_OK;
+}
+
+static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_stream, int with_lists)
+{
+    if (!h || !out || !out->bin || !out->mask || !out->counts)
+        return HOUGH_EINVAL;
+    if (with_lists && (!out->hit_offset || !out->hit_index))
+        return HOUGH_EINVAL;
+    if (!h->voted)
+        return HOUGH_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaMemsetAsync((unsigned char *)h->counters + 64, 0, 192 + (size_t)2 * h->scan_blocks_max * 8, st));
+    CK(launch_peak_sweep(h, st));
+    CK(launch_scan_rows(h, st));
+    CK(launch_compact(h, out, st));
+    if (with_lists) {
+        CK(launch_list_count(h, st));
+        CK(launch_scan_lens(h, out, st));
+        CK(launch_list_fill(h, out, st));
+        CK(launch_sort_lists(h, out, st));
+    }
+    CK(launch_finish_counts(h, out, with_lists, st));
+    return HOUGH_OK;
+}
+
+int hough_peaks(hough_handle *h, const hough_peaks_out *out, void *cuda_stream)
+{
+    return peaks_common(h, out, cuda_stream, 1);
+}
+
+int hough_peaks_only(hough_handle *h, const hough_peaks_out *out, void *cuda_stream)
+{
+    return peaks_common(h, out, cuda_stream, 0);
+}
+
+const uint32_t *hough_accumulator(const hough_handle *h) { return h ? h->acc : nullptr; }
+
+int hough_clear(hough_handle *h, void *cuda_stream)
+{
+    if (!h)
+        return HOUGH_EINVAL;
+    CK(launch_clear(h, (cudaStream_t)cuda_stream));
+    return HOUGH_OK;
+}
+
+int hough_peak_sweep(hough_handle *h, void *cuda_stream)
+{
+    if (!h)
+        return HOUGH_EINVAL;
+    CK(launch_peak_sweep(h, (cudaStream_t)cuda_stream));
+    return HOUGH_OK;
+}
+
+int hough_set_accumulator(hough_handle *h, const uint32_t *acc_dev, void *cuda_stream)
+{
+    if (!h || !acc_dev)
+        return HOUGH_EINVAL;
+    size_t n_bins = (size_t)h->g.n_phi * h->g.n_d0 * h->g.n_kappa;
+    CK(cudaMemcpyAsync(h->acc, acc_dev, n_bins * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    CK(cudaMemsetAsync(h->counters, 0, 64, (cudaStream_t)cuda_stream));
+    h->n_hits = 0;
+    h->voted = 1;
+    return HOUGH_OK;
+}
+
+int hough_process_host(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
+                       const hough_peaks_out *dev, const hough_host_out *host, void *cuda_stream)
+{
+    if (!h || !dev || !host || !host->counts || !host->bin || !host->mask || !host->hit_offset)
+        return HOUGH_EINVAL;
+    if (n > h->cfg.max_hits || (n > 0 && (!x || !y || !layer)))
+        return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n > 0) {
+        CK(cudaMemcpyAsync(h->raw_x, x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_y, y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_layer, layer, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+    }
+    int rc = hough_vote(h, h->raw_x, h->raw_y, h->raw_layer, n, cuda_stream);
+    if (rc != HOUGH_OK)
+        return rc;
+    rc = hough_peaks(h, dev, cuda_stream);
+    if (rc != HOUGH_OK)
+        return rc;
+    CK(cudaMemcpyAsync(host->counts, dev->counts, sizeof(hough_counts), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    uint64_t np = host->counts->n_peaks < h->cfg.cap_peaks ? host->counts->n_peaks : h->cfg.cap_peaks;
+    uint64_t ne = host->counts->n_hit_entries < h->cfg.cap_hits ? host->counts->n_hit_entries : h->cfg.cap_hits;
+    if (np > 0) {
+        CK(cudaMemcpyAsync(host->bin, dev->bin, np * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(host->mask, dev->mask, np * 4, cudaMemcpyDeviceToHost, st));
+    }
+    CK(cudaMemcpyAsync(host->hit_offset, dev->hit_offset, (np + 1) * 8, cudaMemcpyDeviceToHost, st));
+    if (host->hit_index && ne > 0)
+        CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return HOUGH_OK;
+}
+
+int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,
+                int32_t *threads, int32_t *smem_bytes, int32_t *n_sms)
+{
+    if (!h)
+        return HOUGH_EINVAL;
+    if (tile_phi)
+        *tile_phi = h->vote_geom.P;
+    if (tile_d0)
+        *tile_d0 = h->vote_geom.D;
+    if (n_tiles)
+        *n_tiles = h->vote_geom.n_tiles;
+    if (threads)
+        *threads = h->vote_geom.threads;
+    if (smem_bytes)
+        *smem_bytes = h->vote_geom.smem_bytes;
+    if (n_sms)
+        *n_sms = h->n_sms;
+    return HOUGH_OK;
+}
+
+uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
+
+const char *hough_strerror(int code)
+{
+    switch (code) {
+    case HOUGH_OK:
+        return "ok";
+    case HOUGH_EINVAL:
+        return "invalid argument or configuration";
+    case HOUGH_ENOMEM:
+        return "workspace or capacity too small";
+    case HOUGH_ECUDA:
+        return "CUDA runtime error (or no CUDA device)";
+    case HOUGH_ESTATE:
+        return "call order violated";
+    default:
+        return "unknown error code";
+    }
+}

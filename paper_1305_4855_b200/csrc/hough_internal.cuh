@@ -1,0 +1,108 @@
+// hough_internal.cuh -- shared declarations of the CUDA path (libhough_b200.so).
+//
+// Product code.  Shares nothing with oracle/ (see DESIGN.md section 3): the arithmetic
+// recipe of the vote (A1..A7) is restated here with explicit
+// round-to-nearest intrinsics so that nvcc can neither fuse nor reorder it.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hough.h"
+
+// ---------------------------------------------------------------------------------
+// Geometry of one tiled sweep over the hits (vote, hit-list count, hit-list fill).
+// A CTA owns a tile of P phi0 centres x D d0 centres x all kappa bins in shared memory.
+// ---------------------------------------------------------------------------------
+struct SweepGeom {
+    int P, D;            // tile extent in cells
+    int cells_pad;       // P*D rounded up to a multiple of 32 (one lane per cell)
+    int groups;          // cells_pad / 32 : warps needed to cover the tile once
+    int split;           // S : warp sets that share the surviving hits of a chunk
+    int threads;         // 32 * groups * split
+    int chunk;           // hits staged per TMA bulk copy
+    int tiles_phi, tiles_d0, n_tiles;
+    int tile_words;      // 32-bit words of the bin tile in shared memory
+    int smem_bytes;      // dynamic shared memory of the kernel
+    int no_phi_cull;     // tile spans too wide an angle for the interval test
+};
+
+// Device-side constant block handed to every kernel by value.
+struct GridDev {
+    int n_phi, n_d0, n_kappa;
+    int L_min, phi_wrap;
+    int pack;            // masks per 32-bit word of the vote tile: 2 (n_layers <= 16) or 1
+    float klo, khi, inv_dk;
+    float kabs;          // max(|klo|, |khi|)
+    float d0_absmax;     // max |d0 centre|
+    const float *sn, *cs;            // [n_phi]
+    const float *d0c, *twod0, *d0sq; // [n_d0]
+};
+
+struct HitsDev {         // prepared hits, SoA, padded with non-voting entries to a chunk multiple
+    const float *x, *y, *r2;
+    const uint32_t *bit;
+    uint32_t n;          // real hits
+    uint32_t n_pad;      // padded length (multiple of the chunk size)
+};
+
+// Device counters of one event (internal; copied into the caller's hough_counts).
+struct DevCounters {
+    unsigned long long n_votes;
+    unsigned long long n_hit_entries;
+    unsigned int n_peaks;
+    unsigned int n_bad_hits;
+    unsigned int flags;
+    unsigned int pad;
+};
+
+struct hough_handle {
+    hough_config cfg;
+    double *radii;       // host copy
+    int device, n_sms;
+    GridDev g;
+    SweepGeom vote_geom, list_geom;
+    // workspace carve-up (device)
+    uint32_t *acc;
+    float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq;
+    float *hx, *hy, *hr2;
+    uint32_t *hbit;
+    float *raw_x, *raw_y;  // staging of hough_process_host's host buffers
+    int32_t *raw_layer;
+    uint32_t max_hits_pad;
+    uint32_t *flags;      // 1 bit per bin
+    uint32_t *row_base;   // [n_rows + 1] exclusive scan of peaks per (i, j) row
+    uint32_t *list_len;   // [cap_peaks] hit-list length of each reported peak
+    unsigned long long *scan_status; // look-back words of the chained scans
+    unsigned int *scan_ticket;       // [4]
+    DevCounters *counters;
+    uint32_t scan_blocks_max;
+    // sweep tile geometry of the peak kernel
+    int pk_Tj, pk_Li, pk_threads, pk_smem;
+    // state
+    uint32_t n_hits;
+    int voted;
+    uint64_t launches;
+};
+
+// kernels' host launchers (each enqueues on `st`, returns cudaGetLastError())
+cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const int32_t *layer,
+                        uint32_t n, cudaStream_t st);
+cudaError_t launch_vote(hough_handle *h, cudaStream_t st);
+cudaError_t launch_clear(hough_handle *h, cudaStream_t st);
+cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st);
+cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
+cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_sort_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_list_count(hough_handle *h, cudaStream_t st);
+cudaError_t launch_list_fill(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
+                                 cudaStream_t st);
+
+int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split, int bytes_per_bin_x2,
+                    int list_mode);
+int hough_vote_max_smem(void);
+
+#define HOUGH_CHUNK 512       // hits per staged chunk
+#define HOUGH_SCAN_ITEMS 2048 // items per block of the chained scan

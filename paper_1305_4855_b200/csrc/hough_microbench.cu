@@ -1,0 +1,73 @@
+// hough_microbench.cu -- shared-memory atomic micro-benchmark that DEFINES the
+// "shared-atomic roofline" the vote kernel is reported against (SURVEY.md section 8(d),
+// BASELINE.json north_star "% of smem-atomic roofline").  Not part of the hot path.
+#include "hough_internal.cuh"
+
+#define MB_WORDS 8192 // 32 KB table per CTA
+
+template <int MODE>
+__global__ void __launch_bounds__(1024) k_microbench(int iters, uint32_t *sink)
+{
+    __shared__ uint32_t table[MB_WORDS];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int w = tid; w < MB_WORDS; w += blockDim.x)
+        table[w] = 0u;
+    __syncthreads();
+    const uint32_t bit = 1u << (tid & 15);
+    uint32_t rnd = tid * 2654435761u + 12345u;
+    uint32_t base = (uint32_t)(warp * 64 + lane);
+#pragma unroll 8
+    for (int it = 0; it < iters; ++it) {
+        uint32_t idx;
+        if (MODE == 1) {
+            rnd = rnd * 1664525u + 1013904223u;
+            idx = (rnd >> 9) & (MB_WORDS - 1);
+        } else {
+            idx = (base + (uint32_t)it * 32u) & (MB_WORDS - 1); // 32 lanes -> 32 distinct banks
+        }
+        if (MODE == 2) {
+            volatile uint32_t *t = table;
+            t[idx] = t[idx] | bit;
+        } else {
+            atomicOr(&table[idx], bit);
+        }
+    }
+    __syncthreads();
+    uint32_t acc = 0u;
+    for (int w = tid; w < MB_WORDS; w += blockDim.x)
+        acc ^= table[w];
+    if (acc == 0xdeadbeefu)
+        sink[0] = acc;
+}
+
+int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters, void *cuda_stream,
+                          uint64_t *lane_ops)
+{
+    if (mode < 0 || mode > 2 || threads < 32 || threads > 1024 || (threads & 31) || ctas_per_sm < 1 ||
+        iters < 1)
+        return HOUGH_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return HOUGH_ECUDA;
+    }
+    cudaDeviceProp prop;
+    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess)
+        return HOUGH_ECUDA;
+    static uint32_t *sink = nullptr; // 4 bytes of scratch, never freed (benchmark helper only)
+    if (!sink && cudaMalloc(&sink, 4) != cudaSuccess)
+        return HOUGH_ECUDA;
+    int blocks = prop.multiProcessorCount * ctas_per_sm;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (mode == 0)
+        k_microbench<0><<<blocks, threads, 0, st>>>(iters, sink);
+    else if (mode == 1)
+        k_microbench<1><<<blocks, threads, 0, st>>>(iters, sink);
+    else
+        k_microbench<2><<<blocks, threads, 0, st>>>(iters, sink);
+    if (cudaGetLastError() != cudaSuccess)
+        return HOUGH_ECUDA;
+    if (lane_ops)
+        *lane_ops = (uint64_t)blocks * (uint64_t)threads * (uint64_t)iters;
+    return HOUGH_OK;
+}

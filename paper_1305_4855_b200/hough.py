@@ -1,0 +1,300 @@
+"""Thin Python binding of the C ABI in include/hough.h (libhough_b200.so).
+
+Argument marshalling only: every step of the path (hit preparation, staging, vote,
+write-out, peak sweep, compaction, hit lists) runs in the CUDA kernels under ``csrc/``.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback:
+importing this module raises if the shared library cannot be loaded, and every call
+raises ``HoughError`` on a non-zero return code.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libhough_b200.so")
+
+HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3, -4
+TRUNCATED_PEAKS, TRUNCATED_HITS = 1, 2
+OPT_NO_CULL = 1
+
+# every symbol include/hough.h declares (checked by the CPU test-suite)
+SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
+           "hough_accumulator", "hough_process_host", "hough_clear", "hough_peak_sweep",
+           "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
+           "hough_launch_count", "hough_strerror")
+
+
+class HoughError(RuntimeError):
+    pass
+
+
+class Config(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("layer_radius_cm", C.POINTER(C.c_double)),
+                ("phi_min", C.c_double), ("phi_max", C.c_double),
+                ("d0_min", C.c_double), ("d0_max", C.c_double),
+                ("kappa_min", C.c_double), ("kappa_max", C.c_double),
+                ("n_phi", C.c_int32), ("n_d0", C.c_int32), ("n_kappa", C.c_int32),
+                ("L_min", C.c_int32), ("phi_wrap", C.c_int32),
+                ("max_hits", C.c_uint32), ("cap_peaks", C.c_uint32), ("cap_hits", C.c_uint64),
+                ("tile_phi", C.c_int32), ("tile_d0", C.c_int32),
+                ("options", C.c_uint32), ("device", C.c_int32)]
+
+
+class Counts(C.Structure):
+    _fields_ = [("n_votes", C.c_uint64), ("n_hit_entries", C.c_uint64), ("n_peaks", C.c_uint32),
+                ("n_bad_hits", C.c_uint32), ("flags", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class PeaksOut(C.Structure):
+    _fields_ = [("bin", C.c_void_p), ("mask", C.c_void_p), ("hit_offset", C.c_void_p),
+                ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
+
+
+class HostOut(C.Structure):
+    _fields_ = [("bin", C.c_void_p), ("mask", C.c_void_p), ("hit_offset", C.c_void_p),
+                ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
+
+
+COUNTS_DTYPE = np.dtype([("n_votes", "<u8"), ("n_hit_entries", "<u8"), ("n_peaks", "<u4"),
+                         ("n_bad_hits", "<u4"), ("flags", "<u4"), ("reserved", "<u4")])
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s is missing: build it with `python -m paper_1305_4855_b200.build` "
+            "(there is no CPU fallback)" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    lib.hough_workspace_bytes.restype = C.c_size_t
+    lib.hough_workspace_bytes.argtypes = [C.POINTER(Config)]
+    lib.hough_create.restype = C.c_int
+    lib.hough_create.argtypes = [C.POINTER(Config), C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+    lib.hough_destroy.restype = None
+    lib.hough_destroy.argtypes = [C.c_void_p]
+    lib.hough_vote.restype = C.c_int
+    lib.hough_vote.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    for name in ("hough_peaks", "hough_peaks_only"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.POINTER(PeaksOut), C.c_void_p]
+    lib.hough_accumulator.restype = C.c_void_p
+    lib.hough_accumulator.argtypes = [C.c_void_p]
+    lib.hough_process_host.restype = C.c_int
+    lib.hough_process_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32,
+                                       C.POINTER(PeaksOut), C.POINTER(HostOut), C.c_void_p]
+    for name in ("hough_clear", "hough_peak_sweep"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.c_void_p]
+    lib.hough_set_accumulator.restype = C.c_int
+    lib.hough_set_accumulator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.hough_microbench_smem.restype = C.c_int
+    lib.hough_microbench_smem.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                          C.POINTER(C.c_uint64)]
+    lib.hough_query.restype = C.c_int
+    lib.hough_query.argtypes = [C.c_void_p] + [C.POINTER(C.c_int32)] * 6
+    lib.hough_launch_count.restype = C.c_uint64
+    lib.hough_launch_count.argtypes = [C.c_void_p]
+    lib.hough_strerror.restype = C.c_char_p
+    lib.hough_strerror.argtypes = [C.c_int]
+    return lib
+
+
+_lib = _load()
+
+
+def strerror(code: int) -> str:
+    return _lib.hough_strerror(int(code)).decode()
+
+
+def _check(rc: int, what: str):
+    if rc != HOUGH_OK:
+        raise HoughError("%s failed: %s (%d)" % (what, strerror(rc), rc))
+
+
+def make_config(grid, max_hits, cap_peaks, cap_hits, device=0, tile_phi=0, tile_d0=0, options=0):
+    """hough_config from any object with the Grid attributes (see synth.Grid).  Returns
+    (Config, keep-alive objects)."""
+    radii = (C.c_double * len(grid.layer_radii))(*[float(r) for r in grid.layer_radii])
+    cfg = Config(len(grid.layer_radii), C.cast(radii, C.POINTER(C.c_double)),
+                 grid.phi_min, grid.phi_max, grid.d0_min, grid.d0_max, grid.kappa_min, grid.kappa_max,
+                 grid.n_phi, grid.n_d0, grid.n_kappa, grid.L_min, grid.phi_wrap,
+                 int(max_hits), int(cap_peaks), int(cap_hits), int(tile_phi), int(tile_d0),
+                 int(options), int(device))
+    return cfg, radii
+
+
+def workspace_bytes(grid, max_hits, cap_peaks, cap_hits, **kw) -> int:
+    cfg, _keep = make_config(grid, max_hits, cap_peaks, cap_hits, **kw)
+    return int(_lib.hough_workspace_bytes(C.byref(cfg)))
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+class Hough:
+    """One grid on one device.  ``vote`` + ``peaks`` enqueue on a stream and return;
+    ``read`` synchronises and returns numpy views of the results."""
+
+    def __init__(self, grid, max_hits, cap_peaks, cap_hits, device=0, tile_phi=0, tile_d0=0,
+                 options=0):
+        if not torch.cuda.is_available():
+            raise HoughError("no CUDA device: the Hough path has no CPU fallback")
+        self.grid = grid
+        self.device = torch.device("cuda", device)
+        self.cap_peaks, self.cap_hits, self.max_hits = int(cap_peaks), int(cap_hits), int(max_hits)
+        self.cfg, self._keep = make_config(grid, max_hits, cap_peaks, cap_hits, device, tile_phi,
+                                           tile_d0, options)
+        nbytes = int(_lib.hough_workspace_bytes(C.byref(self.cfg)))
+        if nbytes == 0:
+            raise HoughError("hough_workspace_bytes: invalid configuration")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self._h = C.c_void_p()
+        _check(_lib.hough_create(C.byref(self.cfg), C.c_void_p(self.workspace.data_ptr()), nbytes,
+                                 C.byref(self._h)), "hough_create")
+        i32 = dict(dtype=torch.int32, device=self.device)
+        self.peak_bin = torch.empty(self.cap_peaks, **i32)
+        self.peak_mask = torch.empty(self.cap_peaks, **i32)
+        self.hit_offset = torch.empty(self.cap_peaks + 1, dtype=torch.int64, device=self.device)
+        self.hit_index = torch.empty(self.cap_hits, **i32)
+        self.counts = torch.zeros(4, dtype=torch.int64, device=self.device)  # 32 bytes
+        self._out = PeaksOut(self.peak_bin.data_ptr(), self.peak_mask.data_ptr(),
+                             self.hit_offset.data_ptr(), self.hit_index.data_ptr(),
+                             self.counts.data_ptr())
+        self._host = None
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            _lib.hough_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C-ABI calls
+    def vote(self, x, y, layer, stream=None):
+        """hough_vote: x, y float32 / layer int32 CUDA tensors of one event."""
+        n = int(x.numel())
+        assert x.is_cuda and y.is_cuda and layer.is_cuda
+        assert x.dtype == torch.float32 and y.dtype == torch.float32 and layer.dtype == torch.int32
+        assert y.numel() == n and layer.numel() == n
+        assert x.is_contiguous() and y.is_contiguous() and layer.is_contiguous()
+        _check(_lib.hough_vote(self._h, C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()),
+                               C.c_void_p(layer.data_ptr()), n, _stream_ptr(stream)), "hough_vote")
+
+    def peaks(self, stream=None, lists=True):
+        """hough_peaks (or hough_peaks_only): results land in this object's device arrays."""
+        f = _lib.hough_peaks if lists else _lib.hough_peaks_only
+        _check(f(self._h, C.byref(self._out), _stream_ptr(stream)), "hough_peaks")
+
+    def clear(self, stream=None):
+        _check(_lib.hough_clear(self._h, _stream_ptr(stream)), "hough_clear")
+
+    def peak_sweep(self, stream=None):
+        _check(_lib.hough_peak_sweep(self._h, _stream_ptr(stream)), "hough_peak_sweep")
+
+    def set_accumulator(self, acc, stream=None):
+        assert acc.is_cuda and acc.dtype == torch.int32 and acc.numel() == self.grid.n_bins
+        _check(_lib.hough_set_accumulator(self._h, C.c_void_p(acc.data_ptr()), _stream_ptr(stream)),
+               "hough_set_accumulator")
+
+    def accumulator(self) -> torch.Tensor:
+        """Device view (int32 bit patterns of the uint32 masks), shape [n_phi, n_d0, n_kappa]."""
+        ptr = _lib.hough_accumulator(self._h)
+        off = ptr - self.workspace.data_ptr()
+        g = self.grid
+        return self.workspace[off:off + 4 * g.n_bins].view(torch.int32).view(g.n_phi, g.n_d0, g.n_kappa)
+
+    def process_host(self, x, y, layer, stream=None, want_lists=True):
+        """hough_process_host: numpy (ideally pinned) host arrays in, host results out."""
+        x = np.ascontiguousarray(x, np.float32)
+        y = np.ascontiguousarray(y, np.float32)
+        layer = np.ascontiguousarray(layer, np.int32)
+        n = x.shape[0]
+        if self._host is None:
+            pin = dict(pin_memory=True)
+            self._host = dict(
+                bin=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
+                mask=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
+                hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, **pin),
+                hit_index=torch.empty(self.cap_hits, dtype=torch.int32, **pin),
+                counts=torch.zeros(4, dtype=torch.int64, **pin))
+        hb = self._host
+        host = HostOut(hb["bin"].data_ptr(), hb["mask"].data_ptr(), hb["hit_offset"].data_ptr(),
+                       hb["hit_index"].data_ptr() if want_lists else None, hb["counts"].data_ptr())
+        _check(_lib.hough_process_host(self._h, C.c_void_p(x.ctypes.data), C.c_void_p(y.ctypes.data),
+                                       C.c_void_p(layer.ctypes.data), n, C.byref(self._out),
+                                       C.byref(host), _stream_ptr(stream)), "hough_process_host")
+        cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
+        return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
+                          hb["hit_index"].numpy() if want_lists else None)
+
+    # -- results
+    def _pack(self, cnt, b, m, off, idx):
+        n_rep = min(int(cnt["n_peaks"]), self.cap_peaks)
+        n_ent = min(int(cnt["n_hit_entries"]), self.cap_hits)
+        out = {"n_votes": int(cnt["n_votes"]), "n_hit_entries": int(cnt["n_hit_entries"]),
+               "n_peaks": int(cnt["n_peaks"]), "n_bad_hits": int(cnt["n_bad_hits"]),
+               "flags": int(cnt["flags"]),
+               "peak_bin": b[:n_rep].view(np.uint32), "peak_mask": m[:n_rep].view(np.uint32),
+               "hit_offset": off[:n_rep + 1].view(np.uint64)}
+        if idx is not None:
+            out["hit_index"] = idx[:n_ent].view(np.uint32)
+        return out
+
+    def read_counts(self):
+        torch.cuda.synchronize(self.device)
+        return self.counts.cpu().numpy().view(COUNTS_DTYPE)[0]
+
+    def read(self, lists=True):
+        """Synchronise and copy the results of the last vote + peaks to the host."""
+        cnt = self.read_counts()
+        n_rep = min(int(cnt["n_peaks"]), self.cap_peaks)
+        n_ent = min(int(cnt["n_hit_entries"]), self.cap_hits) if lists else 0
+        b = self.peak_bin[:n_rep].cpu().numpy()
+        m = self.peak_mask[:n_rep].cpu().numpy()
+        off = self.hit_offset[:n_rep + 1].cpu().numpy() if lists else np.zeros(n_rep + 1, np.int64)
+        idx = self.hit_index[:n_ent].cpu().numpy() if lists else None
+        return self._pack(cnt, b, m, off, idx)
+
+    def accumulator_host(self) -> np.ndarray:
+        torch.cuda.synchronize(self.device)
+        return self.accumulator().cpu().numpy().view(np.uint32)
+
+    def query(self):
+        v = [C.c_int32() for _ in range(6)]
+        _check(_lib.hough_query(self._h, *[C.byref(a) for a in v]), "hough_query")
+        keys = ("tile_phi", "tile_d0", "n_tiles", "threads", "smem_bytes", "n_sms")
+        return dict(zip(keys, [a.value for a in v]))
+
+    def launch_count(self) -> int:
+        return int(_lib.hough_launch_count(self._h))
+
+
+def microbench_smem(mode, threads=1024, ctas_per_sm=2, iters=4096, device=0, reps=5):
+    """Times hough_microbench_smem with CUDA events; returns lane-ops per second (best of reps)."""
+    st = torch.cuda.current_stream()
+    ops = C.c_uint64()
+    best = None
+    for _ in range(reps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        _check(_lib.hough_microbench_smem(device, mode, threads, ctas_per_sm, iters,
+                                          C.c_void_p(st.cuda_stream), C.byref(ops)),
+               "hough_microbench_smem")
+        e1.record(st)
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return ops.value / (best * 1e-3)

@@ -1,0 +1,241 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit.
+
+Every test drives libhough_b200.so through paper_1305_4855_b200.hough (ctypes marshalling
+only) and compares accumulator masks, vote count, peak list and CSR hit lists with
+oracle/ on the same seeded inputs (BASELINE.json north_star: "GPU results must match the
+oracle bit-exactly (accumulator masks, peak list, hit lists)").
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1305_4855_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def hough():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1305_4855_b200 import hough as hough_mod
+    return hough_mod
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(hough, grid, x, y, layer, cap_peaks, cap_hits, **kw):
+    h = hough.Hough(grid, max_hits=max(len(x), 1), cap_peaks=cap_peaks, cap_hits=cap_hits, **kw)
+    h.vote(dev(x.astype(np.float32)), dev(y.astype(np.float32)), dev(layer.astype(np.int32)))
+    h.peaks()
+    res = h.read()
+    res["acc"] = h.accumulator_host().copy()
+    res["query"] = h.query()
+    h.close()
+    return res
+
+
+def assert_same(res, ref, lists=True):
+    assert res["n_votes"] == ref["n_votes"]
+    assert res["n_bad_hits"] == ref["n_bad_hits"]
+    assert np.array_equal(res["acc"], ref["acc"])
+    assert res["n_peaks"] == ref["n_peaks"]
+    assert np.array_equal(res["peak_bin"], ref["peak_bin"])
+    assert np.array_equal(res["peak_mask"], ref["peak_mask"])
+    if lists:
+        assert res["n_hit_entries"] == ref["n_hit_entries"]
+        assert np.array_equal(res["hit_offset"], ref["hit_offset"])
+        assert np.array_equal(res["hit_index"], ref["hit_index"])
+
+
+def random_hits(rng, n, n_layers=10, rmax=80.0):
+    r = rng.uniform(0.5, rmax, n)
+    phi = rng.uniform(-math.pi, math.pi, n)
+    return ((r * np.cos(phi)).astype(np.float32), (r * np.sin(phi)).astype(np.float32),
+            rng.integers(0, n_layers, n).astype(np.int32))
+
+
+# ------------------------------------------------------------------ small grids, ragged tiles
+@pytest.mark.parametrize("shape,tile,n_hits,seed", [
+    ((8, 4, 32), (0, 0), 20, 0),          # one tile, phi slab wider than a quarter turn
+    ((50, 13, 64), (8, 4), 700, 1),       # ragged in phi0 and d0, several chunks
+    ((37, 5, 96), (6, 2), 1300, 2),       # n_kappa not a multiple of 64 (smaller swizzle)
+    ((64, 1, 128), (16, 1), 300, 3),      # 2-D transform (n_d0 = 1)
+    ((96, 24, 32), (32, 8), 513, 4),      # smallest row, hits = chunk + 1
+    ((33, 9, 256), (4, 8), 100, 5),
+])
+@pytest.mark.parametrize("options", [0, 1])
+def test_random_hits_small_grids(hough, oracle, shape, tile, n_hits, seed, options):
+    rng = np.random.default_rng(seed)
+    d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
+    grid = synth.Grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=3, **d0)
+    x, y, layer = random_hits(rng, n_hits)
+    ref = oracle.run(grid, x, y, layer)
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                  cap_hits=max(ref["n_hit_entries"], 1) + 5, tile_phi=tile[0], tile_d0=tile[1],
+                  options=options)
+    assert_same(res, ref)
+
+
+def test_no_wrap_and_asymmetric_kappa_range(hough, oracle):
+    rng = np.random.default_rng(11)
+    grid = synth.Grid(n_phi=40, n_d0=6, n_kappa=64, L_min=2, phi_min=-1.0, phi_max=2.0,
+                      d0_min=-3.0, d0_max=7.0, kappa_min=-0.002, kappa_max=0.02, phi_wrap=0)
+    x, y, layer = random_hits(rng, 900)
+    ref = oracle.run(grid, x, y, layer)
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                  cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4)
+    assert_same(res, ref)
+
+
+def test_more_than_16_layers_uses_unpacked_tiles(hough, oracle):
+    rng = np.random.default_rng(12)
+    radii = tuple(3.0 + 3.0 * i for i in range(24))
+    grid = synth.Grid(n_phi=48, n_d0=10, n_kappa=64, L_min=4, layer_radii=radii)
+    x, y, layer = random_hits(rng, 1500, n_layers=24)
+    ref = oracle.run(grid, x, y, layer)
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                  cap_hits=ref["n_hit_entries"] + 1)
+    assert_same(res, ref)
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_empty_event(hough, oracle):
+    grid = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=1)
+    e = np.zeros(0, np.float32)
+    res = run_gpu(hough, grid, e, e, np.zeros(0, np.int32), cap_peaks=8, cap_hits=8)
+    assert res["n_votes"] == 0 and res["n_peaks"] == 0 and res["n_hit_entries"] == 0
+    assert not res["acc"].any() and res["hit_offset"].tolist() == [0]
+
+
+def test_bad_layers_and_non_finite_hits(hough, oracle):
+    rng = np.random.default_rng(13)
+    grid = synth.Grid(n_phi=32, n_d0=8, n_kappa=64, L_min=2)
+    x, y, layer = random_hits(rng, 400)
+    layer[::7] = -1
+    layer[3::11] = 10
+    x[5] = np.nan
+    y[6] = np.inf
+    x[8] = -np.inf
+    x[9] = 3.0e19            # x*x overflows: den = inf, kappa = 0 -> a legal vote
+    x[10], y[10] = 0.0, 0.0  # hit at the origin
+    ref = oracle.run(grid, x, y, layer)
+    assert ref["n_bad_hits"] > 0
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                  cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4)
+    assert_same(res, ref)
+
+
+def test_hits_at_the_point_of_closest_approach(hough, oracle):
+    """den = |X - P0|^2 ~ 0: the quotient is ill-conditioned and the cull must stay a superset."""
+    grid = synth.Grid(n_phi=64, n_d0=16, n_kappa=64, L_min=1)
+    phic = grid.phi_min + (np.arange(grid.n_phi) + 0.5) * (grid.phi_max - grid.phi_min) / grid.n_phi
+    d0c = grid.d0_min + (np.arange(grid.n_d0) + 0.5) * (grid.d0_max - grid.d0_min) / grid.n_d0
+    rng = np.random.default_rng(14)
+    xs, ys = [], []
+    for _ in range(600):
+        i, j = rng.integers(0, grid.n_phi), rng.integers(0, grid.n_d0)
+        d = d0c[j] + rng.normal(0, 1e-4)
+        t = rng.normal(0, 1e-3)
+        xs.append(-d * math.sin(phic[i]) + t * math.cos(phic[i]))
+        ys.append(d * math.cos(phic[i]) + t * math.sin(phic[i]))
+    x, y = np.asarray(xs, np.float32), np.asarray(ys, np.float32)
+    layer = rng.integers(0, 10, len(x)).astype(np.int32)
+    ref = oracle.run(grid, x, y, layer)
+    for opt in (0, 1):
+        res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=4, tile_d0=2, options=opt)
+        assert_same(res, ref)
+
+
+def test_truncation_is_deterministic(hough, oracle):
+    rng = np.random.default_rng(15)
+    grid = synth.Grid(n_phi=32, n_d0=8, n_kappa=64, L_min=2)
+    x, y, layer = random_hits(rng, 800)
+    ref = oracle.run(grid, x, y, layer)
+    assert ref["n_peaks"] > 40
+    cap_p = 25
+    full_len = int(ref["hit_offset"][cap_p])
+    cap_h = int(ref["hit_offset"][cap_p - 5]) + 1      # cuts inside list cap_p-5
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=cap_p, cap_hits=cap_h)
+    assert res["flags"] == 3 and res["n_peaks"] == ref["n_peaks"]
+    assert np.array_equal(res["peak_bin"], ref["peak_bin"][:cap_p])
+    assert np.array_equal(res["peak_mask"], ref["peak_mask"][:cap_p])
+    assert res["n_hit_entries"] == full_len
+    assert np.array_equal(res["hit_offset"], ref["hit_offset"][:cap_p + 1])
+    whole = int(ref["hit_offset"][cap_p - 5])           # lists that fit completely
+    assert np.array_equal(res["hit_index"][:whole], ref["hit_index"][:whole])
+
+
+def test_peak_rule_on_handmade_accumulators(hough, oracle):
+    """Plateaus, ties, edges and phi wrap, through hough_set_accumulator + hough_peaks_only."""
+    rng = np.random.default_rng(16)
+    for (shape, wrap, L_min, dens) in [((6, 5, 32), 1, 1, 0.5), ((6, 5, 32), 0, 2, 0.9),
+                                       ((3, 1, 64), 1, 1, 0.3), ((20, 17, 32), 1, 3, 1.0),
+                                       ((5, 30, 64), 0, 1, 0.05)]:
+        d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
+        grid = synth.Grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=L_min,
+                          phi_wrap=wrap, **d0)
+        for variant in range(3):
+            acc = rng.integers(0, 1 << 10, grid.n_bins, dtype=np.uint32)
+            acc[rng.random(grid.n_bins) > dens] = 0
+            if variant == 1:
+                acc[:] = 0x3ff                       # all equal: only lin 0 is a peak
+            if variant == 2:
+                acc &= 0x7                           # few distinct popcounts: many ties
+            pb, pm, n = oracle.peaks(grid, acc)
+            h = hough.Hough(grid, max_hits=1, cap_peaks=grid.n_bins, cap_hits=1)
+            h.set_accumulator(dev(acc.view(np.int32)))
+            h.peaks(lists=False)
+            res = h.read(lists=False)
+            h.close()
+            assert res["n_peaks"] == n
+            assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
+
+
+def test_repeat_runs_are_bit_identical(hough):
+    """The race test of PAPER.md:126: OR of masks is order independent."""
+    w = synth.WORKLOADS["displaced3d"]
+    x, y, layer, _ = synth.generate_event(w.event, 3)
+    h = hough.Hough(w.grid, len(x), w.cap_peaks, w.cap_hits)
+    dx, dy, dl = dev(x), dev(y), dev(layer)
+    outs = []
+    for _ in range(3):
+        h.vote(dx, dy, dl)
+        h.peaks()
+        r = h.read()
+        outs.append((h.accumulator_host().copy(), r["n_votes"], r["peak_bin"].copy(),
+                     r["hit_offset"].copy(), r["hit_index"].copy()))
+    h.close()
+    for o in outs[1:]:
+        assert o[1] == outs[0][1]
+        for a, b in zip(o, outs[0]):
+            if isinstance(a, np.ndarray):
+                assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ the BASELINE.json configs
+@pytest.mark.parametrize("name", ["prompt2d", "displaced3d", "pileup"])
+def test_baseline_configs_full_parity(hough, oracle, name):
+    w = synth.WORKLOADS[name]
+    x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
+    ref = oracle.run(w.grid, x, y, layer)
+    res = run_gpu(hough, w.grid, x, y, layer, cap_peaks=w.cap_peaks, cap_hits=w.cap_hits)
+    assert res["flags"] == 0
+    assert_same(res, ref)
+
+
+def test_process_host_matches_device_path(hough, oracle):
+    w = synth.WORKLOADS["displaced3d"]
+    x, y, layer, _ = synth.generate_event(w.event, 1)
+    ref = oracle.run(w.grid, x, y, layer)
+    h = hough.Hough(w.grid, len(x), w.cap_peaks, w.cap_hits)
+    res = h.process_host(x, y, layer)
+    res["acc"] = h.accumulator_host().copy()
+    h.close()
+    assert_same(res, ref)
