@@ -1,0 +1,408 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Hough-transform hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (hough_vote + hough_peaks: hit preparation,
+staging, vote, write-out, peak sweep, compaction, hit lists) over one batch of the
+workload: BASELINE.json configs[3], 100 independent pile-up events (seeds 0..99), each
+with its own accumulator, back to back on one stream.  `value` is in-range votes cast per
+second over all ranks (inputs resident in HBM); `events_per_s` and `evaluations_per_s`
+(n * n_phi * n_d0 per event, the paper-level work) are reported beside it.  `e2e` is the
+same metric through hough_process_host: pinned HOST buffers in, results copied back to
+the host, every event.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload batch100|pileup|...]
+    python bench.py --impl reference ...   # the CPU oracle, as it stands, on the host cores
+
+N > 1 is launched with torch.distributed.run; ranks take disjoint seed ranges of the same
+event recipe (weak scaling, no data-path collective: the paper runs one event per GPU).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1305_4855_b200 import synth  # noqa: E402  (input generator only)
+
+METRIC = "hough_votes_per_s"
+UNIT = "votes/s"
+# fp32 operations of one closed-form evaluation counting the divide as one:
+# 3 for s, 2 for num, 3 for den, 1 divide, 2 compares, 2 for the bin, 1 convert, 1 min
+FLOP_PER_EVAL = 15.0
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        if self.thread is not None:
+            self.thread.join(timeout=5)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                smax.append(float(r[1]))
+                power.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)),
+                "power_w_max": float(max(power)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_module():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    try:
+        import hough_oracle
+    finally:
+        sys.path.pop(0)
+    hough_oracle.lib()
+    return hough_oracle
+
+
+def time_oracle(workload, seed):
+    """The oracle as it stands on one event of the workload (vote + peaks + hit lists)."""
+    o = oracle_module()
+    x, y, layer, _ = synth.generate_event(workload.event, seed)
+    t0 = time.perf_counter()
+    acc, n_votes, _ = o.vote(workload.grid, x, y, layer)
+    pb, _pm, _n = o.peaks(workload.grid, acc, workload.cap_peaks)
+    o.hitlists(workload.grid, x, y, layer, pb, workload.cap_hits)
+    dt = time.perf_counter() - t0
+    return n_votes, len(x), dt, o.num_threads()
+
+
+def run_reference(args, workload, rank):
+    """--impl reference: the CPU oracle on the host cores, one event per step (bounded sample)."""
+    if rank != 0:
+        return
+    for s in range(args.warmup):
+        if s == 0:  # one warm-up event is enough to page the library in; keep the run short
+            time_oracle(workload, workload.seeds[0])
+    votes, secs, cores = 0, 0.0, 1
+    for s in range(args.steps):
+        nv, _n, dt, cores = time_oracle(workload, workload.seeds[s % len(workload.seeds)])
+        votes += nv
+        secs += dt
+    val = votes / secs
+    sample = "1 event per step (seeds 0..%d of the batch): vote + peaks + hit lists" % (args.steps - 1)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": {"workload": workload.name, "sample": sample},
+            "events_per_s": args.steps / secs,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="batch100", choices=sorted(synth.WORKLOADS))
+    ap.add_argument("--events", type=int, default=0, help="events per step (default: the workload's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the stage-time, sweep-roofline and micro-benchmark legs")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    workload = synth.WORKLOADS[args.workload]
+
+    if args.impl == "reference":
+        run_reference(args, workload, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the Hough path has no CPU fallback)")
+    from paper_1305_4855_b200 import hough
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peaks_info = load_peaks()
+
+    # ---- inputs: this rank's events (weak scaling: rank r takes seeds r*E .. r*E+E-1)
+    n_ev = args.events if args.events > 0 else len(workload.seeds)
+    seeds = [rank * n_ev + s for s in range(n_ev)]
+    events = [synth.generate_event(workload.event, s)[:3] for s in seeds]
+    max_hits = max(len(e[0]) for e in events)
+    d_events = [tuple(torch.from_numpy(a).to(dev) for a in e) for e in events]
+    pin_events = [tuple(torch.from_numpy(a).pin_memory() for a in e) for e in events]
+    h = hough.Hough(workload.grid, max_hits, workload.cap_peaks, workload.cap_hits, device=local_rank)
+    counts_all = torch.zeros(n_ev, hough.COUNTS_WORDS, dtype=torch.int64, device=dev)
+    st = torch.cuda.current_stream()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)  # > the 126 MB L2
+
+    def step():
+        for e in range(n_ev):
+            x, y, layer = d_events[e]
+            h.vote(x, y, layer)
+            h.peaks(counts_out=counts_all[e])
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    cnt = counts_all.cpu().numpy().view(hough.COUNTS_DTYPE).reshape(n_ev)
+    votes_step = int(cnt["n_votes"].sum())
+    evals_step = sum(len(e[0]) for e in events) * workload.grid.n_phi * workload.grid.n_d0
+    evals_done_step = int(cnt["n_evals"].sum())
+    assert int(cnt["flags"].max()) == 0, "output capacities overflowed"
+
+    # ---- timed region: K steps, one CUDA-event pair per step, L2 flushed between steps
+    launches0 = h.launch_count()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    step_ms = []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        step()
+        e1.record(st)
+        e1.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if rank == 0 else None
+    launches = h.launch_count() - launches0
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        v = torch.tensor([votes_step, evals_step, n_ev], dtype=torch.float64, device=dev)
+        dist.all_reduce(v, op=dist.ReduceOp.SUM)
+        votes_all, evals_all, events_all = [float(a) for a in v.tolist()]
+    else:
+        votes_all, evals_all, events_all = float(votes_step), float(evals_step), float(n_ev)
+    secs = total_ms * 1e-3
+    value = votes_all * args.steps / secs
+
+    # ---- e2e: host buffers in, host results out, every event (hough_process_host)
+    def e2e_step():
+        nv = 0
+        for e in range(n_ev):
+            x, y, layer = pin_events[e]
+            r = h.process_host(x.numpy(), y.numpy(), layer.numpy())
+            nv += r["n_votes"]
+        return nv
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    nv_e2e = 0
+    for _ in range(args.steps):
+        nv_e2e += e2e_step()
+    torch.cuda.synchronize(dev)
+    e2e_secs = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_secs], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_secs = float(t.item())
+    assert nv_e2e == votes_step * args.steps
+    h2d = sum(len(e[0]) for e in events) * 12
+    d2h = int(sum(40 + min(int(c["n_peaks"]), workload.cap_peaks) * 16 + 8 +
+                  min(int(c["n_hit_entries"]), workload.cap_hits) * 4 for c in cnt))
+    e2e = {"value": votes_all * args.steps / e2e_secs, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": workload.name, "events_per_step": n_ev,
+                       "grid": [workload.grid.n_phi, workload.grid.n_d0, workload.grid.n_kappa],
+                       "L_min": workload.grid.L_min, "hits_per_event": int(np.mean([len(e[0]) for e in events])),
+                       "l2": "512 MiB flush buffer written between steps, outside the event pairs",
+                       "parallelism": "replicas x%d (events sharded by seed, no collective)" % world},
+            "events_per_s": events_all * args.steps / secs,
+            "evaluations_per_s": evals_all * args.steps / secs,
+            "votes_per_event": votes_step / n_ev,
+            "wall_s_timed_region": t_wall,
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+
+    if rank == 0 and not args.no_extras:
+        line.update(extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_info,
+                           votes_step, evals_step, evals_done_step, flush))
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        nv, _n, dt, cores = time_oracle(workload, workload.seeds[0])
+        line["cpu_baseline"] = {"value": nv / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "events_per_s": 1.0 / dt,
+                                "sample": "1 of the %d events (seed 0), whole path: vote + peaks + "
+                                          "hit lists, %.1f s" % (n_ev, dt)}
+    h.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_info, votes_step,
+           evals_step, evals_done_step, flush):
+    """Per-kernel times measured live (CUDA events on the launching stream, recorded by the
+    library around every kernel), the roofline of the dominant kernel, the shared-atomic
+    micro-benchmark and the HBM roofline of the stand-alone accumulator sweeps."""
+    out = {}
+    ht = hough.Hough(workload.grid, max(len(e[0]) for e in d_events), workload.cap_peaks,
+                     workload.cap_hits, device=local_rank, options=hough.OPT_STAGE_TIMING)
+    acc = {}
+    reps = 2
+    for r in range(reps + 1):
+        for e in range(n_ev):
+            x, y, layer = d_events[e]
+            ht.vote(x, y, layer)
+            ht.peaks()
+            if r > 0:
+                for k, v in ht.stage_times().items():
+                    acc[k] = acc.get(k, 0.0) + v
+    ht.close()
+    per_event = {k: v / (reps * n_ev) for k, v in acc.items()}
+    out["stage_ms_per_event"] = {k: round(v, 5) for k, v in per_event.items()}
+    tot = sum(per_event.values())
+    dom = max(per_event, key=per_event.get)
+    out["stage_share"] = {k: round(v / tot, 4) for k, v in per_event.items()}
+
+    # dominant kernel of the step: the tiled vote sweep (plain-ALU issue bound)
+    vote_s = per_event["vote"] * 1e-3
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    alu_peak = n_sms * 128 * peaks_info["sm_max_mhz"] * 1e6 / 1e12  # fp32 lanes x clock, no FMA
+    achieved = FLOP_PER_EVAL * (evals_step / n_ev) / vote_s / 1e12
+    out["roofline"] = {
+        "kernel": "k_sweep<MODE_VOTE>", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": None,
+        "note": "algorithmic fp32 ops = 15 x n x n_phi x n_d0 per launch (every hit x cell); the "
+                "conservative cull executes only executed_frac of them; peak = SMs x 128 fp32 "
+                "lanes x sm_max_mhz without FMA (the recipe forbids contraction); "
+                + peaks_info["source"],
+        "executed_frac": evals_done_step / evals_step,
+        "achieved_executed": FLOP_PER_EVAL * (evals_done_step / n_ev) / vote_s / 1e12,
+        "dominant_stage_measured": dom}
+
+    # shared-atomic roofline: conflict-free no-return atomicOr micro-benchmark on this box
+    best = 0.0
+    for thr, cps in ((1024, 2), (512, 4), (256, 8)):
+        best = max(best, hough.microbench_smem(0, thr, cps, 4096, device=local_rank))
+    rnd = hough.microbench_smem(1, 512, 4, 4096, device=local_rank)
+    vps = (votes_step / n_ev) / vote_s
+    out["roofline_smem_atomic"] = {"bound": "smem_atomic", "achieved": vps, "peak": best,
+                                   "unit": "lane-atomics/s", "frac": vps / best,
+                                   "peak_random_addresses": rnd,
+                                   "note": "votes cast / vote-kernel time vs the conflict-free "
+                                           "atomicOr micro-benchmark (hough_microbench_smem mode 0)"}
+
+    # HBM roofline of the accumulator sweeps, on the fine grid (512 MiB > L2)
+    fine = synth.WORKLOADS["finegrid"]
+    x, y, layer = [torch.from_numpy(a).to(dev) for a in synth.generate_event(fine.event, 0)[:3]]
+    hf = hough.Hough(fine.grid, len(x), fine.cap_peaks, fine.cap_hits, device=local_rank)
+    hf.vote(x, y, layer)
+    st = torch.cuda.current_stream()
+
+    def timed(fn, n=10):
+        fn()
+        ts = []
+        for _ in range(n):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            fn()
+            e1.record(st)
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.mean(ts)) * 1e-3
+
+    nbytes = fine.grid.n_bins * 4
+    t_sweep = timed(hf.peak_sweep)
+    t_clear = timed(hf.clear)
+    hf.close()
+    hbm = peaks_info["hbm_gbs"]
+    out["roofline_sweep"] = {
+        "kernel": "k_peak_sweep", "workload": "finegrid (512 MiB accumulator, L2 flushed)",
+        "bound": "hbm", "achieved": nbytes / t_sweep / 1e9, "peak": hbm, "unit": "GB/s",
+        "frac": nbytes / t_sweep / 1e9 / hbm, "frac_of_8TBs_nominal": nbytes / t_sweep / 8e12,
+        "traffic": None, "note": "algorithmic bytes = 4 B/bin read once; " + peaks_info["source"]}
+    out["roofline_clear"] = {
+        "kernel": "k_clear", "bound": "hbm", "achieved": nbytes / t_clear / 1e9, "peak": hbm,
+        "unit": "GB/s", "frac": nbytes / t_clear / 1e9 / hbm, "traffic": None}
+    return out
+
+
+if __name__ == "__main__":
+    main()

@@ -57,7 +57,8 @@ extern "C" {
 #define HOUGH_TRUNCATED_HITS 2u  /* n_hit_entries > cap_hits: hit_index holds the first cap_hits entries */
 
 /* hough_config.options */
-#define HOUGH_OPT_NO_CULL 1u /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
+#define HOUGH_OPT_NO_CULL 1u      /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
+#define HOUGH_OPT_STAGE_TIMING 2u /* record a CUDA event after every kernel (see hough_stage_times) */
 
 typedef struct hough_handle hough_handle; /* opaque */
 
@@ -85,10 +86,12 @@ typedef struct hough_config {
     int32_t device;                /* CUDA device ordinal */
 } hough_config;
 
-/* Counters of one event, 32 bytes, same layout on host and device. */
+/* Counters of one event, 40 bytes, same layout on host and device. */
 typedef struct hough_counts {
     uint64_t n_votes;       /* votes cast (in-range solutions over all hit x cell pairs) */
     uint64_t n_hit_entries; /* TRUE total length of the hit lists of the reported peaks */
+    uint64_t n_evals;       /* closed-form evaluations the vote kernel executed after its conservative
+                               cull (<= n * n_phi * n_d0; equal to it with HOUGH_OPT_NO_CULL) */
     uint32_t n_peaks;       /* TRUE number of peaks (may exceed cap_peaks) */
     uint32_t n_bad_hits;    /* hits with layer outside [0, n_layers): cast no vote */
     uint32_t flags;         /* HOUGH_TRUNCATED_* */
@@ -209,6 +212,17 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 
 /* Number of kernel launches enqueued by this handle since creation (for bench accounting). */
 uint64_t hough_launch_count(const hough_handle *h);
+
+/*
+ * Per-kernel device times of the LAST hough_vote + hough_peaks pair, for handles created with
+ * HOUGH_OPT_STAGE_TIMING (otherwise HOUGH_ESTATE).  Synchronises on the last recorded event.
+ * ms[s] = milliseconds of stage s (0 for a stage that did not run), s < min(cap, HOUGH_N_STAGES);
+ * returns the number of stages written or a negative error.  hough_stage_name(s) names stage s
+ * (NULL if out of range).  Meant for measurement runs: the extra event records add launch gaps.
+ */
+#define HOUGH_N_STAGES 10
+int hough_stage_times(hough_handle *h, float *ms, int cap);
+const char *hough_stage_name(int stage);
 
 const char *hough_strerror(int code);
 

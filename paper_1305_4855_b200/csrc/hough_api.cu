@@ -315,6 +315,15 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
         return HOUGH_ECUDA;
     }
     h->n_sms = prop.multiProcessorCount;
+    if (cfg->options & HOUGH_OPT_STAGE_TIMING) {
+        for (int s = 0; s < HOUGH_N_STAGES + 2; ++s)
+            if (cudaEventCreate(&h->ev[s]) != cudaSuccess) {
+                cudaGetLastError();
+                hough_destroy(h);
+                return HOUGH_ECUDA;
+            }
+        h->timing = 1;
+    }
     carve_workspace(cfg, (unsigned char *)workspace, h);
 
     // A1: bin centres in fp64, one rounding to fp32
@@ -390,6 +399,10 @@ void hough_destroy(hough_handle *h)
 {
     if (!h)
         return;
+    if (h->timing)
+        for (int s = 0; s < HOUGH_N_STAGES + 2; ++s)
+            if (h->ev[s])
+                cudaEventDestroy(h->ev[s]);
     free(h->radii);
     delete h;
 }
@@ -414,9 +427,14 @@ int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *l
         return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     h->n_hits = n;
+    if (h->timing)
+        memset(h->ev_set, 0, sizeof(h->ev_set));
+    stage_mark(h, 0, st);
     CK(cudaMemsetAsync(h->counters, 0, 64, st));
     CK(launch_prep(h, x, y, layer, n, st));
+    stage_mark(h, ST_PREP + 1, st);
     CK(launch_vote(h, st));
+    stage_mark(h, ST_VOTE + 1, st);
     h->voted = 1;
     return HOUGH_OK;
 }
@@ -432,15 +450,23 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CK(cudaMemsetAsync((unsigned char *)h->counters + 64, 0, 192 + (size_t)2 * h->scan_blocks_max * 8, st));
     CK(launch_peak_sweep(h, st));
+    stage_mark(h, ST_PEAK_SWEEP + 1, st);
     CK(launch_scan_rows(h, st));
+    stage_mark(h, ST_SCAN_ROWS + 1, st);
     CK(launch_compact(h, out, st));
+    stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
         CK(launch_list_count(h, st));
+        stage_mark(h, ST_LIST_COUNT + 1, st);
         CK(launch_scan_lens(h, out, st));
+        stage_mark(h, ST_SCAN_LENS + 1, st);
         CK(launch_list_fill(h, out, st));
+        stage_mark(h, ST_LIST_FILL + 1, st);
         CK(launch_sort_lists(h, out, st));
+        stage_mark(h, ST_SORT_LISTS + 1, st);
     }
     CK(launch_finish_counts(h, out, with_lists, st));
+    stage_mark(h, ST_FINISH + 1, st);
     return HOUGH_OK;
 }
 
@@ -539,6 +565,47 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 }
 
 uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
+
+static const char *const k_stage_names[HOUGH_N_STAGES] = {
+    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_count", "scan_lens", "list_fill",
+    "sort_lists", "finish"};
+
+const char *hough_stage_name(int stage)
+{
+    return (stage >= 0 && stage < HOUGH_N_STAGES) ? k_stage_names[stage] : nullptr;
+}
+
+int hough_stage_times(hough_handle *h, float *ms, int cap)
+{
+    if (!h || !ms || cap < 1)
+        return HOUGH_EINVAL;
+    if (!h->timing)
+        return HOUGH_ESTATE;
+    int n = cap < HOUGH_N_STAGES ? cap : HOUGH_N_STAGES;
+    int last = -1;
+    for (int s = 0; s < HOUGH_N_STAGES + 1; ++s)
+        if (h->ev_set[s])
+            last = s;
+    if (last < 0)
+        return HOUGH_ESTATE;
+    CK(cudaEventSynchronize(h->ev[last]));
+    // a stage's time runs from the previous recorded event to its own
+    int prev = -1;
+    for (int s = 0; s < HOUGH_N_STAGES + 1; ++s) {
+        if (!h->ev_set[s])
+            continue;
+        if (prev >= 0 && s - 1 < n) {
+            float t = 0.f;
+            CK(cudaEventElapsedTime(&t, h->ev[prev], h->ev[s]));
+            ms[s - 1] = t;
+        }
+        prev = s;
+    }
+    for (int s = 0; s < n; ++s)
+        if (!h->ev_set[s + 1])
+            ms[s] = 0.f;
+    return n;
+}
 
 const char *hough_strerror(int code)
 {

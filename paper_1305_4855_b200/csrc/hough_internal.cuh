@@ -50,10 +50,17 @@ struct HitsDev {         // prepared hits, SoA, padded with non-voting entries t
 struct DevCounters {
     unsigned long long n_votes;
     unsigned long long n_hit_entries;
+    unsigned long long n_evals;
     unsigned int n_peaks;
     unsigned int n_bad_hits;
     unsigned int flags;
     unsigned int pad;
+};
+
+// stages of one event, in launch order (HOUGH_OPT_STAGE_TIMING)
+enum {
+    ST_PREP = 0, ST_VOTE, ST_PEAK_SWEEP, ST_SCAN_ROWS, ST_COMPACT, ST_LIST_COUNT, ST_SCAN_LENS,
+    ST_LIST_FILL, ST_SORT_LISTS, ST_FINISH
 };
 
 struct hough_handle {
@@ -83,7 +90,19 @@ struct hough_handle {
     uint32_t n_hits;
     int voted;
     uint64_t launches;
+    // HOUGH_OPT_STAGE_TIMING: ev[0] = start of hough_vote, ev[s + 1] = end of stage s
+    int timing;
+    cudaEvent_t ev[HOUGH_N_STAGES + 2];
+    unsigned char ev_set[HOUGH_N_STAGES + 2];
 };
+
+static inline void stage_mark(hough_handle *h, int slot, cudaStream_t st)
+{
+    if (h->timing) {
+        cudaEventRecord(h->ev[slot], st);
+        h->ev_set[slot] = 1;
+    }
+}
 
 // kernels' host launchers (each enqueues on `st`, returns cudaGetLastError())
 cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const int32_t *layer,

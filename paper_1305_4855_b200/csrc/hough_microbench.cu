@@ -46,18 +46,27 @@ int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, in
     if (mode < 0 || mode > 2 || threads < 32 || threads > 1024 || (threads & 31) || ctas_per_sm < 1 ||
         iters < 1)
         return HOUGH_EINVAL;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
-        cudaGetLastError();
-        return HOUGH_ECUDA;
-    }
-    cudaDeviceProp prop;
-    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess)
-        return HOUGH_ECUDA;
+    // Slow host queries are done once per device: the caller times this call with events on
+    // the stream, so nothing but the launch may sit between them.
+    static int cached_device = -1, cached_sms = 0;
     static uint32_t *sink = nullptr; // 4 bytes of scratch, never freed (benchmark helper only)
-    if (!sink && cudaMalloc(&sink, 4) != cudaSuccess)
-        return HOUGH_ECUDA;
-    int blocks = prop.multiProcessorCount * ctas_per_sm;
+    if (cached_device != device) {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+            cudaGetLastError();
+            return HOUGH_ECUDA;
+        }
+        if (cudaSetDevice(device) != cudaSuccess ||
+            cudaDeviceGetAttribute(&cached_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
+            return HOUGH_ECUDA;
+        if (sink)
+            cudaFree(sink);
+        sink = nullptr;
+        if (cudaMalloc(&sink, 4) != cudaSuccess)
+            return HOUGH_ECUDA;
+        cached_device = device;
+    }
+    int blocks = cached_sms * ctas_per_sm;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (mode == 0)
         k_microbench<0><<<blocks, threads, 0, st>>>(iters, sink);

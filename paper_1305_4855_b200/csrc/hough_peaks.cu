@@ -479,6 +479,7 @@ __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_p
         hough_counts r;
         r.n_votes = c->n_votes;
         r.n_hit_entries = with_lists ? c->n_hit_entries : 0ull;
+        r.n_evals = c->n_evals;
         r.n_peaks = c->n_peaks;
         r.n_bad_hits = c->n_bad_hits;
         r.flags = 0u;

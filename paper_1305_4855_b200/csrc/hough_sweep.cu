@@ -142,6 +142,7 @@ struct SweepParams {
     int no_cull;
     uint32_t *acc;            // VOTE: global accumulator
     unsigned long long *n_votes;
+    unsigned long long *n_evals;
     // hit lists
     const uint32_t *flags;    // 1 bit per bin
     const uint32_t *row_base; // [n_rows + 1]
@@ -186,7 +187,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
     ptr += 32 * 4;
-    int *nsurv_s = reinterpret_cast<int *>(ptr);
 
     // ---- which tile
     const int tp = blockIdx.x / ge.tiles_d0, td = blockIdx.x % ge.tiles_d0;
@@ -315,6 +315,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     __syncthreads();
 
     unsigned int my_votes = 0;
+    unsigned long long tile_evals = 0; // thread 0: surviving hits x owned cells
     const int row_words = PACK == 2 ? (nk >> 1) : nk;
     uint32_t *my_row = tile + (size_t)c * row_words; // VOTE
     const unsigned short *my_slots = reinterpret_cast<const unsigned short *>(tile) + (size_t)c * nk;
@@ -358,6 +359,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             total += all;
             __syncthreads();
         }
+        tile_evals += (unsigned long long)total * (unsigned)(ni * nj);
         if (tid < EVAL_UNROLL) // non-voting padding up to a multiple of the unroll factor
             surv[total + tid] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
         __syncthreads();
@@ -434,6 +436,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             my_votes += __shfl_xor_sync(0xffffffffu, my_votes, o);
         if (lane == 0 && my_votes)
             atomicAdd(p.n_votes, (unsigned long long)my_votes);
+        if (tid == 0 && tile_evals)
+            atomicAdd(p.n_evals, tile_evals);
     } else if (MODE == MODE_COUNT) {
         // ---- list lengths of this tile's reported peaks -> list_len[global rank]
         for (int cc = tid; cc < ge.cells_pad; cc += ge.threads) {
@@ -506,6 +510,7 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->no_cull = (h->cfg.options & HOUGH_OPT_NO_CULL) ? 1 : 0;
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
+    p->n_evals = &h->counters->n_evals;
     p->flags = h->flags;
     p->row_base = h->row_base;
     p->n_peaks_dev = &h->counters->n_peaks;

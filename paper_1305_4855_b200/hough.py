@@ -20,12 +20,14 @@ LIB_PATH = os.path.join(HERE, "libhough_b200.so")
 HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3, -4
 TRUNCATED_PEAKS, TRUNCATED_HITS = 1, 2
 OPT_NO_CULL = 1
+OPT_STAGE_TIMING = 2
+N_STAGES = 10
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
 SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
            "hough_accumulator", "hough_process_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
-           "hough_launch_count", "hough_strerror")
+           "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror")
 
 
 class HoughError(RuntimeError):
@@ -45,8 +47,9 @@ class Config(C.Structure):
 
 
 class Counts(C.Structure):
-    _fields_ = [("n_votes", C.c_uint64), ("n_hit_entries", C.c_uint64), ("n_peaks", C.c_uint32),
-                ("n_bad_hits", C.c_uint32), ("flags", C.c_uint32), ("reserved", C.c_uint32)]
+    _fields_ = [("n_votes", C.c_uint64), ("n_hit_entries", C.c_uint64), ("n_evals", C.c_uint64),
+                ("n_peaks", C.c_uint32), ("n_bad_hits", C.c_uint32), ("flags", C.c_uint32),
+                ("reserved", C.c_uint32)]
 
 
 class PeaksOut(C.Structure):
@@ -59,8 +62,10 @@ class HostOut(C.Structure):
                 ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
 
 
-COUNTS_DTYPE = np.dtype([("n_votes", "<u8"), ("n_hit_entries", "<u8"), ("n_peaks", "<u4"),
-                         ("n_bad_hits", "<u4"), ("flags", "<u4"), ("reserved", "<u4")])
+COUNTS_DTYPE = np.dtype([("n_votes", "<u8"), ("n_hit_entries", "<u8"), ("n_evals", "<u8"),
+                         ("n_peaks", "<u4"), ("n_bad_hits", "<u4"), ("flags", "<u4"),
+                         ("reserved", "<u4")])
+COUNTS_WORDS = COUNTS_DTYPE.itemsize // 8  # int64 words of one hough_counts block
 
 
 def _load():
@@ -99,6 +104,10 @@ def _load():
     lib.hough_query.argtypes = [C.c_void_p] + [C.POINTER(C.c_int32)] * 6
     lib.hough_launch_count.restype = C.c_uint64
     lib.hough_launch_count.argtypes = [C.c_void_p]
+    lib.hough_stage_times.restype = C.c_int
+    lib.hough_stage_times.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int]
+    lib.hough_stage_name.restype = C.c_char_p
+    lib.hough_stage_name.argtypes = [C.c_int]
     lib.hough_strerror.restype = C.c_char_p
     lib.hough_strerror.argtypes = [C.c_int]
     return lib
@@ -164,7 +173,7 @@ class Hough:
         self.peak_mask = torch.empty(self.cap_peaks, **i32)
         self.hit_offset = torch.empty(self.cap_peaks + 1, dtype=torch.int64, device=self.device)
         self.hit_index = torch.empty(self.cap_hits, **i32)
-        self.counts = torch.zeros(4, dtype=torch.int64, device=self.device)  # 32 bytes
+        self.counts = torch.zeros(COUNTS_WORDS, dtype=torch.int64, device=self.device)
         self._out = PeaksOut(self.peak_bin.data_ptr(), self.peak_mask.data_ptr(),
                              self.hit_offset.data_ptr(), self.hit_index.data_ptr(),
                              self.counts.data_ptr())
@@ -193,10 +202,18 @@ class Hough:
         _check(_lib.hough_vote(self._h, C.c_void_p(x.data_ptr()), C.c_void_p(y.data_ptr()),
                                C.c_void_p(layer.data_ptr()), n, _stream_ptr(stream)), "hough_vote")
 
-    def peaks(self, stream=None, lists=True):
-        """hough_peaks (or hough_peaks_only): results land in this object's device arrays."""
+    def peaks(self, stream=None, lists=True, counts_out=None):
+        """hough_peaks (or hough_peaks_only): results land in this object's device arrays.
+        counts_out: optional int64 CUDA tensor of COUNTS_WORDS words that receives this
+        event's hough_counts instead of self.counts (lets a batch keep every event's counters)."""
         f = _lib.hough_peaks if lists else _lib.hough_peaks_only
-        _check(f(self._h, C.byref(self._out), _stream_ptr(stream)), "hough_peaks")
+        out = self._out
+        if counts_out is not None:
+            assert counts_out.is_cuda and counts_out.dtype == torch.int64
+            assert counts_out.numel() == COUNTS_WORDS and counts_out.is_contiguous()
+            out = PeaksOut(self._out.bin, self._out.mask, self._out.hit_offset, self._out.hit_index,
+                           counts_out.data_ptr())
+        _check(f(self._h, C.byref(out), _stream_ptr(stream)), "hough_peaks")
 
     def clear(self, stream=None):
         _check(_lib.hough_clear(self._h, _stream_ptr(stream)), "hough_clear")
@@ -229,7 +246,7 @@ class Hough:
                 mask=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
                 hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, **pin),
                 hit_index=torch.empty(self.cap_hits, dtype=torch.int32, **pin),
-                counts=torch.zeros(4, dtype=torch.int64, **pin))
+                counts=torch.zeros(COUNTS_WORDS, dtype=torch.int64, **pin))
         hb = self._host
         host = HostOut(hb["bin"].data_ptr(), hb["mask"].data_ptr(), hb["hit_offset"].data_ptr(),
                        hb["hit_index"].data_ptr() if want_lists else None, hb["counts"].data_ptr())
@@ -245,6 +262,7 @@ class Hough:
         n_rep = min(int(cnt["n_peaks"]), self.cap_peaks)
         n_ent = min(int(cnt["n_hit_entries"]), self.cap_hits)
         out = {"n_votes": int(cnt["n_votes"]), "n_hit_entries": int(cnt["n_hit_entries"]),
+               "n_evals": int(cnt["n_evals"]),
                "n_peaks": int(cnt["n_peaks"]), "n_bad_hits": int(cnt["n_bad_hits"]),
                "flags": int(cnt["flags"]),
                "peak_bin": b[:n_rep].view(np.uint32), "peak_mask": m[:n_rep].view(np.uint32),
@@ -280,6 +298,14 @@ class Hough:
 
     def launch_count(self) -> int:
         return int(_lib.hough_launch_count(self._h))
+
+    def stage_times(self) -> dict:
+        """hough_stage_times: {stage name: ms} of the last vote + peaks (needs OPT_STAGE_TIMING)."""
+        ms = (C.c_float * N_STAGES)()
+        n = _lib.hough_stage_times(self._h, ms, N_STAGES)
+        if n < 0:
+            _check(n, "hough_stage_times")
+        return {_lib.hough_stage_name(s).decode(): float(ms[s]) for s in range(n)}
 
 
 def microbench_smem(mode, threads=1024, ctas_per_sm=2, iters=4096, device=0, reps=5):
