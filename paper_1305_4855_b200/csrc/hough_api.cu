@@ -256,27 +256,24 @@ static int choose_geometry(hough_handle *h)
                 return 0;
         }
     }
-    // peak sweep
+    // peak sweep: JW warps x 2 rows per CTA (2 of them halo rows), Li phi0 planes per CTA
     {
-        int Tj = env_int("HOUGH_PEAK_TJ", 14);
-        if (Tj > c.n_d0)
-            Tj = c.n_d0;
+        int JW = env_int("HOUGH_PEAK_JW", 12);
+        int need = (c.n_d0 + 2 + 1) / 2; // warps that cover every row plus the two halo rows
+        if (JW > need)
+            JW = need;
+        if (JW < 2)
+            JW = 2;
+        if (JW > 12)
+            JW = 12; // PEAK_MAX_JW
         int Li = env_int("HOUGH_PEAK_LI", 16);
         if (Li > c.n_phi)
             Li = c.n_phi;
-        for (;;) {
-            size_t smem = (size_t)9 * (Tj + 2) * (nk / 4 + 2) * 4;
-            if (smem <= (size_t)200 * 1024 || Tj == 1) {
-                h->pk_smem = (int)smem;
-                break;
-            }
-            Tj = Tj > 2 ? Tj / 2 : 1;
-        }
-        if (h->pk_smem > 227 * 1024)
-            return 0;
-        h->pk_Tj = Tj;
+        if (Li < 1)
+            Li = 1;
+        h->pk_JW = JW;
         h->pk_Li = Li;
-        h->pk_threads = env_int("HOUGH_PEAK_THREADS", 512);
+        h->pk_smem = 2 * (2 * JW) * 32 * 16;
     }
     return 1;
 }

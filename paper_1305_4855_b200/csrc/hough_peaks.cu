@@ -35,142 +35,197 @@ cudaError_t launch_clear(hough_handle *h, cudaStream_t st)
 }
 
 // ------------------------------------------------------------------ peak sweep
-// A CTA owns Tj d0 rows (plus one halo row on each side) and walks Li phi0 planes with a
-// ring of three planes of byte popcounts in shared memory:
-//   pc[r][w]  popcounts of 4 consecutive kappa bins packed in one word
-//   m3[r][w]  max over kappa-1, kappa, kappa+1 of pc
-//   bx[r][w]  max over the 3x3 (d0, kappa) box = max of m3 over r-1, r, r+1
-// Missing neighbours (grid edges) are zero popcounts, which can never beat a bin with
-// popcount >= L_min >= 1.
+// Register-resident streaming stencil.
+//   * popcounts travel as u16x2 pairs (two bins per register) so that the 3-way maxima are
+//     single VIMNMX3.U16x2 instructions;
+//   * a lane owns 8 consecutive kappa bins of a row (two 16-byte loads, four pair
+//     registers), a warp 256 bins, a thread PEAK_RJ consecutive d0 rows; the CTA owns
+//     PEAK_RJ*JW rows (first and last are halo rows) x 256 bins and walks Li phi0 planes
+//     (+1 halo plane on each side);
+//   * kappa neighbours come from the neighbouring lanes (two shuffles per row), d0
+//     neighbours of the thread's outer rows through a double-buffered shared-memory
+//     exchange (one barrier per plane), phi0 neighbours from the thread's own state;
+//   * the raw masks of plane p+1 are loaded into registers before plane p is processed.
+// With  m3 = max over kappa+-1 of pc,  bx = max over d0+-1 of m3  (the 3x3 box of a plane):
+//   lower-lin neighbours of (i,j,k): box(i-1,j,k), m3(i,j-1,k), pc(i,j,k-1)    -> need pc >  them
+//   higher-lin neighbours          : box(i+1,j,k), m3(i,j+1,k), pc(i,j,k+1)    -> need pc >= them
+// (with phi wrap, plane i-1 of i = 0 is plane n_phi-1, which has HIGHER lin, and plane i+1
+// of i = n_phi-1 is plane 0, which has LOWER lin).  "a > b" on pairs of small numbers is
+// bit 15 / 31 of (a | 0x80008000) - b - 0x00010001, "a >= b" the same without the last term.
+#define PEAK_RJ 2
+#define PEAK_MAX_JW 12
+
 struct PeakParams {
     const uint32_t *acc;
-    uint32_t *flags;
+    unsigned char *flags; // 1 bit per bin, byte q of a row = bins 8q .. 8q+7
     int n_phi, n_d0, nk, L_min, wrap;
-    int Tj, Li;
+    int JW, Li;
 };
 
-__device__ __forceinline__ uint32_t pack_popc(uint4 m)
+__device__ __forceinline__ uint32_t popc_pair(uint32_t a, uint32_t b)
 {
-    return (uint32_t)__popc(m.x) | ((uint32_t)__popc(m.y) << 8) | ((uint32_t)__popc(m.z) << 16) |
-           ((uint32_t)__popc(m.w) << 24);
+    return (uint32_t)__popc(a) | ((uint32_t)__popc(b) << 16);
 }
 
-__global__ void __launch_bounds__(512) k_peak_sweep(const PeakParams p)
+__global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakParams p)
 {
-    extern __shared__ __align__(16) uint32_t sm[];
-    const int WPR = p.nk >> 2;  // byte words per row
-    const int RS = WPR + 2;     // row stride with one zero pad word on each side
-    const int R = p.Tj + 2;
-    const int plane_words = R * RS;
-    uint32_t *pc = sm;                        // [3][R][RS]
-    uint32_t *m3 = sm + 3 * plane_words;      // [3][R][RS]
-    uint32_t *bx = sm + 6 * plane_words;      // [3][R][RS]
-    const int tid = threadIdx.x, nthr = blockDim.x;
-    const int j0 = blockIdx.x * p.Tj;
-    const int ia = blockIdx.y * p.Li, ib = min(ia + p.Li, p.n_phi);
-    const int fw_per_row = p.nk >> 5;
-    const uint32_t lmin4 = (uint32_t)p.L_min * 0x01010101u;
+    extern __shared__ uint4 ex[]; // [2][rows][32] : m3 of every row of the current plane
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rows = PEAK_RJ * p.JW, Tj = rows - 2;
+    const int k0 = blockIdx.x * 256 + lane * 8;
+    const bool kact = k0 < p.nk;
+    const int jfirst = blockIdx.y * Tj - 1;
+    const int ia = blockIdx.z * p.Li, ib = min(ia + p.Li, p.n_phi);
+    const bool edgeL = (lane == 0) && (k0 > 0);
+    const bool edgeR = (lane == 31) && (k0 + 8 < p.nk);
+    const uint32_t HB = 0x80008000u, ONE = 0x00010001u;
+    const uint32_t lmin2 = (uint32_t)p.L_min * ONE;
 
-    for (int w = tid; w < 9 * plane_words; w += nthr)
-        sm[w] = 0u;
-    __syncthreads();
+    int jr[PEAK_RJ];
+    bool rex[PEAK_RJ], rout[PEAK_RJ];
+#pragma unroll
+    for (int t = 0; t < PEAK_RJ; ++t) {
+        int r = warp * PEAK_RJ + t;
+        jr[t] = jfirst + r;
+        rex[t] = kact && jr[t] >= 0 && jr[t] < p.n_d0;
+        rout[t] = rex[t] && r >= 1 && r <= rows - 2;
+    }
 
-    // planes ia-1 .. ib ; plane index q = gi - (ia - 1)
-    for (int gi = ia - 1; gi <= ib; ++gi) {
-        const int q = gi - (ia - 1);
-        const int slot = q % 3;
-        int src = gi;
-        bool exists = true;
-        if (gi < 0) {
+    uint4 na[PEAK_RJ], nb[PEAK_RJ]; // raw masks of the next plane
+    uint32_t ne[PEAK_RJ];           // and the one bin beyond the warp's segment (lanes 0 / 31)
+    auto load_plane = [&](int pl) {
+        int src = pl;
+        bool there = true;
+        if (pl < 0) {
             src = p.n_phi - 1;
-            exists = p.wrap != 0;
-        } else if (gi >= p.n_phi) {
+            there = p.wrap != 0;
+        } else if (pl >= p.n_phi) {
             src = 0;
-            exists = p.wrap != 0;
+            there = p.wrap != 0;
         }
-        uint32_t *pcs = pc + slot * plane_words;
-        uint32_t *m3s = m3 + slot * plane_words;
-        uint32_t *bxs = bx + slot * plane_words;
-        // A: load masks, popcount, pack
-        for (int idx = tid; idx < R * WPR; idx += nthr) {
-            int r = idx / WPR, w = idx - r * WPR;
-            int j = j0 - 1 + r;
-            uint32_t v = 0u;
-            if (exists && j >= 0 && j < p.n_d0) {
-                const uint4 *rowp =
-                    reinterpret_cast<const uint4 *>(p.acc + ((size_t)src * p.n_d0 + j) * p.nk);
-                v = pack_popc(__ldg(rowp + w));
+#pragma unroll
+        for (int t = 0; t < PEAK_RJ; ++t) {
+            na[t] = make_uint4(0u, 0u, 0u, 0u);
+            nb[t] = na[t];
+            ne[t] = 0u;
+            if (there && rex[t]) {
+                const uint32_t *rp = p.acc + ((size_t)src * p.n_d0 + jr[t]) * p.nk + k0;
+                na[t] = __ldg(reinterpret_cast<const uint4 *>(rp));
+                nb[t] = __ldg(reinterpret_cast<const uint4 *>(rp) + 1);
+                if (edgeL)
+                    ne[t] = __ldg(rp - 1);
+                if (edgeR)
+                    ne[t] = __ldg(rp + 8);
             }
-            pcs[r * RS + 1 + w] = v;
+        }
+    };
+
+    // state of the previous plane (the one whose flags are still open)
+    uint32_t s_or[PEAK_RJ][4], s_v[PEAK_RJ][4], s_bx[PEAK_RJ][4];
+#pragma unroll
+    for (int t = 0; t < PEAK_RJ; ++t)
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            s_or[t][q] = s_v[t][q] = s_bx[t][q] = 0u;
+
+    load_plane(ia - 1);
+    for (int pl = ia - 1; pl <= ib; ++pl) {
+        uint4 ca[PEAK_RJ], cb[PEAK_RJ];
+        uint32_t ce[PEAK_RJ];
+#pragma unroll
+        for (int t = 0; t < PEAK_RJ; ++t) {
+            ca[t] = na[t];
+            cb[t] = nb[t];
+            ce[t] = ne[t];
+        }
+        if (pl < ib)
+            load_plane(pl + 1);
+
+        // ---- phase A: pair popcounts, kappa shifts, m3; publish m3 of every row
+        uint32_t c[PEAK_RJ][4], s[PEAK_RJ][5], m3[PEAK_RJ][4];
+        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * 32;
+#pragma unroll
+        for (int t = 0; t < PEAK_RJ; ++t) {
+            c[t][0] = popc_pair(ca[t].x, ca[t].y);
+            c[t][1] = popc_pair(ca[t].z, ca[t].w);
+            c[t][2] = popc_pair(cb[t].x, cb[t].y);
+            c[t][3] = popc_pair(cb[t].z, cb[t].w);
+            uint32_t pe = (uint32_t)__popc(ce[t]);
+            uint32_t pv = __shfl_up_sync(0xffffffffu, c[t][3], 1);
+            uint32_t nx = __shfl_down_sync(0xffffffffu, c[t][0], 1);
+            if (lane == 0)
+                pv = pe << 16;
+            if (lane == 31)
+                nx = pe;
+            s[t][0] = __funnelshift_r(pv, c[t][0], 16);      // bins (k0-1, k0)
+            s[t][1] = __funnelshift_r(c[t][0], c[t][1], 16); // bins (k0+1, k0+2)
+            s[t][2] = __funnelshift_r(c[t][1], c[t][2], 16);
+            s[t][3] = __funnelshift_r(c[t][2], c[t][3], 16);
+            s[t][4] = __funnelshift_r(c[t][3], nx, 16);      // bins (k0+7, k0+8)
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                m3[t][q] = __vimax3_u16x2(c[t][q], s[t][q], s[t][q + 1]);
+            exw[(warp * PEAK_RJ + t) * 32 + lane] = make_uint4(m3[t][0], m3[t][1], m3[t][2], m3[t][3]);
         }
         __syncthreads();
-        // B: max over kappa +-1
-        for (int idx = tid; idx < R * WPR; idx += nthr) {
-            int r = idx / WPR, w = idx - r * WPR;
-            const uint32_t *row = pcs + r * RS + 1 + w;
-            uint32_t cur = row[0], prev = row[-1], next = row[1];
-            uint32_t left = (cur << 8) | (prev >> 24);
-            uint32_t right = (cur >> 8) | (next << 24);
-            m3s[r * RS + 1 + w] = __vmaxu4(cur, __vmaxu4(left, right));
-        }
-        __syncthreads();
-        // C: max over d0 +-1 (interior rows only)
-        for (int idx = tid; idx < p.Tj * WPR; idx += nthr) {
-            int r = idx / WPR + 1, w = idx - (r - 1) * WPR;
-            const uint32_t *c = m3s + r * RS + 1 + w;
-            bxs[r * RS + 1 + w] = __vmaxu4(c[0], __vmaxu4(c[-RS], c[RS]));
-        }
-        __syncthreads();
-        // OUT: plane gi-1 is now complete (needs planes gi-2, gi-1, gi)
-        if (q >= 2) {
-            const int io = gi - 1;
-            const int smid = (q - 1) % 3, sprev = (q - 2) % 3, snext = slot;
-            const uint32_t *pcm = pc + smid * plane_words;
-            const uint32_t *m3m = m3 + smid * plane_words;
-            const uint32_t *bxp = bx + sprev * plane_words;
-            const uint32_t *bxn = bx + snext * plane_words;
-            // With phi wrap, plane -1 of i = 0 is plane n_phi-1 (higher lin: ties lose to
-            // us) and plane +1 of i = n_phi-1 is plane 0 (lower lin: ties win over us).
-            const bool prev_is_high = (io == 0) && p.wrap;
-            const bool next_is_low = (io == p.n_phi - 1) && p.wrap;
-            const int items = p.Tj * WPR;
-            const int items_pad = (items + 31) & ~31;
-            for (int idx = tid; idx < items_pad; idx += nthr) {
-                uint32_t nib = 0u;
-                int r = 0, w = 0;
-                bool ok = idx < items;
-                if (ok) {
-                    r = idx / WPR + 1;
-                    w = idx - (r - 1) * WPR;
-                    int o = r * RS + 1 + w;
-                    uint32_t cur = pcm[o], prev = pcm[o - 1], next = pcm[o + 1];
-                    uint32_t left = (cur << 8) | (prev >> 24);
-                    uint32_t right = (cur >> 8) | (next << 24);
-                    uint32_t lo = __vmaxu4(left, m3m[o - RS]);
-                    uint32_t hi = __vmaxu4(right, m3m[o + RS]);
-                    uint32_t bp = bxp[o], bn = bxn[o];
-                    if (prev_is_high)
-                        hi = __vmaxu4(hi, bp);
-                    else
-                        lo = __vmaxu4(lo, bp);
-                    if (next_is_low)
-                        lo = __vmaxu4(lo, bn);
-                    else
-                        hi = __vmaxu4(hi, bn);
-                    uint32_t m = __vcmpgtu4(cur, lo) & __vcmpgeu4(cur, hi) & __vcmpgeu4(cur, lmin4);
-                    nib = (((m & 0x01010101u) * 0x01020408u) >> 24) & 0xfu;
+
+        // ---- phase B: box maxima, close plane pl-1, open plane pl
+        const bool out_prev = (pl - 1 >= ia);            // plane pl-1 is one of ours
+        const bool open_cur = (pl >= ia) && (pl < ib);   // plane pl is one of ours
+        const uint32_t d_next = ((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u; // next plane has lower lin
+        const uint32_t d_prev = ((pl == 0) && p.wrap) ? 0u : ONE;               // previous plane has higher lin
+#pragma unroll
+        for (int t = 0; t < PEAK_RJ; ++t) {
+            const int r = warp * PEAK_RJ + t;
+            uint32_t dn[4], up[4];
+            if (t > 0) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    dn[q] = m3[t - 1][q];
+            } else {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (r > 0)
+                    v = exw[(r - 1) * 32 + lane];
+                dn[0] = v.x, dn[1] = v.y, dn[2] = v.z, dn[3] = v.w;
+            }
+            if (t < PEAK_RJ - 1) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    up[q] = m3[t + 1][q];
+            } else {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (r < rows - 1)
+                    v = exw[(r + 1) * 32 + lane];
+                up[0] = v.x, up[1] = v.y, up[2] = v.z, up[3] = v.w;
+            }
+            uint32_t bx[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                bx[q] = __vimax3_u16x2(dn[q], m3[t][q], up[q]);
+            if (out_prev && rout[t]) {
+                uint32_t bits = 0u;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    uint32_t g = (s_or[t][q] - bx[q] - d_next) & s_v[t][q] & HB;
+                    bits |= g >> (15 - 2 * q); // bin 2q -> bit 2q, bin 2q+1 -> bit 16+2q
                 }
-                uint32_t bits = nib << ((idx & 7) << 2);
-                bits |= __shfl_xor_sync(0xffffffffu, bits, 1);
-                bits |= __shfl_xor_sync(0xffffffffu, bits, 2);
-                bits |= __shfl_xor_sync(0xffffffffu, bits, 4);
-                int j = j0 + r - 1;
-                if (ok && (idx & 7) == 0 && j < p.n_d0)
-                    p.flags[((size_t)io * p.n_d0 + j) * fw_per_row + (w >> 3)] = bits;
+                bits = (bits | (bits >> 15)) & 0xffu;
+                p.flags[(((size_t)(pl - 1) * p.n_d0 + jr[t]) * p.nk + k0) >> 3] = (unsigned char)bits;
             }
+            if (open_cur) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    uint32_t o = c[t][q] | HB;
+                    uint32_t lo = __vmaxu2(dn[q], s[t][q]);
+                    uint32_t hi = __vimax3_u16x2(up[q], s[t][q + 1], lmin2);
+                    s_v[t][q] = (o - lo - ONE) & (o - hi) & (o - s_bx[t][q] - d_prev);
+                    s_or[t][q] = o;
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                s_bx[t][q] = bx[q];
         }
-        // the slot written next (q+1) % 3 == (q-2) % 3 was last read by OUT above
-        __syncthreads();
     }
 }
 
@@ -178,24 +233,17 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
 {
     PeakParams p;
     p.acc = h->acc;
-    p.flags = h->flags;
+    p.flags = reinterpret_cast<unsigned char *>(h->flags);
     p.n_phi = h->g.n_phi;
     p.n_d0 = h->g.n_d0;
     p.nk = h->g.n_kappa;
     p.L_min = h->g.L_min;
     p.wrap = h->g.phi_wrap;
-    p.Tj = h->pk_Tj;
+    p.JW = h->pk_JW;
     p.Li = h->pk_Li;
-    dim3 grid((h->g.n_d0 + p.Tj - 1) / p.Tj, (h->g.n_phi + p.Li - 1) / p.Li);
-    static int configured = -1;
-    if (configured < h->pk_smem) {
-        cudaError_t e =
-            cudaFuncSetAttribute(k_peak_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, h->pk_smem);
-        if (e != cudaSuccess)
-            return e;
-        configured = h->pk_smem;
-    }
-    k_peak_sweep<<<grid, h->pk_threads, h->pk_smem, st>>>(p);
+    const int Tj = PEAK_RJ * p.JW - 2;
+    dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
+    k_peak_sweep<<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }
