@@ -258,7 +258,7 @@ static int choose_geometry(hough_handle *h)
     }
     // peak sweep: JW warps x 2 rows per CTA (2 of them halo rows), Li phi0 planes per CTA
     {
-        int JW = env_int("HOUGH_PEAK_JW", 12);
+        int JW = env_int("HOUGH_PEAK_JW", 8);
         int need = (c.n_d0 + 2 + 1) / 2; // warps that cover every row plus the two halo rows
         if (JW > need)
             JW = need;

@@ -67,7 +67,13 @@ __device__ __forceinline__ uint32_t popc_pair(uint32_t a, uint32_t b)
     return (uint32_t)__popc(a) | ((uint32_t)__popc(b) << 16);
 }
 
-__global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakParams p)
+struct PeakRaw { // raw masks of one plane for the thread's rows
+    uint4 a[PEAK_RJ], b[PEAK_RJ];
+    uint32_t e[PEAK_RJ]; // the one bin beyond the warp's 256-bin segment (lanes 0 and 31)
+};
+
+template <int MAXJW>
+__global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p)
 {
     extern __shared__ uint4 ex[]; // [2][rows][32] : m3 of every row of the current plane
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -76,81 +82,78 @@ __global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakPa
     const bool kact = k0 < p.nk;
     const int jfirst = blockIdx.y * Tj - 1;
     const int ia = blockIdx.z * p.Li, ib = min(ia + p.Li, p.n_phi);
-    const bool edgeL = (lane == 0) && (k0 > 0);
-    const bool edgeR = (lane == 31) && (k0 + 8 < p.nk);
     const uint32_t HB = 0x80008000u, ONE = 0x00010001u;
     const uint32_t lmin2 = (uint32_t)p.L_min * ONE;
+    const uint32_t plane_stride = (uint32_t)p.n_d0 * (uint32_t)p.nk;
 
-    int jr[PEAK_RJ];
-    bool rex[PEAK_RJ], rout[PEAK_RJ];
+    // Rows or lanes outside the grid load a clamped (valid) address and are masked to zero.
+    uint32_t roff[PEAK_RJ], rmask[PEAK_RJ], fbyte[PEAK_RJ];
+    bool rout[PEAK_RJ];
 #pragma unroll
     for (int t = 0; t < PEAK_RJ; ++t) {
-        int r = warp * PEAK_RJ + t;
-        jr[t] = jfirst + r;
-        rex[t] = kact && jr[t] >= 0 && jr[t] < p.n_d0;
-        rout[t] = rex[t] && r >= 1 && r <= rows - 2;
+        const int r = warp * PEAK_RJ + t, j = jfirst + r;
+        const bool there = kact && j >= 0 && j < p.n_d0;
+        const int jc = min(max(j, 0), p.n_d0 - 1);
+        roff[t] = (uint32_t)jc * (uint32_t)p.nk + (uint32_t)(kact ? k0 : 0);
+        rmask[t] = there ? 0xffffffffu : 0u;
+        rout[t] = there && r >= 1 && r <= rows - 2;
+        fbyte[t] = roff[t] >> 3;
     }
+    const bool e_left = (lane == 0) && (k0 > 0);
+    const bool e_right = (lane == 31) && (k0 + 8 < p.nk);
+    const bool e_any = e_left || e_right;
+    const int e_off = e_left ? -1 : 8;
+    const unsigned char *fb = p.flags;
 
-    uint4 na[PEAK_RJ], nb[PEAK_RJ]; // raw masks of the next plane
-    uint32_t ne[PEAK_RJ];           // and the one bin beyond the warp's segment (lanes 0 / 31)
-    auto load_plane = [&](int pl) {
-        int src = pl;
-        bool there = true;
-        if (pl < 0) {
-            src = p.n_phi - 1;
-            there = p.wrap != 0;
-        } else if (pl >= p.n_phi) {
-            src = 0;
-            there = p.wrap != 0;
-        }
+    auto load_plane = [&](int pl, PeakRaw &R) {
+        const int src = pl < 0 ? p.n_phi - 1 : (pl >= p.n_phi ? 0 : pl);
+        const uint32_t *pb = p.acc + (size_t)src * plane_stride;
 #pragma unroll
         for (int t = 0; t < PEAK_RJ; ++t) {
-            na[t] = make_uint4(0u, 0u, 0u, 0u);
-            nb[t] = na[t];
-            ne[t] = 0u;
-            if (there && rex[t]) {
-                const uint32_t *rp = p.acc + ((size_t)src * p.n_d0 + jr[t]) * p.nk + k0;
-                na[t] = __ldg(reinterpret_cast<const uint4 *>(rp));
-                nb[t] = __ldg(reinterpret_cast<const uint4 *>(rp) + 1);
-                if (edgeL)
-                    ne[t] = __ldg(rp - 1);
-                if (edgeR)
-                    ne[t] = __ldg(rp + 8);
-            }
+            const uint32_t *rp = pb + roff[t];
+            R.a[t] = __ldg(reinterpret_cast<const uint4 *>(rp));
+            R.b[t] = __ldg(reinterpret_cast<const uint4 *>(rp) + 1);
+            R.e[t] = 0u;
+            if (e_any)
+                R.e[t] = __ldg(rp + e_off);
         }
     };
 
-    // state of the previous plane (the one whose flags are still open)
-    uint32_t s_or[PEAK_RJ][4], s_v[PEAK_RJ][4], s_bx[PEAK_RJ][4];
+    // state of the open plane (the previous one): o = pc | HB, thr = what pc must reach
+    // as far as known, bxp = box maxima of the previous plane
+    uint32_t s_o[PEAK_RJ][4], s_thr[PEAK_RJ][4], s_bx[PEAK_RJ][4];
 #pragma unroll
     for (int t = 0; t < PEAK_RJ; ++t)
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            s_or[t][q] = s_v[t][q] = s_bx[t][q] = 0u;
-
-    load_plane(ia - 1);
-    for (int pl = ia - 1; pl <= ib; ++pl) {
-        uint4 ca[PEAK_RJ], cb[PEAK_RJ];
-        uint32_t ce[PEAK_RJ];
-#pragma unroll
-        for (int t = 0; t < PEAK_RJ; ++t) {
-            ca[t] = na[t];
-            cb[t] = nb[t];
-            ce[t] = ne[t];
+        for (int q = 0; q < 4; ++q) {
+            s_o[t][q] = 0u;
+            s_thr[t][q] = 0x7fff7fffu;
+            s_bx[t][q] = 0u;
         }
+
+    auto step = [&](int pl, const PeakRaw &C, PeakRaw &N) {
+        if (pl > ib)
+            return;
         if (pl < ib)
-            load_plane(pl + 1);
+            load_plane(pl + 1, N);
+        const uint32_t pmask = ((pl < 0 || pl >= p.n_phi) && !p.wrap) ? 0u : 0xffffffffu;
+        const bool out_prev = (pl - 1 >= ia);          // plane pl-1 is one of ours: close it
+        const bool open_cur = (pl >= ia) && (pl < ib); // plane pl is one of ours: open it
+        // strictness of the comparison with the neighbouring planes (phi wrap changes lin order)
+        const uint32_t d_next = ((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u;
+        const uint32_t d_prev = ((pl == 0) && p.wrap) ? 0u : ONE;
+        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * 32;
 
         // ---- phase A: pair popcounts, kappa shifts, m3; publish m3 of every row
         uint32_t c[PEAK_RJ][4], s[PEAK_RJ][5], m3[PEAK_RJ][4];
-        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * 32;
 #pragma unroll
         for (int t = 0; t < PEAK_RJ; ++t) {
-            c[t][0] = popc_pair(ca[t].x, ca[t].y);
-            c[t][1] = popc_pair(ca[t].z, ca[t].w);
-            c[t][2] = popc_pair(cb[t].x, cb[t].y);
-            c[t][3] = popc_pair(cb[t].z, cb[t].w);
-            uint32_t pe = (uint32_t)__popc(ce[t]);
+            const uint32_t m = rmask[t] & pmask;
+            c[t][0] = popc_pair(C.a[t].x, C.a[t].y) & m;
+            c[t][1] = popc_pair(C.a[t].z, C.a[t].w) & m;
+            c[t][2] = popc_pair(C.b[t].x, C.b[t].y) & m;
+            c[t][3] = popc_pair(C.b[t].z, C.b[t].w) & m;
+            const uint32_t pe = (uint32_t)__popc(C.e[t]) & m;
             uint32_t pv = __shfl_up_sync(0xffffffffu, c[t][3], 1);
             uint32_t nx = __shfl_down_sync(0xffffffffu, c[t][0], 1);
             if (lane == 0)
@@ -169,11 +172,7 @@ __global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakPa
         }
         __syncthreads();
 
-        // ---- phase B: box maxima, close plane pl-1, open plane pl
-        const bool out_prev = (pl - 1 >= ia);            // plane pl-1 is one of ours
-        const bool open_cur = (pl >= ia) && (pl < ib);   // plane pl is one of ours
-        const uint32_t d_next = ((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u; // next plane has lower lin
-        const uint32_t d_prev = ((pl == 0) && p.wrap) ? 0u : ONE;               // previous plane has higher lin
+        // ---- phase B: box maxima; close plane pl-1; open plane pl
 #pragma unroll
         for (int t = 0; t < PEAK_RJ; ++t) {
             const int r = warp * PEAK_RJ + t;
@@ -183,9 +182,7 @@ __global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakPa
                 for (int q = 0; q < 4; ++q)
                     dn[q] = m3[t - 1][q];
             } else {
-                uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                if (r > 0)
-                    v = exw[(r - 1) * 32 + lane];
+                const uint4 v = exw[max(r - 1, 0) * 32 + lane]; // r = 0 is a halo row: never output
                 dn[0] = v.x, dn[1] = v.y, dn[2] = v.z, dn[3] = v.w;
             }
             if (t < PEAK_RJ - 1) {
@@ -193,9 +190,7 @@ __global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakPa
                 for (int q = 0; q < 4; ++q)
                     up[q] = m3[t + 1][q];
             } else {
-                uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                if (r < rows - 1)
-                    v = exw[(r + 1) * 32 + lane];
+                const uint4 v = exw[min(r + 1, rows - 1) * 32 + lane];
                 up[0] = v.x, up[1] = v.y, up[2] = v.z, up[3] = v.w;
             }
             uint32_t bx[4];
@@ -206,26 +201,34 @@ __global__ void __launch_bounds__(32 * PEAK_MAX_JW, 2) k_peak_sweep(const PeakPa
                 uint32_t bits = 0u;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    uint32_t g = (s_or[t][q] - bx[q] - d_next) & s_v[t][q] & HB;
-                    bits |= g >> (15 - 2 * q); // bin 2q -> bit 2q, bin 2q+1 -> bit 16+2q
+                    const uint32_t thr = __vmaxu2(s_thr[t][q], bx[q] + d_next);
+                    const uint32_t g = (s_o[t][q] - thr) >> (15 - 2 * q); // bin 2q -> bit 2q, 2q+1 -> bit 16+2q
+                    bits |= g & (ONE << (2 * q));
                 }
                 bits = (bits | (bits >> 15)) & 0xffu;
-                p.flags[(((size_t)(pl - 1) * p.n_d0 + jr[t]) * p.nk + k0) >> 3] = (unsigned char)bits;
+                const_cast<unsigned char *>(fb)[(size_t)(pl - 1) * (plane_stride >> 3) + fbyte[t]] =
+                    (unsigned char)bits;
             }
             if (open_cur) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    uint32_t o = c[t][q] | HB;
-                    uint32_t lo = __vmaxu2(dn[q], s[t][q]);
-                    uint32_t hi = __vimax3_u16x2(up[q], s[t][q + 1], lmin2);
-                    s_v[t][q] = (o - lo - ONE) & (o - hi) & (o - s_bx[t][q] - d_prev);
-                    s_or[t][q] = o;
+                    const uint32_t lo = __vmaxu2(dn[q], s[t][q]);            // lower lin: pc must exceed
+                    const uint32_t hi = __vimax3_u16x2(up[q], s[t][q + 1], lmin2); // higher lin: pc must reach
+                    s_thr[t][q] = __vimax3_u16x2(lo + ONE, hi, s_bx[t][q] + d_prev);
+                    s_o[t][q] = c[t][q] | HB;
                 }
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 s_bx[t][q] = bx[q];
         }
+    };
+
+    PeakRaw A, B;
+    load_plane(ia - 1, A);
+    for (int pl = ia - 1; pl <= ib; pl += 2) {
+        step(pl, A, B);
+        step(pl + 1, B, A);
     }
 }
 
@@ -243,7 +246,10 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
     p.Li = h->pk_Li;
     const int Tj = PEAK_RJ * p.JW - 2;
     dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
-    k_peak_sweep<<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+    if (p.JW <= 8)
+        k_peak_sweep<8><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+    else
+        k_peak_sweep<PEAK_MAX_JW><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }
