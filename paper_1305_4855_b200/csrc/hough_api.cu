@@ -129,6 +129,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *flags = cv.take(n_bins / 8);
     void *row_base = cv.take((n_rows + 1) * 4);
     void *list_len = cv.take((size_t)c->cap_peaks * 4);
+    void *pairs = cv.take((size_t)c->cap_hits * 8);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -149,6 +150,8 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->flags = (uint32_t *)flags;
         h->row_base = (uint32_t *)row_base;
         h->list_len = (uint32_t *)list_len;
+        h->pairs = (uint2 *)pairs;
+        h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
         h->scan_status = (unsigned long long *)((unsigned char *)counters + 256);
@@ -210,36 +213,25 @@ static int choose_geometry(hough_handle *h)
         }
         while (split > 1 && 32 * groups * split > 1024)
             --split;
-        if (!sweep_geom_init(h, &h->vote_geom, P, D, split, 8 / h->g.pack, 0)) {
+        if (!sweep_geom_init(h, &h->vote_geom, P, D, split, 0)) {
             // fall back to the smallest tile
-            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 8 / h->g.pack, 0))
+            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 0))
                 return 0;
         }
     }
-    // hit lists: u16 slot per bin + a u32 cursor per possible peak of the tile
+    // hit lists: same tile as the vote by default (the tile itself is small: flag words
+    // and popcount prefixes), so the cull keeps the same efficiency
     {
-        int D = env_int("HOUGH_LIST_TILE_D0", c.n_d0 < 8 ? c.n_d0 : 8);
+        int D = env_int("HOUGH_LIST_TILE_D0", h->vote_geom.D);
         if (D > c.n_d0)
             D = c.n_d0;
-        if (D > 1 && (D & 1))
-            --D;
-        int P = env_int("HOUGH_LIST_TILE_PHI", 0);
-        if (P <= 0) {
-            // bytes per cell ~ 2 nk (slots) + nk/2 (cursors) + 12
-            int per_cell = 2 * nk + nk / 2 + 16;
-            int cells = (budget - staging) / per_cell;
-            P = cells / D;
-            if (P > 32)
-                P = 32;
-            if (P >= 16)
-                P = (P / 8) * 8;
-        }
+        if (D < 1)
+            D = 1;
+        int P = env_int("HOUGH_LIST_TILE_PHI", h->vote_geom.P);
         if (P < 1)
             P = 1;
         if (P > c.n_phi)
             P = c.n_phi;
-        if (P > 1 && (P & 1))
-            --P;
         int groups = (P * D + 31) / 32;
         int split = env_int("HOUGH_LIST_SPLIT", 0);
         if (split <= 0) {
@@ -251,8 +243,8 @@ static int choose_geometry(hough_handle *h)
         }
         while (split > 1 && 32 * groups * split > 1024)
             --split;
-        if (!sweep_geom_init(h, &h->list_geom, P, D, split, 4, 1)) {
-            if (!sweep_geom_init(h, &h->list_geom, 1, 1, 4, 4, 1))
+        if (!sweep_geom_init(h, &h->list_geom, P, D, split, 1)) {
+            if (!sweep_geom_init(h, &h->list_geom, 1, 1, 4, 1))
                 return 0;
         }
     }
@@ -453,12 +445,13 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
-        CK(launch_list_count(h, st));
-        stage_mark(h, ST_LIST_COUNT + 1, st);
+        CK(cudaMemsetAsync(h->list_len, 0, (size_t)h->cfg.cap_peaks * 4, st));
+        CK(launch_list_sweep(h, st));
+        stage_mark(h, ST_LIST_SWEEP + 1, st);
         CK(launch_scan_lens(h, out, st));
         stage_mark(h, ST_SCAN_LENS + 1, st);
-        CK(launch_list_fill(h, out, st));
-        stage_mark(h, ST_LIST_FILL + 1, st);
+        CK(launch_place_lists(h, out, st));
+        stage_mark(h, ST_PLACE_LISTS + 1, st);
         CK(launch_sort_lists(h, out, st));
         stage_mark(h, ST_SORT_LISTS + 1, st);
     }
@@ -564,7 +557,7 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
 
 static const char *const k_stage_names[HOUGH_N_STAGES] = {
-    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_count", "scan_lens", "list_fill",
+    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "scan_lens", "place_lists",
     "sort_lists", "finish"};
 
 const char *hough_stage_name(int stage)

@@ -483,6 +483,120 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------ hit-list placement (a7)
+// The list sweep left list_len[p] = length of peak p's list and n_pairs (peak, hit) pairs in
+// no particular order; after the scan of list_len the pairs are dropped into their lists
+// (the position inside a list is handed out by counting list_len back down), then
+// k_sort_lists orders each list.  If the pair buffer (cap_hits pairs) overflowed, the
+// output is truncated anyway (n_hit_entries > cap_hits) and k_list_fill_slow recomputes
+// the lists that still fit directly from the hits, one warp per peak.
+__global__ void __launch_bounds__(256) k_scatter_pairs(const unsigned long long *__restrict__ n_pairs,
+                                                       unsigned long long pair_cap,
+                                                       const uint2 *__restrict__ pairs,
+                                                       uint32_t *__restrict__ list_len,
+                                                       const unsigned long long *__restrict__ hit_offset,
+                                                       uint32_t *__restrict__ hit_index,
+                                                       unsigned long long cap_hits)
+{
+    const unsigned long long n = *n_pairs;
+    if (n > pair_cap)
+        return; // k_list_fill_slow takes over
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint2 pr = pairs[i];
+        const uint32_t idx = atomicSub(&list_len[pr.x], 1u) - 1u;
+        const unsigned long long pos = hit_offset[pr.x] + idx;
+        if (pos < cap_hits)
+            hit_index[pos] = pr.y;
+    }
+}
+
+struct SlowFillParams {
+    GridDev g;
+    const float *hx, *hy, *hr2;
+    const uint32_t *hbit;
+    uint32_t n_hits;
+    const unsigned long long *n_pairs;
+    unsigned long long pair_cap;
+    const DevCounters *counters;
+    uint32_t cap_peaks;
+    const uint32_t *bin;
+    const unsigned long long *hit_offset;
+    uint32_t *hit_index;
+    unsigned long long cap_hits;
+};
+
+__global__ void __launch_bounds__(256) k_list_fill_slow(const SlowFillParams p)
+{
+    if (*p.n_pairs <= p.pair_cap)
+        return;
+    const GridDev &g = p.g;
+    const int lane = threadIdx.x & 31;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
+    for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
+        unsigned long long pos = p.hit_offset[pk];
+        if (pos >= p.cap_hits)
+            continue;
+        const uint32_t lin = p.bin[pk];
+        const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
+        const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
+        const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
+        for (uint32_t base = 0; base < p.n_hits; base += 32) {
+            const uint32_t hidx = base + lane;
+            bool in = false;
+            if (hidx < p.n_hits && p.hbit[hidx] != 0u) {
+                // DESIGN.md section 2, A3 + A4 (same recipe as the sweeps)
+                float a = __fmul_rn(p.hx[hidx], sn);
+                float b = __fmul_rn(p.hy[hidx], cs);
+                float s = __fsub_rn(b, a);
+                float e = __fsub_rn(s, d0c);
+                float num = __fadd_rn(e, e);
+                float t = __fmul_rn(twod0, s);
+                float u = __fsub_rn(p.hr2[hidx], t);
+                float den = __fadd_rn(u, d0sq);
+                float kappa = __fdiv_rn(num, den);
+                if ((kappa >= g.klo) && (kappa < g.khi)) {
+                    float qf = __fmul_rn(__fsub_rn(kappa, g.klo), g.inv_dk);
+                    in = (uint32_t)min(__float2int_rz(qf), g.n_kappa - 1) == k;
+                }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, in);
+            if (in) {
+                unsigned long long q = pos + __popc(bal & ((1u << lane) - 1u));
+                if (q < p.cap_hits)
+                    p.hit_index[q] = hidx;
+            }
+            pos += __popc(bal);
+        }
+    }
+}
+
+cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    const unsigned long long *off = reinterpret_cast<const unsigned long long *>(out->hit_offset);
+    k_scatter_pairs<<<h->n_sms * 8, 256, 0, st>>>(h->n_pairs, h->cfg.cap_hits, h->pairs, h->list_len, off,
+                                                  out->hit_index, h->cfg.cap_hits);
+    SlowFillParams p;
+    p.g = h->g;
+    p.hx = h->hx;
+    p.hy = h->hy;
+    p.hr2 = h->hr2;
+    p.hbit = h->hbit;
+    p.n_hits = h->n_hits;
+    p.n_pairs = h->n_pairs;
+    p.pair_cap = h->cfg.cap_hits;
+    p.counters = h->counters;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.bin = out->bin;
+    p.hit_offset = off;
+    p.hit_index = out->hit_index;
+    p.cap_hits = h->cfg.cap_hits;
+    k_list_fill_slow<<<h->n_sms * 4, 256, 0, st>>>(p);
+    h->launches += 2;
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------ list order (a7)
 // The fill pass appends with a shared-memory cursor, so a list is complete but in the
 // order the warps happened to run.  One thread per peak sorts its (short) list.

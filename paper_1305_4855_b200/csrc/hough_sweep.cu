@@ -1,16 +1,19 @@
 // hough_sweep.cu -- the tiled sweep of the hits over the (phi0, d0) cells:
 //   MODE_VOTE  : a3 vote into a shared-memory tile with atomicOr, a4 coalesced write-out,
 //                a8 vote count
-//   MODE_COUNT : a7 pass 1, length of each reported peak's hit list
-//   MODE_FILL  : a7 pass 2, the hit indices themselves
-// All three share the staging (TMA 1-D bulk copies of the SoA hit arrays into shared
+//   MODE_LIST  : a7, one sweep that counts every reported peak's hit list (list_len) and
+//                emits its (peak rank, hit index) pairs; k_scatter_pairs (hough_peaks.cu)
+//                places them once the CSR offsets are known
+// Both share the staging (TMA 1-D bulk copies of the SoA hit arrays into shared
 // memory, double buffered), the conservative per-tile hit cull and the exact fp32
 // evaluation of BASELINE.json north_star's closed form.
 #include "hough_internal.cuh"
 
 #define MODE_VOTE 0
-#define MODE_COUNT 1
-#define MODE_FILL 2
+#define MODE_LIST 1
+
+#define PAIR_BUF 2048   // (peak, hit) pairs buffered per CTA between flushes
+#define PAIR_FLUSH 1024 // flush at the end of a chunk once this many are waiting
 
 #define EVAL_UNROLL 2
 
@@ -55,11 +58,10 @@ __device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t
 }
 
 // ------------------------------------------------------------------ the exact evaluation
-// DESIGN.md section 2, A3 + A4: every operation is one binary32 round-to-nearest
-// operation, in this order, never contracted.  Returns the kappa bin or -1.
-__device__ __forceinline__ int eval_bin(float x, float y, float r2, float sn, float cs, float d0c,
-                                        float twod0, float d0sq, float klo, float khi, float inv_dk,
-                                        int nk_minus_1)
+// DESIGN.md section 2, A3: every operation is one binary32 round-to-nearest operation, in
+// this order, never contracted.
+__device__ __forceinline__ float eval_kappa(float x, float y, float r2, float sn, float cs, float d0c,
+                                            float twod0, float d0sq)
 {
     float a = __fmul_rn(x, sn);
     float b = __fmul_rn(y, cs);
@@ -69,12 +71,23 @@ __device__ __forceinline__ int eval_bin(float x, float y, float r2, float sn, fl
     float t = __fmul_rn(twod0, s);
     float u = __fsub_rn(r2, t);
     float den = __fadd_rn(u, d0sq);
-    float kappa = __fdiv_rn(num, den);
-    if (!((kappa >= klo) && (kappa < khi)))
-        return -1;
+    return __fdiv_rn(num, den);
+}
+// A4: the kappa bin of an in-range kappa (truncation, top clamp).
+__device__ __forceinline__ int kappa_bin(float kappa, float klo, float inv_dk, int nk_minus_1)
+{
     float qf = __fmul_rn(__fsub_rn(kappa, klo), inv_dk);
-    int k = __float2int_rz(qf);
-    return min(k, nk_minus_1);
+    return min(__float2int_rz(qf), nk_minus_1);
+}
+__device__ __forceinline__ void smem_red_or(uint32_t addr, uint32_t v)
+{
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t smem_ld(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
 }
 
 // ------------------------------------------------------------------ conservative tile cull
@@ -137,22 +150,20 @@ struct SweepParams {
     GridDev g;
     HitsDev hits;
     SweepGeom geom;
-    int swz_mask;             // XOR swizzle of the word index inside a cell row (vote tile)
-    int slot_swz;             // same for the u16 slot tile of the hit-list passes
+    int swz_mask; // XOR swizzle of the word index inside a cell row (vote tile)
     int no_cull;
-    uint32_t *acc;            // VOTE: global accumulator
+    uint32_t *acc; // VOTE: global accumulator
     unsigned long long *n_votes;
     unsigned long long *n_evals;
-    // hit lists
+    // hit lists (MODE_LIST)
     const uint32_t *flags;    // 1 bit per bin
     const uint32_t *row_base; // [n_rows + 1]
     const unsigned int *n_peaks_dev;
     uint32_t cap_peaks;
-    uint32_t *list_len;       // COUNT out
-    const unsigned long long *hit_offset; // FILL in
-    uint32_t *hit_index;      // FILL out
-    unsigned long long cap_hits;
-    int max_tile_peaks;
+    uint32_t *list_len; // [cap_peaks], zeroed before the sweep
+    uint2 *pairs;       // [pair_cap] (peak rank, hit index)
+    unsigned long long *n_pairs;
+    unsigned long long pair_cap;
 };
 
 template <int MODE, int PACK>
@@ -164,20 +175,17 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const int nk = g.n_kappa;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nwarps = ge.threads >> 5;
+    const int wpr = nk >> 5; // flag words per cell row
 
     // ---- carve shared memory
+    // VOTE: tile = masks [cells_pad][nk / PACK words];
+    // LIST: tile = flag words [wpr][cells_pad] followed by their exclusive popcount prefix
     uint32_t *tile = reinterpret_cast<uint32_t *>(smem_raw);
     unsigned char *ptr = smem_raw + (size_t)ge.tile_words * 4;
-    uint32_t *pk_cnt = nullptr, *cell_lbase = nullptr, *cell_gbase = nullptr, *cell_nrep = nullptr;
-    if (MODE != MODE_VOTE) {
-        pk_cnt = reinterpret_cast<uint32_t *>(ptr);
-        ptr += (size_t)((p.max_tile_peaks + 3) & ~3) * 4;
-        cell_lbase = reinterpret_cast<uint32_t *>(ptr);
-        ptr += (size_t)ge.cells_pad * 4;
-        cell_gbase = reinterpret_cast<uint32_t *>(ptr);
-        ptr += (size_t)ge.cells_pad * 4;
-        cell_nrep = reinterpret_cast<uint32_t *>(ptr);
-        ptr += (size_t)ge.cells_pad * 4;
+    uint2 *pairbuf = nullptr;
+    if (MODE == MODE_LIST) {
+        pairbuf = reinterpret_cast<uint2 *>(ptr);
+        ptr += (size_t)PAIR_BUF * 8;
     }
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
     ptr += (size_t)2 * 4 * ge.chunk * 4;
@@ -187,6 +195,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
     ptr += 32 * 4;
+    unsigned int *s_npairs = reinterpret_cast<unsigned int *>(ptr); // [0] count, [1..2] flush base
+    ptr += 16;
 
     // ---- which tile
     const int tp = blockIdx.x / ge.tiles_d0, td = blockIdx.x % ge.tiles_d0;
@@ -206,7 +216,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         c_2d0 = g.twod0[j0 + jl];
         c_d0sq = g.d0sq[j0 + jl];
     }
-    const int swz = lane & p.swz_mask, sswz = lane & p.slot_swz;
+    const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
 
     TileCull tc;
     tc.snA = g.sn[i0];
@@ -225,6 +235,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         mbar_init(&mbar[0], 1);
         mbar_init(&mbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s_npairs[0] = 0u;
     }
     __syncthreads();
     auto issue = [&](uint32_t ch) {
@@ -240,86 +251,53 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     if (tid == 0 && n_chunks > 0)
         issue(0);
 
-    // ---- clear the tile (a2, shared-memory part)
-    for (int w = tid; w < ge.tile_words; w += ge.threads)
-        tile[w] = 0u;
-
-    uint32_t n_rep = 0;
-    if (MODE != MODE_VOTE) {
-        // Local peak ids of the reported peaks (global rank < n_rep) inside this tile.
-        n_rep = min(*p.n_peaks_dev, p.cap_peaks);
+    uint32_t c_gbase = 0u; // LIST: global rank of the first peak of this thread's cell
+    if (MODE == MODE_VOTE) {
+        // ---- clear the tile (a2, shared-memory part)
+        for (int w = tid; w < ge.tile_words; w += ge.threads)
+            tile[w] = 0u;
+    } else {
+        // ---- flag words of the reported peaks of every cell of the tile, and the number of
+        // reported peaks below each word (peaks of global rank >= n_rep are not reported)
+        const uint32_t n_rep = min(*p.n_peaks_dev, p.cap_peaks);
+        uint32_t *ftile = tile, *ptile = tile + (size_t)wpr * ge.cells_pad;
         for (int cc = tid; cc < ge.cells_pad; cc += ge.threads) {
-            int cil = cc / ge.D, cjl = cc - cil * ge.D;
+            const int cil = cc / ge.D, cjl = cc - cil * ge.D;
             uint32_t gb = 0, nr = 0;
+            const uint32_t *fw = p.flags;
             if (cil < ni && cjl < nj) {
                 size_t row = (size_t)(i0 + cil) * g.n_d0 + (j0 + cjl);
                 gb = p.row_base[row];
                 uint32_t cnt = p.row_base[row + 1] - gb;
                 nr = gb >= n_rep ? 0u : min(cnt, n_rep - gb);
+                fw += row * wpr;
             }
-            cell_gbase[cc] = gb;
-            cell_nrep[cc] = nr;
-        }
-        for (int w = tid; w < p.max_tile_peaks; w += ge.threads)
-            pk_cnt[w] = 0u;
-        __syncthreads();
-        if (warp == 0) { // exclusive scan of cell_nrep over the tile's cells
-            uint32_t carry = 0;
-            for (int base = 0; base < ge.cells_pad; base += 32) {
-                uint32_t v = cell_nrep[base + lane], incl = v;
-                for (int o = 1; o < 32; o <<= 1) {
-                    uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o)
-                        incl += t;
-                }
-                cell_lbase[base + lane] = carry + incl - v;
-                carry += __shfl_sync(0xffffffffu, incl, 31);
+            uint32_t before = 0;
+            for (int w = 0; w < wpr; ++w) {
+                uint32_t f = nr ? fw[w] : 0u;
+                while (before + (uint32_t)__popc(f) > nr) // the capacity cuts inside this word
+                    f &= ~(0x80000000u >> __clz(f));
+                ftile[(size_t)w * ge.cells_pad + cc] = f;
+                ptile[(size_t)w * ge.cells_pad + cc] = before;
+                before += (uint32_t)__popc(f);
             }
         }
-        __syncthreads();
-        // slot[(cell, k)] = local peak id + 1 for reported peaks (u16), 0 otherwise
-        unsigned short *slot = reinterpret_cast<unsigned short *>(tile);
-        const int words_per_row = nk >> 5;
-        for (int cc = warp; cc < ge.cells_pad; cc += nwarps) {
-            uint32_t nr = cell_nrep[cc];
-            if (nr == 0)
-                continue;
-            int cil = cc / ge.D, cjl = cc - cil * ge.D;
-            size_t row = (size_t)(i0 + cil) * g.n_d0 + (j0 + cjl);
-            const uint32_t *fw = p.flags + row * words_per_row;
-            uint32_t rank0 = 0;
-            const int cswz = (cc & 31) & p.slot_swz;
-            for (int wb = 0; wb < words_per_row; wb += 32) {
-                uint32_t f = (wb + lane < words_per_row) ? fw[wb + lane] : 0u;
-                uint32_t pc = __popc(f), incl = pc;
-                for (int o = 1; o < 32; o <<= 1) {
-                    uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o)
-                        incl += t;
-                }
-                uint32_t rank = rank0 + incl - pc;
-                while (f) {
-                    int b = __ffs(f) - 1;
-                    f &= f - 1;
-                    if (rank < nr) {
-                        int k = ((wb + lane) << 5) + b;
-                        int ks = (((k >> 1) ^ cswz) << 1) | (k & 1);
-                        slot[(size_t)cc * nk + ks] = (unsigned short)(cell_lbase[cc] + rank + 1);
-                    }
-                    ++rank;
-                }
-                rank0 += __shfl_sync(0xffffffffu, incl, 31);
-            }
-        }
+        if (cell_ok)
+            c_gbase = p.row_base[(size_t)(i0 + il) * g.n_d0 + (j0 + jl)];
     }
     __syncthreads();
 
     unsigned int my_votes = 0;
     unsigned long long tile_evals = 0; // thread 0: surviving hits x owned cells
-    const int row_words = PACK == 2 ? (nk >> 1) : nk;
-    uint32_t *my_row = tile + (size_t)c * row_words; // VOTE
-    const unsigned short *my_slots = reinterpret_cast<const unsigned short *>(tile) + (size_t)c * nk;
     const int nkm1 = nk - 1;
+    // VOTE: byte address of this cell's row in the tile and its word swizzle (in bytes)
+    const int row_words = PACK == 2 ? (nk >> 1) : nk;
+    const uint32_t row_addr = smem_u32(tile) + (uint32_t)c * (uint32_t)row_words * 4u;
+    const uint32_t swzb = (uint32_t)(lane & p.swz_mask) << 2;
+    // LIST: byte address of this cell's column in the flag tile; the prefix tile follows
+    const uint32_t col_addr = smem_u32(tile) + (uint32_t)c * 4u;
+    const uint32_t word_stride = (uint32_t)ge.cells_pad * 4u;
+    const uint32_t prefix_off = (uint32_t)wpr * word_stride;
 
     for (uint32_t ch = 0; ch < n_chunks; ++ch) {
         const float *st = stage + (size_t)(ch & 1) * 4 * ge.chunk;
@@ -368,28 +346,32 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         for (int hs = set * EVAL_UNROLL; hs < total; hs += ge.split * EVAL_UNROLL) {
 #pragma unroll
             for (int u = 0; u < EVAL_UNROLL; ++u) {
-                float4 hv = surv[hs + u];
-                int k = eval_bin(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq, g.klo, g.khi,
-                                 g.inv_dk, nkm1);
-                if (k >= 0) {
+                const float4 hv = surv[hs + u];
+                const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+                if ((kappa >= klo) && (kappa < khi)) {
+                    const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
                     if (MODE == MODE_VOTE) {
-                        uint32_t bit = __float_as_uint(hv.w);
+                        const uint32_t bit = __float_as_uint(hv.w);
                         if (PACK == 2)
-                            atomicOr(&my_row[(k >> 1) ^ swz], bit << ((k & 1) << 4));
+                            smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
                         else
-                            atomicOr(&my_row[k ^ swz], bit);
+                            smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
                         ++my_votes;
                     } else {
-                        int ks = (((k >> 1) ^ sswz) << 1) | (k & 1);
-                        uint32_t sl = my_slots[ks];
-                        if (sl) {
-                            uint32_t lid = sl - 1;
-                            uint32_t idx = atomicAdd(&pk_cnt[lid], 1u);
-                            if (MODE == MODE_FILL) {
-                                uint32_t gp = cell_gbase[c] + (lid - cell_lbase[c]);
-                                unsigned long long pos = p.hit_offset[gp] + idx;
-                                if (pos < p.cap_hits)
-                                    p.hit_index[pos] = __float_as_uint(hv.w);
+                        const uint32_t wa = col_addr + (k >> 5) * word_stride;
+                        const uint32_t f = smem_ld(wa);
+                        if ((f >> (k & 31u)) & 1u) {
+                            const uint32_t rank = smem_ld(wa + prefix_off) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
+                            const uint32_t gp = c_gbase + rank;
+                            atomicAdd(&p.list_len[gp], 1u);
+                            const uint2 pr = make_uint2(gp, __float_as_uint(hv.w));
+                            const unsigned int pos = atomicAdd(&s_npairs[0], 1u);
+                            if (pos < PAIR_BUF) {
+                                pairbuf[pos] = pr;
+                            } else { // buffer full inside one chunk: straight to global memory
+                                unsigned long long gpos = atomicAdd(p.n_pairs, 1ull);
+                                if (gpos < p.pair_cap)
+                                    p.pairs[gpos] = pr;
                             }
                         }
                     }
@@ -397,6 +379,26 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             }
         }
         __syncthreads(); // survivors and this stage buffer are free again
+
+        if (MODE == MODE_LIST) {
+            const unsigned int np = min(s_npairs[0], (unsigned int)PAIR_BUF);
+            if (np >= PAIR_FLUSH || (ch + 1 == n_chunks && np > 0)) {
+                if (tid == 0) {
+                    unsigned long long b = atomicAdd(p.n_pairs, (unsigned long long)np);
+                    s_npairs[1] = (unsigned int)b;
+                    s_npairs[2] = (unsigned int)(b >> 32);
+                }
+                __syncthreads();
+                const unsigned long long b = ((unsigned long long)s_npairs[2] << 32) | s_npairs[1];
+                for (unsigned int q = tid; q < np; q += ge.threads)
+                    if (b + q < p.pair_cap)
+                        p.pairs[b + q] = pairbuf[q];
+                __syncthreads();
+                if (tid == 0)
+                    s_npairs[0] = 0u;
+                // the next write to s_npairs[0] / pairbuf is behind the barriers of the next cull
+            }
+        }
     }
 
     if (MODE == MODE_VOTE) {
@@ -438,13 +440,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             atomicAdd(p.n_votes, (unsigned long long)my_votes);
         if (tid == 0 && tile_evals)
             atomicAdd(p.n_evals, tile_evals);
-    } else if (MODE == MODE_COUNT) {
-        // ---- list lengths of this tile's reported peaks -> list_len[global rank]
-        for (int cc = tid; cc < ge.cells_pad; cc += ge.threads) {
-            uint32_t nr = cell_nrep[cc], lb = cell_lbase[cc], gb = cell_gbase[cc];
-            for (uint32_t r = 0; r < nr; ++r)
-                p.list_len[gb + r] = pk_cnt[lb + r];
-        }
     }
 }
 
@@ -459,10 +454,10 @@ static int swizzle_mask_for(int row_words)
     return m;
 }
 
-// bytes_per_bin_x2: twice the shared-memory bytes per bin of the tile (VOTE pack 2 -> 4,
-// pack 1 -> 8; slots -> 4).
-int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int bytes_per_bin_x2,
-                    int list_mode)
+// Tile geometry.  Vote tile: cells_pad rows of n_kappa masks, PACK masks per word.
+// List tile: the flag words and their popcount prefixes (2 words per 32 bins per cell)
+// plus the pair buffer.
+int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int list_mode)
 {
     const hough_config &cfg = h->cfg;
     ge->P = P;
@@ -475,21 +470,22 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     ge->tiles_phi = (cfg.n_phi + P - 1) / P;
     ge->tiles_d0 = (cfg.n_d0 + D - 1) / D;
     ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
-    size_t tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * bytes_per_bin_x2 / 2;
-    ge->tile_words = (int)(tile_bytes / 4);
-    size_t extra = 0;
+    size_t tile_bytes, extra = 0;
     if (list_mode) {
-        size_t maxpk = (size_t)((P + 1) / 2) * ((D + 1) / 2) * (cfg.n_kappa / 2);
-        extra = ((maxpk + 3) & ~(size_t)3) * 4 + (size_t)ge->cells_pad * 12;
+        tile_bytes = (size_t)2 * (cfg.n_kappa / 32) * ge->cells_pad * 4;
+        extra = (size_t)PAIR_BUF * 8;
+    } else {
+        tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * 4 / h->g.pack;
     }
-    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16;
+    ge->tile_words = (int)(tile_bytes / 4);
+    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);
     // the interval test needs the slab to span well under a quarter turn
     double span = (cfg.phi_max - cfg.phi_min) * (double)(P - 1) / (double)cfg.n_phi;
     ge->no_phi_cull = (span > 1.0) ? 1 : 0;
     if (ge->threads > 1024 || ge->threads < 32)
         return 0;
-    if (ge->smem_bytes > hough_vote_max_smem())
+    if (tile_bytes + extra + stage > (size_t)hough_vote_max_smem())
         return 0;
     return 1;
 }
@@ -506,7 +502,6 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->geom = ge;
     int row_words = h->g.pack == 2 ? h->g.n_kappa / 2 : h->g.n_kappa;
     p->swz_mask = swizzle_mask_for(row_words);
-    p->slot_swz = swizzle_mask_for(h->g.n_kappa / 2);
     p->no_cull = (h->cfg.options & HOUGH_OPT_NO_CULL) ? 1 : 0;
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
@@ -516,10 +511,9 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->n_peaks_dev = &h->counters->n_peaks;
     p->cap_peaks = h->cfg.cap_peaks;
     p->list_len = h->list_len;
-    p->hit_offset = nullptr;
-    p->hit_index = nullptr;
-    p->cap_hits = h->cfg.cap_hits;
-    p->max_tile_peaks = ((ge.P + 1) / 2) * ((ge.D + 1) / 2) * (h->g.n_kappa / 2);
+    p->pairs = h->pairs;
+    p->n_pairs = h->n_pairs;
+    p->pair_cap = h->cfg.cap_hits;
 }
 
 template <int MODE, int PACK>
@@ -545,20 +539,11 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     return h->g.pack == 2 ? launch_one<MODE_VOTE, 2>(p, st) : launch_one<MODE_VOTE, 1>(p, st);
 }
 
-cudaError_t launch_list_count(hough_handle *h, cudaStream_t st)
+// One sweep: list_len[peak] (true lengths) and the (peak, hit) pairs.
+cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
 {
     SweepParams p;
     fill_params(h, &p, h->list_geom);
     h->launches += 1;
-    return h->g.pack == 2 ? launch_one<MODE_COUNT, 2>(p, st) : launch_one<MODE_COUNT, 1>(p, st);
-}
-
-cudaError_t launch_list_fill(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
-{
-    SweepParams p;
-    fill_params(h, &p, h->list_geom);
-    p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
-    p.hit_index = out->hit_index;
-    h->launches += 1;
-    return h->g.pack == 2 ? launch_one<MODE_FILL, 2>(p, st) : launch_one<MODE_FILL, 1>(p, st);
+    return launch_one<MODE_LIST, 1>(p, st);
 }
