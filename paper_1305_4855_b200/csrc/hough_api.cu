@@ -130,6 +130,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *row_base = cv.take((n_rows + 1) * 4);
     void *list_len = cv.take((size_t)c->cap_peaks * 4);
     void *pairs = cv.take((size_t)c->cap_hits * 8);
+    void *list_tmp = cv.take((size_t)c->cap_hits * 4);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -151,6 +152,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->row_base = (uint32_t *)row_base;
         h->list_len = (uint32_t *)list_len;
         h->pairs = (uint2 *)pairs;
+        h->list_tmp = (uint32_t *)list_tmp;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
@@ -448,12 +450,12 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
         CK(cudaMemsetAsync(h->list_len, 0, (size_t)h->cfg.cap_peaks * 4, st));
         CK(launch_list_sweep(h, st));
         stage_mark(h, ST_LIST_SWEEP + 1, st);
+        CK(launch_rank_pairs(h, out, st));
+        stage_mark(h, ST_RANK_PAIRS + 1, st);
         CK(launch_scan_lens(h, out, st));
         stage_mark(h, ST_SCAN_LENS + 1, st);
         CK(launch_place_lists(h, out, st));
         stage_mark(h, ST_PLACE_LISTS + 1, st);
-        CK(launch_sort_lists(h, out, st));
-        stage_mark(h, ST_SORT_LISTS + 1, st);
     }
     CK(launch_finish_counts(h, out, with_lists, st));
     stage_mark(h, ST_FINISH + 1, st);
@@ -557,8 +559,8 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
 
 static const char *const k_stage_names[HOUGH_N_STAGES] = {
-    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "scan_lens", "place_lists",
-    "sort_lists", "finish"};
+    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "rank_pairs", "scan_lens",
+    "place_lists", "finish"};
 
 const char *hough_stage_name(int stage)
 {

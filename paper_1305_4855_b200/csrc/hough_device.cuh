@@ -1,0 +1,136 @@
+// hough_device.cuh -- device-side helpers shared by the sweep kernels (hough_sweep.cu,
+// hough_lists.cu): TMA bulk-copy / mbarrier PTX wrappers, the exact fp32 evaluation of
+// BASELINE.json north_star's closed form (A3/A4) and the conservative
+// hit cull of DESIGN.md section 4.3.
+#pragma once
+
+#include "hough_internal.cuh"
+
+// ------------------------------------------------------------------ PTX helpers (TMA)
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+// 1-D bulk copy global -> shared through the TMA unit; completion is signalled on `bar`.
+__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// ------------------------------------------------------------------ the exact evaluation
+// DESIGN.md section 2, A3: every operation is one binary32 round-to-nearest operation, in
+// this order, never contracted.
+__device__ __forceinline__ float eval_kappa(float x, float y, float r2, float sn, float cs, float d0c,
+                                            float twod0, float d0sq)
+{
+    float a = __fmul_rn(x, sn);
+    float b = __fmul_rn(y, cs);
+    float s = __fsub_rn(b, a);
+    float e = __fsub_rn(s, d0c);
+    float num = __fadd_rn(e, e); // 2*e, exact
+    float t = __fmul_rn(twod0, s);
+    float u = __fsub_rn(r2, t);
+    float den = __fadd_rn(u, d0sq);
+    return __fdiv_rn(num, den);
+}
+// A4: the kappa bin of an in-range kappa (truncation, top clamp).
+__device__ __forceinline__ int kappa_bin(float kappa, float klo, float inv_dk, int nk_minus_1)
+{
+    float qf = __fmul_rn(__fsub_rn(kappa, klo), inv_dk);
+    return min(__float2int_rz(qf), nk_minus_1);
+}
+__device__ __forceinline__ void smem_red_or(uint32_t addr, uint32_t v)
+{
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t smem_ld(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// ------------------------------------------------------------------ conservative tile cull
+// Can this hit cast a vote anywhere in the tile (phi0 centres between A and B, d0 centres
+// in [dlo, dhi])?  Interval arithmetic on  2|e| <= K (e^2 + c^2),  e = s - d0,
+// c^2 = r^2 - s^2, with slack that dominates every fp32 rounding of the exact recipe
+// (DESIGN.md section 4.3).  May say yes too often, never no wrongly; any NaN says yes.
+struct TileCull {
+    float snA, csA, snB, csB;
+    float dlo, dhi;
+    int phi_all; // tile too wide in phi0: s ranges over [-r, r]
+    int off;     // culling disabled (HOUGH_OPT_NO_CULL)
+};
+
+__device__ __forceinline__ bool hit_may_vote(float x, float y, float r2, const TileCull &tc, float K,
+                                             float d0_absmax)
+{
+    if (tc.off)
+        return true;
+    const float EPS = 3.8146973e-06f; // 2^-18
+    float ax = fabsf(x), ay = fabsf(y);
+    if (!(ax <= 3.0e38f) || !(ay <= 3.0e38f))
+        return false; // inf / NaN coordinates never vote (num/den is NaN)
+    float r = sqrtf(r2);
+    float smin, smax;
+    if (tc.phi_all) {
+        smin = -r;
+        smax = r;
+    } else {
+        float sa = y * tc.csA - x * tc.snA, ca = x * tc.csA + y * tc.snA;
+        float sb = y * tc.csB - x * tc.snB, cb = x * tc.csB + y * tc.snB;
+        smin = fminf(sa, sb);
+        smax = fmaxf(sa, sb);
+        if (ca * cb <= 0.0f) { // s(phi0) has its extremum +-r inside the slab
+            if (sa + sb >= 0.0f)
+                smax = fmaxf(smax, r);
+            else
+                smin = fminf(smin, -r);
+        }
+    }
+    float es = EPS * (ax + ay + d0_absmax) + 1e-30f;
+    smin -= es;
+    smax += es;
+    float elo = smin - tc.dhi, ehi = smax - tc.dlo;
+    float emin = (elo <= 0.0f && ehi >= 0.0f) ? 0.0f : fminf(fabsf(elo), fabsf(ehi));
+    float emax = fmaxf(fabsf(elo), fabsf(ehi));
+    float s2min = (smin <= 0.0f && smax >= 0.0f) ? 0.0f : fminf(smin * smin, smax * smax);
+    float c2max = fmaxf(r2 - s2min, 0.0f);
+    // g(e) = 2e - K e^2 is concave: its minimum over [emin, emax] is at an end point
+    float g0 = 2.0f * emin - K * emin * emin;
+    float g1 = 2.0f * emax - K * emax * emax;
+    float gmin = fminf(g0, g1);
+    float rhs = K * c2max * (1.0f + EPS) +
+                K * EPS * (r2 + 2.0f * d0_absmax * (ax + ay) + d0_absmax * d0_absmax) + 1e-30f;
+    return !(gmin > rhs);
+}
+

@@ -59,8 +59,8 @@ struct DevCounters {
 
 // stages of one event, in launch order (HOUGH_OPT_STAGE_TIMING)
 enum {
-    ST_PREP = 0, ST_VOTE, ST_PEAK_SWEEP, ST_SCAN_ROWS, ST_COMPACT, ST_LIST_SWEEP, ST_SCAN_LENS,
-    ST_PLACE_LISTS, ST_SORT_LISTS, ST_FINISH
+    ST_PREP = 0, ST_VOTE, ST_PEAK_SWEEP, ST_SCAN_ROWS, ST_COMPACT, ST_LIST_SWEEP, ST_RANK_PAIRS,
+    ST_SCAN_LENS, ST_PLACE_LISTS, ST_FINISH
 };
 
 struct hough_handle {
@@ -80,7 +80,8 @@ struct hough_handle {
     uint32_t *flags;      // 1 bit per bin
     uint32_t *row_base;   // [n_rows + 1] exclusive scan of peaks per (i, j) row
     uint32_t *list_len;   // [cap_peaks] hit-list length of each reported peak
-    uint2 *pairs;         // [cap_hits] (peak rank, hit index) pairs of the list sweep
+    uint2 *pairs;         // [cap_hits] (peak, hit index) pairs of the list sweep
+    uint32_t *list_tmp;   // [cap_hits] the lists before ordering
     unsigned long long *n_pairs; // pairs emitted (lives in the per-hough_peaks reset region)
     unsigned long long *scan_status; // look-back words of the chained scans
     unsigned int *scan_ticket;       // [4]
@@ -115,7 +116,7 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
-cudaError_t launch_sort_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_rank_pairs(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,

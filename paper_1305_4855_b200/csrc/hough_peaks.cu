@@ -5,7 +5,7 @@
 //                  one pass over the accumulator (4 B/bin read once), 1 flag bit per bin out
 //   k_scan         single-pass chained prefix sum (decoupled look-back)
 //   k_compact      flag bits -> (lin, mask) records in ascending lin
-//   k_sort_lists   puts each peak's hit list into ascending hit index
+//   k_rank_pairs, k_scatter_pairs, k_order_pairs, k_list_slow   CSR hit lists from the pairs
 //   k_finish       counters -> the caller's hough_counts
 // The peak rule is BASELINE.json north_star's ("popcount reaches at least L_min and ...
 // local maxima in the 3x3x3 neighbourhood (ties go to the lower linear index)"), restated
@@ -483,50 +483,96 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------ hit-list placement (a7)
-// The list sweep left list_len[p] = length of peak p's list and n_pairs (peak, hit) pairs in
-// no particular order; after the scan of list_len the pairs are dropped into their lists
-// (the position inside a list is handed out by counting list_len back down), then
-// k_sort_lists orders each list.  If the pair buffer (cap_hits pairs) overflowed, the
-// output is truncated anyway (n_hit_entries > cap_hits) and k_list_fill_slow recomputes
-// the lists that still fit directly from the hits, one warp per peak.
-__global__ void __launch_bounds__(256) k_scatter_pairs(const unsigned long long *__restrict__ n_pairs,
-                                                       unsigned long long pair_cap,
-                                                       const uint2 *__restrict__ pairs,
-                                                       uint32_t *__restrict__ list_len,
-                                                       const unsigned long long *__restrict__ hit_offset,
-                                                       uint32_t *__restrict__ hit_index,
-                                                       unsigned long long cap_hits)
-{
-    const unsigned long long n = *n_pairs;
-    if (n > pair_cap)
-        return; // k_list_fill_slow takes over
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint2 pr = pairs[i];
-        const uint32_t idx = atomicSub(&list_len[pr.x], 1u) - 1u;
-        const unsigned long long pos = hit_offset[pr.x] + idx;
-        if (pos < cap_hits)
-            hit_index[pos] = pr.y;
-    }
-}
-
-struct SlowFillParams {
+// ------------------------------------------------------------------ hit lists (a7)
+// The list sweep left n_pairs (lin of a reported peak bin, hit index) pairs in no particular
+// order.  Then:
+//   k_rank_pairs    lin -> global peak rank (row_base + flag bits below), list_len[rank]++
+//   k_scan<LENS>    list_len -> hit_offset (CSR), n_hit_entries
+//   k_scatter_pairs pair -> tmp[hit_offset[rank] + slot], slots handed out by counting
+//                   list_len back down: every list complete, in arbitrary order
+//   k_order_pairs   one thread per pair: its place in the ascending list is the number of
+//                   smaller entries of that list (no two entries of a list are equal)
+// If the pair buffer (cap_hits pairs) overflowed, the output is truncated anyway
+// (n_hit_entries > cap_hits); k_list_slow then recounts every list and refills the lists
+// that still fit directly from the hits, one warp per peak, ascending by construction.
+struct ListParams {
     GridDev g;
     const float *hx, *hy, *hr2;
     const uint32_t *hbit;
     uint32_t n_hits;
+    const uint32_t *flags, *row_base;
     const unsigned long long *n_pairs;
     unsigned long long pair_cap;
+    uint2 *pairs;
+    uint32_t *list_len;
     const DevCounters *counters;
     uint32_t cap_peaks;
     const uint32_t *bin;
     const unsigned long long *hit_offset;
+    uint32_t *tmp;
     uint32_t *hit_index;
     unsigned long long cap_hits;
 };
 
-__global__ void __launch_bounds__(256) k_list_fill_slow(const SlowFillParams p)
+__global__ void __launch_bounds__(256) k_rank_pairs(const ListParams p)
+{
+    const unsigned long long n = *p.n_pairs;
+    if (n > p.pair_cap)
+        return; // k_list_slow<0> recounts
+    const uint32_t nk = (uint32_t)p.g.n_kappa, wpr = nk >> 5;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint32_t lin = p.pairs[i].x;
+        const uint32_t row = lin / nk, k = lin - row * nk;
+        const uint32_t *fw = p.flags + (size_t)row * wpr;
+        uint32_t rank = p.row_base[row];
+        for (uint32_t w = 0; w < (k >> 5); ++w)
+            rank += (uint32_t)__popc(fw[w]);
+        rank += (uint32_t)__popc(fw[k >> 5] & ((1u << (k & 31u)) - 1u));
+        p.pairs[i].x = rank;
+        atomicAdd(&p.list_len[rank], 1u);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_scatter_pairs(const ListParams p)
+{
+    const unsigned long long n = *p.n_pairs;
+    if (n > p.pair_cap)
+        return;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint2 pr = p.pairs[i];
+        const uint32_t slot = atomicSub(&p.list_len[pr.x], 1u) - 1u;
+        const unsigned long long pos = p.hit_offset[pr.x] + slot;
+        if (pos < p.cap_hits)
+            p.tmp[pos] = pr.y;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_order_pairs(const ListParams p)
+{
+    const unsigned long long n = *p.n_pairs;
+    if (n > p.pair_cap)
+        return;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint2 pr = p.pairs[i];
+        const unsigned long long b = p.hit_offset[pr.x], e = p.hit_offset[pr.x + 1];
+        if (e > p.cap_hits)
+            continue; // a list cut by the capacity is not part of the valid output
+        const uint32_t *a = p.tmp + b;
+        const uint32_t len = (uint32_t)(e - b);
+        uint32_t r = 0;
+        for (uint32_t m = 0; m < len; ++m)
+            r += a[m] < pr.y;
+        p.hit_index[b + r] = pr.y;
+    }
+}
+
+// FILL = 0: list_len[pk] = true length of every reported peak's list;
+// FILL = 1: write the lists that start below cap_hits, ascending.
+template <int FILL>
+__global__ void __launch_bounds__(256) k_list_slow(const ListParams p)
 {
     if (*p.n_pairs <= p.pair_cap)
         return;
@@ -535,13 +581,14 @@ __global__ void __launch_bounds__(256) k_list_fill_slow(const SlowFillParams p)
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
     const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
     for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
-        unsigned long long pos = p.hit_offset[pk];
-        if (pos >= p.cap_hits)
+        unsigned long long pos = FILL ? p.hit_offset[pk] : 0ull;
+        if (FILL && pos >= p.cap_hits)
             continue;
         const uint32_t lin = p.bin[pk];
         const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
         const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
         const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
+        uint32_t count = 0;
         for (uint32_t base = 0; base < p.n_hits; base += 32) {
             const uint32_t hidx = base + lane;
             bool in = false;
@@ -562,80 +609,62 @@ __global__ void __launch_bounds__(256) k_list_fill_slow(const SlowFillParams p)
                 }
             }
             const unsigned bal = __ballot_sync(0xffffffffu, in);
-            if (in) {
+            if (FILL && in) {
                 unsigned long long q = pos + __popc(bal & ((1u << lane) - 1u));
                 if (q < p.cap_hits)
                     p.hit_index[q] = hidx;
             }
             pos += __popc(bal);
+            count += __popc(bal);
         }
+        if (!FILL && lane == 0)
+            p.list_len[pk] = count;
     }
 }
 
-cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+static void list_params(hough_handle *h, const hough_peaks_out *out, ListParams *p)
 {
-    const unsigned long long *off = reinterpret_cast<const unsigned long long *>(out->hit_offset);
-    k_scatter_pairs<<<h->n_sms * 8, 256, 0, st>>>(h->n_pairs, h->cfg.cap_hits, h->pairs, h->list_len, off,
-                                                  out->hit_index, h->cfg.cap_hits);
-    SlowFillParams p;
-    p.g = h->g;
-    p.hx = h->hx;
-    p.hy = h->hy;
-    p.hr2 = h->hr2;
-    p.hbit = h->hbit;
-    p.n_hits = h->n_hits;
-    p.n_pairs = h->n_pairs;
-    p.pair_cap = h->cfg.cap_hits;
-    p.counters = h->counters;
-    p.cap_peaks = h->cfg.cap_peaks;
-    p.bin = out->bin;
-    p.hit_offset = off;
-    p.hit_index = out->hit_index;
-    p.cap_hits = h->cfg.cap_hits;
-    k_list_fill_slow<<<h->n_sms * 4, 256, 0, st>>>(p);
+    p->g = h->g;
+    p->hx = h->hx;
+    p->hy = h->hy;
+    p->hr2 = h->hr2;
+    p->hbit = h->hbit;
+    p->n_hits = h->n_hits;
+    p->flags = h->flags;
+    p->row_base = h->row_base;
+    p->n_pairs = h->n_pairs;
+    p->pair_cap = h->cfg.cap_hits;
+    p->pairs = h->pairs;
+    p->list_len = h->list_len;
+    p->counters = h->counters;
+    p->cap_peaks = h->cfg.cap_peaks;
+    p->bin = out->bin;
+    p->hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
+    p->tmp = h->list_tmp;
+    p->hit_index = out->hit_index;
+    p->cap_hits = h->cfg.cap_hits;
+}
+
+// after the list sweep, before the scan of list_len
+cudaError_t launch_rank_pairs(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    ListParams p;
+    list_params(h, out, &p);
+    k_rank_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
+    k_list_slow<0><<<h->n_sms * 4, 256, 0, st>>>(p);
     h->launches += 2;
     return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------ list order (a7)
-// The fill pass appends with a shared-memory cursor, so a list is complete but in the
-// order the warps happened to run.  One thread per peak sorts its (short) list.
-__global__ void __launch_bounds__(256) k_sort_lists(const DevCounters *__restrict__ counters,
-                                                    uint32_t cap_peaks,
-                                                    const unsigned long long *__restrict__ hit_offset,
-                                                    uint32_t *__restrict__ hit_index,
-                                                    unsigned long long cap_hits)
+// after the scan of list_len
+cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
 {
-    uint32_t n = min(counters->n_peaks, cap_peaks);
-    uint32_t stride = gridDim.x * blockDim.x;
-    for (uint32_t pk = blockIdx.x * blockDim.x + threadIdx.x; pk < n; pk += stride) {
-        unsigned long long b = hit_offset[pk], e = hit_offset[pk + 1];
-        if (e > cap_hits)
-            continue; // a list cut by the capacity is not part of the valid output
-        uint32_t *a = hit_index + b;
-        int len = (int)(e - b);
-        for (int i = 1; i < len; ++i) {
-            uint32_t v = a[i];
-            int j = i - 1;
-            while (j >= 0 && a[j] > v) {
-                a[j + 1] = a[j];
-                --j;
-            }
-            a[j + 1] = v;
-        }
-    }
-}
-
-cudaError_t launch_sort_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
-{
-    uint32_t blocks = (h->cfg.cap_peaks + 255) / 256;
-    uint32_t maxb = (uint32_t)h->n_sms * 16;
-    if (blocks > maxb)
-        blocks = maxb;
-    k_sort_lists<<<blocks, 256, 0, st>>>(h->counters, h->cfg.cap_peaks,
-                                         reinterpret_cast<const unsigned long long *>(out->hit_offset),
-                                         out->hit_index, h->cfg.cap_hits);
-    h->launches += 1;
+    ListParams p;
+    list_params(h, out, &p);
+    k_scatter_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
+    k_order_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
+    k_list_slow<1><<<h->n_sms * 4, 256, 0, st>>>(p);
+    h->launches += 3;
     return cudaGetLastError();
 }
 

@@ -1,13 +1,13 @@
 // hough_sweep.cu -- the tiled sweep of the hits over the (phi0, d0) cells:
 //   MODE_VOTE  : a3 vote into a shared-memory tile with atomicOr, a4 coalesced write-out,
 //                a8 vote count
-//   MODE_LIST  : a7, one sweep that counts every reported peak's hit list (list_len) and
-//                emits its (peak rank, hit index) pairs; k_scatter_pairs (hough_peaks.cu)
-//                places them once the CSR offsets are known
+//   MODE_LIST  : a7, one sweep that emits a (peak bin, hit index) pair for every vote that
+//                lands in a reported peak; the kernels of hough_peaks.cu rank, count,
+//                place and order them
 // Both share the staging (TMA 1-D bulk copies of the SoA hit arrays into shared
 // memory, double buffered), the conservative per-tile hit cull and the exact fp32
 // evaluation of BASELINE.json north_star's closed form.
-#include "hough_internal.cuh"
+#include "hough_device.cuh"
 
 #define MODE_VOTE 0
 #define MODE_LIST 1
@@ -16,134 +16,6 @@
 #define PAIR_FLUSH 1024 // flush at the end of a chunk once this many are waiting
 
 #define EVAL_UNROLL 2
-
-// ------------------------------------------------------------------ PTX helpers (TMA)
-__device__ __forceinline__ uint32_t smem_u32(const void *p)
-{
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t done;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n"
-            : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!done);
-}
-// 1-D bulk copy global -> shared through the TMA unit; completion is signalled on `bar`.
-__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-            smem_u32(dst)),
-        "l"(src), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
-
-// ------------------------------------------------------------------ the exact evaluation
-// DESIGN.md section 2, A3: every operation is one binary32 round-to-nearest operation, in
-// this order, never contracted.
-__device__ __forceinline__ float eval_kappa(float x, float y, float r2, float sn, float cs, float d0c,
-                                            float twod0, float d0sq)
-{
-    float a = __fmul_rn(x, sn);
-    float b = __fmul_rn(y, cs);
-    float s = __fsub_rn(b, a);
-    float e = __fsub_rn(s, d0c);
-    float num = __fadd_rn(e, e); // 2*e, exact
-    float t = __fmul_rn(twod0, s);
-    float u = __fsub_rn(r2, t);
-    float den = __fadd_rn(u, d0sq);
-    return __fdiv_rn(num, den);
-}
-// A4: the kappa bin of an in-range kappa (truncation, top clamp).
-__device__ __forceinline__ int kappa_bin(float kappa, float klo, float inv_dk, int nk_minus_1)
-{
-    float qf = __fmul_rn(__fsub_rn(kappa, klo), inv_dk);
-    return min(__float2int_rz(qf), nk_minus_1);
-}
-__device__ __forceinline__ void smem_red_or(uint32_t addr, uint32_t v)
-{
-    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-}
-__device__ __forceinline__ uint32_t smem_ld(uint32_t addr)
-{
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-    return v;
-}
-
-// ------------------------------------------------------------------ conservative tile cull
-// Can this hit cast a vote anywhere in the tile (phi0 centres between A and B, d0 centres
-// in [dlo, dhi])?  Interval arithmetic on  2|e| <= K (e^2 + c^2),  e = s - d0,
-// c^2 = r^2 - s^2, with slack that dominates every fp32 rounding of the exact recipe
-// (DESIGN.md section 4.3).  May say yes too often, never no wrongly; any NaN says yes.
-struct TileCull {
-    float snA, csA, snB, csB;
-    float dlo, dhi;
-    int phi_all; // tile too wide in phi0: s ranges over [-r, r]
-    int off;     // culling disabled (HOUGH_OPT_NO_CULL)
-};
-
-__device__ __forceinline__ bool hit_may_vote(float x, float y, float r2, const TileCull &tc, float K,
-                                             float d0_absmax)
-{
-    if (tc.off)
-        return true;
-    const float EPS = 3.8146973e-06f; // 2^-18
-    float ax = fabsf(x), ay = fabsf(y);
-    if (!(ax <= 3.0e38f) || !(ay <= 3.0e38f))
-        return false; // inf / NaN coordinates never vote (num/den is NaN)
-    float r = sqrtf(r2);
-    float smin, smax;
-    if (tc.phi_all) {
-        smin = -r;
-        smax = r;
-    } else {
-        float sa = y * tc.csA - x * tc.snA, ca = x * tc.csA + y * tc.snA;
-        float sb = y * tc.csB - x * tc.snB, cb = x * tc.csB + y * tc.snB;
-        smin = fminf(sa, sb);
-        smax = fmaxf(sa, sb);
-        if (ca * cb <= 0.0f) { // s(phi0) has its extremum +-r inside the slab
-            if (sa + sb >= 0.0f)
-                smax = fmaxf(smax, r);
-            else
-                smin = fminf(smin, -r);
-        }
-    }
-    float es = EPS * (ax + ay + d0_absmax) + 1e-30f;
-    smin -= es;
-    smax += es;
-    float elo = smin - tc.dhi, ehi = smax - tc.dlo;
-    float emin = (elo <= 0.0f && ehi >= 0.0f) ? 0.0f : fminf(fabsf(elo), fabsf(ehi));
-    float emax = fmaxf(fabsf(elo), fabsf(ehi));
-    float s2min = (smin <= 0.0f && smax >= 0.0f) ? 0.0f : fminf(smin * smin, smax * smax);
-    float c2max = fmaxf(r2 - s2min, 0.0f);
-    // g(e) = 2e - K e^2 is concave: its minimum over [emin, emax] is at an end point
-    float g0 = 2.0f * emin - K * emin * emin;
-    float g1 = 2.0f * emax - K * emax * emax;
-    float gmin = fminf(g0, g1);
-    float rhs = K * c2max * (1.0f + EPS) +
-                K * EPS * (r2 + 2.0f * d0_absmax * (ax + ay) + d0_absmax * d0_absmax) + 1e-30f;
-    return !(gmin > rhs);
-}
 
 // ------------------------------------------------------------------ kernel parameters
 struct SweepParams {
@@ -160,8 +32,7 @@ struct SweepParams {
     const uint32_t *row_base; // [n_rows + 1]
     const unsigned int *n_peaks_dev;
     uint32_t cap_peaks;
-    uint32_t *list_len; // [cap_peaks], zeroed before the sweep
-    uint2 *pairs;       // [pair_cap] (peak rank, hit index)
+    uint2 *pairs;       // [pair_cap] (lin of the peak bin, hit index)
     unsigned long long *n_pairs;
     unsigned long long pair_cap;
 };
@@ -179,7 +50,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
 
     // ---- carve shared memory
     // VOTE: tile = masks [cells_pad][nk / PACK words];
-    // LIST: tile = flag words [wpr][cells_pad] followed by their exclusive popcount prefix
+    // LIST: tile = flag words of the reported peaks [wpr][cells_pad]
     uint32_t *tile = reinterpret_cast<uint32_t *>(smem_raw);
     unsigned char *ptr = smem_raw + (size_t)ge.tile_words * 4;
     uint2 *pairbuf = nullptr;
@@ -251,16 +122,17 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     if (tid == 0 && n_chunks > 0)
         issue(0);
 
-    uint32_t c_gbase = 0u; // LIST: global rank of the first peak of this thread's cell
+    // LIST: linear index of bin 0 of this thread's cell
+    const uint32_t c_lin0 = cell_ok ? (uint32_t)(((size_t)(i0 + il) * g.n_d0 + (j0 + jl)) * nk) : 0u;
     if (MODE == MODE_VOTE) {
         // ---- clear the tile (a2, shared-memory part)
         for (int w = tid; w < ge.tile_words; w += ge.threads)
             tile[w] = 0u;
     } else {
-        // ---- flag words of the reported peaks of every cell of the tile, and the number of
-        // reported peaks below each word (peaks of global rank >= n_rep are not reported)
+        // ---- flag words of the reported peaks of every cell of the tile (peaks of global
+        // rank >= n_rep are not reported)
         const uint32_t n_rep = min(*p.n_peaks_dev, p.cap_peaks);
-        uint32_t *ftile = tile, *ptile = tile + (size_t)wpr * ge.cells_pad;
+        uint32_t *ftile = tile;
         for (int cc = tid; cc < ge.cells_pad; cc += ge.threads) {
             const int cil = cc / ge.D, cjl = cc - cil * ge.D;
             uint32_t gb = 0, nr = 0;
@@ -278,12 +150,9 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 while (before + (uint32_t)__popc(f) > nr) // the capacity cuts inside this word
                     f &= ~(0x80000000u >> __clz(f));
                 ftile[(size_t)w * ge.cells_pad + cc] = f;
-                ptile[(size_t)w * ge.cells_pad + cc] = before;
                 before += (uint32_t)__popc(f);
             }
         }
-        if (cell_ok)
-            c_gbase = p.row_base[(size_t)(i0 + il) * g.n_d0 + (j0 + jl)];
     }
     __syncthreads();
 
@@ -297,7 +166,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     // LIST: byte address of this cell's column in the flag tile; the prefix tile follows
     const uint32_t col_addr = smem_u32(tile) + (uint32_t)c * 4u;
     const uint32_t word_stride = (uint32_t)ge.cells_pad * 4u;
-    const uint32_t prefix_off = (uint32_t)wpr * word_stride;
 
     for (uint32_t ch = 0; ch < n_chunks; ++ch) {
         const float *st = stage + (size_t)(ch & 1) * 4 * ge.chunk;
@@ -358,13 +226,9 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                             smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
                         ++my_votes;
                     } else {
-                        const uint32_t wa = col_addr + (k >> 5) * word_stride;
-                        const uint32_t f = smem_ld(wa);
+                        const uint32_t f = smem_ld(col_addr + (k >> 5) * word_stride);
                         if ((f >> (k & 31u)) & 1u) {
-                            const uint32_t rank = smem_ld(wa + prefix_off) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
-                            const uint32_t gp = c_gbase + rank;
-                            atomicAdd(&p.list_len[gp], 1u);
-                            const uint2 pr = make_uint2(gp, __float_as_uint(hv.w));
+                            const uint2 pr = make_uint2(c_lin0 + k, __float_as_uint(hv.w));
                             const unsigned int pos = atomicAdd(&s_npairs[0], 1u);
                             if (pos < PAIR_BUF) {
                                 pairbuf[pos] = pr;
@@ -455,8 +319,8 @@ static int swizzle_mask_for(int row_words)
 }
 
 // Tile geometry.  Vote tile: cells_pad rows of n_kappa masks, PACK masks per word.
-// List tile: the flag words and their popcount prefixes (2 words per 32 bins per cell)
-// plus the pair buffer.
+// List tile: the flag words of the reported peaks (1 word per 32 bins per cell) plus the
+// pair buffer.
 int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int list_mode)
 {
     const hough_config &cfg = h->cfg;
@@ -472,7 +336,7 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
     size_t tile_bytes, extra = 0;
     if (list_mode) {
-        tile_bytes = (size_t)2 * (cfg.n_kappa / 32) * ge->cells_pad * 4;
+        tile_bytes = (size_t)(cfg.n_kappa / 32) * ge->cells_pad * 4;
         extra = (size_t)PAIR_BUF * 8;
     } else {
         tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * 4 / h->g.pack;
@@ -510,7 +374,6 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->row_base = h->row_base;
     p->n_peaks_dev = &h->counters->n_peaks;
     p->cap_peaks = h->cfg.cap_peaks;
-    p->list_len = h->list_len;
     p->pairs = h->pairs;
     p->n_pairs = h->n_pairs;
     p->pair_cap = h->cfg.cap_hits;
@@ -539,7 +402,7 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     return h->g.pack == 2 ? launch_one<MODE_VOTE, 2>(p, st) : launch_one<MODE_VOTE, 1>(p, st);
 }
 
-// One sweep: list_len[peak] (true lengths) and the (peak, hit) pairs.
+// One sweep: the (peak bin, hit) pairs.
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
 {
     SweepParams p;
