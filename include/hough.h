@@ -220,7 +220,7 @@ uint64_t hough_launch_count(const hough_handle *h);
  * returns the number of stages written or a negative error.  hough_stage_name(s) names stage s
  * (NULL if out of range).  Meant for measurement runs: the extra event records add launch gaps.
  */
-#define HOUGH_N_STAGES 10
+#define HOUGH_N_STAGES 9
 int hough_stage_times(hough_handle *h, float *ms, int cap);
 const char *hough_stage_name(int stage);
 

@@ -115,7 +115,8 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     size_t n_rows = (size_t)c->n_phi * c->n_d0;
     uint32_t hp = pad_hits(c->max_hits);
     uint32_t sb = (uint32_t)((n_rows + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
-    uint32_t sb2 = (uint32_t)(((size_t)c->cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
+    const size_t n_sub = (size_t)c->cap_peaks * (size_t)list_segments_bound(c);
+    uint32_t sb2 = (uint32_t)((n_sub + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
     if (sb2 > sb)
         sb = sb2;
     sb += 1;
@@ -128,9 +129,10 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *rx = cv.take((size_t)hp * 4), *ry = cv.take((size_t)hp * 4), *rl = cv.take((size_t)hp * 4);
     void *flags = cv.take(n_bins / 8);
     void *row_base = cv.take((n_rows + 1) * 4);
-    void *list_len = cv.take((size_t)c->cap_peaks * 4);
-    void *pairs = cv.take((size_t)c->cap_hits * 8);
-    void *list_tmp = cv.take((size_t)c->cap_hits * 4);
+    void *list_len = cv.take(n_sub * 4);
+    void *sub_off = cv.take((n_sub + 1) * 8);
+    void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
+    void *ent_idx = cv.take((size_t)c->cap_hits * 4);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -151,8 +153,10 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->flags = (uint32_t *)flags;
         h->row_base = (uint32_t *)row_base;
         h->list_len = (uint32_t *)list_len;
-        h->pairs = (uint2 *)pairs;
-        h->list_tmp = (uint32_t *)list_tmp;
+        h->sub_off = (unsigned long long *)sub_off;
+        h->ent_sub = (uint32_t *)ent_sub;
+        h->ent_hit = (uint32_t *)ent_hit;
+        h->ent_idx = (uint32_t *)ent_idx;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
@@ -215,41 +219,15 @@ static int choose_geometry(hough_handle *h)
         }
         while (split > 1 && 32 * groups * split > 1024)
             --split;
-        if (!sweep_geom_init(h, &h->vote_geom, P, D, split, 0)) {
+        if (!sweep_geom_init(h, &h->vote_geom, P, D, split)) {
             // fall back to the smallest tile
-            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 0))
+            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4))
                 return 0;
         }
     }
-    // hit lists: same tile as the vote by default (the tile itself is small: flag words
-    // and popcount prefixes), so the cull keeps the same efficiency
-    {
-        int D = env_int("HOUGH_LIST_TILE_D0", h->vote_geom.D);
-        if (D > c.n_d0)
-            D = c.n_d0;
-        if (D < 1)
-            D = 1;
-        int P = env_int("HOUGH_LIST_TILE_PHI", h->vote_geom.P);
-        if (P < 1)
-            P = 1;
-        if (P > c.n_phi)
-            P = c.n_phi;
-        int groups = (P * D + 31) / 32;
-        int split = env_int("HOUGH_LIST_SPLIT", 0);
-        if (split <= 0) {
-            split = 512 / (32 * groups);
-            if (split < 1)
-                split = 1;
-            if (split > 8)
-                split = 8;
-        }
-        while (split > 1 && 32 * groups * split > 1024)
-            --split;
-        if (!sweep_geom_init(h, &h->list_geom, P, D, split, 1)) {
-            if (!sweep_geom_init(h, &h->list_geom, 1, 1, 4, 1))
-                return 0;
-        }
-    }
+    // hit lists: warp sub-tiles, hit segments (hough_lists.cu)
+    if (!list_geom_init(h))
+        return 0;
     // peak sweep: JW warps x 2 rows per CTA (2 of them halo rows), Li phi0 planes per CTA
     {
         int JW = env_int("HOUGH_PEAK_JW", 8);
@@ -447,11 +425,9 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
-        CK(cudaMemsetAsync(h->list_len, 0, (size_t)h->cfg.cap_peaks * 4, st));
+        CK(cudaMemsetAsync(h->list_len, 0, (size_t)h->cfg.cap_peaks * h->list_geom.S * 4, st));
         CK(launch_list_sweep(h, st));
         stage_mark(h, ST_LIST_SWEEP + 1, st);
-        CK(launch_rank_pairs(h, out, st));
-        stage_mark(h, ST_RANK_PAIRS + 1, st);
         CK(launch_scan_lens(h, out, st));
         stage_mark(h, ST_SCAN_LENS + 1, st);
         CK(launch_place_lists(h, out, st));
@@ -559,8 +535,8 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
 
 static const char *const k_stage_names[HOUGH_N_STAGES] = {
-    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "rank_pairs", "scan_lens",
-    "place_lists", "finish"};
+    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "scan_lens", "place_lists",
+    "finish"};
 
 const char *hough_stage_name(int stage)
 {

@@ -27,6 +27,21 @@ struct SweepGeom {
     int no_phi_cull;     // tile spans too wide an angle for the interval test
 };
 
+// Geometry of the hit-list sweep (hough_lists.cu): a warp owns a sub-tile of SP x SD = 32
+// cells, a CTA a super-tile of WP x WD sub-tiles and one of S segments of the event's hits.
+#define LIST_WARPS 16
+#define LIST_MAX_SEGMENTS 16
+struct ListGeom {
+    int SP, SD, WP, WD;
+    int tiles_phi, tiles_d0;
+    int S;               // hit segments (sub-lists per peak)
+    int max_pk;          // bound on the peaks of one sub-tile
+    int widx_off, laneq_off, queue_off; // byte offsets inside the warp's shared-memory block
+    int warp_bytes;      // shared memory per warp
+    int smem_bytes;      // dynamic shared memory of the kernel
+    int no_phi_cull_tile, no_phi_cull_sub;
+};
+
 // Device-side constant block handed to every kernel by value.
 struct GridDev {
     int n_phi, n_d0, n_kappa;
@@ -59,8 +74,8 @@ struct DevCounters {
 
 // stages of one event, in launch order (HOUGH_OPT_STAGE_TIMING)
 enum {
-    ST_PREP = 0, ST_VOTE, ST_PEAK_SWEEP, ST_SCAN_ROWS, ST_COMPACT, ST_LIST_SWEEP, ST_RANK_PAIRS,
-    ST_SCAN_LENS, ST_PLACE_LISTS, ST_FINISH
+    ST_PREP = 0, ST_VOTE, ST_PEAK_SWEEP, ST_SCAN_ROWS, ST_COMPACT, ST_LIST_SWEEP, ST_SCAN_LENS,
+    ST_PLACE_LISTS, ST_FINISH
 };
 
 struct hough_handle {
@@ -68,7 +83,8 @@ struct hough_handle {
     double *radii;       // host copy
     int device, n_sms;
     GridDev g;
-    SweepGeom vote_geom, list_geom;
+    SweepGeom vote_geom;
+    ListGeom list_geom;
     // workspace carve-up (device)
     uint32_t *acc;
     float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq;
@@ -79,10 +95,10 @@ struct hough_handle {
     uint32_t max_hits_pad;
     uint32_t *flags;      // 1 bit per bin
     uint32_t *row_base;   // [n_rows + 1] exclusive scan of peaks per (i, j) row
-    uint32_t *list_len;   // [cap_peaks] hit-list length of each reported peak
-    uint2 *pairs;         // [cap_hits] (peak, hit index) pairs of the list sweep
-    uint32_t *list_tmp;   // [cap_hits] the lists before ordering
-    unsigned long long *n_pairs; // pairs emitted (lives in the per-hough_peaks reset region)
+    uint32_t *list_len;   // [cap_peaks * S_max] length of sub-list (peak, segment)
+    unsigned long long *sub_off; // [cap_peaks * S_max + 1] its exclusive scan
+    uint32_t *ent_sub, *ent_hit, *ent_idx; // [cap_hits] entries (sub-list, hit, place) of the list sweep
+    unsigned long long *n_pairs; // entries emitted (lives in the per-hough_peaks reset region)
     unsigned long long *scan_status; // look-back words of the chained scans
     unsigned int *scan_ticket;       // [4]
     DevCounters *counters;
@@ -116,13 +132,14 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
-cudaError_t launch_rank_pairs(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st);
 
-int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split, int list_mode);
+int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split);
+int list_geom_init(hough_handle *h);
+int list_segments_bound(const hough_config *c);
 int hough_vote_max_smem(void);
 
 #define HOUGH_CHUNK 512       // hits per staged chunk

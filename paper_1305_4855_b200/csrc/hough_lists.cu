@@ -1,0 +1,554 @@
+// hough_lists.cu -- a7, the hit lists of the reported peaks (DESIGN.md
+// section 4.4): "each peak is emitted with its sorted hit list" (BASELINE.json north_star),
+// hit list of a peak = the hits whose own vote at the peak's (phi0, d0) cell lands in the
+// peak's kappa bin, ascending hit index, CSR (A7).
+//
+// One sweep re-evaluates the votes and keeps those that land in a reported peak bin.  It
+// is organised so that every entry already knows its final place in its list:
+//   * a WARP owns a sub-tile of 32 (phi0, d0) cells (lane = cell) and walks the hits of ONE
+//     segment of the event in ascending hit order, so the entries of a cell come out
+//     ascending; a private shared-memory counter per peak hands out idx = 0, 1, 2, ...;
+//   * the event's hits are cut into S segments (whole staged chunks); CTA = (super-tile of
+//     LIST_WARPS sub-tiles, segment).  Sub-list (peak p, segment s) has the id p*S + s; the
+//     concatenation of a peak's sub-lists in segment order is its ascending list;
+//   * sub_len[p*S + s] is written at the end of the CTA, k_scan<LENS> turns it into
+//     sub_off (and hit_offset[p] = sub_off[p*S]), k_scatter_entries drops entry
+//     (sub, hit, idx) at hit_index[sub_off[sub] + idx].  No sort, no atomics on the lists.
+// The hits are culled twice with the conservative interval test of DESIGN.md section 4.3:
+// per CTA against the super-tile (lane = hit, order-preserving compaction) and per warp
+// against its sub-tile (lane = hit, ballot), then the exact recipe runs on the survivors.
+// If the entry buffer (cap_hits entries) overflows, the output is truncated anyway
+// (n_hit_entries > cap_hits); k_list_slow then refills the lists that still fit directly
+// from the hits, one warp per peak.
+#include "hough_device.cuh"
+
+#define LIST_QUEUE 64  // entries a warp buffers before it flushes (>= 2 * 32)
+#define LIST_ROUND 128 // CTA survivors a warp culls at a time
+#define LIST_LQ 8      // pending votes per lane before the warp drains them
+
+struct ListSweepParams {
+    GridDev g;
+    HitsDev hits;
+    ListGeom geom;
+    int no_cull;
+    const uint32_t *flags;    // 1 bit per bin
+    const uint32_t *row_base; // [n_rows + 1]
+    const unsigned int *n_peaks_dev;
+    uint32_t cap_peaks;
+    uint32_t *sub_len;        // [cap_peaks * S], zeroed before the sweep
+    uint32_t *ent_sub, *ent_hit, *ent_idx; // [ent_cap] entries
+    unsigned long long *n_entries;
+    unsigned long long ent_cap;
+};
+
+__device__ __forceinline__ unsigned short lds_u16(uint32_t addr)
+{
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t addr, unsigned short v)
+{
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(v) : "memory");
+}
+
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+// Per-warp shared-memory block (byte offsets; wpr = n_kappa / 32):
+//   flags   [wpr][32] u32   flag words of the reported peaks of the warp's cells
+//   prefix  [wpr][32] u16   reported peaks of the cell below each word
+//   count   [max_pk]  u16   entries handed out so far, per local peak id
+//   widx    [LIST_ROUND + 2] u16   survivors of the warp-level cull (indices into surv)
+//   laneq   [LIST_LQ][32] u32      per lane: pending (kappa bin << 10 | surv index)
+//   flushq  [3][LIST_QUEUE] u32    finished entries on their way to global memory
+__global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepParams p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const GridDev &g = p.g;
+    const ListGeom &ge = p.geom;
+    const int nk = g.n_kappa, wpr = nk >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int S = ge.S;
+
+    // ---- which super-tile, which hit segment
+    const int seg = blockIdx.x % S, tile_id = blockIdx.x / S;
+    const int tp = tile_id / ge.tiles_d0, td = tile_id % ge.tiles_d0;
+    const uint32_t n_chunks = p.hits.n_pad / HOUGH_CHUNK;
+    const uint32_t ch0 = (uint32_t)(((unsigned long long)n_chunks * seg) / S);
+    const uint32_t ch1 = (uint32_t)(((unsigned long long)n_chunks * (seg + 1)) / S);
+    if (ch0 >= ch1)
+        return; // empty segment: its sub-lists stay 0
+
+    // ---- carve shared memory
+    unsigned char *wbase = smem_raw + (size_t)warp * ge.warp_bytes;
+    uint32_t *wflags = reinterpret_cast<uint32_t *>(wbase);
+    unsigned short *wpre = reinterpret_cast<unsigned short *>(wbase + (size_t)wpr * 128);
+    unsigned short *wcnt = wpre + (size_t)wpr * 32;
+    unsigned short *widx = reinterpret_cast<unsigned short *>(wbase + ge.widx_off);
+    uint32_t *laneq = reinterpret_cast<uint32_t *>(wbase + ge.laneq_off);
+    uint32_t *wq = reinterpret_cast<uint32_t *>(wbase + ge.queue_off);
+    unsigned char *ptr = smem_raw + (size_t)LIST_WARPS * ge.warp_bytes;
+    float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
+    ptr += (size_t)2 * 4 * HOUGH_CHUNK * 4;
+    float4 *surv = reinterpret_cast<float4 *>(ptr); // [chunk + 2]
+    ptr += (size_t)(HOUGH_CHUNK + 2) * 16;
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
+    ptr += 16;
+    int *warp_cnt = reinterpret_cast<int *>(ptr); // [LIST_WARPS]
+
+    // ---- this warp's sub-tile and this lane's cell
+    const int wp = warp / ge.WD, wd = warp % ge.WD;
+    const int i0 = tp * ge.WP * ge.SP, j0 = td * ge.WD * ge.SD; // super-tile origin
+    const int si0 = i0 + wp * ge.SP, sj0 = j0 + wd * ge.SD;
+    const int sni = max(0, min(ge.SP, g.n_phi - si0)), snj = max(0, min(ge.SD, g.n_d0 - sj0));
+    const int il = lane / ge.SD, jl = lane - il * ge.SD;
+    const bool cell_ok = (il < sni) && (jl < snj);
+    const bool warp_ok = sni > 0 && snj > 0;
+    float c_sn = 0.f, c_cs = 0.f, c_d0 = 0.f, c_2d0 = 0.f, c_d0sq = __int_as_float(0x7fc00000);
+    uint32_t c_row = 0;
+    if (cell_ok) {
+        c_sn = g.sn[si0 + il];
+        c_cs = g.cs[si0 + il];
+        c_d0 = g.d0c[sj0 + jl];
+        c_2d0 = g.twod0[sj0 + jl];
+        c_d0sq = g.d0sq[sj0 + jl];
+        c_row = (uint32_t)(si0 + il) * (uint32_t)g.n_d0 + (uint32_t)(sj0 + jl);
+    }
+    const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
+
+    // super-tile extent (CTA-level cull) and sub-tile extent (warp-level cull)
+    const int ni = min(ge.WP * ge.SP, g.n_phi - i0), nj = min(ge.WD * ge.SD, g.n_d0 - j0);
+    TileCull tc, wc;
+    tc.snA = g.sn[i0];
+    tc.csA = g.cs[i0];
+    tc.snB = g.sn[i0 + ni - 1];
+    tc.csB = g.cs[i0 + ni - 1];
+    tc.dlo = g.d0c[j0];
+    tc.dhi = g.d0c[j0 + nj - 1];
+    tc.phi_all = ge.no_phi_cull_tile;
+    tc.off = p.no_cull;
+    wc = tc;
+    if (warp_ok) {
+        wc.snA = g.sn[si0];
+        wc.csA = g.cs[si0];
+        wc.snB = g.sn[si0 + sni - 1];
+        wc.csB = g.cs[si0 + sni - 1];
+        wc.dlo = g.d0c[sj0];
+        wc.dhi = g.d0c[sj0 + snj - 1];
+        wc.phi_all = ge.no_phi_cull_sub;
+    }
+
+    if (tid == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint32_t chunk_bytes = (uint32_t)HOUGH_CHUNK * 4;
+    auto issue = [&](uint32_t ch) { // buffer and parity follow (ch - ch0)
+        const uint32_t q = ch - ch0;
+        float *dst = stage + (size_t)(q & 1) * 4 * HOUGH_CHUNK;
+        uint64_t *bar = &mbar[q & 1];
+        mbar_expect_tx(bar, 4 * chunk_bytes);
+        size_t off = (size_t)ch * HOUGH_CHUNK;
+        tma_load_1d(dst, p.hits.x + off, chunk_bytes, bar);
+        tma_load_1d(dst + HOUGH_CHUNK, p.hits.y + off, chunk_bytes, bar);
+        tma_load_1d(dst + 2 * HOUGH_CHUNK, p.hits.r2 + off, chunk_bytes, bar);
+        tma_load_1d(dst + 3 * HOUGH_CHUNK, p.hits.bit + off, chunk_bytes, bar);
+    };
+    if (tid == 0)
+        issue(ch0);
+
+    // ---- per warp: flag words of the reported peaks of its 32 cells, the number of reported
+    // peaks below each word, the local peak ids and their counters
+    const uint32_t n_rep = min(*p.n_peaks_dev, p.cap_peaks);
+    uint32_t c_gbase = 0, c_nrep = 0;
+    {
+        uint32_t nr = 0;
+        const uint32_t *fw = p.flags;
+        if (cell_ok) {
+            c_gbase = p.row_base[c_row];
+            const uint32_t cnt = p.row_base[c_row + 1] - c_gbase;
+            nr = c_gbase >= n_rep ? 0u : min(cnt, n_rep - c_gbase);
+            fw += (size_t)c_row * wpr;
+        }
+        uint32_t before = 0;
+        for (int w = 0; w < wpr; ++w) {
+            uint32_t f = nr ? fw[w] : 0u;
+            while (before + (uint32_t)__popc(f) > nr) // the capacity cuts inside this word
+                f &= ~(0x80000000u >> __clz(f));
+            wflags[w * 32 + lane] = f;
+            wpre[w * 32 + lane] = (unsigned short)before;
+            before += (uint32_t)__popc(f);
+        }
+        c_nrep = before;
+    }
+    uint32_t c_lbase = c_nrep; // exclusive warp scan
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, c_lbase, o);
+        if (lane >= o)
+            c_lbase += t;
+    }
+    const uint32_t w_npk = __shfl_sync(0xffffffffu, c_lbase, 31);
+    c_lbase -= c_nrep;
+    for (uint32_t q = lane; q < w_npk; q += 32)
+        wcnt[q] = 0;
+    __syncwarp();
+
+    const int nkm1 = nk - 1;
+    const uint32_t fl_addr = smem_u32(wflags) + (uint32_t)lane * 4u;  // + (k >> 5) * 128
+    const uint32_t pre_addr = smem_u32(wpre) + (uint32_t)lane * 2u;   // + (k >> 5) * 64
+    const uint32_t cnt_addr = smem_u32(wcnt) + c_lbase * 2u;          // + rank * 2
+    const uint32_t lq_addr = smem_u32(laneq) + (uint32_t)lane * 4u;   // + e * 128
+    const uint32_t sub0 = c_gbase * (uint32_t)S + (uint32_t)seg;      // + rank * S
+    uint32_t *q_sub = wq, *q_hit = wq + LIST_QUEUE, *q_idx = wq + 2 * LIST_QUEUE;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    uint32_t qn = 0; // entries waiting in this warp's flush queue (warp-uniform)
+    uint32_t nl = 0; // entries waiting in this lane's queue
+
+    auto flush = [&]() {
+        __syncwarp();
+        unsigned long long b = 0;
+        if (lane == 0)
+            b = atomicAdd(p.n_entries, (unsigned long long)qn);
+        b = __shfl_sync(0xffffffffu, b, 0);
+        for (uint32_t e = lane; e < qn; e += 32)
+            if (b + e < p.ent_cap) {
+                p.ent_sub[b + e] = q_sub[e];
+                p.ent_hit[b + e] = q_hit[e];
+                p.ent_idx[b + e] = q_idx[e];
+            }
+        qn = 0;
+        __syncwarp();
+    };
+
+    // Every lane turns its pending votes into entries, oldest first: rank of the bin among
+    // the cell's reported peaks -> local peak id -> its counter (the place in the sub-list).
+    auto drain = [&]() {
+        for (uint32_t e = 0;; ++e) {
+            const bool act = e < nl;
+            const unsigned bh = __ballot_sync(0xffffffffu, act);
+            if (!bh)
+                break;
+            if (act) {
+                const uint32_t ent = smem_ld(lq_addr + e * 128u);
+                const uint32_t k = ent >> 10;
+                const uint32_t f = smem_ld(fl_addr + (k >> 5) * 128u);
+                const uint32_t rank = lds_u16(pre_addr + (k >> 5) * 64u) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
+                const uint32_t ca = cnt_addr + rank * 2u;
+                const unsigned short n = lds_u16(ca);
+                sts_u16(ca, (unsigned short)(n + 1));
+                const uint32_t pos = qn + (uint32_t)__popc(bh & lt_mask);
+                q_sub[pos] = sub0 + rank * (uint32_t)S;
+                q_hit[pos] = __float_as_uint(surv[ent & 1023u].w);
+                q_idx[pos] = n;
+            }
+            qn += (uint32_t)__popc(bh);
+            if (qn > LIST_QUEUE - 32)
+                flush();
+        }
+        nl = 0;
+    };
+
+    // one hit against the warp's 32 cells: exact recipe, then the peak test of the bin
+    auto process = [&](const float4 hv, const uint32_t sidx) {
+        const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+        if ((kappa >= klo) && (kappa < khi)) {
+            const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
+            const uint32_t f = smem_ld(fl_addr + (k >> 5) * 128u);
+            if ((f >> (k & 31u)) & 1u) {
+                sts_u32(lq_addr + nl * 128u, (k << 10) | sidx);
+                ++nl;
+            }
+        }
+    };
+
+    for (uint32_t ch = ch0; ch < ch1; ++ch) {
+        const uint32_t q = ch - ch0;
+        const float *st = stage + (size_t)(q & 1) * 4 * HOUGH_CHUNK;
+        mbar_wait(&mbar[q & 1], (q >> 1) & 1);
+        if (tid == 0 && ch + 1 < ch1)
+            issue(ch + 1); // the other buffer was released by the barrier ending the previous chunk
+
+        // ---- CTA-level cull against the super-tile, order-preserving compaction
+        int total = 0;
+        for (int base = 0; base < HOUGH_CHUNK; base += 32 * LIST_WARPS) {
+            const int hidx = base + tid;
+            const float hx = st[hidx], hy = st[HOUGH_CHUNK + hidx], hr2 = st[2 * HOUGH_CHUNK + hidx];
+            const uint32_t hb = __float_as_uint(st[3 * HOUGH_CHUNK + hidx]);
+            const bool keep = (hb != 0u) && hit_may_vote(hx, hy, hr2, tc, g.kabs, g.d0_absmax);
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            if (lane == 0)
+                warp_cnt[warp] = __popc(bal);
+            __syncthreads();
+            int before = 0, all = 0;
+#pragma unroll
+            for (int w = 0; w < LIST_WARPS; ++w) {
+                const int cw = warp_cnt[w];
+                before += (w < warp) ? cw : 0;
+                all += cw;
+            }
+            if (keep)
+                surv[total + before + __popc(bal & lt_mask)] =
+                    make_float4(hx, hy, hr2, __uint_as_float(ch * HOUGH_CHUNK + hidx));
+            total += all;
+            __syncthreads();
+        }
+        if (tid == 0) // a non-voting entry that pads odd batches
+            surv[total] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+        __syncthreads();
+
+        if (warp_ok) {
+            for (int base = 0; base < total; base += LIST_ROUND) {
+                // ---- warp-level cull against the sub-tile (lane = hit) -> widx[0 .. nw)
+                int nw = 0;
+#pragma unroll
+                for (int r = 0; r < LIST_ROUND / 32; ++r) {
+                    const int idx = base + r * 32 + lane;
+                    bool kw = false;
+                    if (idx < total) {
+                        const float4 hv = surv[idx];
+                        kw = hit_may_vote(hv.x, hv.y, hv.z, wc, g.kabs, g.d0_absmax);
+                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, kw);
+                    if (kw)
+                        widx[nw + __popc(bal & lt_mask)] = (unsigned short)idx;
+                    nw += __popc(bal);
+                }
+                if (lane == 0)
+                    widx[nw] = (unsigned short)total; // pad to an even count with the non-voting entry
+                __syncwarp();
+                // ---- lane = cell: the exact recipe on the survivors, two at a time
+                const uint32_t *wpair = reinterpret_cast<const uint32_t *>(widx);
+                for (int t = 0; t < nw; t += 2) {
+                    const uint32_t two = wpair[t >> 1];
+                    const uint32_t a = two & 0xffffu, b = two >> 16;
+                    const float4 h0 = surv[a], h1 = surv[b];
+                    process(h0, a);
+                    process(h1, b);
+                    if (__any_sync(0xffffffffu, nl > LIST_LQ - 2))
+                        drain();
+                }
+                __syncwarp();
+            }
+            drain(); // surv is about to be reused
+        }
+        __syncthreads(); // survivors and this stage buffer are free again
+    }
+
+    if (qn)
+        flush();
+    // ---- true lengths of this segment's sub-lists
+    for (uint32_t r = 0; r < c_nrep; ++r)
+        p.sub_len[(size_t)(c_gbase + r) * S + seg] = wcnt[c_lbase + r];
+}
+
+// ------------------------------------------------------------------ placement
+struct ListPlaceParams {
+    GridDev g;
+    const float *hx, *hy, *hr2;
+    const uint32_t *hbit;
+    uint32_t n_hits;
+    const unsigned long long *n_entries;
+    unsigned long long ent_cap;
+    const uint32_t *ent_sub, *ent_hit, *ent_idx;
+    const unsigned long long *sub_off;
+    const DevCounters *counters;
+    uint32_t cap_peaks;
+    const uint32_t *bin;
+    const unsigned long long *hit_offset;
+    uint32_t *hit_index;
+    unsigned long long cap_hits;
+};
+
+__global__ void __launch_bounds__(256) k_scatter_entries(const ListPlaceParams p)
+{
+    const unsigned long long n = *p.n_entries;
+    if (n > p.ent_cap)
+        return; // k_list_slow takes over
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const unsigned long long pos = p.sub_off[p.ent_sub[i]] + p.ent_idx[i];
+        if (pos < p.cap_hits)
+            p.hit_index[pos] = p.ent_hit[i];
+    }
+}
+
+// Entry buffer overflowed: write the lists that start below cap_hits straight from the
+// hits, one warp per peak, ascending by construction.
+__global__ void __launch_bounds__(256) k_list_slow(const ListPlaceParams p)
+{
+    if (*p.n_entries <= p.ent_cap)
+        return;
+    const GridDev &g = p.g;
+    const int lane = threadIdx.x & 31;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
+    for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
+        unsigned long long pos = p.hit_offset[pk];
+        if (pos >= p.cap_hits)
+            continue;
+        const uint32_t lin = p.bin[pk];
+        const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
+        const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
+        const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
+        for (uint32_t base = 0; base < p.n_hits; base += 32) {
+            const uint32_t hidx = base + lane;
+            bool in = false;
+            if (hidx < p.n_hits && p.hbit[hidx] != 0u) {
+                const float kappa = eval_kappa(p.hx[hidx], p.hy[hidx], p.hr2[hidx], sn, cs, d0c, twod0, d0sq);
+                if ((kappa >= g.klo) && (kappa < g.khi))
+                    in = (uint32_t)kappa_bin(kappa, g.klo, g.inv_dk, g.n_kappa - 1) == k;
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, in);
+            if (in) {
+                unsigned long long q = pos + __popc(bal & ((1u << lane) - 1u));
+                if (q < p.cap_hits)
+                    p.hit_index[q] = hidx;
+            }
+            pos += __popc(bal);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ host side
+// Sub-tile = SP x SD = 32 cells (8 x 4 by default), super-tile = WP x WD sub-tiles, S hit
+// segments chosen so that the CTAs fill a whole number of waves as nearly as possible.
+static int list_segments_min(const hough_config *c)
+{
+    uint32_t hp = ((c->max_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
+    int s_min = (int)((hp + 65534u) / 65535u); // u16 counters: at most 65535 hits per segment
+    return s_min < 1 ? 1 : s_min;
+}
+
+// Upper bound of S for a configuration (sizes the sub-list tables of the workspace).
+int list_segments_bound(const hough_config *c)
+{
+    const int s_min = list_segments_min(c);
+    int s_max = LIST_MAX_SEGMENTS;
+    while (s_max > s_min && (unsigned long long)s_max * c->cap_peaks > (1ull << 26))
+        --s_max;
+    return s_max > s_min ? s_max : s_min;
+}
+
+int list_geom_init(hough_handle *h)
+{
+    const hough_config &c = h->cfg;
+    ListGeom *ge = &h->list_geom;
+    int SD = 4;
+    while (SD > c.n_d0)
+        SD >>= 1;
+    ge->SD = SD;
+    ge->SP = 32 / SD;
+    ge->WD = 1;
+    while (ge->WD < 4 && ge->WD * 2 * SD <= c.n_d0)
+        ge->WD *= 2;
+    ge->WP = LIST_WARPS / ge->WD;
+    ge->tiles_phi = (c.n_phi + ge->WP * ge->SP - 1) / (ge->WP * ge->SP);
+    ge->tiles_d0 = (c.n_d0 + ge->WD * ge->SD - 1) / (ge->WD * ge->SD);
+    const int wpr = c.n_kappa / 32;
+    ge->max_pk = ((ge->SP + 1) / 2) * ((ge->SD + 1) / 2) * ((c.n_kappa + 1) / 2);
+    ge->widx_off = (wpr * 192 + ge->max_pk * 2 + 15) & ~15;
+    ge->laneq_off = (ge->widx_off + (LIST_ROUND + 2) * 2 + 15) & ~15;
+    ge->queue_off = ge->laneq_off + LIST_LQ * 32 * 4;
+    ge->warp_bytes = (ge->queue_off + 3 * LIST_QUEUE * 4 + 127) & ~127;
+    ge->smem_bytes = LIST_WARPS * ge->warp_bytes + 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 2) * 16 + 16 +
+                     LIST_WARPS * 4 + 16;
+    if (ge->smem_bytes > hough_vote_max_smem())
+        return 0;
+    const double dphi = (c.phi_max - c.phi_min) / (double)c.n_phi;
+    ge->no_phi_cull_tile = (dphi * (ge->WP * ge->SP - 1) > 1.0) ? 1 : 0;
+    ge->no_phi_cull_sub = (dphi * (ge->SP - 1) > 1.0) ? 1 : 0;
+    if (cudaFuncSetAttribute(k_list_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes) !=
+        cudaSuccess)
+        return 0;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_list_sweep, 32 * LIST_WARPS, ge->smem_bytes) !=
+            cudaSuccess ||
+        per_sm < 1)
+        return 0;
+    // segments: whole chunks, at most 65535 hits each (u16 counters), bounded sub-list table
+    const uint32_t n_chunks_max = (h->max_hits_pad + HOUGH_CHUNK - 1) / HOUGH_CHUNK;
+    const int s_min = list_segments_min(&c), s_bound = list_segments_bound(&c);
+    int s_max = s_bound;
+    if ((uint32_t)s_max > n_chunks_max)
+        s_max = n_chunks_max > (uint32_t)s_min ? (int)n_chunks_max : s_min;
+    const double slots = (double)h->n_sms * per_sm;
+    const double tiles = (double)ge->tiles_phi * ge->tiles_d0;
+    int best = s_min;
+    double best_score = -1.0;
+    for (int s = s_min; s <= s_max; ++s) {
+        const double r = tiles * s / slots;
+        const double eff = r / ceil(r);
+        const double score = eff - 0.002 * s; // prefer fewer segments when the fill is equal
+        if (score > best_score) {
+            best_score = score;
+            best = s;
+        }
+    }
+    ge->S = best;
+    const char *e = getenv("HOUGH_LIST_SEGMENTS");
+    if (e && atoi(e) >= s_min && atoi(e) <= s_bound)
+        ge->S = atoi(e);
+    return 1;
+}
+
+cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
+{
+    ListSweepParams p;
+    p.g = h->g;
+    p.hits.x = h->hx;
+    p.hits.y = h->hy;
+    p.hits.r2 = h->hr2;
+    p.hits.bit = h->hbit;
+    p.hits.n = h->n_hits;
+    p.hits.n_pad = ((h->n_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
+    p.geom = h->list_geom;
+    p.no_cull = (h->cfg.options & HOUGH_OPT_NO_CULL) ? 1 : 0;
+    p.flags = h->flags;
+    p.row_base = h->row_base;
+    p.n_peaks_dev = &h->counters->n_peaks;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.sub_len = h->list_len;
+    p.ent_sub = h->ent_sub;
+    p.ent_hit = h->ent_hit;
+    p.ent_idx = h->ent_idx;
+    p.n_entries = h->n_pairs;
+    p.ent_cap = h->cfg.cap_hits;
+    h->launches += 1;
+    if (p.hits.n_pad == 0)
+        return cudaSuccess;
+    const int blocks = h->list_geom.tiles_phi * h->list_geom.tiles_d0 * h->list_geom.S;
+    k_list_sweep<<<blocks, 32 * LIST_WARPS, h->list_geom.smem_bytes, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    ListPlaceParams p;
+    p.g = h->g;
+    p.hx = h->hx;
+    p.hy = h->hy;
+    p.hr2 = h->hr2;
+    p.hbit = h->hbit;
+    p.n_hits = h->n_hits;
+    p.n_entries = h->n_pairs;
+    p.ent_cap = h->cfg.cap_hits;
+    p.ent_sub = h->ent_sub;
+    p.ent_hit = h->ent_hit;
+    p.ent_idx = h->ent_idx;
+    p.sub_off = h->sub_off;
+    p.counters = h->counters;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.bin = out->bin;
+    p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
+    p.hit_index = out->hit_index;
+    p.cap_hits = h->cfg.cap_hits;
+    k_scatter_entries<<<h->n_sms * 16, 256, 0, st>>>(p);
+    k_list_slow<<<h->n_sms * 4, 256, 0, st>>>(p);
+    h->launches += 2;
+    return cudaGetLastError();
+}

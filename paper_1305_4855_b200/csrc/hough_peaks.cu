@@ -5,7 +5,6 @@
 //                  one pass over the accumulator (4 B/bin read once), 1 flag bit per bin out
 //   k_scan         single-pass chained prefix sum (decoupled look-back)
 //   k_compact      flag bits -> (lin, mask) records in ascending lin
-//   k_rank_pairs, k_scatter_pairs, k_order_pairs, k_list_slow   CSR hit lists from the pairs
 //   k_finish       counters -> the caller's hough_counts
 // The peak rule is BASELINE.json north_star's ("popcount reaches at least L_min and ...
 // local maxima in the 3x3x3 neighbourhood (ties go to the lower linear index)"), restated
@@ -260,7 +259,8 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
 // (flag << 62) | value, flag 1 = aggregate, 2 = inclusive prefix; written with one
 // 64-bit store so that no fence is needed between flag and value.
 //   SCAN_ROWS : item i = number of flag bits of accumulator row i  -> row_base (u32)
-//   SCAN_LENS : item i = list_len[i], i < min(n_peaks, cap_peaks)  -> hit_offset (u64)
+//   SCAN_LENS : item i = length of sub-list i = peak*S + segment, i < min(n_peaks, cap_peaks)*S
+//               -> sub_off (u64); hit_offset[peak] = sub_off[peak*S]
 #define SCAN_ROWS 0
 #define SCAN_LENS 1
 #define SCAN_THREADS 256
@@ -274,6 +274,8 @@ struct ScanParams {
     const uint32_t *list_len;
     uint32_t cap_peaks;
     unsigned long long *hit_offset;
+    unsigned long long *sub_off;
+    uint32_t S;
     unsigned long long cap_hits;
     DevCounters *counters;
     unsigned int *ticket;
@@ -291,7 +293,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
         s_ticket = atomicAdd(p.ticket, 1u);
     __syncthreads();
     const unsigned int t = s_ticket;
-    const uint32_t n = KIND == SCAN_ROWS ? p.n_rows : min(p.counters->n_peaks, p.cap_peaks);
+    const uint32_t n = KIND == SCAN_ROWS ? p.n_rows : min(p.counters->n_peaks, p.cap_peaks) * p.S;
     const unsigned long long base = (unsigned long long)t * HOUGH_SCAN_ITEMS;
     if (n == 0) {
         if (t == 0 && tid == 0) {
@@ -373,17 +375,21 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
     for (int q = 0; q < SCAN_PER_THREAD; ++q) {
         unsigned long long i = base + (unsigned long long)tid * SCAN_PER_THREAD + q;
         if (i < n) {
-            if (KIND == SCAN_ROWS)
+            if (KIND == SCAN_ROWS) {
                 p.row_base[i] = (uint32_t)run;
-            else
-                p.hit_offset[i] = run;
+            } else {
+                p.sub_off[i] = run;
+                if (i % p.S == 0)
+                    p.hit_offset[i / p.S] = run;
+            }
             run += v[q];
             if (i == (unsigned long long)n - 1) { // the last item closes the scan
                 if (KIND == SCAN_ROWS) {
                     p.row_base[n] = (uint32_t)run;
                     p.counters->n_peaks = (unsigned int)run;
                 } else {
-                    p.hit_offset[n] = run;
+                    p.sub_off[n] = run;
+                    p.hit_offset[n / p.S] = run;
                     p.counters->n_hit_entries = run;
                 }
             }
@@ -400,6 +406,8 @@ static void scan_params(hough_handle *h, ScanParams *p, const hough_peaks_out *o
     p->list_len = h->list_len;
     p->cap_peaks = h->cfg.cap_peaks;
     p->hit_offset = out ? reinterpret_cast<unsigned long long *>(out->hit_offset) : nullptr;
+    p->sub_off = h->sub_off;
+    p->S = (uint32_t)h->list_geom.S;
     p->cap_hits = h->cfg.cap_hits;
     p->counters = h->counters;
     p->ticket = h->scan_ticket + which;
@@ -420,7 +428,7 @@ cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaSt
 {
     ScanParams p;
     scan_params(h, &p, out, 1);
-    uint32_t blocks = (h->cfg.cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS;
+    uint32_t blocks = (uint32_t)(((size_t)h->cfg.cap_peaks * h->list_geom.S + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
     k_scan<SCAN_LENS><<<blocks, SCAN_THREADS, 0, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
@@ -480,191 +488,6 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
     k_compact<<<blocks, 256, 0, st>>>(h->flags, h->row_base, h->acc, n_rows, h->g.n_kappa,
                                       h->cfg.cap_peaks, out->bin, out->mask);
     h->launches += 1;
-    return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------ hit lists (a7)
-// The list sweep left n_pairs (lin of a reported peak bin, hit index) pairs in no particular
-// order.  Then:
-//   k_rank_pairs    lin -> global peak rank (row_base + flag bits below), list_len[rank]++
-//   k_scan<LENS>    list_len -> hit_offset (CSR), n_hit_entries
-//   k_scatter_pairs pair -> tmp[hit_offset[rank] + slot], slots handed out by counting
-//                   list_len back down: every list complete, in arbitrary order
-//   k_order_pairs   one thread per pair: its place in the ascending list is the number of
-//                   smaller entries of that list (no two entries of a list are equal)
-// If the pair buffer (cap_hits pairs) overflowed, the output is truncated anyway
-// (n_hit_entries > cap_hits); k_list_slow then recounts every list and refills the lists
-// that still fit directly from the hits, one warp per peak, ascending by construction.
-struct ListParams {
-    GridDev g;
-    const float *hx, *hy, *hr2;
-    const uint32_t *hbit;
-    uint32_t n_hits;
-    const uint32_t *flags, *row_base;
-    const unsigned long long *n_pairs;
-    unsigned long long pair_cap;
-    uint2 *pairs;
-    uint32_t *list_len;
-    const DevCounters *counters;
-    uint32_t cap_peaks;
-    const uint32_t *bin;
-    const unsigned long long *hit_offset;
-    uint32_t *tmp;
-    uint32_t *hit_index;
-    unsigned long long cap_hits;
-};
-
-__global__ void __launch_bounds__(256) k_rank_pairs(const ListParams p)
-{
-    const unsigned long long n = *p.n_pairs;
-    if (n > p.pair_cap)
-        return; // k_list_slow<0> recounts
-    const uint32_t nk = (uint32_t)p.g.n_kappa, wpr = nk >> 5;
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint32_t lin = p.pairs[i].x;
-        const uint32_t row = lin / nk, k = lin - row * nk;
-        const uint32_t *fw = p.flags + (size_t)row * wpr;
-        uint32_t rank = p.row_base[row];
-        for (uint32_t w = 0; w < (k >> 5); ++w)
-            rank += (uint32_t)__popc(fw[w]);
-        rank += (uint32_t)__popc(fw[k >> 5] & ((1u << (k & 31u)) - 1u));
-        p.pairs[i].x = rank;
-        atomicAdd(&p.list_len[rank], 1u);
-    }
-}
-
-__global__ void __launch_bounds__(256) k_scatter_pairs(const ListParams p)
-{
-    const unsigned long long n = *p.n_pairs;
-    if (n > p.pair_cap)
-        return;
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint2 pr = p.pairs[i];
-        const uint32_t slot = atomicSub(&p.list_len[pr.x], 1u) - 1u;
-        const unsigned long long pos = p.hit_offset[pr.x] + slot;
-        if (pos < p.cap_hits)
-            p.tmp[pos] = pr.y;
-    }
-}
-
-__global__ void __launch_bounds__(256) k_order_pairs(const ListParams p)
-{
-    const unsigned long long n = *p.n_pairs;
-    if (n > p.pair_cap)
-        return;
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint2 pr = p.pairs[i];
-        const unsigned long long b = p.hit_offset[pr.x], e = p.hit_offset[pr.x + 1];
-        if (e > p.cap_hits)
-            continue; // a list cut by the capacity is not part of the valid output
-        const uint32_t *a = p.tmp + b;
-        const uint32_t len = (uint32_t)(e - b);
-        uint32_t r = 0;
-        for (uint32_t m = 0; m < len; ++m)
-            r += a[m] < pr.y;
-        p.hit_index[b + r] = pr.y;
-    }
-}
-
-// FILL = 0: list_len[pk] = true length of every reported peak's list;
-// FILL = 1: write the lists that start below cap_hits, ascending.
-template <int FILL>
-__global__ void __launch_bounds__(256) k_list_slow(const ListParams p)
-{
-    if (*p.n_pairs <= p.pair_cap)
-        return;
-    const GridDev &g = p.g;
-    const int lane = threadIdx.x & 31;
-    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
-    const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
-    for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
-        unsigned long long pos = FILL ? p.hit_offset[pk] : 0ull;
-        if (FILL && pos >= p.cap_hits)
-            continue;
-        const uint32_t lin = p.bin[pk];
-        const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
-        const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
-        const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
-        uint32_t count = 0;
-        for (uint32_t base = 0; base < p.n_hits; base += 32) {
-            const uint32_t hidx = base + lane;
-            bool in = false;
-            if (hidx < p.n_hits && p.hbit[hidx] != 0u) {
-                // DESIGN.md section 2, A3 + A4 (same recipe as the sweeps)
-                float a = __fmul_rn(p.hx[hidx], sn);
-                float b = __fmul_rn(p.hy[hidx], cs);
-                float s = __fsub_rn(b, a);
-                float e = __fsub_rn(s, d0c);
-                float num = __fadd_rn(e, e);
-                float t = __fmul_rn(twod0, s);
-                float u = __fsub_rn(p.hr2[hidx], t);
-                float den = __fadd_rn(u, d0sq);
-                float kappa = __fdiv_rn(num, den);
-                if ((kappa >= g.klo) && (kappa < g.khi)) {
-                    float qf = __fmul_rn(__fsub_rn(kappa, g.klo), g.inv_dk);
-                    in = (uint32_t)min(__float2int_rz(qf), g.n_kappa - 1) == k;
-                }
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, in);
-            if (FILL && in) {
-                unsigned long long q = pos + __popc(bal & ((1u << lane) - 1u));
-                if (q < p.cap_hits)
-                    p.hit_index[q] = hidx;
-            }
-            pos += __popc(bal);
-            count += __popc(bal);
-        }
-        if (!FILL && lane == 0)
-            p.list_len[pk] = count;
-    }
-}
-
-static void list_params(hough_handle *h, const hough_peaks_out *out, ListParams *p)
-{
-    p->g = h->g;
-    p->hx = h->hx;
-    p->hy = h->hy;
-    p->hr2 = h->hr2;
-    p->hbit = h->hbit;
-    p->n_hits = h->n_hits;
-    p->flags = h->flags;
-    p->row_base = h->row_base;
-    p->n_pairs = h->n_pairs;
-    p->pair_cap = h->cfg.cap_hits;
-    p->pairs = h->pairs;
-    p->list_len = h->list_len;
-    p->counters = h->counters;
-    p->cap_peaks = h->cfg.cap_peaks;
-    p->bin = out->bin;
-    p->hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
-    p->tmp = h->list_tmp;
-    p->hit_index = out->hit_index;
-    p->cap_hits = h->cfg.cap_hits;
-}
-
-// after the list sweep, before the scan of list_len
-cudaError_t launch_rank_pairs(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
-{
-    ListParams p;
-    list_params(h, out, &p);
-    k_rank_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
-    k_list_slow<0><<<h->n_sms * 4, 256, 0, st>>>(p);
-    h->launches += 2;
-    return cudaGetLastError();
-}
-
-// after the scan of list_len
-cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
-{
-    ListParams p;
-    list_params(h, out, &p);
-    k_scatter_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
-    k_order_pairs<<<h->n_sms * 8, 256, 0, st>>>(p);
-    k_list_slow<1><<<h->n_sms * 4, 256, 0, st>>>(p);
-    h->launches += 3;
     return cudaGetLastError();
 }
 

@@ -1,19 +1,10 @@
-// hough_sweep.cu -- the tiled sweep of the hits over the (phi0, d0) cells:
-//   MODE_VOTE  : a3 vote into a shared-memory tile with atomicOr, a4 coalesced write-out,
-//                a8 vote count
-//   MODE_LIST  : a7, one sweep that emits a (peak bin, hit index) pair for every vote that
-//                lands in a reported peak; the kernels of hough_peaks.cu rank, count,
-//                place and order them
-// Both share the staging (TMA 1-D bulk copies of the SoA hit arrays into shared
-// memory, double buffered), the conservative per-tile hit cull and the exact fp32
-// evaluation of BASELINE.json north_star's closed form.
+// hough_sweep.cu -- the tiled vote sweep of the hits over the (phi0, d0) cells: a3 vote into a
+// shared-memory tile with shared atomic OR, a4 coalesced write-out, a8 vote count
+// (DESIGN.md 4.1).  Hits are staged by TMA 1-D bulk copies of the
+// SoA arrays into shared memory (double buffered), culled per tile by the conservative
+// interval test and evaluated with the exact fp32 recipe of BASELINE.json north_star's
+// closed form (hough_device.cuh).
 #include "hough_device.cuh"
-
-#define MODE_VOTE 0
-#define MODE_LIST 1
-
-#define PAIR_BUF 2048   // (peak, hit) pairs buffered per CTA between flushes
-#define PAIR_FLUSH 1024 // flush at the end of a chunk once this many are waiting
 
 #define EVAL_UNROLL 2
 
@@ -27,17 +18,9 @@ struct SweepParams {
     uint32_t *acc; // VOTE: global accumulator
     unsigned long long *n_votes;
     unsigned long long *n_evals;
-    // hit lists (MODE_LIST)
-    const uint32_t *flags;    // 1 bit per bin
-    const uint32_t *row_base; // [n_rows + 1]
-    const unsigned int *n_peaks_dev;
-    uint32_t cap_peaks;
-    uint2 *pairs;       // [pair_cap] (lin of the peak bin, hit index)
-    unsigned long long *n_pairs;
-    unsigned long long pair_cap;
 };
 
-template <int MODE, int PACK>
+template <int PACK>
 __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -46,18 +29,10 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const int nk = g.n_kappa;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nwarps = ge.threads >> 5;
-    const int wpr = nk >> 5; // flag words per cell row
 
-    // ---- carve shared memory
-    // VOTE: tile = masks [cells_pad][nk / PACK words];
-    // LIST: tile = flag words of the reported peaks [wpr][cells_pad]
+    // ---- carve shared memory: tile = masks [cells_pad][nk / PACK words], then staging
     uint32_t *tile = reinterpret_cast<uint32_t *>(smem_raw);
     unsigned char *ptr = smem_raw + (size_t)ge.tile_words * 4;
-    uint2 *pairbuf = nullptr;
-    if (MODE == MODE_LIST) {
-        pairbuf = reinterpret_cast<uint2 *>(ptr);
-        ptr += (size_t)PAIR_BUF * 8;
-    }
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
     ptr += (size_t)2 * 4 * ge.chunk * 4;
     float4 *surv = reinterpret_cast<float4 *>(ptr); // [chunk + EVAL_UNROLL]
@@ -65,9 +40,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
-    ptr += 32 * 4;
-    unsigned int *s_npairs = reinterpret_cast<unsigned int *>(ptr); // [0] count, [1..2] flush base
-    ptr += 16;
 
     // ---- which tile
     const int tp = blockIdx.x / ge.tiles_d0, td = blockIdx.x % ge.tiles_d0;
@@ -106,7 +78,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         mbar_init(&mbar[0], 1);
         mbar_init(&mbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        s_npairs[0] = 0u;
     }
     __syncthreads();
     auto issue = [&](uint32_t ch) {
@@ -122,50 +93,18 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     if (tid == 0 && n_chunks > 0)
         issue(0);
 
-    // LIST: linear index of bin 0 of this thread's cell
-    const uint32_t c_lin0 = cell_ok ? (uint32_t)(((size_t)(i0 + il) * g.n_d0 + (j0 + jl)) * nk) : 0u;
-    if (MODE == MODE_VOTE) {
-        // ---- clear the tile (a2, shared-memory part)
-        for (int w = tid; w < ge.tile_words; w += ge.threads)
-            tile[w] = 0u;
-    } else {
-        // ---- flag words of the reported peaks of every cell of the tile (peaks of global
-        // rank >= n_rep are not reported)
-        const uint32_t n_rep = min(*p.n_peaks_dev, p.cap_peaks);
-        uint32_t *ftile = tile;
-        for (int cc = tid; cc < ge.cells_pad; cc += ge.threads) {
-            const int cil = cc / ge.D, cjl = cc - cil * ge.D;
-            uint32_t gb = 0, nr = 0;
-            const uint32_t *fw = p.flags;
-            if (cil < ni && cjl < nj) {
-                size_t row = (size_t)(i0 + cil) * g.n_d0 + (j0 + cjl);
-                gb = p.row_base[row];
-                uint32_t cnt = p.row_base[row + 1] - gb;
-                nr = gb >= n_rep ? 0u : min(cnt, n_rep - gb);
-                fw += row * wpr;
-            }
-            uint32_t before = 0;
-            for (int w = 0; w < wpr; ++w) {
-                uint32_t f = nr ? fw[w] : 0u;
-                while (before + (uint32_t)__popc(f) > nr) // the capacity cuts inside this word
-                    f &= ~(0x80000000u >> __clz(f));
-                ftile[(size_t)w * ge.cells_pad + cc] = f;
-                before += (uint32_t)__popc(f);
-            }
-        }
-    }
+    // ---- clear the tile (a2, shared-memory part)
+    for (int w = tid; w < ge.tile_words; w += ge.threads)
+        tile[w] = 0u;
     __syncthreads();
 
     unsigned int my_votes = 0;
     unsigned long long tile_evals = 0; // thread 0: surviving hits x owned cells
     const int nkm1 = nk - 1;
-    // VOTE: byte address of this cell's row in the tile and its word swizzle (in bytes)
+    // byte address of this cell's row in the tile and its word swizzle (in bytes)
     const int row_words = PACK == 2 ? (nk >> 1) : nk;
     const uint32_t row_addr = smem_u32(tile) + (uint32_t)c * (uint32_t)row_words * 4u;
     const uint32_t swzb = (uint32_t)(lane & p.swz_mask) << 2;
-    // LIST: byte address of this cell's column in the flag tile; the prefix tile follows
-    const uint32_t col_addr = smem_u32(tile) + (uint32_t)c * 4u;
-    const uint32_t word_stride = (uint32_t)ge.cells_pad * 4u;
 
     for (uint32_t ch = 0; ch < n_chunks; ++ch) {
         const float *st = stage + (size_t)(ch & 1) * 4 * ge.chunk;
@@ -199,8 +138,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             }
             if (keep) {
                 int pos = total + before + __popc(bal & ((1u << lane) - 1u));
-                uint32_t payload = (MODE == MODE_VOTE) ? hb : (uint32_t)(ch * ge.chunk + hidx);
-                surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(payload));
+                surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(hb));
             }
             total += all;
             __syncthreads();
@@ -218,54 +156,19 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
                 if ((kappa >= klo) && (kappa < khi)) {
                     const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
-                    if (MODE == MODE_VOTE) {
-                        const uint32_t bit = __float_as_uint(hv.w);
-                        if (PACK == 2)
-                            smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
-                        else
-                            smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
-                        ++my_votes;
-                    } else {
-                        const uint32_t f = smem_ld(col_addr + (k >> 5) * word_stride);
-                        if ((f >> (k & 31u)) & 1u) {
-                            const uint2 pr = make_uint2(c_lin0 + k, __float_as_uint(hv.w));
-                            const unsigned int pos = atomicAdd(&s_npairs[0], 1u);
-                            if (pos < PAIR_BUF) {
-                                pairbuf[pos] = pr;
-                            } else { // buffer full inside one chunk: straight to global memory
-                                unsigned long long gpos = atomicAdd(p.n_pairs, 1ull);
-                                if (gpos < p.pair_cap)
-                                    p.pairs[gpos] = pr;
-                            }
-                        }
-                    }
+                    const uint32_t bit = __float_as_uint(hv.w);
+                    if (PACK == 2)
+                        smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
+                    else
+                        smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
+                    ++my_votes;
                 }
             }
         }
         __syncthreads(); // survivors and this stage buffer are free again
-
-        if (MODE == MODE_LIST) {
-            const unsigned int np = min(s_npairs[0], (unsigned int)PAIR_BUF);
-            if (np >= PAIR_FLUSH || (ch + 1 == n_chunks && np > 0)) {
-                if (tid == 0) {
-                    unsigned long long b = atomicAdd(p.n_pairs, (unsigned long long)np);
-                    s_npairs[1] = (unsigned int)b;
-                    s_npairs[2] = (unsigned int)(b >> 32);
-                }
-                __syncthreads();
-                const unsigned long long b = ((unsigned long long)s_npairs[2] << 32) | s_npairs[1];
-                for (unsigned int q = tid; q < np; q += ge.threads)
-                    if (b + q < p.pair_cap)
-                        p.pairs[b + q] = pairbuf[q];
-                __syncthreads();
-                if (tid == 0)
-                    s_npairs[0] = 0u;
-                // the next write to s_npairs[0] / pairbuf is behind the barriers of the next cull
-            }
-        }
     }
 
-    if (MODE == MODE_VOTE) {
+    {
         // ---- a4: write the tile out, kappa fastest, 16-byte stores
         if (PACK == 2) {
             const int W = nk >> 1;               // words per cell row
@@ -318,10 +221,8 @@ static int swizzle_mask_for(int row_words)
     return m;
 }
 
-// Tile geometry.  Vote tile: cells_pad rows of n_kappa masks, PACK masks per word.
-// List tile: the flag words of the reported peaks (1 word per 32 bins per cell) plus the
-// pair buffer.
-int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int list_mode)
+// Tile geometry: cells_pad rows of n_kappa masks, PACK masks per word, plus the staging.
+int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split)
 {
     const hough_config &cfg = h->cfg;
     ge->P = P;
@@ -334,13 +235,7 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     ge->tiles_phi = (cfg.n_phi + P - 1) / P;
     ge->tiles_d0 = (cfg.n_d0 + D - 1) / D;
     ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
-    size_t tile_bytes, extra = 0;
-    if (list_mode) {
-        tile_bytes = (size_t)(cfg.n_kappa / 32) * ge->cells_pad * 4;
-        extra = (size_t)PAIR_BUF * 8;
-    } else {
-        tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * 4 / h->g.pack;
-    }
+    const size_t tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * 4 / h->g.pack, extra = 0;
     ge->tile_words = (int)(tile_bytes / 4);
     size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);
@@ -370,27 +265,20 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
     p->n_evals = &h->counters->n_evals;
-    p->flags = h->flags;
-    p->row_base = h->row_base;
-    p->n_peaks_dev = &h->counters->n_peaks;
-    p->cap_peaks = h->cfg.cap_peaks;
-    p->pairs = h->pairs;
-    p->n_pairs = h->n_pairs;
-    p->pair_cap = h->cfg.cap_hits;
 }
 
-template <int MODE, int PACK>
+template <int PACK>
 static cudaError_t launch_one(const SweepParams &p, cudaStream_t st)
 {
-    static int configured_smem = -1; // per (MODE, PACK) instantiation
+    static int configured_smem = -1; // per PACK instantiation
     if (configured_smem < p.geom.smem_bytes) {
-        cudaError_t e = cudaFuncSetAttribute(k_sweep<MODE, PACK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(k_sweep<PACK>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              p.geom.smem_bytes);
         if (e != cudaSuccess)
             return e;
         configured_smem = p.geom.smem_bytes;
     }
-    k_sweep<MODE, PACK><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
+    k_sweep<PACK><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -399,14 +287,6 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     SweepParams p;
     fill_params(h, &p, h->vote_geom);
     h->launches += 1;
-    return h->g.pack == 2 ? launch_one<MODE_VOTE, 2>(p, st) : launch_one<MODE_VOTE, 1>(p, st);
+    return h->g.pack == 2 ? launch_one<2>(p, st) : launch_one<1>(p, st);
 }
 
-// One sweep: the (peak bin, hit) pairs.
-cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
-{
-    SweepParams p;
-    fill_params(h, &p, h->list_geom);
-    h->launches += 1;
-    return launch_one<MODE_LIST, 1>(p, st);
-}

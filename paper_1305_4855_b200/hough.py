@@ -21,7 +21,7 @@ HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3,
 TRUNCATED_PEAKS, TRUNCATED_HITS = 1, 2
 OPT_NO_CULL = 1
 OPT_STAGE_TIMING = 2
-N_STAGES = 10
+N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
 SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
