@@ -24,6 +24,7 @@
 
 #define LIST_QUEUE 64  // entries a warp buffers before it flushes (>= 2 * 32)
 #define LIST_ROUND 128 // CTA survivors a warp culls at a time
+#define LIST_CHUNK 256 // hits staged per TMA bulk copy (divides HOUGH_CHUNK)
 #define LIST_LQ 8      // pending votes per lane before the warp drains them
 
 struct ListSweepParams {
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
     // ---- which super-tile, which hit segment
     const int seg = blockIdx.x % S, tile_id = blockIdx.x / S;
     const int tp = tile_id / ge.tiles_d0, td = tile_id % ge.tiles_d0;
-    const uint32_t n_chunks = p.hits.n_pad / HOUGH_CHUNK;
+    const uint32_t n_chunks = p.hits.n_pad / LIST_CHUNK;
     const uint32_t ch0 = (uint32_t)(((unsigned long long)n_chunks * seg) / S);
     const uint32_t ch1 = (uint32_t)(((unsigned long long)n_chunks * (seg + 1)) / S);
     if (ch0 >= ch1)
@@ -92,9 +93,9 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
     uint32_t *wq = reinterpret_cast<uint32_t *>(wbase + ge.queue_off);
     unsigned char *ptr = smem_raw + (size_t)LIST_WARPS * ge.warp_bytes;
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
-    ptr += (size_t)2 * 4 * HOUGH_CHUNK * 4;
+    ptr += (size_t)2 * 4 * LIST_CHUNK * 4;
     float4 *surv = reinterpret_cast<float4 *>(ptr); // [chunk + 2]
-    ptr += (size_t)(HOUGH_CHUNK + 2) * 16;
+    ptr += (size_t)(LIST_CHUNK + 2) * 16;
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [LIST_WARPS]
@@ -147,17 +148,17 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    const uint32_t chunk_bytes = (uint32_t)HOUGH_CHUNK * 4;
+    const uint32_t chunk_bytes = (uint32_t)LIST_CHUNK * 4;
     auto issue = [&](uint32_t ch) { // buffer and parity follow (ch - ch0)
         const uint32_t q = ch - ch0;
-        float *dst = stage + (size_t)(q & 1) * 4 * HOUGH_CHUNK;
+        float *dst = stage + (size_t)(q & 1) * 4 * LIST_CHUNK;
         uint64_t *bar = &mbar[q & 1];
         mbar_expect_tx(bar, 4 * chunk_bytes);
-        size_t off = (size_t)ch * HOUGH_CHUNK;
+        size_t off = (size_t)ch * LIST_CHUNK;
         tma_load_1d(dst, p.hits.x + off, chunk_bytes, bar);
-        tma_load_1d(dst + HOUGH_CHUNK, p.hits.y + off, chunk_bytes, bar);
-        tma_load_1d(dst + 2 * HOUGH_CHUNK, p.hits.r2 + off, chunk_bytes, bar);
-        tma_load_1d(dst + 3 * HOUGH_CHUNK, p.hits.bit + off, chunk_bytes, bar);
+        tma_load_1d(dst + LIST_CHUNK, p.hits.y + off, chunk_bytes, bar);
+        tma_load_1d(dst + 2 * LIST_CHUNK, p.hits.r2 + off, chunk_bytes, bar);
+        tma_load_1d(dst + 3 * LIST_CHUNK, p.hits.bit + off, chunk_bytes, bar);
     };
     if (tid == 0)
         issue(ch0);
@@ -268,18 +269,22 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
 
     for (uint32_t ch = ch0; ch < ch1; ++ch) {
         const uint32_t q = ch - ch0;
-        const float *st = stage + (size_t)(q & 1) * 4 * HOUGH_CHUNK;
+        const float *st = stage + (size_t)(q & 1) * 4 * LIST_CHUNK;
         mbar_wait(&mbar[q & 1], (q >> 1) & 1);
         if (tid == 0 && ch + 1 < ch1)
             issue(ch + 1); // the other buffer was released by the barrier ending the previous chunk
 
         // ---- CTA-level cull against the super-tile, order-preserving compaction
         int total = 0;
-        for (int base = 0; base < HOUGH_CHUNK; base += 32 * LIST_WARPS) {
+        for (int base = 0; base < LIST_CHUNK; base += 32 * LIST_WARPS) {
             const int hidx = base + tid;
-            const float hx = st[hidx], hy = st[HOUGH_CHUNK + hidx], hr2 = st[2 * HOUGH_CHUNK + hidx];
-            const uint32_t hb = __float_as_uint(st[3 * HOUGH_CHUNK + hidx]);
-            const bool keep = (hb != 0u) && hit_may_vote(hx, hy, hr2, tc, g.kabs, g.d0_absmax);
+            float hx = 0.f, hy = 0.f, hr2 = 0.f;
+            bool keep = false;
+            if (hidx < LIST_CHUNK) {
+                hx = st[hidx], hy = st[LIST_CHUNK + hidx], hr2 = st[2 * LIST_CHUNK + hidx];
+                const uint32_t hb = __float_as_uint(st[3 * LIST_CHUNK + hidx]);
+                keep = (hb != 0u) && hit_may_vote(hx, hy, hr2, tc, g.kabs, g.d0_absmax);
+            }
             const unsigned bal = __ballot_sync(0xffffffffu, keep);
             if (lane == 0)
                 warp_cnt[warp] = __popc(bal);
@@ -293,7 +298,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
             }
             if (keep)
                 surv[total + before + __popc(bal & lt_mask)] =
-                    make_float4(hx, hy, hr2, __uint_as_float(ch * HOUGH_CHUNK + hidx));
+                    make_float4(hx, hy, hr2, __uint_as_float(ch * LIST_CHUNK + hidx));
             total += all;
             __syncthreads();
         }
@@ -455,7 +460,7 @@ int list_geom_init(hough_handle *h)
     ge->laneq_off = (ge->widx_off + (LIST_ROUND + 2) * 2 + 15) & ~15;
     ge->queue_off = ge->laneq_off + LIST_LQ * 32 * 4;
     ge->warp_bytes = (ge->queue_off + 3 * LIST_QUEUE * 4 + 127) & ~127;
-    ge->smem_bytes = LIST_WARPS * ge->warp_bytes + 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 2) * 16 + 16 +
+    ge->smem_bytes = LIST_WARPS * ge->warp_bytes + 2 * 4 * LIST_CHUNK * 4 + (LIST_CHUNK + 2) * 16 + 16 +
                      LIST_WARPS * 4 + 16;
     if (ge->smem_bytes > hough_vote_max_smem())
         return 0;
@@ -471,7 +476,7 @@ int list_geom_init(hough_handle *h)
         per_sm < 1)
         return 0;
     // segments: whole chunks, at most 65535 hits each (u16 counters), bounded sub-list table
-    const uint32_t n_chunks_max = (h->max_hits_pad + HOUGH_CHUNK - 1) / HOUGH_CHUNK;
+    const uint32_t n_chunks_max = (h->max_hits_pad + LIST_CHUNK - 1) / LIST_CHUNK;
     const int s_min = list_segments_min(&c), s_bound = list_segments_bound(&c);
     int s_max = s_bound;
     if ((uint32_t)s_max > n_chunks_max)
