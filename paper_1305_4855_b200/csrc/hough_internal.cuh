@@ -36,7 +36,6 @@ struct ListGeom {
     int tiles_phi, tiles_d0;
     int S;               // hit segments (sub-lists per peak)
     int max_pk;          // bound on the peaks of one sub-tile
-    int widx_off, laneq_off, queue_off; // byte offsets inside the warp's shared-memory block
     int warp_bytes;      // shared memory per warp
     int smem_bytes;      // dynamic shared memory of the kernel
     int no_phi_cull_tile, no_phi_cull_sub;

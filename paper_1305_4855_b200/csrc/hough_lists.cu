@@ -58,13 +58,33 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
-// Per-warp shared-memory block (byte offsets; wpr = n_kappa / 32):
-//   flags   [wpr][32] u32   flag words of the reported peaks of the warp's cells
-//   prefix  [wpr][32] u16   reported peaks of the cell below each word
-//   count   [max_pk]  u16   entries handed out so far, per local peak id
+// Per-warp shared-memory block; the fixed-size parts come first so that the hot loop
+// addresses them with immediates off one register (wpr = n_kappa / 32):
 //   widx    [LIST_ROUND + 2] u16   survivors of the warp-level cull (indices into surv)
 //   laneq   [LIST_LQ][32] u32      per lane: pending (kappa bin << 10 | surv index)
 //   flushq  [3][LIST_QUEUE] u32    finished entries on their way to global memory
+//   flags   [wpr][32] u32   flag words of the reported peaks of the warp's cells
+//   prefix  [wpr][32] u16   reported peaks of the cell below each word
+//   count   [max_pk]  u16   entries handed out so far, per local peak id
+#define OFF_WIDX 0
+#define OFF_LANEQ 384
+#define OFF_FLUSHQ (OFF_LANEQ + LIST_LQ * 128)
+#define OFF_FLAGS (OFF_FLUSHQ + 3 * LIST_QUEUE * 4)
+static_assert((LIST_ROUND + 2) * 2 <= OFF_LANEQ && OFF_FLAGS % 128 == 0, "per-warp block layout");
+
+template <int OFF>
+__device__ __forceinline__ uint32_t lds_off(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFF));
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
 __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -85,12 +105,11 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
 
     // ---- carve shared memory
     unsigned char *wbase = smem_raw + (size_t)warp * ge.warp_bytes;
-    uint32_t *wflags = reinterpret_cast<uint32_t *>(wbase);
-    unsigned short *wpre = reinterpret_cast<unsigned short *>(wbase + (size_t)wpr * 128);
+    unsigned short *widx = reinterpret_cast<unsigned short *>(wbase + OFF_WIDX);
+    uint32_t *wq = reinterpret_cast<uint32_t *>(wbase + OFF_FLUSHQ);
+    uint32_t *wflags = reinterpret_cast<uint32_t *>(wbase + OFF_FLAGS);
+    unsigned short *wpre = reinterpret_cast<unsigned short *>(wbase + OFF_FLAGS + (size_t)wpr * 128);
     unsigned short *wcnt = wpre + (size_t)wpr * 32;
-    unsigned short *widx = reinterpret_cast<unsigned short *>(wbase + ge.widx_off);
-    uint32_t *laneq = reinterpret_cast<uint32_t *>(wbase + ge.laneq_off);
-    uint32_t *wq = reinterpret_cast<uint32_t *>(wbase + ge.queue_off);
     unsigned char *ptr = smem_raw + (size_t)LIST_WARPS * ge.warp_bytes;
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
     ptr += (size_t)2 * 4 * LIST_CHUNK * 4;
@@ -200,15 +219,16 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
     __syncwarp();
 
     const int nkm1 = nk - 1;
-    const uint32_t fl_addr = smem_u32(wflags) + (uint32_t)lane * 4u;  // + (k >> 5) * 128
+    const uint32_t wb = smem_u32(wbase);                              // the warp's block
+    const uint32_t wl4 = wb + (uint32_t)lane * 4u;                    // this lane's column in it
+    const uint32_t sv = smem_u32(surv);
     const uint32_t pre_addr = smem_u32(wpre) + (uint32_t)lane * 2u;   // + (k >> 5) * 64
     const uint32_t cnt_addr = smem_u32(wcnt) + c_lbase * 2u;          // + rank * 2
-    const uint32_t lq_addr = smem_u32(laneq) + (uint32_t)lane * 4u;   // + e * 128
     const uint32_t sub0 = c_gbase * (uint32_t)S + (uint32_t)seg;      // + rank * S
     uint32_t *q_sub = wq, *q_hit = wq + LIST_QUEUE, *q_idx = wq + 2 * LIST_QUEUE;
     const uint32_t lt_mask = (1u << lane) - 1u;
     uint32_t qn = 0; // entries waiting in this warp's flush queue (warp-uniform)
-    uint32_t nl = 0; // entries waiting in this lane's queue
+    uint32_t lqp = wl4; // + OFF_LANEQ: next free slot of this lane's queue (128 bytes apart)
 
     auto flush = [&]() {
         __syncwarp();
@@ -229,15 +249,16 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
     // Every lane turns its pending votes into entries, oldest first: rank of the bin among
     // the cell's reported peaks -> local peak id -> its counter (the place in the sub-list).
     auto drain = [&]() {
+        const uint32_t nl = (lqp - wl4) >> 7;
         for (uint32_t e = 0;; ++e) {
             const bool act = e < nl;
             const unsigned bh = __ballot_sync(0xffffffffu, act);
             if (!bh)
                 break;
             if (act) {
-                const uint32_t ent = smem_ld(lq_addr + e * 128u);
+                const uint32_t ent = lds_off<OFF_LANEQ>(wl4 + e * 128u);
                 const uint32_t k = ent >> 10;
-                const uint32_t f = smem_ld(fl_addr + (k >> 5) * 128u);
+                const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
                 const uint32_t rank = lds_u16(pre_addr + (k >> 5) * 64u) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
                 const uint32_t ca = cnt_addr + rank * 2u;
                 const unsigned short n = lds_u16(ca);
@@ -251,7 +272,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
             if (qn > LIST_QUEUE - 32)
                 flush();
         }
-        nl = 0;
+        lqp = wl4;
     };
 
     // one hit against the warp's 32 cells: exact recipe, then the peak test of the bin
@@ -259,10 +280,10 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
         const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
         if ((kappa >= klo) && (kappa < khi)) {
             const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
-            const uint32_t f = smem_ld(fl_addr + (k >> 5) * 128u);
+            const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
             if ((f >> (k & 31u)) & 1u) {
-                sts_u32(lq_addr + nl * 128u, (k << 10) | sidx);
-                ++nl;
+                asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(lqp), "n"(OFF_LANEQ), "r"((k << 10) | sidx) : "memory");
+                lqp += 128u;
             }
         }
     };
@@ -327,14 +348,13 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
                     widx[nw] = (unsigned short)total; // pad to an even count with the non-voting entry
                 __syncwarp();
                 // ---- lane = cell: the exact recipe on the survivors, two at a time
-                const uint32_t *wpair = reinterpret_cast<const uint32_t *>(widx);
                 for (int t = 0; t < nw; t += 2) {
-                    const uint32_t two = wpair[t >> 1];
+                    const uint32_t two = lds_off<OFF_WIDX>((wl4 & ~127u) + (uint32_t)t * 2u); // the block is 128-byte aligned
                     const uint32_t a = two & 0xffffu, b = two >> 16;
-                    const float4 h0 = surv[a], h1 = surv[b];
+                    const float4 h0 = lds_f4(sv + a * 16u), h1 = lds_f4(sv + b * 16u);
                     process(h0, a);
                     process(h1, b);
-                    if (__any_sync(0xffffffffu, nl > LIST_LQ - 2))
+                    if (__any_sync(0xffffffffu, lqp > wl4 + (LIST_LQ - 2) * 128u))
                         drain();
                 }
                 __syncwarp();
@@ -456,10 +476,7 @@ int list_geom_init(hough_handle *h)
     ge->tiles_d0 = (c.n_d0 + ge->WD * ge->SD - 1) / (ge->WD * ge->SD);
     const int wpr = c.n_kappa / 32;
     ge->max_pk = ((ge->SP + 1) / 2) * ((ge->SD + 1) / 2) * ((c.n_kappa + 1) / 2);
-    ge->widx_off = (wpr * 192 + ge->max_pk * 2 + 15) & ~15;
-    ge->laneq_off = (ge->widx_off + (LIST_ROUND + 2) * 2 + 15) & ~15;
-    ge->queue_off = ge->laneq_off + LIST_LQ * 32 * 4;
-    ge->warp_bytes = (ge->queue_off + 3 * LIST_QUEUE * 4 + 127) & ~127;
+    ge->warp_bytes = (OFF_FLAGS + wpr * 192 + ge->max_pk * 2 + 127) & ~127;
     ge->smem_bytes = LIST_WARPS * ge->warp_bytes + 2 * 4 * LIST_CHUNK * 4 + (LIST_CHUNK + 2) * 16 + 16 +
                      LIST_WARPS * 4 + 16;
     if (ge->smem_bytes > hough_vote_max_smem())
