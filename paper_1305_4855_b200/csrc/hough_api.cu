@@ -116,7 +116,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     uint32_t hp = pad_hits(c->max_hits);
     uint32_t sb = (uint32_t)((n_rows + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
     const size_t n_sub = (size_t)c->cap_peaks * (size_t)list_segments_bound(c);
-    uint32_t sb2 = (uint32_t)((n_sub + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
+    uint32_t sb2 = (uint32_t)(((size_t)c->cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
     if (sb2 > sb)
         sb = sb2;
     sb += 1;
@@ -130,7 +130,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *flags = cv.take(n_bins / 8);
     void *row_base = cv.take((n_rows + 1) * 4);
     void *list_len = cv.take(n_sub * 4);
-    void *sub_off = cv.take((n_sub + 1) * 8);
+    void *peak_len = cv.take((size_t)c->cap_peaks * 4);
     void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
@@ -153,7 +153,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->flags = (uint32_t *)flags;
         h->row_base = (uint32_t *)row_base;
         h->list_len = (uint32_t *)list_len;
-        h->sub_off = (unsigned long long *)sub_off;
+        h->peak_len = (uint32_t *)peak_len;
         h->ent_sub = (uint32_t *)ent_sub;
         h->ent_hit = (uint32_t *)ent_hit;
         h->ent_idx = (uint32_t *)ent_idx;
@@ -425,7 +425,6 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
-        CK(cudaMemsetAsync(h->list_len, 0, (size_t)h->cfg.cap_peaks * h->list_geom.S * 4, st));
         CK(launch_list_sweep(h, st));
         stage_mark(h, ST_LIST_SWEEP + 1, st);
         CK(launch_scan_lens(h, out, st));

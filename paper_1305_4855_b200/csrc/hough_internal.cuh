@@ -94,8 +94,8 @@ struct hough_handle {
     uint32_t max_hits_pad;
     uint32_t *flags;      // 1 bit per bin
     uint32_t *row_base;   // [n_rows + 1] exclusive scan of peaks per (i, j) row
-    uint32_t *list_len;   // [cap_peaks * S_max] length of sub-list (peak, segment)
-    unsigned long long *sub_off; // [cap_peaks * S_max + 1] its exclusive scan
+    uint32_t *list_len;   // [cap_peaks * S_max] length of sub-list (peak, segment), then its start in the peak's list
+    uint32_t *peak_len;   // [cap_peaks] list length per peak
     uint32_t *ent_sub, *ent_hit, *ent_idx; // [cap_hits] entries (sub-list, hit, place) of the list sweep
     unsigned long long *n_pairs; // entries emitted (lives in the per-hough_peaks reset region)
     unsigned long long *scan_status; // look-back words of the chained scans

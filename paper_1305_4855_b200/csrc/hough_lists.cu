@@ -11,9 +11,10 @@
 //   * the event's hits are cut into S segments (whole staged chunks); CTA = (super-tile of
 //     LIST_WARPS sub-tiles, segment).  Sub-list (peak p, segment s) has the id p*S + s; the
 //     concatenation of a peak's sub-lists in segment order is its ascending list;
-//   * sub_len[p*S + s] is written at the end of the CTA, k_scan<LENS> turns it into
-//     sub_off (and hit_offset[p] = sub_off[p*S]), k_scatter_entries drops entry
-//     (sub, hit, idx) at hit_index[sub_off[sub] + idx].  No sort, no atomics on the lists.
+//   * sub_len[p*S + s] is written at the end of the CTA; k_scan<LENS> sums a peak's S
+//     lengths into hit_offset and leaves their exclusive prefix in sub_len;
+//     k_scatter_entries drops entry (sub, hit, idx) at
+//     hit_index[hit_offset[sub / S] + sub_len[sub] + idx].  No sort, no atomics on the lists.
 // The hits are culled twice with the conservative interval test of DESIGN.md section 4.3:
 // per CTA against the super-tile (lane = hit, order-preserving compaction) and per warp
 // against its sub-tile (lane = hit, ballot), then the exact recipe runs on the survivors.
@@ -380,7 +381,8 @@ struct ListPlaceParams {
     const unsigned long long *n_entries;
     unsigned long long ent_cap;
     const uint32_t *ent_sub, *ent_hit, *ent_idx;
-    const unsigned long long *sub_off;
+    const uint32_t *sub_pre; // [n_rep * S] start of every sub-list inside its peak's list
+    uint32_t S;
     const DevCounters *counters;
     uint32_t cap_peaks;
     const uint32_t *bin;
@@ -396,7 +398,8 @@ __global__ void __launch_bounds__(256) k_scatter_entries(const ListPlaceParams p
         return; // k_list_slow takes over
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const unsigned long long pos = p.sub_off[p.ent_sub[i]] + p.ent_idx[i];
+        const uint32_t sub = p.ent_sub[i];
+        const unsigned long long pos = p.hit_offset[sub / p.S] + p.sub_pre[sub] + p.ent_idx[i];
         if (pos < p.cap_hits)
             p.hit_index[pos] = p.ent_hit[i];
     }
@@ -505,7 +508,7 @@ int list_geom_init(hough_handle *h)
     for (int s = s_min; s <= s_max; ++s) {
         const double r = tiles * s / slots;
         const double eff = r / ceil(r);
-        const double score = eff - 0.002 * s; // prefer fewer segments when the fill is equal
+        const double score = eff - 0.004 * s; // prefer fewer segments when the fill is equal
         if (score > best_score) {
             best_score = score;
             best = s;
@@ -516,6 +519,16 @@ int list_geom_init(hough_handle *h)
     if (e && atoi(e) >= s_min && atoi(e) <= s_bound)
         ge->S = atoi(e);
     return 1;
+}
+
+// sub_len[0 .. n_rep * S) = 0 (only the part this event uses)
+__global__ void __launch_bounds__(256) k_zero_sub_len(uint32_t *sub_len, const DevCounters *counters,
+                                                      uint32_t cap_peaks, uint32_t S)
+{
+    const size_t n = (size_t)min(counters->n_peaks, cap_peaks) * S;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        sub_len[i] = 0u;
 }
 
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
@@ -540,9 +553,11 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
     p.ent_idx = h->ent_idx;
     p.n_entries = h->n_pairs;
     p.ent_cap = h->cfg.cap_hits;
-    h->launches += 1;
+    k_zero_sub_len<<<h->n_sms * 8, 256, 0, st>>>(h->list_len, h->counters, h->cfg.cap_peaks,
+                                                 (uint32_t)h->list_geom.S);
+    h->launches += 2;
     if (p.hits.n_pad == 0)
-        return cudaSuccess;
+        return cudaGetLastError();
     const int blocks = h->list_geom.tiles_phi * h->list_geom.tiles_d0 * h->list_geom.S;
     k_list_sweep<<<blocks, 32 * LIST_WARPS, h->list_geom.smem_bytes, st>>>(p);
     return cudaGetLastError();
@@ -562,7 +577,8 @@ cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cuda
     p.ent_sub = h->ent_sub;
     p.ent_hit = h->ent_hit;
     p.ent_idx = h->ent_idx;
-    p.sub_off = h->sub_off;
+    p.sub_pre = h->list_len;
+    p.S = (uint32_t)h->list_geom.S;
     p.counters = h->counters;
     p.cap_peaks = h->cfg.cap_peaks;
     p.bin = out->bin;

@@ -259,8 +259,8 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
 // (flag << 62) | value, flag 1 = aggregate, 2 = inclusive prefix; written with one
 // 64-bit store so that no fence is needed between flag and value.
 //   SCAN_ROWS : item i = number of flag bits of accumulator row i  -> row_base (u32)
-//   SCAN_LENS : item i = length of sub-list i = peak*S + segment, i < min(n_peaks, cap_peaks)*S
-//               -> sub_off (u64); hit_offset[peak] = sub_off[peak*S]
+//   SCAN_LENS : item i = peak_len[i] = length of peak i's list (k_sub_prefix),
+//               i < min(n_peaks, cap_peaks)  -> hit_offset (u64)
 #define SCAN_ROWS 0
 #define SCAN_LENS 1
 #define SCAN_THREADS 256
@@ -271,10 +271,9 @@ struct ScanParams {
     int fw_per_row;
     uint32_t n_rows;
     uint32_t *row_base;
-    const uint32_t *list_len;
+    const uint32_t *list_len; // LENS: peak_len
     uint32_t cap_peaks;
     unsigned long long *hit_offset;
-    unsigned long long *sub_off;
     uint32_t S;
     unsigned long long cap_hits;
     DevCounters *counters;
@@ -293,7 +292,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
         s_ticket = atomicAdd(p.ticket, 1u);
     __syncthreads();
     const unsigned int t = s_ticket;
-    const uint32_t n = KIND == SCAN_ROWS ? p.n_rows : min(p.counters->n_peaks, p.cap_peaks) * p.S;
+    const uint32_t n = KIND == SCAN_ROWS ? p.n_rows : min(p.counters->n_peaks, p.cap_peaks);
     const unsigned long long base = (unsigned long long)t * HOUGH_SCAN_ITEMS;
     if (n == 0) {
         if (t == 0 && tid == 0) {
@@ -378,9 +377,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
             if (KIND == SCAN_ROWS) {
                 p.row_base[i] = (uint32_t)run;
             } else {
-                p.sub_off[i] = run;
-                if (i % p.S == 0)
-                    p.hit_offset[i / p.S] = run;
+                p.hit_offset[i] = run;
             }
             run += v[q];
             if (i == (unsigned long long)n - 1) { // the last item closes the scan
@@ -388,8 +385,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
                     p.row_base[n] = (uint32_t)run;
                     p.counters->n_peaks = (unsigned int)run;
                 } else {
-                    p.sub_off[n] = run;
-                    p.hit_offset[n / p.S] = run;
+                    p.hit_offset[n] = run;
                     p.counters->n_hit_entries = run;
                 }
             }
@@ -403,10 +399,9 @@ static void scan_params(hough_handle *h, ScanParams *p, const hough_peaks_out *o
     p->fw_per_row = h->g.n_kappa >> 5;
     p->n_rows = (uint32_t)h->g.n_phi * (uint32_t)h->g.n_d0;
     p->row_base = h->row_base;
-    p->list_len = h->list_len;
+    p->list_len = h->peak_len;
     p->cap_peaks = h->cfg.cap_peaks;
     p->hit_offset = out ? reinterpret_cast<unsigned long long *>(out->hit_offset) : nullptr;
-    p->sub_off = h->sub_off;
     p->S = (uint32_t)h->list_geom.S;
     p->cap_hits = h->cfg.cap_hits;
     p->counters = h->counters;
@@ -424,11 +419,47 @@ cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// A peak's list is the concatenation of its S sub-lists (hough_lists.cu): replace the S
+// lengths sub_len[p*S .. p*S+S) by their exclusive prefix and put the sum in peak_len[p].
+// 256 peaks per block, staged through shared memory so that global traffic is coalesced.
+__global__ void __launch_bounds__(256) k_sub_prefix(uint32_t *sub_len, uint32_t *peak_len,
+                                                    const DevCounters *counters, uint32_t cap_peaks, uint32_t S)
+{
+    extern __shared__ uint32_t sp[]; // [256][S + 1]
+    const uint32_t n = min(counters->n_peaks, cap_peaks);
+    const uint32_t p0 = blockIdx.x * 256u;
+    if (p0 >= n)
+        return;
+    const uint32_t np = min(256u, n - p0), words = np * S;
+    uint32_t *g = sub_len + (size_t)p0 * S;
+    for (uint32_t w = threadIdx.x; w < words; w += 256u)
+        sp[(w / S) * (S + 1) + (w % S)] = g[w];
+    __syncthreads();
+    if (threadIdx.x < np) {
+        uint32_t *row = sp + threadIdx.x * (S + 1), run = 0;
+        for (uint32_t s = 0; s < S; ++s) {
+            const uint32_t len = row[s];
+            row[s] = run;
+            run += len;
+        }
+        peak_len[p0 + threadIdx.x] = run;
+    }
+    __syncthreads();
+    for (uint32_t w = threadIdx.x; w < words; w += 256u)
+        g[w] = sp[(w / S) * (S + 1) + (w % S)];
+}
+
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
 {
+    {
+        const uint32_t S = (uint32_t)h->list_geom.S;
+        k_sub_prefix<<<(h->cfg.cap_peaks + 255) / 256, 256, 256 * (S + 1) * 4, st>>>(
+            h->list_len, h->peak_len, h->counters, h->cfg.cap_peaks, S);
+        h->launches += 1;
+    }
     ScanParams p;
     scan_params(h, &p, out, 1);
-    uint32_t blocks = (uint32_t)(((size_t)h->cfg.cap_peaks * h->list_geom.S + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS);
+    uint32_t blocks = (h->cfg.cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS;
     k_scan<SCAN_LENS><<<blocks, SCAN_THREADS, 0, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
