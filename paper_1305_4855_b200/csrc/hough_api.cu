@@ -219,9 +219,10 @@ static int choose_geometry(hough_handle *h)
         }
         while (split > 1 && 32 * groups * split > 1024)
             --split;
-        if (!sweep_geom_init(h, &h->vote_geom, P, D, split)) {
+        const int fit = (c.tile_phi == 0 && env_int("HOUGH_TILE_PHI", 0) == 0 && env_int("HOUGH_FIT_WAVES", 1)) ? 1 : 0;
+        if (!sweep_geom_init(h, &h->vote_geom, P, D, split, fit)) {
             // fall back to the smallest tile
-            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4))
+            if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 0))
                 return 0;
         }
     }

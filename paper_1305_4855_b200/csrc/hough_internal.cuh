@@ -22,6 +22,7 @@ struct SweepGeom {
     int threads;         // 32 * groups * split
     int chunk;           // hits staged per TMA bulk copy
     int tiles_phi, tiles_d0, n_tiles;
+    int n_big, P_small;  // the first n_big phi0 slabs are P rows high, the rest P_small
     int tile_words;      // 32-bit words of the bin tile in shared memory
     int smem_bytes;      // dynamic shared memory of the kernel
     int no_phi_cull;     // tile spans too wide an angle for the interval test
@@ -136,7 +137,7 @@ cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cuda
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st);
 
-int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split);
+int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split, int fit_waves);
 int list_geom_init(hough_handle *h);
 int list_segments_bound(const hough_config *c);
 int hough_vote_max_smem(void);

@@ -333,7 +333,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
                 // ---- warp-level cull against the sub-tile (lane = hit) -> widx[0 .. nw)
                 int nw = 0;
 #pragma unroll
-                for (int r = 0; r < LIST_ROUND / 32; ++r) {
+                for (int r = 0; r < LIST_ROUND / 32 && base + r * 32 < total; ++r) {
                     const int idx = base + r * 32 + lane;
                     bool kw = false;
                     if (idx < total) {

@@ -41,13 +41,17 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
 
-    // ---- which tile
+    // ---- which tile: the first n_big phi0 slabs are P rows high, the others P_small
+    // (two heights so that the CTAs fill whole waves)
     const int tp = blockIdx.x / ge.tiles_d0, td = blockIdx.x % ge.tiles_d0;
-    const int i0 = tp * ge.P, j0 = td * ge.D;
-    const int ni = min(ge.P, g.n_phi - i0), nj = min(ge.D, g.n_d0 - j0);
+    const int Pt = tp < ge.n_big ? ge.P : ge.P_small;
+    const int i0 = tp < ge.n_big ? tp * ge.P : ge.n_big * ge.P + (tp - ge.n_big) * ge.P_small;
+    const int j0 = td * ge.D;
+    const int ni = min(Pt, g.n_phi - i0), nj = min(ge.D, g.n_d0 - j0);
 
-    // ---- this thread's cell and its constants (registers)
-    const int grp = warp % ge.groups, set = warp / ge.groups;
+    // ---- this thread's cell and its constants (registers); warps beyond groups * split idle
+    const int groups = (Pt * ge.D + 31) >> 5, split = nwarps / groups;
+    const int grp = warp % groups, set = warp / groups;
     const int c = grp * 32 + lane;
     const int il = c / ge.D, jl = c - il * ge.D;
     const bool cell_ok = (il < ni) && (jl < nj);
@@ -70,6 +74,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     tc.dhi = g.d0c[j0 + nj - 1];
     tc.phi_all = ge.no_phi_cull;
     tc.off = p.no_cull;
+    const bool warp_ok = set < split;
 
     const uint32_t n_chunks = p.hits.n_pad / ge.chunk;
     const uint32_t chunk_bytes = (uint32_t)ge.chunk * 4;
@@ -148,20 +153,22 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             surv[total + tid] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
         __syncthreads();
 
-        // ---- evaluate: lane = cell, the warp walks the survivors
-        for (int hs = set * EVAL_UNROLL; hs < total; hs += ge.split * EVAL_UNROLL) {
+        // ---- evaluate: lane = cell, the `split` warps of a cell group interleave the survivors
+        if (warp_ok) {
+            for (int hs = set * EVAL_UNROLL; hs < total; hs += split * EVAL_UNROLL) {
 #pragma unroll
-            for (int u = 0; u < EVAL_UNROLL; ++u) {
-                const float4 hv = surv[hs + u];
-                const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-                if ((kappa >= klo) && (kappa < khi)) {
-                    const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
-                    const uint32_t bit = __float_as_uint(hv.w);
-                    if (PACK == 2)
-                        smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
-                    else
-                        smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
-                    ++my_votes;
+                for (int u = 0; u < EVAL_UNROLL; ++u) {
+                    const float4 hv = surv[hs + u];
+                    const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+                    if ((kappa >= klo) && (kappa < khi)) {
+                        const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
+                        const uint32_t bit = __float_as_uint(hv.w);
+                        if (PACK == 2)
+                            smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
+                        else
+                            smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
+                        ++my_votes;
+                    }
                 }
             }
         }
@@ -172,7 +179,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         // ---- a4: write the tile out, kappa fastest, 16-byte stores
         if (PACK == 2) {
             const int W = nk >> 1;               // words per cell row
-            const int pairs = (ge.P * ge.D) * (W >> 1);
+            const int pairs = (Pt * ge.D) * (W >> 1);
             for (int q = tid; q < pairs; q += ge.threads) {
                 int cc = q / (W >> 1), kw = (q - cc * (W >> 1)) << 1;
                 int cil = cc / ge.D, cjl = cc - cil * ge.D;
@@ -187,7 +194,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             }
         } else {
             const int W = nk;
-            const int quads = (ge.P * ge.D) * (W >> 2);
+            const int quads = (Pt * ge.D) * (W >> 2);
             for (int q = tid; q < quads; q += ge.threads) {
                 int cc = q / (W >> 2), kw = (q - cc * (W >> 2)) << 2;
                 int cil = cc / ge.D, cjl = cc - cil * ge.D;
@@ -222,7 +229,7 @@ static int swizzle_mask_for(int row_words)
 }
 
 // Tile geometry: cells_pad rows of n_kappa masks, PACK masks per word, plus the staging.
-int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split)
+int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int fit_waves)
 {
     const hough_config &cfg = h->cfg;
     ge->P = P;
@@ -246,6 +253,48 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
         return 0;
     if (tile_bytes + extra + stage > (size_t)hough_vote_max_smem())
         return 0;
+    ge->n_big = ge->tiles_phi;
+    ge->P_small = P;
+    // Two slab heights: n_big slabs of P rows first, then slabs of P - (one cell group) rows,
+    // chosen so that the CTAs fill whole waves (cost model: a wave takes as long as its
+    // highest tile).
+    const int step = (D <= 32 && 32 % D == 0) ? 32 / D : 0;
+    if (fit_waves && step > 0 && P % step == 0 && P - step >= step) {
+        int per_sm = 0;
+        cudaError_t e = h->g.pack == 2
+                            ? cudaFuncSetAttribute(k_sweep<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes)
+                            : cudaFuncSetAttribute(k_sweep<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes);
+        if (e == cudaSuccess)
+            e = h->g.pack == 2
+                    ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<2>, ge->threads, ge->smem_bytes)
+                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<1>, ge->threads, ge->smem_bytes);
+        if (e != cudaSuccess || per_sm < 1) {
+            cudaGetLastError();
+            return 1;
+        }
+        const long long slots = (long long)h->n_sms * per_sm, T = ge->tiles_d0;
+        const int Ps = P - step, n_phi = cfg.n_phi;
+        const int ns_min = (n_phi + P - 1) / P, ns_max = (n_phi + Ps - 1) / Ps;
+        long long best_cost = (long long)P * ((ns_min * T + slots - 1) / slots);
+        for (int ns = ns_min + 1; ns <= ns_max; ++ns) {
+            int a = (n_phi - ns * Ps + step - 1) / step;
+            if (n_phi - ns * Ps <= 0)
+                a = 0;
+            if (a > ns)
+                continue;
+            if (ns > a && (long long)a * P + (long long)(ns - a - 1) * Ps >= n_phi)
+                continue; // the last slab would be empty
+            const long long w_big = (a * T + slots - 1) / slots, w_all = (ns * T + slots - 1) / slots;
+            const long long cost = P * w_big + Ps * (w_all - w_big);
+            if (cost < best_cost) {
+                best_cost = cost;
+                ge->tiles_phi = ns;
+                ge->n_big = a;
+                ge->P_small = Ps;
+            }
+        }
+        ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
+    }
     return 1;
 }
 
