@@ -106,6 +106,35 @@ class ClockSampler:
                 "power_w_max": float(max(power)), "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def shard_seeds(rank, n_ev):
+    """Weak scaling: rank r takes seeds r*E .. r*E+E-1 of the same event recipe (no exchange)."""
+    return [rank * n_ev + s for s in range(n_ev)]
+
+
+def aggregate(dist, dev, total_ms, votes_step, evals_step, n_ev, world):
+    """(max-over-ranks time, summed votes, summed evaluations, summed events) -- the only
+    collectives of the job, outside the timed region."""
+    if world <= 1:
+        return float(total_ms), float(votes_step), float(evals_step), float(n_ev)
+    import torch
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    v = torch.tensor([votes_step, evals_step, n_ev], dtype=torch.float64, device=dev)
+    dist.all_reduce(v, op=dist.ReduceOp.SUM)
+    votes_all, evals_all, events_all = [float(a) for a in v.tolist()]
+    return float(t.item()), votes_all, evals_all, events_all
+
+
+def ncu_traffic(kernel_key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel, from the committed
+    `ncu --set full` summary (profiles/ncu_traffic.json), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f).get(kernel_key)
+
+
 def oracle_module():
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     try:
@@ -191,7 +220,7 @@ def main():
 
     # ---- inputs: this rank's events (weak scaling: rank r takes seeds r*E .. r*E+E-1)
     n_ev = args.events if args.events > 0 else len(workload.seeds)
-    seeds = [rank * n_ev + s for s in range(n_ev)]
+    seeds = shard_seeds(rank, n_ev)
     events = [synth.generate_event(workload.event, s)[:3] for s in seeds]
     max_hits = max(len(e[0]) for e in events)
     d_events = [tuple(torch.from_numpy(a).to(dev) for a in e) for e in events]
@@ -243,15 +272,8 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     launches = h.launch_count() - launches0
     total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        v = torch.tensor([votes_step, evals_step, n_ev], dtype=torch.float64, device=dev)
-        dist.all_reduce(v, op=dist.ReduceOp.SUM)
-        votes_all, evals_all, events_all = [float(a) for a in v.tolist()]
-    else:
-        votes_all, evals_all, events_all = float(votes_step), float(evals_step), float(n_ev)
+    total_ms, votes_all, evals_all, events_all = aggregate(dist, dev, total_ms, votes_step, evals_step,
+                                                           n_ev, world)
     secs = total_ms * 1e-3
     value = votes_all * args.steps / secs
 
@@ -346,8 +368,8 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
     alu_peak = n_sms * 128 * peaks_info["sm_max_mhz"] * 1e6 / 1e12  # fp32 lanes x clock, no FMA
     achieved = FLOP_PER_EVAL * (evals_step / n_ev) / vote_s / 1e12
     out["roofline"] = {
-        "kernel": "k_sweep<MODE_VOTE>", "bound": "alu", "achieved": achieved, "peak": alu_peak,
-        "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": None,
+        "kernel": "k_sweep (vote)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": ncu_traffic("vote"),
         "note": "algorithmic fp32 ops = 15 x n x n_phi x n_d0 per launch (every hit x cell); the "
                 "conservative cull executes only executed_frac of them; peak = SMs x 128 fp32 "
                 "lanes x sm_max_mhz without FMA (the recipe forbids contraction); "
@@ -397,7 +419,8 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
         "kernel": "k_peak_sweep", "workload": "finegrid (512 MiB accumulator, L2 flushed)",
         "bound": "hbm", "achieved": nbytes / t_sweep / 1e9, "peak": hbm, "unit": "GB/s",
         "frac": nbytes / t_sweep / 1e9 / hbm, "frac_of_8TBs_nominal": nbytes / t_sweep / 8e12,
-        "traffic": None, "note": "algorithmic bytes = 4 B/bin read once; " + peaks_info["source"]}
+        "traffic": ncu_traffic("peak_sweep_finegrid"),
+        "note": "algorithmic bytes = 4 B/bin read once; " + peaks_info["source"]}
     out["roofline_clear"] = {
         "kernel": "k_clear", "bound": "hbm", "achieved": nbytes / t_clear / 1e9, "peak": hbm,
         "unit": "GB/s", "frac": nbytes / t_clear / 1e9 / hbm, "traffic": None}

@@ -239,3 +239,58 @@ def test_process_host_matches_device_path(hough, oracle):
     res["acc"] = h.accumulator_host().copy()
     h.close()
     assert_same(res, ref)
+
+
+def test_batch_events_back_to_back_on_one_handle(hough, oracle):
+    """BASELINE.json configs[3]: events shaped like "pileup", one handle, one stream, each with
+    its own accumulator -- the second and third event must not see anything of the first.
+    (bench.py times all 100 seeds; the oracle needs ~10 s per event, so three are compared.)"""
+    w = synth.WORKLOADS["batch100"]
+    h = hough.Hough(w.grid, 20000, w.cap_peaks, w.cap_hits)
+    for seed in (w.seeds[1], w.seeds[57], w.seeds[99]):
+        x, y, layer, _ = synth.generate_event(w.event, seed)
+        h.vote(dev(x), dev(y), dev(layer))
+        h.peaks()
+        res = h.read()
+        res["acc"] = h.accumulator_host().copy()
+        ref = oracle.run(w.grid, x, y, layer)
+        assert res["flags"] == 0
+        assert_same(res, ref)
+    h.close()
+
+
+def test_finegrid_sampled_parity(hough, oracle):
+    """BASELINE.json configs[4] at full size (134M bins, ~62k hits), in bench.py's launch
+    configuration.  The oracle would need minutes for the whole vote, so: accumulator rows of
+    4096 sampled (phi0, d0) cells + every row of 2 whole phi0 planes, bit for bit; the whole
+    peak list against the oracle's peak rule applied to the (row-checked) accumulator; the
+    complete hit lists of 3000 sampled peaks and of the first/last 50; CSR consistency and
+    n_hit_entries = sum of all list lengths = votes that landed in reported peaks."""
+    w = synth.WORKLOADS["finegrid"]
+    g = w.grid
+    x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
+    h = hough.Hough(g, len(x), w.cap_peaks, w.cap_hits)
+    h.vote(dev(x), dev(y), dev(layer))
+    h.peaks()
+    res = h.read()
+    acc = h.accumulator_host().copy().reshape(g.n_phi, g.n_d0, g.n_kappa)
+    h.close()
+    assert res["flags"] == 0 and res["n_bad_hits"] == 0
+    rng = np.random.default_rng(5)
+    ci = np.concatenate([rng.integers(0, g.n_phi, 4096), np.repeat([0, g.n_phi - 1], g.n_d0)])
+    cj = np.concatenate([rng.integers(0, g.n_d0, 4096), np.tile(np.arange(g.n_d0), 2)])
+    rows, _nv = oracle.vote_cells(g, x, y, layer, ci, cj)
+    assert np.array_equal(acc[ci, cj, :], rows)
+    # vote count: sum of popcounts <= n_votes <= evaluations (SURVEY.md 8(c) C)
+    pop = int(np.unpackbits(acc.view(np.uint8)).sum())
+    assert pop <= res["n_votes"] <= len(x) * g.n_phi * g.n_d0
+    pb, pm, n = oracle.peaks(g, acc)
+    assert res["n_peaks"] == n
+    assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
+    off = res["hit_offset"].astype(np.int64)
+    assert off[0] == 0 and np.all(np.diff(off) >= 0) and off[-1] == res["n_hit_entries"]
+    sel = np.unique(np.concatenate([rng.integers(0, n, 3000), np.arange(50), np.arange(n - 50, n)]))
+    soff, sidx, _tot = oracle.hitlists(g, x, y, layer, pb[sel])
+    for q, pk in enumerate(sel):
+        got = res["hit_index"][off[pk]:off[pk + 1]]
+        assert np.array_equal(got, sidx[int(soff[q]):int(soff[q + 1])]), pk
