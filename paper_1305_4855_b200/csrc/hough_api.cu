@@ -229,24 +229,34 @@ static int choose_geometry(hough_handle *h)
     // hit lists: warp sub-tiles, hit segments (hough_lists.cu)
     if (!list_geom_init(h))
         return 0;
-    // peak sweep: JW warps x 2 rows per CTA (2 of them halo rows), Li phi0 planes per CTA
+    // peak sweep: JW warps x RJ rows per thread and CTA (2 of the rows are halo rows), Li
+    // phi0 planes per CTA.  RJ = 2: 8 warps, more registers; RJ = 1: 16 warps, more exchange.
     {
-        int JW = env_int("HOUGH_PEAK_JW", 8);
-        int need = (c.n_d0 + 2 + 1) / 2; // warps that cover every row plus the two halo rows
+        int RJ = env_int("HOUGH_PEAK_RJ", 2);
+        if (RJ != 1)
+            RJ = 2;
+        int KW = env_int("HOUGH_PEAK_KW", 1); // warps side by side along kappa (256 bins each)
+        if (KW < 1 || KW > 4 || KW * 256 > ((c.n_kappa + 255) / 256) * 256)
+            KW = 1;
+        const int max_jw = 16 / KW; // at most 16 warps per CTA
+        int JW = env_int("HOUGH_PEAK_JW", RJ == 1 ? 16 : 8);
+        int need = (c.n_d0 + 2 + RJ - 1) / RJ; // warps that cover every row plus the two halo rows
         if (JW > need)
             JW = need;
-        if (JW < 2)
-            JW = 2;
-        if (JW > 12)
-            JW = 12; // PEAK_MAX_JW
+        if (JW * RJ < 3)
+            JW = (3 + RJ - 1) / RJ;
+        if (JW > max_jw)
+            JW = max_jw;
         int Li = env_int("HOUGH_PEAK_LI", 16);
         if (Li > c.n_phi)
             Li = c.n_phi;
         if (Li < 1)
             Li = 1;
         h->pk_JW = JW;
+        h->pk_RJ = RJ;
+        h->pk_KW = KW;
         h->pk_Li = Li;
-        h->pk_smem = 2 * (2 * JW) * 32 * 16;
+        h->pk_smem = 2 * (RJ * JW) * KW * 32 * 16;
     }
     return 1;
 }

@@ -104,7 +104,7 @@ struct hough_handle {
     DevCounters *counters;
     uint32_t scan_blocks_max;
     // sweep tile geometry of the peak kernel
-    int pk_JW, pk_Li, pk_smem;
+    int pk_JW, pk_KW, pk_RJ, pk_Li, pk_smem;
     // state
     uint32_t n_hits;
     int voted;

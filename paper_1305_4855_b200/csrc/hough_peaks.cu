@@ -51,14 +51,12 @@ cudaError_t launch_clear(hough_handle *h, cudaStream_t st)
 // (with phi wrap, plane i-1 of i = 0 is plane n_phi-1, which has HIGHER lin, and plane i+1
 // of i = n_phi-1 is plane 0, which has LOWER lin).  "a > b" on pairs of small numbers is
 // bit 15 / 31 of (a | 0x80008000) - b - 0x00010001, "a >= b" the same without the last term.
-#define PEAK_RJ 2
-#define PEAK_MAX_JW 12
 
 struct PeakParams {
     const uint32_t *acc;
     unsigned char *flags; // 1 bit per bin, byte q of a row = bins 8q .. 8q+7
     int n_phi, n_d0, nk, L_min, wrap;
-    int JW, Li;
+    int JW, KW, RJ, Li;
 };
 
 __device__ __forceinline__ uint32_t popc_pair(uint32_t a, uint32_t b)
@@ -66,18 +64,22 @@ __device__ __forceinline__ uint32_t popc_pair(uint32_t a, uint32_t b)
     return (uint32_t)__popc(a) | ((uint32_t)__popc(b) << 16);
 }
 
+template <int PEAK_RJ>
 struct PeakRaw { // raw masks of one plane for the thread's rows
     uint4 a[PEAK_RJ], b[PEAK_RJ];
     uint32_t e[PEAK_RJ]; // the one bin beyond the warp's 256-bin segment (lanes 0 and 31)
 };
 
-template <int MAXJW>
-__global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p)
+template <int PEAK_RJ, int MAXJW>
+__global__ void __launch_bounds__(32 * MAXJW, (PEAK_RJ == 2 && MAXJW == 16) ? 1 : 2) k_peak_sweep(const PeakParams p)
 {
     extern __shared__ uint4 ex[]; // [2][rows][32] : m3 of every row of the current plane
+    // warp = (jw, kw): KW warps side by side along kappa so that the CTA's rows are whole
+    // (or long) contiguous pieces of memory, JW warps along d0
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int KW = p.KW, kw = warp % KW, jw = warp / KW;
     const int rows = PEAK_RJ * p.JW, Tj = rows - 2;
-    const int k0 = blockIdx.x * 256 + lane * 8;
+    const int k0 = (blockIdx.x * KW + kw) * 256 + lane * 8;
     const bool kact = k0 < p.nk;
     const int jfirst = blockIdx.y * Tj - 1;
     const int ia = blockIdx.z * p.Li, ib = min(ia + p.Li, p.n_phi);
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
     bool rout[PEAK_RJ];
 #pragma unroll
     for (int t = 0; t < PEAK_RJ; ++t) {
-        const int r = warp * PEAK_RJ + t, j = jfirst + r;
+        const int r = jw * PEAK_RJ + t, j = jfirst + r;
         const bool there = kact && j >= 0 && j < p.n_d0;
         const int jc = min(max(j, 0), p.n_d0 - 1);
         roff[t] = (uint32_t)jc * (uint32_t)p.nk + (uint32_t)(kact ? k0 : 0);
@@ -104,7 +106,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
     const int e_off = e_left ? -1 : 8;
     const unsigned char *fb = p.flags;
 
-    auto load_plane = [&](int pl, PeakRaw &R) {
+    auto load_plane = [&](int pl, PeakRaw<PEAK_RJ> &R) {
         const int src = pl < 0 ? p.n_phi - 1 : (pl >= p.n_phi ? 0 : pl);
         const uint32_t *pb = p.acc + (size_t)src * plane_stride;
 #pragma unroll
@@ -130,7 +132,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
             s_bx[t][q] = 0u;
         }
 
-    auto step = [&](int pl, const PeakRaw &C, PeakRaw &N) {
+    auto step = [&](int pl, const PeakRaw<PEAK_RJ> &C, PeakRaw<PEAK_RJ> &N) {
         if (pl > ib)
             return;
         if (pl < ib)
@@ -141,7 +143,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
         // strictness of the comparison with the neighbouring planes (phi wrap changes lin order)
         const uint32_t d_next = ((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u;
         const uint32_t d_prev = ((pl == 0) && p.wrap) ? 0u : ONE;
-        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * 32;
+        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * KW * 32;
 
         // ---- phase A: pair popcounts, kappa shifts, m3; publish m3 of every row
         uint32_t c[PEAK_RJ][4], s[PEAK_RJ][5], m3[PEAK_RJ][4];
@@ -167,21 +169,29 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 m3[t][q] = __vimax3_u16x2(c[t][q], s[t][q], s[t][q + 1]);
-            exw[(warp * PEAK_RJ + t) * 32 + lane] = make_uint4(m3[t][0], m3[t][1], m3[t][2], m3[t][3]);
+            exw[((jw * PEAK_RJ + t) * KW + kw) * 32 + lane] = make_uint4(m3[t][0], m3[t][1], m3[t][2], m3[t][3]);
         }
-        __syncthreads();
+        // A warp only needs the rows of the warps below and above it: pair barriers (named
+        // barrier 1 + jw*KW + kw joins warps (jw, kw) and (jw+1, kw)) instead of a CTA-wide
+        // one.  Lower id first on both sides, so the chain cannot deadlock; the exchange
+        // buffer is double buffered, and passing the pair barriers of plane p+1 implies that
+        // the neighbours have finished reading plane p.
+        if (jw > 0)
+            asm volatile("bar.sync %0, 64;" ::"r"(1 + (jw - 1) * KW + kw) : "memory");
+        if (jw < p.JW - 1)
+            asm volatile("bar.sync %0, 64;" ::"r"(1 + jw * KW + kw) : "memory");
 
         // ---- phase B: box maxima; close plane pl-1; open plane pl
 #pragma unroll
         for (int t = 0; t < PEAK_RJ; ++t) {
-            const int r = warp * PEAK_RJ + t;
+            const int r = jw * PEAK_RJ + t;
             uint32_t dn[4], up[4];
             if (t > 0) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
                     dn[q] = m3[t - 1][q];
             } else {
-                const uint4 v = exw[max(r - 1, 0) * 32 + lane]; // r = 0 is a halo row: never output
+                const uint4 v = exw[(max(r - 1, 0) * KW + kw) * 32 + lane]; // r = 0 is a halo row: never output
                 dn[0] = v.x, dn[1] = v.y, dn[2] = v.z, dn[3] = v.w;
             }
             if (t < PEAK_RJ - 1) {
@@ -189,7 +199,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
                 for (int q = 0; q < 4; ++q)
                     up[q] = m3[t + 1][q];
             } else {
-                const uint4 v = exw[min(r + 1, rows - 1) * 32 + lane];
+                const uint4 v = exw[(min(r + 1, rows - 1) * KW + kw) * 32 + lane];
                 up[0] = v.x, up[1] = v.y, up[2] = v.z, up[3] = v.w;
             }
             uint32_t bx[4];
@@ -223,7 +233,7 @@ __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p
         }
     };
 
-    PeakRaw A, B;
+    PeakRaw<PEAK_RJ> A, B;
     load_plane(ia - 1, A);
     for (int pl = ia - 1; pl <= ib; pl += 2) {
         step(pl, A, B);
@@ -243,12 +253,16 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
     p.wrap = h->g.phi_wrap;
     p.JW = h->pk_JW;
     p.Li = h->pk_Li;
-    const int Tj = PEAK_RJ * p.JW - 2;
-    dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
-    if (p.JW <= 8)
-        k_peak_sweep<8><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+    p.RJ = h->pk_RJ;
+    p.KW = h->pk_KW;
+    const int Tj = p.RJ * p.JW - 2;
+    dim3 grid((p.nk + 256 * p.KW - 1) / (256 * p.KW), (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
+    if (p.RJ == 1)
+        k_peak_sweep<1, 16><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
+    else if (p.JW * p.KW <= 8)
+        k_peak_sweep<2, 8><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
     else
-        k_peak_sweep<PEAK_MAX_JW><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+        k_peak_sweep<2, 16><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }
