@@ -324,6 +324,15 @@ def main():
         line.update(extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_info,
                            votes_step, evals_step, evals_done_step, flush))
     if rank == 0 and not args.no_cpu_baseline and world == 1:
+        # single-threaded oracle on the small 3-D config ("(a) single-threaded")
+        o = oracle_module()
+        small = synth.WORKLOADS["displaced3d"]
+        nthr = o.num_threads()
+        o.set_num_threads(1)
+        nv1, _n1, dt1, _c = time_oracle(small, small.seeds[0])
+        o.set_num_threads(nthr)
+        line["cpu_baseline_1thread"] = {"value": nv1 / dt1, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                        "sample": "displaced3d (configs[1]), 1 event, %.1f s" % dt1}
         nv, _n, dt, cores = time_oracle(workload, workload.seeds[0])
         line["cpu_baseline"] = {"value": nv / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "events_per_s": 1.0 / dt,
@@ -389,6 +398,32 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
                                    "peak_random_addresses": rnd,
                                    "note": "votes cast / vote-kernel time vs the conflict-free "
                                            "atomicOr micro-benchmark (hough_microbench_smem mode 0)"}
+
+    # the unpruned sweep (HOUGH_OPT_NO_CULL: every hit x cell is evaluated), SURVEY.md 8(d):
+    # "report the fraction honestly for both the pruned and unpruned kernels"
+    hn = hough.Hough(workload.grid, max(len(e[0]) for e in d_events), workload.cap_peaks,
+                     workload.cap_hits, device=local_rank,
+                     options=hough.OPT_STAGE_TIMING | hough.OPT_NO_CULL)
+    t_nc, n_nc = 0.0, min(n_ev, 3)
+    for r in range(2):
+        for e in range(n_nc):
+            x, y, layer = d_events[e]
+            hn.vote(x, y, layer)
+            hn.peaks(lists=False)
+            if r > 0:
+                t_nc += hn.stage_times()["vote"]
+    hn.close()
+    vote_nc_s = t_nc / n_nc * 1e-3
+    out["vote_unpruned"] = {
+        "ms_per_event": vote_nc_s * 1e3, "evaluations_per_s": (evals_step / n_ev) / vote_nc_s,
+        "alu_frac": FLOP_PER_EVAL * (evals_step / n_ev) / vote_nc_s / 1e12 / alu_peak,
+        "smem_atomic_frac": (votes_step / n_ev) / vote_nc_s / best,
+        "note": "same kernel with the conservative cull switched off: executed = algorithmic evaluations"}
+    # issue-slot utilisation and shared-memory bank-conflict rate of the sweeps, from the
+    # committed ncu --set full capture (profiles/r1h_pileup_sweeps_ncu_full.md)
+    prof = ncu_traffic("_sweeps")
+    if prof:
+        out["ncu_sweeps"] = prof
 
     # HBM roofline of the accumulator sweeps, on the fine grid (512 MiB > L2)
     fine = synth.WORKLOADS["finegrid"]
