@@ -101,6 +101,25 @@ struct Carve {
     }
 };
 
+static int env_int(const char *name, int dflt);
+
+// u16 entries of the kappa-code cache: HOUGH_KC_PERCENT % of the worst case (default 0 = off:
+// measured slower than re-evaluating; 35 holds config 3/4)
+// (every hit x every cell + 25 % row overhead); 0 switches the cache off.
+size_t kc_entries_for(const hough_config *c)
+{
+    const int pct = env_int("HOUGH_KC_PERCENT", 0);
+    if (pct <= 0)
+        return 0;
+    const double hp = (double)(((c->max_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK);
+    double e = hp * (double)c->n_phi * (double)c->n_d0 * 1.25 * (double)pct / 100.0;
+    if (e < 1048576.0)
+        e = 1048576.0;
+    if (e > 6.0e10)
+        e = 6.0e10;
+    return ((size_t)e + 1023) & ~(size_t)1023;
+}
+
 static uint32_t pad_hits(uint32_t n)
 {
     uint32_t p = ((n + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
@@ -133,6 +152,10 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *peak_len = cv.take((size_t)c->cap_peaks * 4);
     void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
+    const size_t kc_cap = kc_entries_for(c);
+    const uint32_t kc_chunks = hp / HOUGH_CHUNK;
+    void *kc_buf = cv.take(kc_cap * 2);
+    void *kc_tab = cv.take(kc_cap ? n_rows * (size_t)kc_chunks * 8 : 0);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -157,6 +180,11 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ent_sub = (uint32_t *)ent_sub;
         h->ent_hit = (uint32_t *)ent_hit;
         h->ent_idx = (uint32_t *)ent_idx;
+        h->kc_buf = (unsigned short *)kc_buf;
+        h->kc_cap = kc_cap;
+        h->kc_tab = (uint2 *)kc_tab;
+        h->kc_chunks = kc_chunks;
+        h->kc_on = kc_cap > 0;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
