@@ -216,7 +216,7 @@ static int choose_geometry(hough_handle *h)
     const hough_config &c = h->cfg;
     const int nk = c.n_kappa;
     const int budget = env_int("HOUGH_SMEM_BUDGET", 113 * 1024);
-    const int staging = 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 8) * 16 + 256;
+    const int staging = 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 8) * 16 + 1024;
     // vote
     {
         int cell_bytes = nk * 4 / h->g.pack;
@@ -225,7 +225,12 @@ static int choose_geometry(hough_handle *h)
             D = c.n_d0;
         int P = c.tile_phi > 0 ? c.tile_phi : env_int("HOUGH_TILE_PHI", 0);
         if (P <= 0) {
-            int cells = (budget - staging) / cell_bytes;
+            // whole cell groups (32 lanes) only: a padded group costs a full group of
+            // shared memory and lanes (fine grid: 11 x 8 cells = 96 KB + staging -> 1 CTA/SM,
+            // 41 % issue; 8 x 8 = 64 KB -> 2 CTAs/SM)
+            int cells = ((budget - staging) / cell_bytes / 32) * 32;
+            if (cells < 32)
+                cells = (budget - staging) / cell_bytes;
             P = cells / D;
             if (P > 32)
                 P = 32;
