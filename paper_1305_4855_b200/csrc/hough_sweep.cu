@@ -6,7 +6,7 @@
 // closed form (hough_device.cuh).
 #include "hough_device.cuh"
 
-#define EVAL_UNROLL 2
+#define EVAL_UNROLL 4
 
 // ------------------------------------------------------------------ kernel parameters
 struct SweepParams {
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         if (KC && tid == 0) {
             // rows of the kappa-code cache for this chunk's survivors: (cells + 32) u16 each
             unsigned long long base = ~0ull;
-            const unsigned long long need = (unsigned long long)(total + 1) * (unsigned)kc_row; // + a row the padding entry may write
+            const unsigned long long need = (unsigned long long)(total + EVAL_UNROLL - 1) * (unsigned)kc_row; // + rows the padding entries may write
             if (total > 0) {
                 const unsigned long long b = atomicAdd(&p.counters->kc_cursor, need);
                 if (b + need <= p.kc_cap)
