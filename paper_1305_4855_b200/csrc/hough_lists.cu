@@ -63,7 +63,7 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 
 // Per-warp shared-memory block; the fixed-size parts come first so that the hot loop
 // addresses them with immediates off one register (wpr = n_kappa / 32):
-//   widx    [LIST_ROUND + 2] u16   survivors of the warp-level cull (indices into surv)
+//   widx    [LIST_ROUND + 4] u16   survivors of the warp-level cull (indices into surv)
 //   laneq   [LIST_LQ][32] u32      per lane: pending (kappa bin << 10 | surv index)
 //   flushq  [3][LIST_QUEUE] u32    finished entries on their way to global memory
 //   flags   [wpr][32] u32   flag words of the reported peaks of the warp's cells
@@ -73,7 +73,7 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 #define OFF_LANEQ 384
 #define OFF_FLUSHQ (OFF_LANEQ + LIST_LQ * 128)
 #define OFF_FLAGS (OFF_FLUSHQ + 3 * LIST_QUEUE * 4)
-static_assert((LIST_ROUND + 2) * 2 <= OFF_LANEQ && OFF_FLAGS % 128 == 0, "per-warp block layout");
+static_assert((LIST_ROUND + 4) * 2 <= OFF_LANEQ && OFF_FLAGS % 128 == 0, "per-warp block layout");
 
 template <int OFF>
 __device__ __forceinline__ uint32_t lds_off(uint32_t addr)
@@ -349,17 +349,21 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
                         widx[nw + __popc(bal & lt_mask)] = (unsigned short)idx;
                     nw += __popc(bal);
                 }
-                if (lane == 0)
-                    widx[nw] = (unsigned short)total; // pad to an even count with the non-voting entry
+                if (lane < 3)
+                    widx[nw + lane] = (unsigned short)total; // pad to a multiple of 4 with the non-voting entry
                 __syncwarp();
-                // ---- lane = cell: the exact recipe on the survivors, two at a time
-                for (int t = 0; t < nw; t += 2) {
-                    const uint32_t two = lds_off<OFF_WIDX>((wl4 & ~127u) + (uint32_t)t * 2u); // the block is 128-byte aligned
-                    const uint32_t a = two & 0xffffu, b = two >> 16;
+                // ---- lane = cell: the exact recipe on the survivors, four at a time
+                for (int t = 0; t < nw; t += 4) {
+                    const uint32_t wa = (wl4 & ~127u) + (uint32_t)t * 2u; // the block is 128-byte aligned
+                    const uint32_t two0 = lds_off<OFF_WIDX>(wa), two1 = lds_off<OFF_WIDX + 4>(wa);
+                    const uint32_t a = two0 & 0xffffu, b = two0 >> 16, c2 = two1 & 0xffffu, d2 = two1 >> 16;
                     const float4 h0 = lds_f4(sv + a * 16u), h1 = lds_f4(sv + b * 16u);
+                    const float4 h2 = lds_f4(sv + c2 * 16u), h3 = lds_f4(sv + d2 * 16u);
                     process(h0, a);
                     process(h1, b);
-                    if (__any_sync(0xffffffffu, lqp > wl4 + (LIST_LQ - 2) * 128u))
+                    process(h2, c2);
+                    process(h3, d2);
+                    if (__any_sync(0xffffffffu, lqp > wl4 + (LIST_LQ - 4) * 128u))
                         drain();
                 }
                 __syncwarp();
