@@ -279,11 +279,21 @@ def main():
 
     # ---- e2e: host buffers in, host results out, every event (hough_process_host)
     def e2e_step():
+        # hough_submit_host / hough_collect_host: the copies of event e-1 overlap event e
         nv = 0
         for e in range(n_ev):
             x, y, layer = pin_events[e]
-            r = h.process_host(x.numpy(), y.numpy(), layer.numpy())
-            nv += r["n_votes"]
+            h.submit_host(x.numpy(), y.numpy(), layer.numpy(), e & 1)
+            if e > 0:
+                nv += h.collect_host((e - 1) & 1)["n_votes"]
+        nv += h.collect_host((n_ev - 1) & 1)["n_votes"]
+        return nv
+
+    def e2e_step_sync():
+        nv = 0
+        for e in range(n_ev):
+            x, y, layer = pin_events[e]
+            nv += h.process_host(x.numpy(), y.numpy(), layer.numpy())["n_votes"]
         return nv
 
     e2e_step()
@@ -303,7 +313,14 @@ def main():
     d2h = int(sum(40 + min(int(c["n_peaks"]), workload.cap_peaks) * 16 + 8 +
                   min(int(c["n_hit_entries"]), workload.cap_hits) * 4 for c in cnt))
     e2e = {"value": votes_all * args.steps / e2e_secs, "unit": UNIT, "h2d_bytes_per_step": h2d,
-           "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs}
+           "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs,
+           "api": "hough_submit_host + hough_collect_host (two events in flight, copies on a second stream)"}
+    if rank == 0 and world == 1:
+        t0 = time.perf_counter()
+        e2e_step_sync()
+        torch.cuda.synchronize(dev)
+        e2e["events_per_s_one_at_a_time"] = n_ev / (time.perf_counter() - t0)  # hough_process_host
+
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,

@@ -177,6 +177,26 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
                        void *cuda_stream);
 
 /*
+ * The same in two halves, so that the device->host copies of one event overlap the
+ * computation of the next (the paper's production model: transfers of neighbouring events
+ * overlap, steady-state throughput).  `slot` is 0 or 1 and names one of
+ * two in-flight events; each slot needs its own `dev` arrays (and `host` buffers).
+ *   hough_submit_host   copies x, y, layer host->device on `cuda_stream`, enqueues hough_vote
+ *                       + hough_peaks into `dev`, records the slot's event; returns at once.
+ *   hough_collect_host  waits (on `copy_stream`) for the slot's event, copies counts, then
+ *                       the filled prefixes of the peak arrays and hit lists to `host`, and
+ *                       SYNCHRONISES `copy_stream` before returning.
+ * Pattern:  submit(e, e&1);  if (e > 0) collect(e-1, (e-1)&1);  ...  collect(last).
+ * A slot must be collected before it is submitted again.  The host arrays must be pinned
+ * for the copies to overlap.  Errors as hough_process_host; HOUGH_ESTATE if the slot was
+ * not submitted.
+ */
+int hough_submit_host(hough_handle *h, const float *x, const float *y, const int32_t *layer,
+                      uint32_t n, const hough_peaks_out *dev, int32_t slot, void *cuda_stream);
+int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host,
+                       int32_t slot, void *copy_stream);
+
+/*
  * Stand-alone accumulator kernels, used for the
  * HBM-roofline measurements and as cross-checks:
  *   hough_clear       zero the global accumulator (pure HBM write);

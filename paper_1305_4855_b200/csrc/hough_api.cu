@@ -416,6 +416,9 @@ void hough_destroy(hough_handle *h)
         for (int s = 0; s < HOUGH_N_STAGES + 2; ++s)
             if (h->ev[s])
                 cudaEventDestroy(h->ev[s]);
+    for (int s = 0; s < 2; ++s)
+        if (h->slot_ev[s])
+            cudaEventDestroy(h->slot_ev[s]);
     free(h->radii);
     delete h;
 }
@@ -552,6 +555,60 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
     if (host->hit_index && ne > 0)
         CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return HOUGH_OK;
+}
+
+int hough_submit_host(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
+                      const hough_peaks_out *dev, int32_t slot, void *cuda_stream)
+{
+    if (!h || !dev || slot < 0 || slot > 1)
+        return HOUGH_EINVAL;
+    if (n > h->cfg.max_hits || (n > 0 && (!x || !y || !layer)))
+        return HOUGH_EINVAL;
+    if (h->slot_busy[slot])
+        return HOUGH_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!h->slot_ev[slot])
+        CK(cudaEventCreateWithFlags(&h->slot_ev[slot], cudaEventDisableTiming));
+    if (n > 0) {
+        CK(cudaMemcpyAsync(h->raw_x, x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_y, y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_layer, layer, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+    }
+    int rc = hough_vote(h, h->raw_x, h->raw_y, h->raw_layer, n, cuda_stream);
+    if (rc != HOUGH_OK)
+        return rc;
+    rc = hough_peaks(h, dev, cuda_stream);
+    if (rc != HOUGH_OK)
+        return rc;
+    CK(cudaEventRecord(h->slot_ev[slot], st));
+    h->slot_busy[slot] = 1;
+    return HOUGH_OK;
+}
+
+int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host, int32_t slot,
+                       void *copy_stream)
+{
+    if (!h || !dev || !host || !host->counts || !host->bin || !host->mask || !host->hit_offset || slot < 0 ||
+        slot > 1)
+        return HOUGH_EINVAL;
+    if (!h->slot_busy[slot])
+        return HOUGH_ESTATE;
+    cudaStream_t st = (cudaStream_t)copy_stream;
+    CK(cudaStreamWaitEvent(st, h->slot_ev[slot], 0));
+    CK(cudaMemcpyAsync(host->counts, dev->counts, sizeof(hough_counts), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    uint64_t np = host->counts->n_peaks < h->cfg.cap_peaks ? host->counts->n_peaks : h->cfg.cap_peaks;
+    uint64_t ne = host->counts->n_hit_entries < h->cfg.cap_hits ? host->counts->n_hit_entries : h->cfg.cap_hits;
+    if (np > 0) {
+        CK(cudaMemcpyAsync(host->bin, dev->bin, np * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(host->mask, dev->mask, np * 4, cudaMemcpyDeviceToHost, st));
+    }
+    CK(cudaMemcpyAsync(host->hit_offset, dev->hit_offset, (np + 1) * 8, cudaMemcpyDeviceToHost, st));
+    if (host->hit_index && ne > 0)
+        CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    h->slot_busy[slot] = 0;
     return HOUGH_OK;
 }
 

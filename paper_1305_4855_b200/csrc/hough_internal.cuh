@@ -113,6 +113,9 @@ struct hough_handle {
     uint32_t scan_blocks_max;
     // sweep tile geometry of the peak kernel
     int pk_JW, pk_KW, pk_RJ, pk_Li, pk_smem;
+    // hough_submit_host / hough_collect_host: one event per slot marks the end of the slot's work
+    cudaEvent_t slot_ev[2];
+    unsigned char slot_busy[2];
     // state
     uint32_t n_hits;
     int voted;

@@ -25,7 +25,7 @@ N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
 SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
-           "hough_accumulator", "hough_process_host", "hough_clear", "hough_peak_sweep",
+           "hough_accumulator", "hough_process_host", "hough_submit_host", "hough_collect_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
            "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror")
 
@@ -91,6 +91,12 @@ def _load():
     lib.hough_process_host.restype = C.c_int
     lib.hough_process_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32,
                                        C.POINTER(PeaksOut), C.POINTER(HostOut), C.c_void_p]
+    lib.hough_submit_host.restype = C.c_int
+    lib.hough_submit_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32,
+                                      C.POINTER(PeaksOut), C.c_int32, C.c_void_p]
+    lib.hough_collect_host.restype = C.c_int
+    lib.hough_collect_host.argtypes = [C.c_void_p, C.POINTER(PeaksOut), C.POINTER(HostOut), C.c_int32,
+                                       C.c_void_p]
     for name in ("hough_clear", "hough_peak_sweep"):
         f = getattr(lib, name)
         f.restype = C.c_int
@@ -256,6 +262,48 @@ class Hough:
         cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
         return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
                           hb["hit_index"].numpy() if want_lists else None)
+
+    def _slot(self, slot):
+        """Device and pinned host arrays of one in-flight event (submit_host / collect_host)."""
+        if not hasattr(self, "_slots"):
+            self._slots, self._copy_stream = {}, torch.cuda.Stream(device=self.device)
+        if slot not in self._slots:
+            i32 = dict(dtype=torch.int32, device=self.device)
+            pin = dict(pin_memory=True)
+            d = dict(bin=torch.empty(self.cap_peaks, **i32), mask=torch.empty(self.cap_peaks, **i32),
+                     hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, device=self.device),
+                     hit_index=torch.empty(self.cap_hits, **i32),
+                     counts=torch.zeros(COUNTS_WORDS, dtype=torch.int64, device=self.device))
+            hb = dict(bin=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
+                      mask=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
+                      hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, **pin),
+                      hit_index=torch.empty(self.cap_hits, dtype=torch.int32, **pin),
+                      counts=torch.zeros(COUNTS_WORDS, dtype=torch.int64, **pin))
+            out = PeaksOut(d["bin"].data_ptr(), d["mask"].data_ptr(), d["hit_offset"].data_ptr(),
+                           d["hit_index"].data_ptr(), d["counts"].data_ptr())
+            host = HostOut(hb["bin"].data_ptr(), hb["mask"].data_ptr(), hb["hit_offset"].data_ptr(),
+                           hb["hit_index"].data_ptr(), hb["counts"].data_ptr())
+            self._slots[slot] = (d, hb, out, host)
+        return self._slots[slot]
+
+    def submit_host(self, x, y, layer, slot, stream=None):
+        """hough_submit_host: host arrays in (pinned for overlap), compute enqueued, returns at once."""
+        x = np.ascontiguousarray(x, np.float32)
+        y = np.ascontiguousarray(y, np.float32)
+        layer = np.ascontiguousarray(layer, np.int32)
+        _d, _hb, out, _host = self._slot(slot)
+        _check(_lib.hough_submit_host(self._h, C.c_void_p(x.ctypes.data), C.c_void_p(y.ctypes.data),
+                                      C.c_void_p(layer.ctypes.data), x.shape[0], C.byref(out), int(slot),
+                                      _stream_ptr(stream)), "hough_submit_host")
+
+    def collect_host(self, slot):
+        """hough_collect_host: results of the event submitted in `slot`, copied on a second stream."""
+        _d, hb, out, host = self._slot(slot)
+        _check(_lib.hough_collect_host(self._h, C.byref(out), C.byref(host), int(slot),
+                                       C.c_void_p(self._copy_stream.cuda_stream)), "hough_collect_host")
+        cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
+        return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
+                          hb["hit_index"].numpy())
 
     # -- results
     def _pack(self, cnt, b, m, off, idx):

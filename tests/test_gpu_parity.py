@@ -294,3 +294,30 @@ def test_finegrid_sampled_parity(hough, oracle):
     for q, pk in enumerate(sel):
         got = res["hit_index"][off[pk]:off[pk + 1]]
         assert np.array_equal(got, sidx[int(soff[q]):int(soff[q + 1])]), pk
+
+
+def test_submit_collect_pipeline_matches_oracle(hough, oracle):
+    """hough_submit_host / hough_collect_host with two events in flight: every event's results
+    (copied on the second stream while the next event computes) equal the oracle's."""
+    w = synth.WORKLOADS["displaced3d"]
+    evs = [synth.generate_event(w.event, s)[:3] for s in (2, 3, 4, 5, 6)]
+    refs = [oracle.run(w.grid, *e) for e in evs]
+    pins = [[torch.from_numpy(a).pin_memory() for a in e] for e in evs]
+    h = hough.Hough(w.grid, max(len(e[0]) for e in evs), w.cap_peaks, w.cap_hits)
+    got = []
+    for e, pe in enumerate(pins):
+        h.submit_host(pe[0].numpy(), pe[1].numpy(), pe[2].numpy(), e & 1)
+        if e > 0:
+            r = h.collect_host((e - 1) & 1)
+            got.append({k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in r.items()})
+    r = h.collect_host((len(pins) - 1) & 1)
+    got.append({k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in r.items()})
+    with pytest.raises(hough.HoughError):
+        h.collect_host(0)          # nothing submitted in that slot any more
+    h.close()
+    for res, ref in zip(got, refs):
+        assert res["n_votes"] == ref["n_votes"] and res["n_peaks"] == ref["n_peaks"]
+        assert np.array_equal(res["peak_bin"], ref["peak_bin"])
+        assert np.array_equal(res["peak_mask"], ref["peak_mask"])
+        assert np.array_equal(res["hit_offset"], ref["hit_offset"])
+        assert np.array_equal(res["hit_index"], ref["hit_index"])
