@@ -316,6 +316,7 @@ def main():
            "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs,
            "api": "hough_submit_host + hough_collect_host (two events in flight, copies on a second stream)"}
     if rank == 0 and world == 1:
+        h.process_host(*[t.numpy() for t in pin_events[0]])  # allocates its pinned buffers
         t0 = time.perf_counter()
         e2e_step_sync()
         torch.cuda.synchronize(dev)
@@ -437,7 +438,7 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
         "smem_atomic_frac": (votes_step / n_ev) / vote_nc_s / best,
         "note": "same kernel with the conservative cull switched off: executed = algorithmic evaluations"}
     # issue-slot utilisation and shared-memory bank-conflict rate of the sweeps, from the
-    # committed ncu --set full capture (profiles/r1h_pileup_sweeps_ncu_full.md)
+    # committed ncu --set full capture (profiles/r1i_pileup_sweeps_ncu_full.md)
     prof = ncu_traffic("_sweeps")
     if prof:
         out["ncu_sweeps"] = prof
