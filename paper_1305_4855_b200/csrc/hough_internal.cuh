@@ -34,6 +34,7 @@ struct SweepGeom {
 #define LIST_MAX_SEGMENTS 16
 struct ListGeom {
     int SP, SD, WP, WD;
+    int warps;           // warps per CTA (<= LIST_WARPS)
     int tiles_phi, tiles_d0;
     int S;               // hit segments (sub-lists per peak)
     int max_pk;          // bound on the peaks of one sub-tile

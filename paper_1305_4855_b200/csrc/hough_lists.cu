@@ -88,7 +88,8 @@ __device__ __forceinline__ float4 lds_f4(uint32_t addr)
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-__global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepParams p)
+template <int WARPS> // warps per CTA = sub-tiles per super-tile (ListGeom::warps)
+__global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     if (p.kc_on && !p.counters->kc_overflow)
@@ -115,7 +116,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
     uint32_t *wflags = reinterpret_cast<uint32_t *>(wbase + OFF_FLAGS);
     unsigned short *wpre = reinterpret_cast<unsigned short *>(wbase + OFF_FLAGS + (size_t)wpr * 128);
     unsigned short *wcnt = wpre + (size_t)wpr * 32;
-    unsigned char *ptr = smem_raw + (size_t)LIST_WARPS * ge.warp_bytes;
+    unsigned char *ptr = smem_raw + (size_t)WARPS * ge.warp_bytes;
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
     ptr += (size_t)2 * 4 * LIST_CHUNK * 4;
     float4 *surv = reinterpret_cast<float4 *>(ptr); // [chunk + 2]
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
 
         // ---- CTA-level cull against the super-tile, order-preserving compaction
         int total = 0;
-        for (int base = 0; base < LIST_CHUNK; base += 32 * LIST_WARPS) {
+        for (int base = 0; base < LIST_CHUNK; base += 32 * WARPS) {
             const int hidx = base + tid;
             float hx = 0.f, hy = 0.f, hr2 = 0.f;
             bool keep = false;
@@ -317,7 +318,7 @@ __global__ void __launch_bounds__(32 * LIST_WARPS) k_list_sweep(const ListSweepP
             __syncthreads();
             int before = 0, all = 0;
 #pragma unroll
-            for (int w = 0; w < LIST_WARPS; ++w) {
+            for (int w = 0; w < WARPS; ++w) {
                 const int cw = warp_cnt[w];
                 before += (w < warp) ? cw : 0;
                 all += cw;
@@ -662,6 +663,22 @@ int list_segments_bound(const hough_config *c)
     return s_max > s_min ? s_max : s_min;
 }
 
+static const void *list_sweep_fn(int warps)
+{
+    switch (warps) {
+    case 16:
+        return (const void *)k_list_sweep<16>;
+    case 8:
+        return (const void *)k_list_sweep<8>;
+    case 4:
+        return (const void *)k_list_sweep<4>;
+    case 2:
+        return (const void *)k_list_sweep<2>;
+    default:
+        return (const void *)k_list_sweep<1>;
+    }
+}
+
 int list_geom_init(hough_handle *h)
 {
     const hough_config &c = h->cfg;
@@ -669,30 +686,44 @@ int list_geom_init(hough_handle *h)
     int SD = 4;
     while (SD > c.n_d0)
         SD >>= 1;
+    int SP = 32 / SD, warps = LIST_WARPS;
+    const int wpr = c.n_kappa / 32;
+    // The per-warp tables grow with n_kappa: fewer warps per CTA first, then fewer cells per
+    // warp (idle lanes), until the CTA fits (n_kappa = 256: 16 warps; 2048: 4; 16384: 1 warp
+    // of 8 cells).
+    for (;;) {
+        ge->max_pk = ((SP + 1) / 2) * ((SD + 1) / 2) * ((c.n_kappa + 1) / 2);
+        ge->warp_bytes = (OFF_FLAGS + wpr * 192 + ge->max_pk * 2 + 127) & ~127;
+        ge->smem_bytes = warps * ge->warp_bytes + 2 * 4 * LIST_CHUNK * 4 + (LIST_CHUNK + 2) * 16 + 16 +
+                         LIST_WARPS * 4 + 16;
+        if (ge->smem_bytes <= hough_vote_max_smem())
+            break;
+        if (warps > 1)
+            warps >>= 1;
+        else if (SP > 1)
+            SP >>= 1;
+        else if (SD > 1)
+            SD >>= 1;
+        else
+            return 0;
+    }
     ge->SD = SD;
-    ge->SP = 32 / SD;
+    ge->SP = SP;
+    ge->warps = warps;
     ge->WD = 1;
-    while (ge->WD < 4 && ge->WD * 2 * SD <= c.n_d0)
+    while (ge->WD < 4 && ge->WD * 2 <= warps && ge->WD * 2 * SD <= c.n_d0)
         ge->WD *= 2;
-    ge->WP = LIST_WARPS / ge->WD;
+    ge->WP = warps / ge->WD;
     ge->tiles_phi = (c.n_phi + ge->WP * ge->SP - 1) / (ge->WP * ge->SP);
     ge->tiles_d0 = (c.n_d0 + ge->WD * ge->SD - 1) / (ge->WD * ge->SD);
-    const int wpr = c.n_kappa / 32;
-    ge->max_pk = ((ge->SP + 1) / 2) * ((ge->SD + 1) / 2) * ((c.n_kappa + 1) / 2);
-    ge->warp_bytes = (OFF_FLAGS + wpr * 192 + ge->max_pk * 2 + 127) & ~127;
-    ge->smem_bytes = LIST_WARPS * ge->warp_bytes + 2 * 4 * LIST_CHUNK * 4 + (LIST_CHUNK + 2) * 16 + 16 +
-                     LIST_WARPS * 4 + 16;
-    if (ge->smem_bytes > hough_vote_max_smem())
-        return 0;
     const double dphi = (c.phi_max - c.phi_min) / (double)c.n_phi;
     ge->no_phi_cull_tile = (dphi * (ge->WP * ge->SP - 1) > 1.0) ? 1 : 0;
     ge->no_phi_cull_sub = (dphi * (ge->SP - 1) > 1.0) ? 1 : 0;
-    if (cudaFuncSetAttribute(k_list_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes) !=
-        cudaSuccess)
+    const void *fn = list_sweep_fn(ge->warps);
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes) != cudaSuccess)
         return 0;
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_list_sweep, 32 * LIST_WARPS, ge->smem_bytes) !=
-            cudaSuccess ||
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * ge->warps, ge->smem_bytes) != cudaSuccess ||
         per_sm < 1)
         return 0;
     // segments: whole chunks, at most 65535 hits each (u16 counters), bounded sub-list table
@@ -801,8 +832,9 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
         }
     }
     const int blocks = h->list_geom.tiles_phi * h->list_geom.tiles_d0 * h->list_geom.S;
-    k_list_sweep<<<blocks, 32 * LIST_WARPS, h->list_geom.smem_bytes, st>>>(p);
-    return cudaGetLastError();
+    void *args[] = {(void *)&p};
+    return cudaLaunchKernel(list_sweep_fn(h->list_geom.warps), dim3(blocks), dim3(32 * h->list_geom.warps), args,
+                            (size_t)h->list_geom.smem_bytes, st);
 }
 
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)

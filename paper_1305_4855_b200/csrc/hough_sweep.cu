@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nwarps = ge.threads >> 5;
 
-    // ---- carve shared memory: tile = masks [cells_pad][nk / PACK words], then staging
+    // ---- carve shared memory: tile = masks [P * D cells][nk / PACK words], then staging
     uint32_t *tile = reinterpret_cast<uint32_t *>(smem_raw);
     unsigned char *ptr = smem_raw + (size_t)ge.tile_words * 4;
     float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
@@ -270,7 +270,7 @@ static int swizzle_mask_for(int row_words)
     return m;
 }
 
-// Tile geometry: cells_pad rows of n_kappa masks, PACK masks per word, plus the staging.
+// Tile geometry: P x D rows of n_kappa masks, PACK masks per word, plus the staging.
 int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int fit_waves)
 {
     const hough_config &cfg = h->cfg;
@@ -284,7 +284,8 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     ge->tiles_phi = (cfg.n_phi + P - 1) / P;
     ge->tiles_d0 = (cfg.n_d0 + D - 1) / D;
     ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
-    const size_t tile_bytes = (size_t)ge->cells_pad * cfg.n_kappa * 4 / h->g.pack, extra = 0;
+    // rows for the P x D cells only: padding lanes of the last cell group never vote
+    const size_t tile_bytes = (size_t)(P * D) * cfg.n_kappa * 4 / h->g.pack, extra = 0;
     ge->tile_words = (int)(tile_bytes / 4);
     size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16 + 16 + (size_t)ge->chunk * 2;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);

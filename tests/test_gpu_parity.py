@@ -321,3 +321,41 @@ def test_submit_collect_pipeline_matches_oracle(hough, oracle):
         assert np.array_equal(res["peak_mask"], ref["peak_mask"])
         assert np.array_equal(res["hit_offset"], ref["hit_offset"])
         assert np.array_equal(res["hit_index"], ref["hit_index"])
+
+
+def test_second_vote_replaces_the_event_and_peaks_can_be_repeated(hough, oracle):
+    """Reading B15: a second hough_vote before hough_peaks replaces the event; hough_peaks
+    may be called again on the same accumulator and gives the same answer."""
+    rng = np.random.default_rng(21)
+    grid = synth.Grid(n_phi=48, n_d0=12, n_kappa=64, L_min=2)
+    xa, ya, la = random_hits(rng, 900)
+    xb, yb, lb = random_hits(rng, 350)
+    ref = oracle.run(grid, xb, yb, lb)
+    h = hough.Hough(grid, 900, grid.n_bins // 2 + 1, ref["n_hit_entries"] + 1000)
+    h.vote(dev(xa), dev(ya), dev(la))
+    h.vote(dev(xb), dev(yb), dev(lb))
+    for _ in range(2):
+        h.peaks()
+        res = h.read()
+        res["acc"] = h.accumulator_host().copy()
+        assert_same(res, ref)
+    h.close()
+
+
+def test_many_kappa_bins_and_single_cell_tiles(hough, oracle):
+    """n_kappa = 2048 (a cell row of 4 KB: few cells per tile) and the 1 x 1 tile override."""
+    rng = np.random.default_rng(22)
+    grid = synth.Grid(n_phi=24, n_d0=6, n_kappa=2048, L_min=2)
+    x, y, layer = random_hits(rng, 600)
+    ref = oracle.run(grid, x, y, layer)
+    for tile in ((0, 0), (1, 1)):
+        res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=tile[0], tile_d0=tile[1])
+        assert_same(res, ref)
+    # the largest n_kappa the library accepts: one warp of 8 cells per list CTA
+    grid = synth.Grid(n_phi=6, n_d0=2, n_kappa=16384, L_min=1)
+    x, y, layer = random_hits(rng, 300)
+    ref = oracle.run(grid, x, y, layer)
+    res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                  cap_hits=ref["n_hit_entries"] + 1)
+    assert_same(res, ref)
