@@ -52,6 +52,37 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
     return cudaGetLastError();
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize holds the LAST value set, not the largest: a
+// handle with a small tile must not take the limit away from a live handle with a large one.
+cudaError_t ensure_dynamic_smem(const void *kernel, int bytes)
+{
+    struct Entry {
+        const void *fn;
+        int device, bytes;
+    };
+    static Entry table[64];
+    static int n_entries = 0;
+    int device = 0;
+    cudaGetDevice(&device);
+    Entry *e = nullptr;
+    for (int i = 0; i < n_entries; ++i)
+        if (table[i].fn == kernel && table[i].device == device)
+            e = &table[i];
+    if (e && e->bytes >= bytes)
+        return cudaSuccess;
+    cudaError_t rc = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (rc != cudaSuccess)
+        return rc;
+    if (!e && n_entries < 64) {
+        e = &table[n_entries++];
+        e->fn = kernel;
+        e->device = device;
+    }
+    if (e)
+        e->bytes = bytes;
+    return cudaSuccess;
+}
+
 // ------------------------------------------------------------------ configuration
 static int cfg_valid(const hough_config *c)
 {

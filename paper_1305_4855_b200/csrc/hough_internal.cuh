@@ -154,6 +154,8 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split
 int list_geom_init(hough_handle *h);
 int list_segments_bound(const hough_config *c);
 int hough_vote_max_smem(void);
+// Raise (never lower) a kernel's dynamic shared-memory limit on the current device.
+cudaError_t ensure_dynamic_smem(const void *kernel, int bytes);
 
 #define HOUGH_CHUNK 512       // hits per staged chunk
 #define HOUGH_SCAN_ITEMS 2048 // items per block of the chained scan

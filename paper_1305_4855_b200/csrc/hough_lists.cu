@@ -720,7 +720,7 @@ int list_geom_init(hough_handle *h)
     ge->no_phi_cull_tile = (dphi * (ge->WP * ge->SP - 1) > 1.0) ? 1 : 0;
     ge->no_phi_cull_sub = (dphi * (ge->SP - 1) > 1.0) ? 1 : 0;
     const void *fn = list_sweep_fn(ge->warps);
-    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes) != cudaSuccess)
+    if (ensure_dynamic_smem(fn, ge->smem_bytes) != cudaSuccess)
         return 0;
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 32 * ge->warps, ge->smem_bytes) != cudaSuccess ||
@@ -818,12 +818,9 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
             max_pk = 32ll * ((nk + 1) / 2);
         r.warp_bytes = (int)((R_OFF_FLAGS + (nk / 32 + 1) * 192 + max_pk * 2 + 127) & ~127ll);
         const int smem = REPLAY_WARPS * r.warp_bytes;
-        static int configured = -1;
-        if (smem > 48 * 1024 && configured < smem) {
-            if (cudaFuncSetAttribute(k_list_replay, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-                return cudaGetLastError();
-            configured = smem;
-        }
+        if (smem > 48 * 1024 && smem <= hough_vote_max_smem() &&
+            ensure_dynamic_smem((const void *)k_list_replay, smem) != cudaSuccess)
+            return cudaGetLastError();
         if (smem <= hough_vote_max_smem()) {
             k_list_replay<<<h->vote_geom.n_tiles * r.S, 32 * REPLAY_WARPS, smem, st>>>(r);
             h->launches += 1;

@@ -304,9 +304,8 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     const int step = (D <= 32 && 32 % D == 0) ? 32 / D : 0;
     if (fit_waves && step > 0 && P % step == 0 && P - step >= step) {
         int per_sm = 0;
-        cudaError_t e = h->g.pack == 2
-                            ? cudaFuncSetAttribute(k_sweep<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes)
-                            : cudaFuncSetAttribute(k_sweep<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ge->smem_bytes);
+        cudaError_t e = h->g.pack == 2 ? ensure_dynamic_smem((const void *)k_sweep<2, false>, ge->smem_bytes)
+                                       : ensure_dynamic_smem((const void *)k_sweep<1, false>, ge->smem_bytes);
         if (e == cudaSuccess)
             e = h->g.pack == 2
                     ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<2, false>, ge->threads, ge->smem_bytes)
@@ -367,14 +366,9 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
 template <int PACK, bool KC>
 static cudaError_t launch_one(const SweepParams &p, cudaStream_t st)
 {
-    static int configured_smem = -1; // per PACK instantiation
-    if (configured_smem < p.geom.smem_bytes) {
-        cudaError_t e = cudaFuncSetAttribute(k_sweep<PACK, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             p.geom.smem_bytes);
-        if (e != cudaSuccess)
-            return e;
-        configured_smem = p.geom.smem_bytes;
-    }
+    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK, KC>, p.geom.smem_bytes);
+    if (e != cudaSuccess)
+        return e;
     k_sweep<PACK, KC><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
     return cudaGetLastError();
 }

@@ -359,3 +359,41 @@ def test_many_kappa_bins_and_single_cell_tiles(hough, oracle):
     res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
                   cap_hits=ref["n_hit_entries"] + 1)
     assert_same(res, ref)
+
+
+def test_random_configurations_share_the_process(hough, oracle):
+    """60 random grids / detectors / tile overrides / hit counts in ONE process, handles created
+    and destroyed back to back: besides parity this guards the per-kernel shared-memory limit
+    (a small-tile handle must not lower it under a later large-tile one)."""
+    for seed in range(60):
+        rng = np.random.default_rng(1000 + seed)
+        n_phi = int(rng.integers(3, 90))
+        n_d0 = int(rng.choice([1, 2, 3, 5, 8, 13, 20, 33, 40]))
+        nk = int(rng.choice([32, 64, 96, 128, 160, 256, 512, 1024]))
+        nl = int(rng.choice([3, 10, 16, 17, 32]))
+        wrap = int(rng.integers(0, 2))
+        kw = dict(n_phi=n_phi, n_d0=n_d0, n_kappa=nk, L_min=int(rng.integers(1, min(nl, 4) + 1)),
+                  layer_radii=tuple(2.0 + 70.0 * (i + 1) / nl for i in range(nl)), phi_wrap=wrap)
+        if n_d0 == 1:
+            kw.update(d0_min=0.0, d0_max=0.0)
+        elif rng.random() < 0.5:
+            kw.update(d0_min=float(rng.uniform(-20, 0)), d0_max=float(rng.uniform(1, 25)))
+        if rng.random() < 0.5:
+            a = float(rng.uniform(-0.03, 0.01))
+            kw.update(kappa_min=a, kappa_max=a + float(rng.uniform(0.002, 0.05)))
+        if not wrap or rng.random() < 0.3:
+            a = float(rng.uniform(-3, 0))
+            kw.update(phi_min=a, phi_max=a + float(rng.uniform(0.5, 6.0)))
+        grid = synth.Grid(**kw)
+        n = int(rng.choice([0, 1, 31, 200, 513, 1500, 3000]))
+        r, ph = rng.uniform(0.3, 80, n), rng.uniform(-math.pi, math.pi, n)
+        x, y = (r * np.cos(ph)).astype(np.float32), (r * np.sin(ph)).astype(np.float32)
+        layer = rng.integers(-1 if rng.random() < 0.2 else 0, nl + (1 if rng.random() < 0.2 else 0),
+                             n).astype(np.int32)
+        ref = oracle.run(grid, x, y, layer)
+        tile = (0, 0) if rng.random() < 0.5 else (int(rng.integers(1, 20)),
+                                                  int(rng.integers(1, min(n_d0, 12) + 1)))
+        res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                      cap_hits=max(ref["n_hit_entries"], 1) + 3, tile_phi=tile[0], tile_d0=tile[1],
+                      options=int(rng.integers(0, 2)))
+        assert_same(res, ref)
