@@ -75,7 +75,7 @@ typedef struct hough_config {
     double phi_min, phi_max;       /* phi_max > phi_min */
     double d0_min, d0_max;         /* d0_max >= d0_min (equal only if n_d0 == 1) */
     double kappa_min, kappa_max;   /* kappa_max > kappa_min */
-    int32_t n_phi, n_d0, n_kappa;  /* >= 1; n_kappa a multiple of 32; n_phi*n_d0*n_kappa < 2^32 */
+    int32_t n_phi, n_d0, n_kappa;  /* >= 1; n_kappa a multiple of 32, <= 16384; n_phi*n_d0*n_kappa < 2^32 */
     int32_t L_min;                 /* 1..n_layers */
     int32_t phi_wrap;              /* 1: phi0 is periodic in the peak test (needs n_phi >= 3); 0: not */
     uint32_t max_hits;             /* largest n accepted by hough_vote / hough_process_host */

@@ -158,4 +158,4 @@ int hough_vote_max_smem(void);
 cudaError_t ensure_dynamic_smem(const void *kernel, int bytes);
 
 #define HOUGH_CHUNK 512       // hits per staged chunk
-#define HOUGH_SCAN_ITEMS 2048 // items per block of the chained scan
+#define HOUGH_SCAN_ITEMS 512  // items per block of the chained scan
