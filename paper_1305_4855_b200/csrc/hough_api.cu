@@ -311,7 +311,10 @@ static int choose_geometry(hough_handle *h)
             JW = (3 + RJ - 1) / RJ;
         if (JW > max_jw)
             JW = max_jw;
-        int Li = env_int("HOUGH_PEAK_LI", 16);
+        // planes per CTA: 24 (8 % halo planes) when that still leaves >= 4 waves of CTAs, else 16
+        const long long ctas24 = (long long)((c.n_kappa + 255) / 256) * ((c.n_d0 + RJ * JW - 3) / (RJ * JW - 2)) *
+                                 ((c.n_phi + 23) / 24);
+        int Li = env_int("HOUGH_PEAK_LI", ctas24 >= 8LL * h->n_sms ? 24 : 16);
         if (Li > c.n_phi)
             Li = c.n_phi;
         if (Li < 1)

@@ -11,6 +11,8 @@
 // in DESIGN.md section 2 A6: with key(b) = (popcount, -lin) a bin is a peak iff its key
 // beats the key of every existing neighbour, i.e. popcount > every neighbour of lower lin
 // and >= every neighbour of higher lin.
+#include <type_traits>
+
 #include "hough_internal.cuh"
 
 // ------------------------------------------------------------------ clear
@@ -104,7 +106,6 @@ __global__ void __launch_bounds__(32 * MAXJW, (PEAK_RJ == 2 && MAXJW == 16) ? 1 
     const bool e_right = (lane == 31) && (k0 + 8 < p.nk);
     const bool e_any = e_left || e_right;
     const int e_off = e_left ? -1 : 8;
-    const unsigned char *fb = p.flags;
 
     auto load_plane = [&](int pl, PeakRaw<PEAK_RJ> &R) {
         const int src = pl < 0 ? p.n_phi - 1 : (pl >= p.n_phi ? 0 : pl);
@@ -132,18 +133,38 @@ __global__ void __launch_bounds__(32 * MAXJW, (PEAK_RJ == 2 && MAXJW == 16) ? 1 
             s_bx[t][q] = 0u;
         }
 
-    auto step = [&](int pl, const PeakRaw<PEAK_RJ> &C, PeakRaw<PEAK_RJ> &N) {
-        if (pl > ib)
+    // shared-memory exchange through 32-bit addresses: this thread's rows, and the rows of
+    // the warps below / above (r = 0 and r = rows-1 are halo rows and never output)
+    const uint32_t ex0 = (uint32_t)__cvta_generic_to_shared(ex);
+    const uint32_t ex_half = (uint32_t)rows * (uint32_t)KW * 512u;
+    uint32_t ex_mine[PEAK_RJ];
+#pragma unroll
+    for (int t = 0; t < PEAK_RJ; ++t)
+        ex_mine[t] = ex0 + (uint32_t)(((jw * PEAK_RJ + t) * KW + kw) * 32 + lane) * 16u;
+    const uint32_t ex_dn = ex0 + (uint32_t)((max(jw * PEAK_RJ - 1, 0) * KW + kw) * 32 + lane) * 16u;
+    const uint32_t ex_up = ex0 + (uint32_t)((min(jw * PEAK_RJ + PEAK_RJ, rows - 1) * KW + kw) * 32 + lane) * 16u;
+    const int bar_dn = 1 + (jw - 1) * KW + kw, bar_up = 1 + jw * KW + kw;
+    const bool has_dn = jw > 0, has_up = jw < p.JW - 1;
+    // flag byte of the plane being closed, per row (advanced by one plane per step)
+    long long fo[PEAK_RJ];
+#pragma unroll
+    for (int t = 0; t < PEAK_RJ; ++t)
+        fo[t] = (long long)fbyte[t] + ((long long)ia - 3) * (long long)(plane_stride >> 3);
+    uint32_t exo = 0;
+
+    // One plane.  STEADY: an interior plane (0 < pl < n_phi) that is ours and whose predecessor
+    // is ours too: masks and the strictness of the comparisons are compile-time constants.
+    auto step = [&](int pl, const PeakRaw<PEAK_RJ> &C, PeakRaw<PEAK_RJ> &N, auto steady_tag) {
+        constexpr bool STEADY = decltype(steady_tag)::value;
+        if (!STEADY && pl > ib)
             return;
-        if (pl < ib)
+        if (STEADY || pl < ib)
             load_plane(pl + 1, N);
-        const uint32_t pmask = ((pl < 0 || pl >= p.n_phi) && !p.wrap) ? 0u : 0xffffffffu;
-        const bool out_prev = (pl - 1 >= ia);          // plane pl-1 is one of ours: close it
-        const bool open_cur = (pl >= ia) && (pl < ib); // plane pl is one of ours: open it
+        const uint32_t pmask = STEADY ? 0xffffffffu : (((pl < 0 || pl >= p.n_phi) && !p.wrap) ? 0u : 0xffffffffu);
+        const bool out_prev = STEADY ? true : (pl - 1 >= ia); // plane pl-1 is one of ours: close it
         // strictness of the comparison with the neighbouring planes (phi wrap changes lin order)
-        const uint32_t d_next = ((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u;
-        const uint32_t d_prev = ((pl == 0) && p.wrap) ? 0u : ONE;
-        uint4 *exw = ex + (size_t)((pl - ia + 1) & 1) * rows * KW * 32;
+        const uint32_t d_next = STEADY ? 0u : (((pl - 1 == p.n_phi - 1) && p.wrap) ? ONE : 0u);
+        const uint32_t d_prev = STEADY ? ONE : (((pl == 0) && p.wrap) ? 0u : ONE);
 
         // ---- phase A: pair popcounts, kappa shifts, m3; publish m3 of every row
         uint32_t c[PEAK_RJ][4], s[PEAK_RJ][5], m3[PEAK_RJ][4];
@@ -169,75 +190,74 @@ __global__ void __launch_bounds__(32 * MAXJW, (PEAK_RJ == 2 && MAXJW == 16) ? 1 
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 m3[t][q] = __vimax3_u16x2(c[t][q], s[t][q], s[t][q + 1]);
-            exw[((jw * PEAK_RJ + t) * KW + kw) * 32 + lane] = make_uint4(m3[t][0], m3[t][1], m3[t][2], m3[t][3]);
+            asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(ex_mine[t] + exo), "r"(m3[t][0]), "r"(m3[t][1]),
+                         "r"(m3[t][2]), "r"(m3[t][3])
+                         : "memory");
         }
         // A warp only needs the rows of the warps below and above it: pair barriers (named
         // barrier 1 + jw*KW + kw joins warps (jw, kw) and (jw+1, kw)) instead of a CTA-wide
         // one.  Lower id first on both sides, so the chain cannot deadlock; the exchange
         // buffer is double buffered, and passing the pair barriers of plane p+1 implies that
         // the neighbours have finished reading plane p.
-        if (jw > 0)
-            asm volatile("bar.sync %0, 64;" ::"r"(1 + (jw - 1) * KW + kw) : "memory");
-        if (jw < p.JW - 1)
-            asm volatile("bar.sync %0, 64;" ::"r"(1 + jw * KW + kw) : "memory");
+        if (has_dn)
+            asm volatile("bar.sync %0, 64;" ::"r"(bar_dn) : "memory");
+        if (has_up)
+            asm volatile("bar.sync %0, 64;" ::"r"(bar_up) : "memory");
 
-        // ---- phase B: box maxima; close plane pl-1; open plane pl
+        // ---- phase B: box maxima; close plane pl-1; open plane pl (always computed: a plane
+        // that is not ours is simply never stored)
+        uint4 vdn, vup;
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(vdn.x), "=r"(vdn.y), "=r"(vdn.z), "=r"(vdn.w) : "r"(ex_dn + exo));
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(vup.x), "=r"(vup.y), "=r"(vup.z), "=r"(vup.w) : "r"(ex_up + exo));
 #pragma unroll
         for (int t = 0; t < PEAK_RJ; ++t) {
-            const int r = jw * PEAK_RJ + t;
             uint32_t dn[4], up[4];
             if (t > 0) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
                     dn[q] = m3[t - 1][q];
             } else {
-                const uint4 v = exw[(max(r - 1, 0) * KW + kw) * 32 + lane]; // r = 0 is a halo row: never output
-                dn[0] = v.x, dn[1] = v.y, dn[2] = v.z, dn[3] = v.w;
+                dn[0] = vdn.x, dn[1] = vdn.y, dn[2] = vdn.z, dn[3] = vdn.w;
             }
             if (t < PEAK_RJ - 1) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
                     up[q] = m3[t + 1][q];
             } else {
-                const uint4 v = exw[(min(r + 1, rows - 1) * KW + kw) * 32 + lane];
-                up[0] = v.x, up[1] = v.y, up[2] = v.z, up[3] = v.w;
+                up[0] = vup.x, up[1] = vup.y, up[2] = vup.z, up[3] = vup.w;
             }
-            uint32_t bx[4];
+            uint32_t bits = 0u;
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
-                bx[q] = __vimax3_u16x2(dn[q], m3[t][q], up[q]);
-            if (out_prev && rout[t]) {
-                uint32_t bits = 0u;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const uint32_t thr = __vmaxu2(s_thr[t][q], bx[q] + d_next);
-                    const uint32_t g = (s_o[t][q] - thr) >> (15 - 2 * q); // bin 2q -> bit 2q, 2q+1 -> bit 16+2q
-                    bits |= g & (ONE << (2 * q));
-                }
-                bits = (bits | (bits >> 15)) & 0xffu;
-                const_cast<unsigned char *>(fb)[(size_t)(pl - 1) * (plane_stride >> 3) + fbyte[t]] =
-                    (unsigned char)bits;
+            for (int q = 0; q < 4; ++q) {
+                const uint32_t bx = __vimax3_u16x2(dn[q], m3[t][q], up[q]);
+                const uint32_t thr = __vmaxu2(s_thr[t][q], bx + d_next);
+                const uint32_t g = (s_o[t][q] - thr) >> (15 - 2 * q); // bin 2q -> bit 2q, 2q+1 -> bit 16+2q
+                bits |= g & (ONE << (2 * q));
+                const uint32_t lo = __vmaxu2(dn[q], s[t][q]);                  // lower lin: pc must exceed
+                const uint32_t hi = __vimax3_u16x2(up[q], s[t][q + 1], lmin2); // higher lin: pc must reach
+                s_thr[t][q] = __vimax3_u16x2(lo + ONE, hi, s_bx[t][q] + d_prev);
+                s_o[t][q] = c[t][q] | HB;
+                s_bx[t][q] = bx;
             }
-            if (open_cur) {
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const uint32_t lo = __vmaxu2(dn[q], s[t][q]);            // lower lin: pc must exceed
-                    const uint32_t hi = __vimax3_u16x2(up[q], s[t][q + 1], lmin2); // higher lin: pc must reach
-                    s_thr[t][q] = __vimax3_u16x2(lo + ONE, hi, s_bx[t][q] + d_prev);
-                    s_o[t][q] = c[t][q] | HB;
-                }
-            }
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                s_bx[t][q] = bx[q];
+            fo[t] += (long long)(plane_stride >> 3);
+            if (out_prev && rout[t])
+                p.flags[fo[t]] = (unsigned char)((bits | (bits >> 15)) & 0xffu);
         }
+        exo ^= ex_half;
     };
 
     PeakRaw<PEAK_RJ> A, B;
     load_plane(ia - 1, A);
+    const int st_lo = max(ia + 1, 1), st_hi = min(ib - 1, p.n_phi - 1); // steady planes: [st_lo, st_hi]
     for (int pl = ia - 1; pl <= ib; pl += 2) {
-        step(pl, A, B);
-        step(pl + 1, B, A);
+        if (pl >= st_lo && pl <= st_hi)
+            step(pl, A, B, std::true_type());
+        else
+            step(pl, A, B, std::false_type());
+        if (pl + 1 >= st_lo && pl + 1 <= st_hi)
+            step(pl + 1, B, A, std::true_type());
+        else
+            step(pl + 1, B, A, std::false_type());
     }
 }
 
