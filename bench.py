@@ -135,6 +135,16 @@ def ncu_traffic(kernel_key):
         return json.load(f).get(kernel_key)
 
 
+def input_digest(event):
+    """SHA-256 over x, y, layer of one generated event (inputs are seeded and
+    reproducible; the digest lets two runs prove they measured the same hits)."""
+    import hashlib
+    h = hashlib.sha256()
+    for a in event:
+        h.update(np.ascontiguousarray(a).tobytes())
+    return h.hexdigest()
+
+
 def oracle_module():
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     try:
@@ -332,6 +342,8 @@ def main():
                        "L_min": workload.grid.L_min, "hits_per_event": int(np.mean([len(e[0]) for e in events])),
                        "l2": "512 MiB flush buffer written between steps, outside the event pairs",
                        "parallelism": "replicas x%d (events sharded by seed, no collective)" % world},
+            "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(np.min(step_ms)),
+            "inputs_sha256_first_event": input_digest(events[0]),
             "events_per_s": events_all * args.steps / secs,
             "evaluations_per_s": evals_all * args.steps / secs,
             "votes_per_event": votes_step / n_ev,

@@ -70,3 +70,12 @@ def test_oracle_regression_fixture(oracle):
         assert r["peak_mask"].tolist() == rec["peak_mask"]
         assert r["hit_offset"].tolist() == rec["hit_offset"]
         assert r["hit_index"].tolist() == rec["hit_index"]
+
+
+def test_first_batch_event_digest_is_stable():
+    """The inputs bench.py measures are reproducible bit for bit (its JSON line carries the
+    SHA-256 of the first event; this pins the generator's draw order and dtype handling)."""
+    import bench
+    w = synth.WORKLOADS["batch100"]
+    e = synth.generate_event(w.event, w.seeds[0])[:3]
+    assert bench.input_digest(e) == "6c3d9e0a77886577e984fbb164db541f5f97a879b8efe0c25b6346838d03ea5a"
