@@ -19,8 +19,8 @@
 // per CTA against the super-tile (lane = hit, order-preserving compaction) and per warp
 // against its sub-tile (lane = hit, ballot), then the exact recipe runs on the survivors.
 // If the entry buffer (cap_hits entries) overflows, the output is truncated anyway
-// (n_hit_entries > cap_hits); k_list_slow then refills the lists that still fit directly
-// from the hits, one warp per peak.
+// (n_hit_entries > cap_hits); k_scatter_entries then refills the lists that still fit
+// directly from the hits, one warp per peak (list_slow).
 #include "hough_device.cuh"
 
 #define LIST_QUEUE 64  // entries a warp buffers before it flushes (>= 2 * 32)
@@ -592,26 +592,10 @@ struct ListPlaceParams {
     unsigned long long cap_hits;
 };
 
-__global__ void __launch_bounds__(256) k_scatter_entries(const ListPlaceParams p)
-{
-    const unsigned long long n = *p.n_entries;
-    if (n > p.ent_cap)
-        return; // k_list_slow takes over
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const uint32_t sub = p.ent_sub[i];
-        const unsigned long long pos = p.hit_offset[sub / p.S] + p.sub_pre[sub] + p.ent_idx[i];
-        if (pos < p.cap_hits)
-            p.hit_index[pos] = p.ent_hit[i];
-    }
-}
-
 // Entry buffer overflowed: write the lists that start below cap_hits straight from the
 // hits, one warp per peak, ascending by construction.
-__global__ void __launch_bounds__(256) k_list_slow(const ListPlaceParams p)
+__device__ void list_slow(const ListPlaceParams &p)
 {
-    if (*p.n_entries <= p.ent_cap)
-        return;
     const GridDev &g = p.g;
     const int lane = threadIdx.x & 31;
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
@@ -640,6 +624,22 @@ __global__ void __launch_bounds__(256) k_list_slow(const ListPlaceParams p)
             }
             pos += __popc(bal);
         }
+    }
+}
+
+__global__ void __launch_bounds__(256) k_scatter_entries(const ListPlaceParams p)
+{
+    const unsigned long long n = *p.n_entries;
+    if (n > p.ent_cap) {
+        list_slow(p);
+        return;
+    }
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint32_t sub = p.ent_sub[i];
+        const unsigned long long pos = p.hit_offset[sub / p.S] + p.sub_pre[sub] + p.ent_idx[i];
+        if (pos < p.cap_hits)
+            p.hit_index[pos] = p.ent_hit[i];
     }
 }
 
@@ -857,7 +857,6 @@ cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cuda
     p.hit_index = out->hit_index;
     p.cap_hits = h->cfg.cap_hits;
     k_scatter_entries<<<h->n_sms * 16, 256, 0, st>>>(p);
-    k_list_slow<<<h->n_sms * 4, 256, 0, st>>>(p);
-    h->launches += 2;
+    h->launches += 1;
     return cudaGetLastError();
 }
