@@ -668,6 +668,8 @@ static const void *list_sweep_fn(int warps)
     switch (warps) {
     case 16:
         return (const void *)k_list_sweep<16>;
+    case 12:
+        return (const void *)k_list_sweep<12>;
     case 8:
         return (const void *)k_list_sweep<8>;
     case 4:
@@ -687,6 +689,12 @@ int list_geom_init(hough_handle *h)
     while (SD > c.n_d0)
         SD >>= 1;
     int SP = 32 / SD, warps = LIST_WARPS;
+    {
+        const char *e = getenv("HOUGH_LIST_WARPS"); // 16 (default), 12, 8, 4, 2, 1
+        const int w = e ? atoi(e) : 0;
+        if (w == 12 || w == 8 || w == 4 || w == 2 || w == 1)
+            warps = w;
+    }
     const int wpr = c.n_kappa / 32;
     // The per-warp tables grow with n_kappa: fewer warps per CTA first, then fewer cells per
     // warp (idle lanes), until the CTA fits (n_kappa = 256: 16 warps; 2048: 4; 16384: 1 warp
@@ -699,7 +707,7 @@ int list_geom_init(hough_handle *h)
         if (ge->smem_bytes <= hough_vote_max_smem())
             break;
         if (warps > 1)
-            warps >>= 1;
+            warps = warps == 12 ? 8 : warps >> 1;
         else if (SP > 1)
             SP >>= 1;
         else if (SD > 1)
@@ -713,6 +721,12 @@ int list_geom_init(hough_handle *h)
     ge->WD = 1;
     while (ge->WD < 4 && ge->WD * 2 <= warps && ge->WD * 2 * SD <= c.n_d0)
         ge->WD *= 2;
+    {
+        const char *e = getenv("HOUGH_LIST_WD"); // sub-tiles side by side along d0 (1, 2, 4, ...)
+        const int wd = e ? atoi(e) : 0;
+        if (wd >= 1 && wd <= warps && warps % wd == 0)
+            ge->WD = wd;
+    }
     ge->WP = warps / ge->WD;
     ge->tiles_phi = (c.n_phi + ge->WP * ge->SP - 1) / (ge->WP * ge->SP);
     ge->tiles_d0 = (c.n_d0 + ge->WD * ge->SD - 1) / (ge->WD * ge->SD);
