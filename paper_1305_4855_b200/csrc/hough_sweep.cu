@@ -119,8 +119,10 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const int nkm1 = nk - 1;
     // byte address of this cell's row in the tile and its word swizzle (in bytes)
     const int row_words = PACK == 2 ? (nk >> 1) : nk;
-    const uint32_t row_addr = smem_u32(tile) + (uint32_t)c * (uint32_t)row_words * 4u;
-    const uint32_t swzb = (uint32_t)(lane & p.swz_mask) << 2;
+    uint32_t row_addr = smem_u32(tile) + (uint32_t)c * (uint32_t)row_words * 4u;
+    uint32_t swzb = (uint32_t)(lane & p.swz_mask) << 2;
+    // keep both in registers: recomputing them inside the vote path costs more than it saves
+    asm volatile("" : "+r"(row_addr), "+r"(swzb));
 
     for (uint32_t ch = 0; ch < n_chunks; ++ch) {
         const float *st = stage + (size_t)(ch & 1) * 4 * ge.chunk;
