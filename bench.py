@@ -410,10 +410,12 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
         "kernel": "k_sweep (vote)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
         "unit": "TFLOP/s", "frac": achieved / alu_peak, "traffic": ncu_traffic("vote"),
         "note": "algorithmic fp32 ops = 15 x n x n_phi x n_d0 per launch (every hit x cell); the "
-                "conservative cull executes only executed_frac of them; peak = SMs x 128 fp32 "
+                "conservative cull proves that 1 - executed_frac of them cannot vote and skips them, so "
+                "frac can exceed 1 (frac_executed counts only the evaluations run); peak = SMs x 128 fp32 "
                 "lanes x sm_max_mhz without FMA (the recipe forbids contraction); "
                 + peaks_info["source"],
         "executed_frac": evals_done_step / evals_step,
+        "frac_executed": FLOP_PER_EVAL * (evals_done_step / n_ev) / vote_s / 1e12 / alu_peak,
         "achieved_executed": FLOP_PER_EVAL * (evals_done_step / n_ev) / vote_s / 1e12,
         "dominant_stage_measured": dom}
 
