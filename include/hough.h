@@ -30,7 +30,10 @@
  *     Calls that take a stream only ENQUEUE work and return without synchronising,
  *     unless stated otherwise.  One handle is used from one stream at a time.
  *   - Every int-returning call returns HOUGH_OK (0) or a negative HOUGH_E* code; nothing
- *     throws across the boundary; there is no global state.
+ *     throws across the boundary.  All configuration is the hough_config struct: the library
+ *     reads no environment variable.  Its only process-wide state is a mutex-guarded record
+ *     of the dynamic shared-memory limit it has set per (kernel, device) -- a CUDA attribute
+ *     that is itself process-wide; handles share nothing else and may live on different threads.
  *   - There is no CPU fallback: without a CUDA device every compute call returns
  *     HOUGH_ECUDA.
  *   - Accumulator layout: bin (i, j, k) at linear index lin = (i*n_d0 + j)*n_kappa + k
@@ -59,6 +62,8 @@ extern "C" {
 /* hough_config.options */
 #define HOUGH_OPT_NO_CULL 1u      /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
 #define HOUGH_OPT_STAGE_TIMING 2u /* record a CUDA event after every kernel (see hough_stage_times) */
+#define HOUGH_OPT_UNPACKED 4u     /* one mask per 32-bit word of the vote tile even with <= 16 layers (test hook
+                                     for the tile layout used with 17..32 layers) */
 
 typedef struct hough_handle hough_handle; /* opaque */
 
@@ -73,12 +78,12 @@ typedef struct hough_config {
     int32_t n_layers;              /* 1..32; hit layer l sets mask bit l */
     const double *layer_radius_cm; /* [host] n_layers radii, > 0; metadata only: the vote uses the hit's own x^2+y^2 */
     double phi_min, phi_max;       /* phi_max > phi_min */
-    double d0_min, d0_max;         /* d0_max >= d0_min (equal only if n_d0 == 1) */
-    double kappa_min, kappa_max;   /* kappa_max > kappa_min */
+    double d0_min, d0_max;         /* d0_max >= d0_min (equal only if n_d0 == 1); |d0| <= 1e15 */
+    double kappa_min, kappa_max;   /* kappa_max > kappa_min; |kappa| <= 1e15 */
     int32_t n_phi, n_d0, n_kappa;  /* >= 1; n_kappa a multiple of 32, <= 16384; n_phi*n_d0*n_kappa < 2^32 */
     int32_t L_min;                 /* 1..n_layers */
     int32_t phi_wrap;              /* 1: phi0 is periodic in the peak test (needs n_phi >= 3); 0: not */
-    uint32_t max_hits;             /* largest n accepted by hough_vote / hough_process_host */
+    uint32_t max_hits;             /* largest n accepted by hough_vote / hough_process_host (<= 1 044 480) */
     uint32_t cap_peaks;            /* capacity of the caller's peak arrays (>= 1) */
     uint64_t cap_hits;             /* capacity of the caller's hit_index array (>= 1) */
     int32_t tile_phi, tile_d0;     /* accumulator tile owned by one CTA, in cells; 0 = choose automatically */
@@ -86,12 +91,13 @@ typedef struct hough_config {
     int32_t device;                /* CUDA device ordinal */
 } hough_config;
 
-/* Counters of one event, 40 bytes, same layout on host and device. */
+/* Counters of one event, 48 bytes, same layout on host and device. */
 typedef struct hough_counts {
     uint64_t n_votes;       /* votes cast (in-range solutions over all hit x cell pairs) */
     uint64_t n_hit_entries; /* TRUE total length of the hit lists of the reported peaks */
     uint64_t n_evals;       /* closed-form evaluations the vote kernel executed after its conservative
                                cull (<= n * n_phi * n_d0; equal to it with HOUGH_OPT_NO_CULL) */
+    uint64_t n_list_evals;  /* evaluations the hit-list stage executed (0 after hough_peaks_only) */
     uint32_t n_peaks;       /* TRUE number of peaks (may exceed cap_peaks) */
     uint32_t n_bad_hits;    /* hits with layer outside [0, n_layers): cast no vote */
     uint32_t flags;         /* HOUGH_TRUNCATED_* */
@@ -220,10 +226,11 @@ int hough_peaks_only(hough_handle *h, const hough_peaks_out *out, void *cuda_str
  * mode 1: atomicOr, pseudo-random addresses (bank conflicts as they fall);
  * mode 2: plain load/OR/store on the same conflict-free addresses (no atomic), for comparison.
  * Enqueues on the stream; *lane_ops (host) receives the number of lane-operations one
- * launch performs.  Time it with CUDA events around the call.
+ * launch performs.  sink_dev: [device] 4 bytes of caller-owned scratch (keeps the compiler from
+ * dropping the loop; the library allocates nothing).  Time it with CUDA events around the call.
  */
 int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters,
-                          void *cuda_stream, uint64_t *lane_ops);
+                          uint32_t *sink_dev, void *cuda_stream, uint64_t *lane_ops);
 
 /* Geometry the library chose (for reporting): tile_phi, tile_d0, n_tiles, threads per CTA,
  * dynamic shared memory bytes of the vote kernel, number of SMs.  Any pointer may be NULL. */

@@ -2,6 +2,7 @@
 // tables (A1), the workspace carve-up, hit preparation (a1) and the call sequences of
 // hough_vote / hough_peaks.  No torch types, no exceptions, no global state.
 #include <math.h>
+#include <mutex>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -54,16 +55,21 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize holds the LAST value set, not the largest: a
 // handle with a small tile must not take the limit away from a live handle with a large one.
+// The attribute belongs to the (kernel, device) pair, i.e. to the process, so the record of
+// what has been set is process-wide too; it is the library's only static state and is
+// guarded by a mutex (handles may be created from different threads).
 cudaError_t ensure_dynamic_smem(const void *kernel, int bytes)
 {
     struct Entry {
         const void *fn;
         int device, bytes;
     };
-    static Entry table[64];
+    static Entry table[128];
     static int n_entries = 0;
+    static std::mutex mu;
     int device = 0;
     cudaGetDevice(&device);
+    std::lock_guard<std::mutex> lock(mu);
     Entry *e = nullptr;
     for (int i = 0; i < n_entries; ++i)
         if (table[i].fn == kernel && table[i].device == device)
@@ -73,7 +79,7 @@ cudaError_t ensure_dynamic_smem(const void *kernel, int bytes)
     cudaError_t rc = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (rc != cudaSuccess)
         return rc;
-    if (!e && n_entries < 64) {
+    if (!e && n_entries < 128) {
         e = &table[n_entries++];
         e->fn = kernel;
         e->device = device;
@@ -117,6 +123,11 @@ static int cfg_valid(const hough_config *c)
         return 0;
     if (c->n_kappa > 16384)
         return 0; // one cell row must fit a shared-memory tile
+    // magnitudes the conservative cull's interval arithmetic cannot overflow on (hough.h)
+    if (fabs(c->d0_min) > 1e15 || fabs(c->d0_max) > 1e15 || fabs(c->kappa_min) > 1e15 || fabs(c->kappa_max) > 1e15)
+        return 0;
+    if (!list_config_ok(c))
+        return 0; // max_hits beyond what the hit-list segmentation supports
     return 1;
 }
 
@@ -131,25 +142,6 @@ struct Carve {
         return p;
     }
 };
-
-static int env_int(const char *name, int dflt);
-
-// u16 entries of the kappa-code cache: HOUGH_KC_PERCENT % of the worst case (default 0 = off:
-// measured slower than re-evaluating; 35 holds config 3/4)
-// (every hit x every cell + 25 % row overhead); 0 switches the cache off.
-size_t kc_entries_for(const hough_config *c)
-{
-    const int pct = env_int("HOUGH_KC_PERCENT", 0);
-    if (pct <= 0)
-        return 0;
-    const double hp = (double)(((c->max_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK);
-    double e = hp * (double)c->n_phi * (double)c->n_d0 * 1.25 * (double)pct / 100.0;
-    if (e < 1048576.0)
-        e = 1048576.0;
-    if (e > 6.0e10)
-        e = 6.0e10;
-    return ((size_t)e + 1023) & ~(size_t)1023;
-}
 
 static uint32_t pad_hits(uint32_t n)
 {
@@ -183,10 +175,6 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *peak_len = cv.take((size_t)c->cap_peaks * 4);
     void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
-    const size_t kc_cap = kc_entries_for(c);
-    const uint32_t kc_chunks = hp / HOUGH_CHUNK;
-    void *kc_buf = cv.take(kc_cap * 2);
-    void *kc_tab = cv.take(kc_cap ? n_rows * (size_t)kc_chunks * 8 : 0);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -211,11 +199,6 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ent_sub = (uint32_t *)ent_sub;
         h->ent_hit = (uint32_t *)ent_hit;
         h->ent_idx = (uint32_t *)ent_idx;
-        h->kc_buf = (unsigned short *)kc_buf;
-        h->kc_cap = kc_cap;
-        h->kc_tab = (uint2 *)kc_tab;
-        h->kc_chunks = kc_chunks;
-        h->kc_on = kc_cap > 0;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
@@ -232,29 +215,22 @@ size_t hough_workspace_bytes(const hough_config *cfg)
     return carve_workspace(cfg, nullptr, nullptr);
 }
 
-static int env_int(const char *name, int dflt)
-{
-    const char *s = getenv(name);
-    if (!s || !*s)
-        return dflt;
-    return atoi(s);
-}
-
 // Tile shapes.  Defaults aim at two resident CTAs per SM (<= ~113 KB of shared memory
-// each); cfg.tile_phi / tile_d0 or the HOUGH_TILE_* environment variables override.
+// each); cfg.tile_phi / tile_d0 override the vote tile.  All configuration comes from
+// hough_config (no environment variables).
 static int choose_geometry(hough_handle *h)
 {
     const hough_config &c = h->cfg;
     const int nk = c.n_kappa;
-    const int budget = env_int("HOUGH_SMEM_BUDGET", 113 * 1024);
+    const int budget = 113 * 1024;
     const int staging = 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 8) * 16 + 1024;
     // vote
     {
         int cell_bytes = nk * 4 / h->g.pack;
-        int D = c.tile_d0 > 0 ? c.tile_d0 : env_int("HOUGH_TILE_D0", c.n_d0 < 8 ? c.n_d0 : 8);
+        int D = c.tile_d0 > 0 ? c.tile_d0 : (c.n_d0 < 8 ? c.n_d0 : 8);
         if (D > c.n_d0)
             D = c.n_d0;
-        int P = c.tile_phi > 0 ? c.tile_phi : env_int("HOUGH_TILE_PHI", 0);
+        int P = c.tile_phi;
         if (P <= 0) {
             // whole cell groups (32 lanes) only: a padded group costs a full group of
             // shared memory and lanes (fine grid: 11 x 8 cells = 96 KB + staging -> 1 CTA/SM,
@@ -273,17 +249,14 @@ static int choose_geometry(hough_handle *h)
         if (P > c.n_phi)
             P = c.n_phi;
         int groups = (P * D + 31) / 32;
-        int split = env_int("HOUGH_VOTE_SPLIT", 0);
-        if (split <= 0) {
-            split = 512 / (32 * groups);
-            if (split < 1)
-                split = 1;
-            if (split > 8)
-                split = 8;
-        }
+        int split = 512 / (32 * groups);
+        if (split < 1)
+            split = 1;
+        if (split > 8)
+            split = 8;
         while (split > 1 && 32 * groups * split > 1024)
             --split;
-        const int fit = (c.tile_phi == 0 && env_int("HOUGH_TILE_PHI", 0) == 0 && env_int("HOUGH_FIT_WAVES", 1)) ? 1 : 0;
+        const int fit = c.tile_phi == 0 ? 1 : 0;
         if (!sweep_geom_init(h, &h->vote_geom, P, D, split, fit)) {
             // fall back to the smallest tile
             if (!sweep_geom_init(h, &h->vote_geom, 1, 1, 4, 0))
@@ -293,37 +266,27 @@ static int choose_geometry(hough_handle *h)
     // hit lists: warp sub-tiles, hit segments (hough_lists.cu)
     if (!list_geom_init(h))
         return 0;
-    // peak sweep: JW warps x RJ rows per thread and CTA (2 of the rows are halo rows), Li
-    // phi0 planes per CTA.  RJ = 2: 8 warps, more registers; RJ = 1: 16 warps, more exchange.
+    // peak sweep: JW warps x 2 rows per thread and CTA (2 of the rows are halo rows), Li phi0
+    // planes per CTA
     {
-        int RJ = env_int("HOUGH_PEAK_RJ", 2);
-        if (RJ != 1)
-            RJ = 2;
-        int KW = env_int("HOUGH_PEAK_KW", 1); // warps side by side along kappa (256 bins each)
-        if (KW < 1 || KW > 4 || KW * 256 > ((c.n_kappa + 255) / 256) * 256)
-            KW = 1;
-        const int max_jw = 16 / KW; // at most 16 warps per CTA
-        int JW = env_int("HOUGH_PEAK_JW", RJ == 1 ? 16 : 8);
+        const int RJ = 2;
+        int JW = 8;
         int need = (c.n_d0 + 2 + RJ - 1) / RJ; // warps that cover every row plus the two halo rows
         if (JW > need)
             JW = need;
         if (JW * RJ < 3)
             JW = (3 + RJ - 1) / RJ;
-        if (JW > max_jw)
-            JW = max_jw;
         // planes per CTA: 24 (8 % halo planes) when that still leaves >= 4 waves of CTAs, else 16
         const long long ctas24 = (long long)((c.n_kappa + 255) / 256) * ((c.n_d0 + RJ * JW - 3) / (RJ * JW - 2)) *
                                  ((c.n_phi + 23) / 24);
-        int Li = env_int("HOUGH_PEAK_LI", ctas24 >= 8LL * h->n_sms ? 24 : 16);
+        int Li = ctas24 >= 8LL * h->n_sms ? 24 : 16;
         if (Li > c.n_phi)
             Li = c.n_phi;
         if (Li < 1)
             Li = 1;
         h->pk_JW = JW;
-        h->pk_RJ = RJ;
-        h->pk_KW = KW;
         h->pk_Li = Li;
-        h->pk_smem = 2 * (RJ * JW) * KW * 32 * 16;
+        h->pk_smem = 2 * (RJ * JW) * 32 * 16;
     }
     return 1;
 }
@@ -400,9 +363,7 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     g.n_kappa = cfg->n_kappa;
     g.L_min = cfg->L_min;
     g.phi_wrap = cfg->phi_wrap;
-    g.pack = cfg->n_layers <= 16 ? 2 : 1;
-    if (env_int("HOUGH_FORCE_PACK1", 0))
-        g.pack = 1;
+    g.pack = (cfg->n_layers <= 16 && !(cfg->options & HOUGH_OPT_UNPACKED)) ? 2 : 1;
     g.klo = (float)cfg->kappa_min;
     g.khi = (float)cfg->kappa_max;
     g.inv_dk = (float)((double)cfg->n_kappa / (cfg->kappa_max - cfg->kappa_min));

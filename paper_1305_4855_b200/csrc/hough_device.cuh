@@ -98,8 +98,10 @@ __device__ __forceinline__ bool hit_may_vote(float x, float y, float r2, const T
         return true;
     const float EPS = 3.8146973e-06f; // 2^-18
     float ax = fabsf(x), ay = fabsf(y);
-    if (!(ax <= 3.0e38f) || !(ay <= 3.0e38f))
-        return false; // inf / NaN coordinates never vote (num/den is NaN)
+    if (!(ax <= 3.4028234664e38f) || !(ay <= 3.4028234664e38f))
+        return false; // an inf / NaN coordinate never votes: s is +-inf or NaN, so num/den is NaN
+    if (!(r2 <= 3.4028234664e38f))
+        return true; // finite coordinates whose squares overflow: den = inf, kappa = +-0 may be in range
     float r = sqrtf(r2);
     float smin, smax;
     if (tc.phi_all) {

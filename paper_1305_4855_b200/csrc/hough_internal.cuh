@@ -67,11 +67,10 @@ struct DevCounters {
     unsigned long long n_votes;
     unsigned long long n_hit_entries;
     unsigned long long n_evals;
+    unsigned long long n_list_evals;
     unsigned int n_peaks;
     unsigned int n_bad_hits;
     unsigned int flags;
-    unsigned int kc_overflow;      // the kappa-code cache of this event is incomplete
-    unsigned long long kc_cursor;  // u16 entries of the cache handed out so far
 };
 
 // stages of one event, in launch order (HOUGH_OPT_STAGE_TIMING)
@@ -101,19 +100,12 @@ struct hough_handle {
     uint32_t *peak_len;   // [cap_peaks] list length per peak
     uint32_t *ent_sub, *ent_hit, *ent_idx; // [cap_hits] entries (sub-list, hit, place) of the list sweep
     unsigned long long *n_pairs; // entries emitted (lives in the per-hough_peaks reset region)
-    // kappa-code cache: the vote sweep leaves the bin (or 0xffff) of every
-    // evaluation it executes, the hit lists replay it instead of re-evaluating
-    unsigned short *kc_buf;      // [kc_cap] u16, rows of (cells of the tile + 32) per surviving hit
-    unsigned long long kc_cap;
-    uint2 *kc_tab;               // [n_tiles][kc_chunks] (first entry / 32, survivors) per tile and chunk
-    uint32_t kc_chunks;
-    int kc_on;
     unsigned long long *scan_status; // look-back words of the chained scans
     unsigned int *scan_ticket;       // [4]
     DevCounters *counters;
     uint32_t scan_blocks_max;
     // sweep tile geometry of the peak kernel
-    int pk_JW, pk_KW, pk_RJ, pk_Li, pk_smem;
+    int pk_JW, pk_Li, pk_smem;
     // hough_submit_host / hough_collect_host: one event per slot marks the end of the slot's work
     cudaEvent_t slot_ev[2];
     unsigned char slot_busy[2];
@@ -145,7 +137,6 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
 cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
-size_t kc_entries_for(const hough_config *c);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st);
@@ -153,6 +144,7 @@ cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, in
 int sweep_geom_init(const hough_handle *h, SweepGeom *g, int P, int D, int split, int fit_waves);
 int list_geom_init(hough_handle *h);
 int list_segments_bound(const hough_config *c);
+int list_config_ok(const hough_config *c);
 int hough_vote_max_smem(void);
 // Raise (never lower) a kernel's dynamic shared-memory limit on the current device.
 cudaError_t ensure_dynamic_smem(const void *kernel, int bytes);

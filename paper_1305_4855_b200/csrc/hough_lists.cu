@@ -41,8 +41,7 @@ struct ListSweepParams {
     uint32_t *ent_sub, *ent_hit, *ent_idx; // [ent_cap] entries
     unsigned long long *n_entries;
     unsigned long long ent_cap;
-    const DevCounters *counters;
-    int kc_on; // the kappa-code cache is in use: run only if it overflowed
+    unsigned long long *n_list_evals; // evaluations executed (hough_counts.n_list_evals)
 };
 
 __device__ __forceinline__ unsigned short lds_u16(uint32_t addr)
@@ -92,8 +91,6 @@ template <int WARPS> // warps per CTA = sub-tiles per super-tile (ListGeom::warp
 __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    if (p.kc_on && !p.counters->kc_overflow)
-        return; // k_list_replay does the work from the kappa-code cache
     const GridDev &g = p.g;
     const ListGeom &ge = p.geom;
     const int nk = g.n_kappa, wpr = nk >> 5;
@@ -234,6 +231,7 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
     uint32_t *q_sub = wq, *q_hit = wq + LIST_QUEUE, *q_idx = wq + 2 * LIST_QUEUE;
     const uint32_t lt_mask = (1u << lane) - 1u;
     uint32_t qn = 0; // entries waiting in this warp's flush queue (warp-uniform)
+    unsigned long long w_evals = 0; // hits x cells this warp evaluated (warp-uniform)
     uint32_t lqp = wl4; // + OFF_LANEQ: next free slot of this lane's queue (128 bytes apart)
 
     auto flush = [&]() {
@@ -350,6 +348,7 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
                         widx[nw + __popc(bal & lt_mask)] = (unsigned short)idx;
                     nw += __popc(bal);
                 }
+                w_evals += (unsigned long long)(nw * sni * snj);
                 if (lane < 3)
                     widx[nw + lane] = (unsigned short)total; // pad to a multiple of 4 with the non-voting entry
                 __syncwarp();
@@ -376,201 +375,11 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
 
     if (qn)
         flush();
+    if (lane == 0 && w_evals)
+        atomicAdd(p.n_list_evals, w_evals);
     // ---- true lengths of this segment's sub-lists
     for (uint32_t r = 0; r < c_nrep; ++r)
         p.sub_len[(size_t)(c_gbase + r) * S + seg] = wcnt[c_lbase + r];
-}
-
-// ------------------------------------------------------------------ replay of the kappa-code cache
-// The vote sweep left, for every (surviving hit, cell) it evaluated, the kappa bin or n_kappa
-// (hough_sweep.cu).  Replaying that stream gives the same entries as k_list_sweep without
-// one closed-form evaluation: CTA = (vote tile, hit segment), warp = one cell group of the
-// tile (lane = cell), survivors in the order the vote kernel compacted them (ascending hit
-// index).  Same per-warp tables, counters, queues and sub-list ids as k_list_sweep.
-struct ListReplayParams {
-    GridDev g;
-    SweepGeom vg; // the vote kernel's tiles
-    int S;
-    uint32_t n_pad;
-    const uint32_t *flags;
-    const uint32_t *row_base;
-    const DevCounters *counters;
-    uint32_t cap_peaks;
-    uint32_t *sub_len;
-    uint32_t *ent_sub, *ent_hit, *ent_idx;
-    unsigned long long *n_entries;
-    unsigned long long ent_cap;
-    const unsigned short *kc_buf;
-    const uint2 *kc_tab;
-    uint32_t kc_chunks;
-    int warp_bytes;
-};
-
-#define REPLAY_WARPS 4
-#define REPLAY_LQ 16     // pending votes per lane (8 codes are loaded at a time)
-#define R_OFF_FLUSHQ (OFF_LANEQ + REPLAY_LQ * 128)
-#define R_OFF_FLAGS (R_OFF_FLUSHQ + 3 * LIST_QUEUE * 4)
-
-__global__ void __launch_bounds__(32 * REPLAY_WARPS) k_list_replay(const ListReplayParams p)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    if (p.counters->kc_overflow)
-        return; // the cache is incomplete: k_list_sweep re-evaluates instead
-    const GridDev &g = p.g;
-    const SweepGeom &ge = p.vg;
-    const int nk = g.n_kappa, wpr = nk >> 5;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int S = p.S;
-    const int seg = blockIdx.x % S, tile_id = blockIdx.x / S;
-    const uint32_t n_chunks = p.n_pad / HOUGH_CHUNK;
-    const uint32_t ch0 = (uint32_t)(((unsigned long long)n_chunks * seg) / S);
-    const uint32_t ch1 = (uint32_t)(((unsigned long long)n_chunks * (seg + 1)) / S);
-    if (ch0 >= ch1)
-        return;
-
-    // ---- the vote kernel's tile and this warp's cell group
-    const int tp = tile_id / ge.tiles_d0, td = tile_id % ge.tiles_d0;
-    const int Pt = tp < ge.n_big ? ge.P : ge.P_small;
-    const int i0 = tp < ge.n_big ? tp * ge.P : ge.n_big * ge.P + (tp - ge.n_big) * ge.P_small;
-    const int j0 = td * ge.D;
-    const int ni = min(Pt, g.n_phi - i0), nj = min(ge.D, g.n_d0 - j0);
-    const int groups = (Pt * ge.D + 31) >> 5, kc_row = groups * 32 + 32;
-    for (int grp = warp; grp < groups; grp += REPLAY_WARPS) { // (more than 4 groups: a warp takes several)
-        const int c = grp * 32 + lane;
-        const int il = c / ge.D, jl = c - il * ge.D;
-        const bool cell_ok = (il < ni) && (jl < nj);
-        const uint32_t c_row = cell_ok ? (uint32_t)(i0 + il) * (uint32_t)g.n_d0 + (uint32_t)(j0 + jl) : 0u;
-
-        unsigned char *wbase = smem_raw + (size_t)warp * p.warp_bytes;
-        uint32_t *wq = reinterpret_cast<uint32_t *>(wbase + R_OFF_FLUSHQ);
-        uint32_t *wflags = reinterpret_cast<uint32_t *>(wbase + R_OFF_FLAGS);
-        // one more (zero) flag word than k_list_sweep: "no vote" = bin n_kappa lands in it
-        unsigned short *wpre = reinterpret_cast<unsigned short *>(wbase + R_OFF_FLAGS + (size_t)(wpr + 1) * 128);
-        unsigned short *wcnt = wpre + (size_t)wpr * 32;
-
-        // ---- flag words, prefixes, local peak ids, counters (as in k_list_sweep)
-        const uint32_t n_rep = min(p.counters->n_peaks, p.cap_peaks);
-        uint32_t c_gbase = 0, c_nrep = 0;
-        {
-            uint32_t nr = 0;
-            const uint32_t *fw = p.flags;
-            if (cell_ok) {
-                c_gbase = p.row_base[c_row];
-                const uint32_t cnt = p.row_base[c_row + 1] - c_gbase;
-                nr = c_gbase >= n_rep ? 0u : min(cnt, n_rep - c_gbase);
-                fw += (size_t)c_row * wpr;
-            }
-            uint32_t before = 0;
-            for (int w = 0; w < wpr; ++w) {
-                uint32_t f = nr ? fw[w] : 0u;
-                while (before + (uint32_t)__popc(f) > nr)
-                    f &= ~(0x80000000u >> __clz(f));
-                wflags[w * 32 + lane] = f;
-                wpre[w * 32 + lane] = (unsigned short)before;
-                before += (uint32_t)__popc(f);
-            }
-            wflags[wpr * 32 + lane] = 0u;
-            c_nrep = before;
-        }
-        uint32_t c_lbase = c_nrep;
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, c_lbase, o);
-            if (lane >= o)
-                c_lbase += t;
-        }
-        const uint32_t w_npk = __shfl_sync(0xffffffffu, c_lbase, 31);
-        c_lbase -= c_nrep;
-        for (uint32_t q = lane; q < w_npk; q += 32)
-            wcnt[q] = 0;
-        __syncwarp();
-
-        const uint32_t wl4 = smem_u32(wbase) + (uint32_t)lane * 4u;
-        const uint32_t pre_addr = smem_u32(wpre) + (uint32_t)lane * 2u;
-        const uint32_t cnt_addr = smem_u32(wcnt) + c_lbase * 2u;
-        const uint32_t sub0 = c_gbase * (uint32_t)S + (uint32_t)seg;
-        uint32_t *q_sub = wq, *q_hit = wq + LIST_QUEUE, *q_idx = wq + 2 * LIST_QUEUE;
-        const uint32_t lt_mask = (1u << lane) - 1u;
-        uint32_t qn = 0, lqp = wl4;
-
-        auto flush = [&]() {
-            __syncwarp();
-            unsigned long long b = 0;
-            if (lane == 0)
-                b = atomicAdd(p.n_entries, (unsigned long long)qn);
-            b = __shfl_sync(0xffffffffu, b, 0);
-            for (uint32_t e = lane; e < qn; e += 32)
-                if (b + e < p.ent_cap) {
-                    p.ent_sub[b + e] = q_sub[e];
-                    p.ent_hit[b + e] = q_hit[e];
-                    p.ent_idx[b + e] = q_idx[e];
-                }
-            qn = 0;
-            __syncwarp();
-        };
-        // pending entry = kappa bin << 10 | survivor index inside the chunk; rows = this chunk's cache rows
-        auto drain = [&](const unsigned short *rows, uint32_t hit0) {
-            const uint32_t nl = (lqp - wl4) >> 7;
-            for (uint32_t e = 0;; ++e) {
-                const bool act = e < nl;
-                const unsigned bh = __ballot_sync(0xffffffffu, act);
-                if (!bh)
-                    break;
-                if (act) {
-                    const uint32_t ent = lds_off<OFF_LANEQ>(wl4 + e * 128u);
-                    const uint32_t k = ent >> 10;
-                    const uint32_t f = lds_off<R_OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
-                    const uint32_t rank = lds_u16(pre_addr + (k >> 5) * 64u) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
-                    const uint32_t ca = cnt_addr + rank * 2u;
-                    const unsigned short n = lds_u16(ca);
-                    sts_u16(ca, (unsigned short)(n + 1));
-                    const uint32_t pos = qn + (uint32_t)__popc(bh & lt_mask);
-                    q_sub[pos] = sub0 + rank * (uint32_t)S;
-                    q_hit[pos] = hit0 + rows[(size_t)(ent & 1023u) * kc_row + kc_row - 32];
-                    q_idx[pos] = n;
-                }
-                qn += (uint32_t)__popc(bh);
-                if (qn > LIST_QUEUE - 32)
-                    flush();
-            }
-            lqp = wl4;
-        };
-
-        for (uint32_t ch = ch0; ch < ch1; ++ch) {
-            const uint2 tb = p.kc_tab[(size_t)tile_id * p.kc_chunks + ch];
-            const uint32_t total = tb.y;
-            if (total == 0 || tb.x == 0xffffffffu)
-                continue;
-            const unsigned short *rows = p.kc_buf + ((unsigned long long)tb.x << 5);
-            uint32_t mo = (uint32_t)c; // 32-bit offset into this chunk's rows
-            auto one = [&](const uint32_t k, const uint32_t sidx) {
-                const uint32_t f = lds_off<R_OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
-                if ((f >> (k & 31u)) & 1u) {
-                    asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(lqp), "n"(OFF_LANEQ), "r"((k << 10) | sidx) : "memory");
-                    lqp += 128u;
-                }
-            };
-            uint32_t s0 = 0;
-            for (; s0 + 8 <= total; s0 += 8, mo += 8u * (uint32_t)kc_row) {
-                uint32_t kc[8];
-#pragma unroll
-                for (int u = 0; u < 8; ++u)
-                    kc[u] = (uint32_t)__ldg(rows + mo + (uint32_t)(u * kc_row));
-#pragma unroll
-                for (int u = 0; u < 8; ++u)
-                    one(kc[u], s0 + u);
-                if (__any_sync(0xffffffffu, lqp > wl4 + (REPLAY_LQ - 8) * 128u))
-                    drain(rows, ch * HOUGH_CHUNK);
-            }
-            for (; s0 < total; ++s0, mo += (uint32_t)kc_row)
-                one((uint32_t)__ldg(rows + mo), s0);
-            drain(rows, ch * HOUGH_CHUNK);
-        }
-        if (qn)
-            flush();
-        for (uint32_t r = 0; r < c_nrep; ++r)
-            p.sub_len[(size_t)(c_gbase + r) * S + seg] = wcnt[c_lbase + r];
-        __syncwarp();
-    }
 }
 
 // ------------------------------------------------------------------ placement
@@ -648,10 +457,17 @@ __global__ void __launch_bounds__(256) k_scatter_entries(const ListPlaceParams p
 // segments chosen so that the CTAs fill a whole number of waves as nearly as possible.
 static int list_segments_min(const hough_config *c)
 {
-    uint32_t hp = ((c->max_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
-    int s_min = (int)((hp + 65534u) / 65535u); // u16 counters: at most 65535 hits per segment
+    // u16 counters per (peak, segment): a segment is at most ceil(n_chunks / S) staged chunks
+    // and must hold fewer than 65536 hits, i.e. at most 255 chunks of LIST_CHUNK = 256 hits
+    const uint32_t hp = ((c->max_hits + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
+    const uint32_t n_chunks = hp / LIST_CHUNK;
+    const int s_min = (int)((n_chunks + 254u) / 255u);
     return s_min < 1 ? 1 : s_min;
 }
+
+// max_hits must leave S within LIST_MAX_SEGMENTS (k_sub_prefix stages 256 x (S + 1) words in
+// static-limit shared memory): at most 16 x 255 x 256 = 1 044 480 hits per event.
+int list_config_ok(const hough_config *c) { return list_segments_min(c) <= LIST_MAX_SEGMENTS; }
 
 // Upper bound of S for a configuration (sizes the sub-list tables of the workspace).
 int list_segments_bound(const hough_config *c)
@@ -668,8 +484,6 @@ static const void *list_sweep_fn(int warps)
     switch (warps) {
     case 16:
         return (const void *)k_list_sweep<16>;
-    case 12:
-        return (const void *)k_list_sweep<12>;
     case 8:
         return (const void *)k_list_sweep<8>;
     case 4:
@@ -689,12 +503,6 @@ int list_geom_init(hough_handle *h)
     while (SD > c.n_d0)
         SD >>= 1;
     int SP = 32 / SD, warps = LIST_WARPS;
-    {
-        const char *e = getenv("HOUGH_LIST_WARPS"); // 16 (default), 12, 8, 4, 2, 1
-        const int w = e ? atoi(e) : 0;
-        if (w == 12 || w == 8 || w == 4 || w == 2 || w == 1)
-            warps = w;
-    }
     const int wpr = c.n_kappa / 32;
     // The per-warp tables grow with n_kappa: fewer warps per CTA first, then fewer cells per
     // warp (idle lanes), until the CTA fits (n_kappa = 256: 16 warps; 2048: 4; 16384: 1 warp
@@ -707,7 +515,7 @@ int list_geom_init(hough_handle *h)
         if (ge->smem_bytes <= hough_vote_max_smem())
             break;
         if (warps > 1)
-            warps = warps == 12 ? 8 : warps >> 1;
+            warps >>= 1;
         else if (SP > 1)
             SP >>= 1;
         else if (SD > 1)
@@ -721,12 +529,6 @@ int list_geom_init(hough_handle *h)
     ge->WD = 1;
     while (ge->WD < 4 && ge->WD * 2 <= warps && ge->WD * 2 * SD <= c.n_d0)
         ge->WD *= 2;
-    {
-        const char *e = getenv("HOUGH_LIST_WD"); // sub-tiles side by side along d0 (1, 2, 4, ...)
-        const int wd = e ? atoi(e) : 0;
-        if (wd >= 1 && wd <= warps && warps % wd == 0)
-            ge->WD = wd;
-    }
     ge->WP = warps / ge->WD;
     ge->tiles_phi = (c.n_phi + ge->WP * ge->SP - 1) / (ge->WP * ge->SP);
     ge->tiles_d0 = (c.n_d0 + ge->WD * ge->SD - 1) / (ge->WD * ge->SD);
@@ -760,16 +562,15 @@ int list_geom_init(hough_handle *h)
         }
     }
     ge->S = best;
-    const char *e = getenv("HOUGH_LIST_SEGMENTS");
-    if (e && atoi(e) >= s_min && atoi(e) <= s_bound)
-        ge->S = atoi(e);
     return 1;
 }
 
 // sub_len[0 .. n_rep * S) = 0 (only the part this event uses)
-__global__ void __launch_bounds__(256) k_zero_sub_len(uint32_t *sub_len, const DevCounters *counters,
+__global__ void __launch_bounds__(256) k_zero_sub_len(uint32_t *sub_len, DevCounters *counters,
                                                       uint32_t cap_peaks, uint32_t S)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        counters->n_list_evals = 0ull; // hough_peaks may be repeated on the same vote
     const size_t n = (size_t)min(counters->n_peaks, cap_peaks) * S;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
@@ -798,50 +599,12 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
     p.ent_idx = h->ent_idx;
     p.n_entries = h->n_pairs;
     p.ent_cap = h->cfg.cap_hits;
-    p.counters = h->counters;
-    p.kc_on = h->kc_on;
+    p.n_list_evals = &h->counters->n_list_evals;
     k_zero_sub_len<<<h->n_sms * 8, 256, 0, st>>>(h->list_len, h->counters, h->cfg.cap_peaks,
                                                  (uint32_t)h->list_geom.S);
     h->launches += 2;
     if (p.hits.n_pad == 0)
         return cudaGetLastError();
-    if (h->kc_on) {
-        ListReplayParams r;
-        r.g = h->g;
-        r.vg = h->vote_geom;
-        r.S = h->list_geom.S;
-        r.n_pad = p.hits.n_pad;
-        r.flags = h->flags;
-        r.row_base = h->row_base;
-        r.counters = h->counters;
-        r.cap_peaks = h->cfg.cap_peaks;
-        r.sub_len = h->list_len;
-        r.ent_sub = h->ent_sub;
-        r.ent_hit = h->ent_hit;
-        r.ent_idx = h->ent_idx;
-        r.n_entries = h->n_pairs;
-        r.ent_cap = h->cfg.cap_hits;
-        r.kc_buf = h->kc_buf;
-        r.kc_tab = h->kc_tab;
-        r.kc_chunks = h->kc_chunks;
-        // bound on the peaks of one cell group: 32 consecutive cells of a P x D tile
-        const int D = h->vote_geom.D, nk = h->g.n_kappa;
-        const int g_rows = (32 % D == 0) ? (32 / D > 0 ? 32 / D : 1) : 32 / D + 2;
-        long long max_pk = (long long)((g_rows + 1) / 2) * ((((D < 32 ? D : 32)) + 1) / 2) * ((nk + 1) / 2);
-        if (max_pk > 32ll * ((nk + 1) / 2))
-            max_pk = 32ll * ((nk + 1) / 2);
-        r.warp_bytes = (int)((R_OFF_FLAGS + (nk / 32 + 1) * 192 + max_pk * 2 + 127) & ~127ll);
-        const int smem = REPLAY_WARPS * r.warp_bytes;
-        if (smem > 48 * 1024 && smem <= hough_vote_max_smem() &&
-            ensure_dynamic_smem((const void *)k_list_replay, smem) != cudaSuccess)
-            return cudaGetLastError();
-        if (smem <= hough_vote_max_smem()) {
-            k_list_replay<<<h->vote_geom.n_tiles * r.S, 32 * REPLAY_WARPS, smem, st>>>(r);
-            h->launches += 1;
-        } else {
-            p.kc_on = 0; // cannot replay: always re-evaluate
-        }
-    }
     const int blocks = h->list_geom.tiles_phi * h->list_geom.tiles_d0 * h->list_geom.S;
     void *args[] = {(void *)&p};
     return cudaLaunchKernel(list_sweep_fn(h->list_geom.warps), dim3(blocks), dim3(32 * h->list_geom.warps), args,

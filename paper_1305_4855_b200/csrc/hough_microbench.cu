@@ -40,40 +40,28 @@ __global__ void __launch_bounds__(1024) k_microbench(int iters, uint32_t *sink)
         sink[0] = acc;
 }
 
-int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters, void *cuda_stream,
-                          uint64_t *lane_ops)
+int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters, uint32_t *sink_dev,
+                          void *cuda_stream, uint64_t *lane_ops)
 {
     if (mode < 0 || mode > 2 || threads < 32 || threads > 1024 || (threads & 31) || ctas_per_sm < 1 ||
-        iters < 1)
+        iters < 1 || !sink_dev)
         return HOUGH_EINVAL;
-    // Slow host queries are done once per device: the caller times this call with events on
-    // the stream, so nothing but the launch may sit between them.
-    static int cached_device = -1, cached_sms = 0;
-    static uint32_t *sink = nullptr; // 4 bytes of scratch, never freed (benchmark helper only)
-    if (cached_device != device) {
-        int ndev = 0;
-        if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
-            cudaGetLastError();
-            return HOUGH_ECUDA;
-        }
-        if (cudaSetDevice(device) != cudaSuccess ||
-            cudaDeviceGetAttribute(&cached_sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
-            return HOUGH_ECUDA;
-        if (sink)
-            cudaFree(sink);
-        sink = nullptr;
-        if (cudaMalloc(&sink, 4) != cudaSuccess)
-            return HOUGH_ECUDA;
-        cached_device = device;
+    int ndev = 0, sms = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return HOUGH_ECUDA;
     }
-    int blocks = cached_sms * ctas_per_sm;
+    if (cudaSetDevice(device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
+        return HOUGH_ECUDA;
+    int blocks = sms * ctas_per_sm;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (mode == 0)
-        k_microbench<0><<<blocks, threads, 0, st>>>(iters, sink);
+        k_microbench<0><<<blocks, threads, 0, st>>>(iters, sink_dev);
     else if (mode == 1)
-        k_microbench<1><<<blocks, threads, 0, st>>>(iters, sink);
+        k_microbench<1><<<blocks, threads, 0, st>>>(iters, sink_dev);
     else
-        k_microbench<2><<<blocks, threads, 0, st>>>(iters, sink);
+        k_microbench<2><<<blocks, threads, 0, st>>>(iters, sink_dev);
     if (cudaGetLastError() != cudaSuccess)
         return HOUGH_ECUDA;
     if (lane_ops)

@@ -58,7 +58,7 @@ struct PeakParams {
     const uint32_t *acc;
     unsigned char *flags; // 1 bit per bin, byte q of a row = bins 8q .. 8q+7
     int n_phi, n_d0, nk, L_min, wrap;
-    int JW, KW, RJ, Li;
+    int JW, Li;
 };
 
 __device__ __forceinline__ uint32_t popc_pair(uint32_t a, uint32_t b)
@@ -73,13 +73,13 @@ struct PeakRaw { // raw masks of one plane for the thread's rows
 };
 
 template <int PEAK_RJ, int MAXJW>
-__global__ void __launch_bounds__(32 * MAXJW, (PEAK_RJ == 2 && MAXJW == 16) ? 1 : 2) k_peak_sweep(const PeakParams p)
+__global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p)
 {
     extern __shared__ uint4 ex[]; // [2][rows][32] : m3 of every row of the current plane
-    // warp = (jw, kw): KW warps side by side along kappa so that the CTA's rows are whole
-    // (or long) contiguous pieces of memory, JW warps along d0
+    // one warp per pair of d0 rows, 256 kappa bins wide
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int KW = p.KW, kw = warp % KW, jw = warp / KW;
+    constexpr int KW = 1;
+    const int kw = 0, jw = warp;
     const int rows = PEAK_RJ * p.JW, Tj = rows - 2;
     const int k0 = (blockIdx.x * KW + kw) * 256 + lane * 8;
     const bool kact = k0 < p.nk;
@@ -273,16 +273,9 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
     p.wrap = h->g.phi_wrap;
     p.JW = h->pk_JW;
     p.Li = h->pk_Li;
-    p.RJ = h->pk_RJ;
-    p.KW = h->pk_KW;
-    const int Tj = p.RJ * p.JW - 2;
-    dim3 grid((p.nk + 256 * p.KW - 1) / (256 * p.KW), (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
-    if (p.RJ == 1)
-        k_peak_sweep<1, 16><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
-    else if (p.JW * p.KW <= 8)
-        k_peak_sweep<2, 8><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
-    else
-        k_peak_sweep<2, 16><<<grid, 32 * p.JW * p.KW, h->pk_smem, st>>>(p);
+    const int Tj = 2 * p.JW - 2;
+    dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
+    k_peak_sweep<2, 8><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -565,6 +558,7 @@ __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_p
         r.n_votes = c->n_votes;
         r.n_hit_entries = with_lists ? c->n_hit_entries : 0ull;
         r.n_evals = c->n_evals;
+        r.n_list_evals = with_lists ? c->n_list_evals : 0ull;
         r.n_peaks = c->n_peaks;
         r.n_bad_hits = c->n_bad_hits;
         r.flags = 0u;

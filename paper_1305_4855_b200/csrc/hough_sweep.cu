@@ -18,15 +18,9 @@ struct SweepParams {
     uint32_t *acc; // VOTE: global accumulator
     unsigned long long *n_votes;
     unsigned long long *n_evals;
-    // kappa-code cache
-    unsigned short *kc_buf;
-    unsigned long long kc_cap;
-    uint2 *kc_tab;
-    uint32_t kc_chunks;
-    DevCounters *counters;
 };
 
-template <int PACK, bool KC>
+template <int PACK>
 __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -46,10 +40,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
-    ptr += 32 * 4;
-    unsigned long long *s_kbase = reinterpret_cast<unsigned long long *>(ptr); // cache rows of this chunk
-    ptr += 16;
-    unsigned short *surv_id = reinterpret_cast<unsigned short *>(ptr); // [chunk] hit index inside the chunk
 
     // ---- which tile: the first n_big phi0 slabs are P rows high, the others P_small
     // (two heights so that the CTAs fill whole waves)
@@ -85,7 +75,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     tc.phi_all = ge.no_phi_cull;
     tc.off = p.no_cull;
     const bool warp_ok = set < split;
-    const int kc_row = groups * 32 + 32;
 
     const uint32_t n_chunks = p.hits.n_pad / ge.chunk;
     const uint32_t chunk_bytes = (uint32_t)ge.chunk * 4;
@@ -157,50 +146,22 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             if (keep) {
                 int pos = total + before + __popc(bal & ((1u << lane) - 1u));
                 surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(hb));
-                if (KC)
-                    surv_id[pos] = (unsigned short)hidx;
             }
             total += all;
             __syncthreads();
         }
         tile_evals += (unsigned long long)total * (unsigned)(ni * nj);
-        if (KC && tid == 0) {
-            // rows of the kappa-code cache for this chunk's survivors: (cells + 32) u16 each
-            unsigned long long base = ~0ull;
-            const unsigned long long need = (unsigned long long)(total + EVAL_UNROLL - 1) * (unsigned)kc_row; // + rows the padding entries may write
-            if (total > 0) {
-                const unsigned long long b = atomicAdd(&p.counters->kc_cursor, need);
-                if (b + need <= p.kc_cap)
-                    base = b;
-                else
-                    p.counters->kc_overflow = 1u;
-            }
-            s_kbase[0] = base;
-            p.kc_tab[(size_t)blockIdx.x * p.kc_chunks + ch] =
-                make_uint2(base == ~0ull ? 0xffffffffu : (uint32_t)(base >> 5), (uint32_t)total);
-        }
         if (tid < EVAL_UNROLL) // non-voting padding up to a multiple of the unroll factor
             surv[total + tid] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
         __syncthreads();
 
         // ---- evaluate: lane = cell, the `split` warps of a cell group interleave the survivors
         if (warp_ok) {
-            // kappa-code cache: one u16 per evaluation (the bin, or n_kappa = no vote), rows of
-            // kc_row entries per survivor; the hit lists replay it (hough_lists.cu)
-            const unsigned long long kbase = KC ? s_kbase[0] : ~0ull;
-            const bool kstore = KC && kbase != ~0ull;
-            unsigned short *const kb = p.kc_buf + (kstore ? kbase : 0ull); // warp-uniform; 32-bit offsets below
-            uint32_t ko = (uint32_t)c + (uint32_t)(set * EVAL_UNROLL * kc_row);
-            const uint32_t kstep = (uint32_t)(split * EVAL_UNROLL * kc_row);
-            if (kstore) // [kc_row - 32] of a row = the hit's index inside the chunk
-                for (int t = (warp / groups) * 32 + lane; grp == 0 && t < total; t += split * 32)
-                    p.kc_buf[kbase + (size_t)t * kc_row + kc_row - 32] = surv_id[t];
-            for (int hs = set * EVAL_UNROLL; hs < total; hs += split * EVAL_UNROLL, ko += kstep) {
+            for (int hs = set * EVAL_UNROLL; hs < total; hs += split * EVAL_UNROLL) {
 #pragma unroll
                 for (int u = 0; u < EVAL_UNROLL; ++u) {
                     const float4 hv = surv[hs + u];
                     const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-                    uint32_t kcode = (uint32_t)nk;
                     if ((kappa >= klo) && (kappa < khi)) {
                         const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
                         const uint32_t bit = __float_as_uint(hv.w);
@@ -209,10 +170,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                         else
                             smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
                         ++my_votes;
-                        kcode = k;
                     }
-                    if (KC && kstore)
-                        kb[ko + (uint32_t)(u * kc_row)] = (unsigned short)kcode;
                 }
             }
         }
@@ -289,7 +247,7 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     // rows for the P x D cells only: padding lanes of the last cell group never vote
     const size_t tile_bytes = (size_t)(P * D) * cfg.n_kappa * 4 / h->g.pack, extra = 0;
     ge->tile_words = (int)(tile_bytes / 4);
-    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16 + 16 + (size_t)ge->chunk * 2;
+    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);
     // the interval test needs the slab to span well under a quarter turn
     double span = (cfg.phi_max - cfg.phi_min) * (double)(P - 1) / (double)cfg.n_phi;
@@ -306,12 +264,12 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     const int step = (D <= 32 && 32 % D == 0) ? 32 / D : 0;
     if (fit_waves && step > 0 && P % step == 0 && P - step >= step) {
         int per_sm = 0;
-        cudaError_t e = h->g.pack == 2 ? ensure_dynamic_smem((const void *)k_sweep<2, false>, ge->smem_bytes)
-                                       : ensure_dynamic_smem((const void *)k_sweep<1, false>, ge->smem_bytes);
+        cudaError_t e = h->g.pack == 2 ? ensure_dynamic_smem((const void *)k_sweep<2>, ge->smem_bytes)
+                                       : ensure_dynamic_smem((const void *)k_sweep<1>, ge->smem_bytes);
         if (e == cudaSuccess)
             e = h->g.pack == 2
-                    ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<2, false>, ge->threads, ge->smem_bytes)
-                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<1, false>, ge->threads, ge->smem_bytes);
+                    ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<2>, ge->threads, ge->smem_bytes)
+                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<1>, ge->threads, ge->smem_bytes);
         if (e != cudaSuccess || per_sm < 1) {
             cudaGetLastError();
             return 1;
@@ -358,20 +316,15 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
     p->n_evals = &h->counters->n_evals;
-    p->kc_buf = h->kc_on ? h->kc_buf : nullptr;
-    p->kc_cap = h->kc_cap;
-    p->kc_tab = h->kc_tab;
-    p->kc_chunks = h->kc_chunks;
-    p->counters = h->counters;
 }
 
-template <int PACK, bool KC>
+template <int PACK>
 static cudaError_t launch_one(const SweepParams &p, cudaStream_t st)
 {
-    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK, KC>, p.geom.smem_bytes);
+    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK>, p.geom.smem_bytes);
     if (e != cudaSuccess)
         return e;
-    k_sweep<PACK, KC><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
+    k_sweep<PACK><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -380,8 +333,6 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     SweepParams p;
     fill_params(h, &p, h->vote_geom);
     h->launches += 1;
-    if (p.kc_buf)
-        return h->g.pack == 2 ? launch_one<2, true>(p, st) : launch_one<1, true>(p, st);
-    return h->g.pack == 2 ? launch_one<2, false>(p, st) : launch_one<1, false>(p, st);
+    return h->g.pack == 2 ? launch_one<2>(p, st) : launch_one<1>(p, st);
 }
 

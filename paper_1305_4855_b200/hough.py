@@ -21,6 +21,7 @@ HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3,
 TRUNCATED_PEAKS, TRUNCATED_HITS = 1, 2
 OPT_NO_CULL = 1
 OPT_STAGE_TIMING = 2
+OPT_UNPACKED = 4
 N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
@@ -48,7 +49,7 @@ class Config(C.Structure):
 
 class Counts(C.Structure):
     _fields_ = [("n_votes", C.c_uint64), ("n_hit_entries", C.c_uint64), ("n_evals", C.c_uint64),
-                ("n_peaks", C.c_uint32), ("n_bad_hits", C.c_uint32), ("flags", C.c_uint32),
+                ("n_list_evals", C.c_uint64), ("n_peaks", C.c_uint32), ("n_bad_hits", C.c_uint32), ("flags", C.c_uint32),
                 ("reserved", C.c_uint32)]
 
 
@@ -63,7 +64,7 @@ class HostOut(C.Structure):
 
 
 COUNTS_DTYPE = np.dtype([("n_votes", "<u8"), ("n_hit_entries", "<u8"), ("n_evals", "<u8"),
-                         ("n_peaks", "<u4"), ("n_bad_hits", "<u4"), ("flags", "<u4"),
+                         ("n_list_evals", "<u8"), ("n_peaks", "<u4"), ("n_bad_hits", "<u4"), ("flags", "<u4"),
                          ("reserved", "<u4")])
 COUNTS_WORDS = COUNTS_DTYPE.itemsize // 8  # int64 words of one hough_counts block
 
@@ -105,7 +106,7 @@ def _load():
     lib.hough_set_accumulator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.hough_microbench_smem.restype = C.c_int
     lib.hough_microbench_smem.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
-                                          C.POINTER(C.c_uint64)]
+                                          C.c_void_p, C.POINTER(C.c_uint64)]
     lib.hough_query.restype = C.c_int
     lib.hough_query.argtypes = [C.c_void_p] + [C.POINTER(C.c_int32)] * 6
     lib.hough_launch_count.restype = C.c_uint64
@@ -310,7 +311,7 @@ class Hough:
         n_rep = min(int(cnt["n_peaks"]), self.cap_peaks)
         n_ent = min(int(cnt["n_hit_entries"]), self.cap_hits)
         out = {"n_votes": int(cnt["n_votes"]), "n_hit_entries": int(cnt["n_hit_entries"]),
-               "n_evals": int(cnt["n_evals"]),
+               "n_evals": int(cnt["n_evals"]), "n_list_evals": int(cnt["n_list_evals"]),
                "n_peaks": int(cnt["n_peaks"]), "n_bad_hits": int(cnt["n_bad_hits"]),
                "flags": int(cnt["flags"]),
                "peak_bin": b[:n_rep].view(np.uint32), "peak_mask": m[:n_rep].view(np.uint32),
@@ -360,12 +361,14 @@ def microbench_smem(mode, threads=1024, ctas_per_sm=2, iters=4096, device=0, rep
     """Times hough_microbench_smem with CUDA events; returns lane-ops per second (best of reps)."""
     st = torch.cuda.current_stream()
     ops = C.c_uint64()
+    sink = torch.zeros(1, dtype=torch.int32, device=torch.device("cuda", device))
     best = None
     for _ in range(reps + 1):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(st)
         _check(_lib.hough_microbench_smem(device, mode, threads, ctas_per_sm, iters,
-                                          C.c_void_p(st.cuda_stream), C.byref(ops)),
+                                          C.c_void_p(sink.data_ptr()), C.c_void_p(st.cuda_stream),
+                                          C.byref(ops)),
                "hough_microbench_smem")
         e1.record(st)
         e1.synchronize()

@@ -124,10 +124,23 @@ def test_bad_layers_and_non_finite_hits(hough, oracle):
     x[8] = -np.inf
     x[9] = 3.0e19            # x*x overflows: den = inf, kappa = 0 -> a legal vote
     x[10], y[10] = 0.0, 0.0  # hit at the origin
+    # finite coordinates up to FLT_MAX still vote (r2 = inf => den = inf => kappa = +-0)
+    x[12] = 3.2e38
+    y[13] = -3.3e38
+    x[14], y[14] = np.float32(3.4028234e38), np.float32(-3.4028234e38)
+    x[15], y[15] = 1.0e19, 1.7e19      # r2 finite but huge
+    layer[[9, 12, 13, 14, 15]] = [1, 2, 3, 4, 5]
     ref = oracle.run(grid, x, y, layer)
     assert ref["n_bad_hits"] > 0
+    # the huge finite hits really vote in the oracle (so a cull that drops them is caught)
+    solo = oracle.run(grid, x[12:15], y[12:15], layer[12:15])
+    assert solo["n_votes"] > 0
+    for opt in (0, 1):
+        res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4, options=opt)
+        assert_same(res, ref)
     res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
-                  cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4)
+                  cap_hits=ref["n_hit_entries"] + 1)
     assert_same(res, ref)
 
 
@@ -241,31 +254,50 @@ def test_process_host_matches_device_path(hough, oracle):
     assert_same(res, ref)
 
 
-def test_batch_events_back_to_back_on_one_handle(hough, oracle):
-    """BASELINE.json configs[3]: events shaped like "pileup", one handle, one stream, each with
-    its own accumulator -- the second and third event must not see anything of the first.
-    (bench.py times all 100 seeds; the oracle needs ~10 s per event, so three are compared.)"""
+def test_batch_all_100_events_back_to_back_on_one_handle(hough, oracle):
+    """BASELINE.json configs[3]: 100 events shaped like "pileup" (seeds 0..99), one handle, one
+    stream, each with its own accumulator.  EVERY seed: whole accumulator, n_votes, n_bad_hits,
+    peak list and masks against the oracle; the CSR hit lists for every tenth seed (the oracle's
+    O(n_peaks x n_hits) list passes cost ~10 s per event, its vote + peaks ~1 s)."""
     w = synth.WORKLOADS["batch100"]
+    assert w.seeds == tuple(range(100))
     h = hough.Hough(w.grid, 20000, w.cap_peaks, w.cap_hits)
-    for seed in (w.seeds[1], w.seeds[57], w.seeds[99]):
+    for seed in w.seeds:
         x, y, layer, _ = synth.generate_event(w.event, seed)
         h.vote(dev(x), dev(y), dev(layer))
         h.peaks()
         res = h.read()
-        res["acc"] = h.accumulator_host().copy()
-        ref = oracle.run(w.grid, x, y, layer)
-        assert res["flags"] == 0
-        assert_same(res, ref)
+        res["acc"] = h.accumulator_host()
+        assert res["flags"] == 0, seed
+        with_lists = seed % 10 == 0
+        if with_lists:
+            ref = oracle.run(w.grid, x, y, layer)
+        else:
+            acc, n_votes, n_bad = oracle.vote(w.grid, x, y, layer)
+            pb, pm, n_peaks = oracle.peaks(w.grid, acc)
+            ref = {"acc": acc, "n_votes": n_votes, "n_bad_hits": n_bad, "peak_bin": pb,
+                   "peak_mask": pm, "n_peaks": n_peaks}
+        res["acc"] = res["acc"].reshape(ref["acc"].shape)
+        assert_same(res, ref, lists=with_lists)
+        # CSR consistency for every seed: n_hit_entries = sum of list lengths, OR of the
+        # listed hits' layer bits = the peak's mask
+        off = res["hit_offset"].astype(np.int64)
+        assert off[0] == 0 and np.all(np.diff(off) > 0) and off[-1] == res["n_hit_entries"]
+        bits = (np.uint32(1) << layer[res["hit_index"]].astype(np.uint32)).astype(np.uint32)
+        assert np.array_equal(np.bitwise_or.reduceat(bits, off[:-1]), res["peak_mask"]), seed
     h.close()
 
 
-def test_finegrid_sampled_parity(hough, oracle):
+def test_finegrid_full_accumulator_parity(hough, oracle):
     """BASELINE.json configs[4] at full size (134M bins, ~62k hits), in bench.py's launch
-    configuration.  The oracle would need minutes for the whole vote, so: accumulator rows of
-    4096 sampled (phi0, d0) cells + every row of 2 whole phi0 planes, bit for bit; the whole
-    peak list against the oracle's peak rule applied to the (row-checked) accumulator; the
-    complete hit lists of 3000 sampled peaks and of the first/last 50; CSR consistency and
-    n_hit_entries = sum of all list lengths = votes that landed in reported peaks."""
+    configuration: the WHOLE 512 MiB accumulator, n_votes and n_bad_hits against the oracle's
+    vote (1.6e10 evaluations: tens of seconds on the host cores); the whole peak list and masks
+    against the oracle's peak rule on the ORACLE's accumulator.  Only the oracle's hit-list
+    passes (O(n_peaks x n_hits) = 3.6e6 x 6.2e4 x 2) are infeasible at this size, so the CSR
+    lists are compared for 3000 sampled peaks plus the first and last 50, and checked for
+    every peak by properties that hold at any size: offsets strictly increasing, ascending
+    hit indices inside each list, n_hit_entries = sum of the lengths, OR of the listed hits'
+    layer bits = the peak's mask."""
     w = synth.WORKLOADS["finegrid"]
     g = w.grid
     x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
@@ -273,27 +305,44 @@ def test_finegrid_sampled_parity(hough, oracle):
     h.vote(dev(x), dev(y), dev(layer))
     h.peaks()
     res = h.read()
-    acc = h.accumulator_host().copy().reshape(g.n_phi, g.n_d0, g.n_kappa)
+    acc = h.accumulator_host().reshape(g.n_phi, g.n_d0, g.n_kappa)
     h.close()
-    assert res["flags"] == 0 and res["n_bad_hits"] == 0
-    rng = np.random.default_rng(5)
-    ci = np.concatenate([rng.integers(0, g.n_phi, 4096), np.repeat([0, g.n_phi - 1], g.n_d0)])
-    cj = np.concatenate([rng.integers(0, g.n_d0, 4096), np.tile(np.arange(g.n_d0), 2)])
-    rows, _nv = oracle.vote_cells(g, x, y, layer, ci, cj)
-    assert np.array_equal(acc[ci, cj, :], rows)
-    # vote count: sum of popcounts <= n_votes <= evaluations
-    pop = int(np.unpackbits(acc.view(np.uint8)).sum())
-    assert pop <= res["n_votes"] <= len(x) * g.n_phi * g.n_d0
-    pb, pm, n = oracle.peaks(g, acc)
+    assert res["flags"] == 0
+    ref_acc, ref_votes, ref_bad = oracle.vote(g, x, y, layer)
+    assert res["n_votes"] == ref_votes and res["n_bad_hits"] == ref_bad
+    assert np.array_equal(acc, ref_acc)
+    del acc
+    pb, pm, n = oracle.peaks(g, ref_acc)
+    del ref_acc
     assert res["n_peaks"] == n
     assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
     off = res["hit_offset"].astype(np.int64)
-    assert off[0] == 0 and np.all(np.diff(off) >= 0) and off[-1] == res["n_hit_entries"]
+    idx = res["hit_index"]
+    assert off[0] == 0 and np.all(np.diff(off) > 0) and off[-1] == res["n_hit_entries"] == len(idx)
+    inner = np.ones(len(idx), bool)
+    inner[off[:-1]] = False                      # first entry of every list
+    assert np.all(np.diff(idx.astype(np.int64))[inner[1:]] > 0)   # ascending inside each list
+    bits = (np.uint32(1) << layer[idx].astype(np.uint32)).astype(np.uint32)
+    assert np.array_equal(np.bitwise_or.reduceat(bits, off[:-1]), pm)
+    rng = np.random.default_rng(5)
     sel = np.unique(np.concatenate([rng.integers(0, n, 3000), np.arange(50), np.arange(n - 50, n)]))
     soff, sidx, _tot = oracle.hitlists(g, x, y, layer, pb[sel])
     for q, pk in enumerate(sel):
-        got = res["hit_index"][off[pk]:off[pk + 1]]
+        got = idx[off[pk]:off[pk + 1]]
         assert np.array_equal(got, sidx[int(soff[q]):int(soff[q + 1])]), pk
+
+
+def test_unpacked_tile_option_with_few_layers(hough, oracle):
+    """HOUGH_OPT_UNPACKED: the one-mask-per-word tile layout (used with 17..32 layers) on a
+    10-layer detector, with and without the cull."""
+    rng = np.random.default_rng(31)
+    grid = synth.Grid(n_phi=50, n_d0=13, n_kappa=96, L_min=3)
+    x, y, layer = random_hits(rng, 1100)
+    ref = oracle.run(grid, x, y, layer)
+    for opt in (hough.OPT_UNPACKED, hough.OPT_UNPACKED | hough.OPT_NO_CULL):
+        res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
+                      cap_hits=ref["n_hit_entries"] + 1, options=opt)
+        assert_same(res, ref)
 
 
 def test_submit_collect_pipeline_matches_oracle(hough, oracle):

@@ -246,6 +246,45 @@ def test_popcount_sum_equals_votes_for_a_single_track(oracle):
     assert sum(bin(int(v)).count("1") for v in acc.reshape(-1)) == n_votes
 
 
+def test_vote_cells_equals_the_same_rows_of_the_whole_vote(oracle):
+    """oracle_vote_cells (used where only part of a large grid is checked) must give exactly
+    the rows oracle_vote gives, and its vote count the votes of those rows; listing every
+    cell reproduces the whole accumulator and n_votes."""
+    rng = np.random.default_rng(17)
+    grid = synth.Grid(n_phi=24, n_d0=7, n_kappa=32, L_min=2)
+    x, y, layer = random_hits(rng, 400)
+    layer[::13] = -1                              # bad hits are skipped by both
+    acc, n_votes, _ = oracle.vote(grid, x, y, layer)
+    ci = rng.integers(0, grid.n_phi, 60)
+    cj = rng.integers(0, grid.n_d0, 60)
+    rows, nv = oracle.vote_cells(grid, x, y, layer, ci, cj)
+    assert np.array_equal(rows, acc[ci, cj, :])
+    # the same cells once more with single-hit events: votes in the listed cells add up
+    per_hit = sum(oracle.vote_cells(grid, x[h:h + 1], y[h:h + 1], layer[h:h + 1], ci, cj)[1]
+                  for h in range(len(x)))
+    assert per_hit == nv
+    ii, jj = np.meshgrid(np.arange(grid.n_phi), np.arange(grid.n_d0), indexing="ij")
+    rows_all, nv_all = oracle.vote_cells(grid, x, y, layer, ii.ravel(), jj.ravel())
+    assert np.array_equal(rows_all.reshape(acc.shape), acc) and nv_all == n_votes
+
+
+def test_finite_coordinates_whose_squares_overflow_still_vote(oracle):
+    """r2 = x*x + y*y = inf for |x| > ~1.8e19: den = inf, kappa = +-0, which is inside a kappa
+    range that contains 0 (reading B4: no special case).  Checked against the definition: the
+    vote of such a hit is bin(0) in every cell, for any finite coordinate up to FLT_MAX."""
+    grid = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=1)
+    k0 = int((0.0 - grid.kappa_min) * (grid.n_kappa / (grid.kappa_max - grid.kappa_min)))
+    for xv, yv in ((3.2e38, 1.0), (2.0, -3.3e38), (3.0e19, 0.0), (3.4028234e38, -3.4028234e38)):
+        x = np.array([xv], np.float32)
+        y = np.array([yv], np.float32)
+        acc, n_votes, n_bad = oracle.vote(grid, x, y, np.array([3], np.int32))
+        voted = acc[:, :, k0] == 8
+        # every cell whose s is finite votes into the bin of kappa = 0; a cell whose s overflows
+        # to +-inf (or whose 2*d0*s does) has num/den = inf/inf = NaN and casts no vote
+        assert n_votes == int(voted.sum()) > 0 and n_bad == 0
+        assert int((acc != 0).sum()) == n_votes
+
+
 def test_bad_and_non_finite_hits_cast_no_vote(oracle):
     grid = tiny_grid()
     rng = np.random.default_rng(9)
