@@ -291,6 +291,42 @@ static int choose_geometry(hough_handle *h)
     return 1;
 }
 
+// Constants and admissibility of the fast bin path (hough_device.cuh approx_bin; DESIGN.md
+// 4.5).  With klo, khi, inv_dk the fp32 constants of A1 taken as reals, the estimate is
+//   t = trunc( e * rcp(den) * c1 + c0 ),  c1 = 2 inv_dk 2^16 (exact),  c0 = RN(-klo inv_dk 2^16 + delta).
+// One binary32 rounding of a coordinate below n_kappa * 2^16 is at most U = n_kappa / 256
+// steps.  Error budget against the exact qf * 2^16: E = (7A + 3) U + 1 with A = K / W; khi's
+// own coordinate is within (2A + 1) U of n_kappa * 2^16; delta = ceil((12 A + 8) max(U, 1)).
+static void approx_bin_init(hough_handle *h, const float *d0c, int nd)
+{
+    ApproxBin &ab = h->ab;
+    memset(&ab, 0, sizeof(ab));
+    if (h->cfg.options & HOUGH_OPT_EXACT_ONLY)
+        return;
+    const double klo = (double)h->g.klo, khi = (double)h->g.khi, inv = (double)h->g.inv_dk;
+    const int nk = h->g.n_kappa;
+    const double W = khi - klo, K = fmax(fabs(klo), fabs(khi));
+    if (!(W > 0.0) || !(inv > 0.0) || K > 1048576.0 || W / nk < ldexp(1.0, -40))
+        return;
+    for (int j = 0; j < nd; ++j) { // den = r2 - 2 d0 s + d0^2 must be 0 or normal with a normal reciprocal
+        const double a = fabs((double)d0c[j]);
+        if (a != 0.0 && (a < ldexp(1.0, -20) || a > 1048576.0))
+            return;
+    }
+    const double steps = 65536.0, U = fmax(nk / 256.0, 1.0);
+    const double delta = ceil((12.0 * K / W + 8.0) * U);
+    if (16.0 * delta > steps)
+        return; // more than 1/8 of every bin would fall back to the exact recipe anyway
+    // the bin coordinates of klo and khi must sit where the budget assumes them
+    if (fabs((khi - klo) * inv - nk) * steps > 0.25 * delta)
+        return;
+    ab.c1 = (float)ldexp(inv, APPROX_FRAC_BITS + 1);
+    ab.c0 = (float)(-klo * inv * steps + delta);
+    ab.lim = (uint32_t)((double)nk * steps + 2.0 * delta);
+    ab.edge = (uint32_t)(2.0 * delta);
+    ab.ok = isfinite(ab.c1) && isfinite(ab.c0) ? 1 : 0;
+}
+
 int hough_create(const hough_config *cfg, void *workspace, size_t workspace_bytes, hough_handle **out)
 {
     if (!out)
@@ -374,6 +410,7 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     g.d0c = h->t_d0c;
     g.twod0 = h->t_twod0;
     g.d0sq = h->t_d0sq;
+    approx_bin_init(h, d0c, nd);
     int ok = 1;
     ok &= cudaMemcpy(h->t_sn, sn, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_cs, cs, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;

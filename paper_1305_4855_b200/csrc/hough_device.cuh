@@ -68,6 +68,37 @@ __device__ __forceinline__ int kappa_bin(float kappa, float klo, float inv_dk, i
     float qf = __fmul_rn(__fsub_rn(kappa, klo), inv_dk);
     return min(__float2int_rz(qf), nk_minus_1);
 }
+// ------------------------------------------------------------------ the fast bin path
+// The exact recipe costs ~14 issue slots for the IEEE divide, the two range compares and the
+// bin.  The sweeps only need the BIN, so they first compute a 16.16 fixed-point estimate
+//     t = trunc( e * rcp(den) * c1 + c0 )  ~=  (kappa - klo) * inv_dk * 2^16 + delta
+// (MUFU.RCP + FMUL + FFMA + F2I; e and den are the exact binary32 values of the recipe) and
+// use it only where it provably equals the exact result.  With U = n_kappa / 256 (one
+// binary32 rounding of a coordinate below n_kappa * 2^16, in steps of 2^-16 bin) and
+// A = max(|klo|, |khi|) / (khi - klo):  |estimate - exact qf * 2^16| <= E = (7A + 3) U + 1
+// (2 ulp for the reciprocal, one rounding each for the product, the folded constant and the
+// FMA, the truncation, plus the three roundings of the exact path itself).
+// delta = ceil((12A + 8) max(U, 1)) > E + the offset of khi's own coordinate, so
+//   (unsigned)t >= lim              kappa is outside [klo, khi) by more than E: no vote;
+//   (t & 0xffff) <  edge = 2 delta   within delta of a bin edge (or of klo / khi; NaN gives
+//                                    t = 0): the exact recipe decides;
+//   otherwise                        the exact bin is t >> 16.
+// Preconditions, checked on the host (approx_bin_init) and per hit (hit_is_wild): den is 0,
+// +-inf, NaN or a normal number whose reciprocal is normal, so that MUFU.RCP's flush-to-zero
+// never changes the outcome.  Hits outside that range take the exact recipe everywhere.
+__device__ __forceinline__ uint32_t approx_bin(float e, float den, float c1, float c0)
+{
+    float rho;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rho) : "f"(den));
+    const float p = __fmul_rn(e, rho);
+    return (uint32_t)__float2int_rz(__fmaf_rn(p, c1, c0));
+}
+// r2 outside [2^-40, 2^80] (or NaN): the reciprocal of den could be flushed
+__device__ __forceinline__ bool hit_is_wild(float r2)
+{
+    return !((r2 >= 9.094947017729282e-13f) && (r2 <= 1.2089258196146292e24f));
+}
+
 __device__ __forceinline__ void smem_red_or(uint32_t addr, uint32_t v)
 {
     asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");

@@ -55,6 +55,16 @@ struct GridDev {
     const float *d0c, *twod0, *d0sq; // [n_d0]
 };
 
+// constants of the fast bin path (hough_device.cuh approx_bin; built by hough_create).
+// t = trunc(e * rcp(den) * c1 + c0) is the kappa-bin coordinate in 16.16 fixed point, shifted by delta.
+#define APPROX_FRAC_BITS 16
+struct ApproxBin {
+    float c1, c0;
+    uint32_t lim;  // n_kappa * 2^16 + 2 delta: (unsigned)t >= lim -> no vote
+    uint32_t edge; // 2 delta: (t & 0xffff) < edge -> the exact recipe decides
+    int ok;        // 0: the fast path is off for this grid
+};
+
 struct HitsDev {         // prepared hits, SoA, padded with non-voting entries to a chunk multiple
     const float *x, *y, *r2;
     const uint32_t *bit;
@@ -84,6 +94,7 @@ struct hough_handle {
     double *radii;       // host copy
     int device, n_sms;
     GridDev g;
+    ApproxBin ab;
     SweepGeom vote_geom;
     ListGeom list_geom;
     // workspace carve-up (device)

@@ -42,6 +42,7 @@ struct ListSweepParams {
     unsigned long long *n_entries;
     unsigned long long ent_cap;
     unsigned long long *n_list_evals; // evaluations executed (hough_counts.n_list_evals)
+    ApproxBin ab;
 };
 
 __device__ __forceinline__ unsigned short lds_u16(uint32_t addr)
@@ -87,7 +88,11 @@ __device__ __forceinline__ float4 lds_f4(uint32_t addr)
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-template <int WARPS> // warps per CTA = sub-tiles per super-tile (ListGeom::warps)
+// WARPS: warps per CTA = sub-tiles per super-tile (ListGeom::warps).  APPROX: the hot loop
+// finds the bin with the fixed-point estimate of hough_device.cuh; only
+// candidates (the estimated bin is a reported peak, or the estimate is not decisive) reach
+// the drain, which settles the undecided ones with the exact recipe.
+template <int WARPS, bool APPROX>
 __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -141,6 +146,8 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
         c_row = (uint32_t)(si0 + il) * (uint32_t)g.n_d0 + (uint32_t)(sj0 + jl);
     }
     const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
+    const float ab_c1 = p.ab.c1, ab_c0 = p.ab.c0;
+    const uint32_t ab_lim = p.ab.lim, ab_edge = p.ab.edge;
 
     // super-tile extent (CTA-level cull) and sub-tile extent (warp-level cull)
     const int ni = min(ge.WP * ge.SP, g.n_phi - i0), nj = min(ge.WD * ge.SD, g.n_d0 - j0);
@@ -255,13 +262,37 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
     auto drain = [&]() {
         const uint32_t nl = (lqp - wl4) >> 7;
         for (uint32_t e = 0;; ++e) {
-            const bool act = e < nl;
-            const unsigned bh = __ballot_sync(0xffffffffu, act);
-            if (!bh)
+            bool act = e < nl;
+            if (!__any_sync(0xffffffffu, act))
                 break;
+            uint32_t k = 0, hit = 0;
             if (act) {
                 const uint32_t ent = lds_off<OFF_LANEQ>(wl4 + e * 128u);
-                const uint32_t k = ent >> 10;
+                if (APPROX) {
+                    // ent = (t & ~511) | index: the bin is t >> 16 unless the coordinate is within
+                    // edge (rounded up to a multiple of 512) steps above a bin edge, where the exact
+                    // recipe decides
+                    const float4 hv = surv[ent & 511u];
+                    hit = __float_as_uint(hv.w);
+                    k = ent >> APPROX_FRAC_BITS;
+                    act = hit != 0xffffffffu; // the padding entry never counts
+                    if ((ent & 0xfe00u) < ((ab_edge + 511u) & ~511u)) {
+                        // r2 is recomputed from x, y (A2): the staged copy of a hit outside the
+                        // estimate's range holds NaN instead
+                        const float r2 = __fadd_rn(__fmul_rn(hv.x, hv.x), __fmul_rn(hv.y, hv.y));
+                        const float kappa = eval_kappa(hv.x, hv.y, r2, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+                        act = act && (kappa >= klo) && (kappa < khi);
+                        k = act ? (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1) : 0u;
+                        const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
+                        act = act && ((f >> (k & 31u)) & 1u);
+                    }
+                } else {
+                    hit = __float_as_uint(surv[ent & 1023u].w);
+                    k = ent >> 10;
+                }
+            }
+            const unsigned bh = __ballot_sync(0xffffffffu, act);
+            if (act) {
                 const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
                 const uint32_t rank = lds_u16(pre_addr + (k >> 5) * 64u) + (uint32_t)__popc(f & ((1u << (k & 31u)) - 1u));
                 const uint32_t ca = cnt_addr + rank * 2u;
@@ -269,7 +300,7 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
                 sts_u16(ca, (unsigned short)(n + 1));
                 const uint32_t pos = qn + (uint32_t)__popc(bh & lt_mask);
                 q_sub[pos] = sub0 + rank * (uint32_t)S;
-                q_hit[pos] = __float_as_uint(surv[ent & 1023u].w);
+                q_hit[pos] = hit;
                 q_idx[pos] = n;
             }
             qn += (uint32_t)__popc(bh);
@@ -279,15 +310,36 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
         lqp = wl4;
     };
 
-    // one hit against the warp's 32 cells: exact recipe, then the peak test of the bin
+    // one hit against the warp's 32 cells: the bin, then the peak test of the bin
     auto process = [&](const float4 hv, const uint32_t sidx) {
-        const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-        if ((kappa >= klo) && (kappa < khi)) {
-            const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
-            const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
-            if ((f >> (k & 31u)) & 1u) {
-                asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(lqp), "n"(OFF_LANEQ), "r"((k << 10) | sidx) : "memory");
-                lqp += 128u;
+        if (APPROX) {
+            // e and den are the exact binary32 values of the recipe (A3)
+            const float a = __fmul_rn(hv.x, c_sn);
+            const float b = __fmul_rn(hv.y, c_cs);
+            const float sv_ = __fsub_rn(b, a);
+            const float e = __fsub_rn(sv_, c_d0);
+            const float den = __fadd_rn(__fsub_rn(hv.z, __fmul_rn(c_2d0, sv_)), c_d0sq);
+            const uint32_t t = approx_bin(e, den, ab_c1, ab_c0);
+            if (t < ab_lim) {
+                // flag word of bin t >> 16 (it may be n_kappa, just above khi: that word is not a
+                // flag word, but then the estimate is undecided anyway)
+                const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((t >> (APPROX_FRAC_BITS + 5)) << 7));
+                const bool near = (t & 0xffffu) < ab_edge;
+                if (near || ((f >> ((t >> APPROX_FRAC_BITS) & 31u)) & 1u)) {
+                    // pending entry: the coordinate with its low 9 bits replaced by the index into surv
+                    asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(lqp), "n"(OFF_LANEQ), "r"((t & ~511u) | sidx) : "memory");
+                    lqp += 128u;
+                }
+            }
+        } else {
+            const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+            if ((kappa >= klo) && (kappa < khi)) {
+                const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
+                const uint32_t f = lds_off<OFF_FLAGS>(wl4 + ((k << 2) & ~127u));
+                if ((f >> (k & 31u)) & 1u) {
+                    asm volatile("st.shared.u32 [%0+%1], %2;" ::"r"(lqp), "n"(OFF_LANEQ), "r"((k << 10) | sidx) : "memory");
+                    lqp += 128u;
+                }
             }
         }
     };
@@ -321,14 +373,22 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
                 before += (w < warp) ? cw : 0;
                 all += cw;
             }
-            if (keep)
+            if (keep) // a hit outside the estimate's range is staged with r2 = NaN: every estimate says "undecided"
                 surv[total + before + __popc(bal & lt_mask)] =
-                    make_float4(hx, hy, hr2, __uint_as_float(ch * LIST_CHUNK + hidx));
+                    make_float4(hx, hy, (APPROX && hit_is_wild(hr2)) ? __int_as_float(0x7fc00000) : hr2,
+                                __uint_as_float(ch * LIST_CHUNK + hidx));
             total += all;
             __syncthreads();
         }
-        if (tid == 0) // a non-voting entry that pads odd batches
-            surv[total] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+        __syncthreads();
+        if (tid == 0) { // the entry that pads odd batches: non-voting (exact path) / marked as padding
+            if (APPROX) {
+                const float4 h0 = surv[0]; // an ordinary evaluation whose entries the drain drops
+                surv[total] = make_float4(h0.x, h0.y, h0.z, __uint_as_float(0xffffffffu));
+            } else {
+                surv[total] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+            }
+        }
         __syncthreads();
 
         if (warp_ok) {
@@ -479,20 +539,25 @@ int list_segments_bound(const hough_config *c)
     return s_max > s_min ? s_max : s_min;
 }
 
-static const void *list_sweep_fn(int warps)
+template <bool APPROX>
+static const void *list_sweep_fn_t(int warps)
 {
     switch (warps) {
     case 16:
-        return (const void *)k_list_sweep<16>;
+        return (const void *)k_list_sweep<16, APPROX>;
     case 8:
-        return (const void *)k_list_sweep<8>;
+        return (const void *)k_list_sweep<8, APPROX>;
     case 4:
-        return (const void *)k_list_sweep<4>;
+        return (const void *)k_list_sweep<4, APPROX>;
     case 2:
-        return (const void *)k_list_sweep<2>;
+        return (const void *)k_list_sweep<2, APPROX>;
     default:
-        return (const void *)k_list_sweep<1>;
+        return (const void *)k_list_sweep<1, APPROX>;
     }
+}
+static const void *list_sweep_fn(int warps, int approx)
+{
+    return approx ? list_sweep_fn_t<true>(warps) : list_sweep_fn_t<false>(warps);
 }
 
 int list_geom_init(hough_handle *h)
@@ -535,7 +600,7 @@ int list_geom_init(hough_handle *h)
     const double dphi = (c.phi_max - c.phi_min) / (double)c.n_phi;
     ge->no_phi_cull_tile = (dphi * (ge->WP * ge->SP - 1) > 1.0) ? 1 : 0;
     ge->no_phi_cull_sub = (dphi * (ge->SP - 1) > 1.0) ? 1 : 0;
-    const void *fn = list_sweep_fn(ge->warps);
+    const void *fn = list_sweep_fn(ge->warps, h->ab.ok);
     if (ensure_dynamic_smem(fn, ge->smem_bytes) != cudaSuccess)
         return 0;
     int per_sm = 0;
@@ -600,6 +665,7 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
     p.n_entries = h->n_pairs;
     p.ent_cap = h->cfg.cap_hits;
     p.n_list_evals = &h->counters->n_list_evals;
+    p.ab = h->ab;
     k_zero_sub_len<<<h->n_sms * 8, 256, 0, st>>>(h->list_len, h->counters, h->cfg.cap_peaks,
                                                  (uint32_t)h->list_geom.S);
     h->launches += 2;
@@ -607,7 +673,7 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st)
         return cudaGetLastError();
     const int blocks = h->list_geom.tiles_phi * h->list_geom.tiles_d0 * h->list_geom.S;
     void *args[] = {(void *)&p};
-    return cudaLaunchKernel(list_sweep_fn(h->list_geom.warps), dim3(blocks), dim3(32 * h->list_geom.warps), args,
+    return cudaLaunchKernel(list_sweep_fn(h->list_geom.warps, h->ab.ok), dim3(blocks), dim3(32 * h->list_geom.warps), args,
                             (size_t)h->list_geom.smem_bytes, st);
 }
 

@@ -18,9 +18,13 @@ struct SweepParams {
     uint32_t *acc; // VOTE: global accumulator
     unsigned long long *n_votes;
     unsigned long long *n_evals;
+    ApproxBin ab;
 };
 
-template <int PACK>
+// APPROX: bins come from the fixed-point estimate wherever it provably equals the exact
+// recipe (hough_device.cuh approx_bin); near a bin edge, and for hits whose
+// r^2 is outside the estimate's admissible range, the exact recipe runs.
+template <int PACK, bool APPROX>
 __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -40,6 +44,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
+    ptr += 32 * 4;
+    int *s_nwild = reinterpret_cast<int *>(ptr);
 
     // ---- which tile: the first n_big phi0 slabs are P rows high, the others P_small
     // (two heights so that the CTAs fill whole waves)
@@ -103,6 +109,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         tile[w] = 0u;
     __syncthreads();
 
+    const float ab_c1 = p.ab.c1, ab_c0 = p.ab.c0;
+    const uint32_t ab_lim = p.ab.lim, ab_edge = p.ab.edge;
     unsigned int my_votes = 0;
     unsigned long long tile_evals = 0; // thread 0: surviving hits x owned cells
     const int nkm1 = nk - 1;
@@ -119,11 +127,14 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         if (tid == 0 && ch + 1 < n_chunks)
             issue(ch + 1); // the other buffer was released by the barrier ending chunk ch-1
 
-        // ---- cull + order-preserving compaction of the survivors
+        // ---- cull + compaction of the survivors: ordinary hits from the front of surv, hits
+        // outside the fast path's range ("wild") from its back
         int total = 0;
+        if (APPROX && tid == 0)
+            s_nwild[0] = 0; // (the barrier inside the loop orders it before the first use)
         for (int base = 0; base < ge.chunk; base += ge.threads) {
             int hidx = base + tid;
-            bool keep = false;
+            bool keep = false, wild = false;
             float hx = 0.f, hy = 0.f, hr2 = 0.f;
             uint32_t hb = 0;
             if (hidx < ge.chunk) {
@@ -132,6 +143,10 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 hr2 = st[2 * ge.chunk + hidx];
                 hb = __float_as_uint(st[3 * ge.chunk + hidx]);
                 keep = (hb != 0u) && hit_may_vote(hx, hy, hr2, tc, g.kabs, g.d0_absmax);
+                if (APPROX) {
+                    wild = keep && hit_is_wild(hr2);
+                    keep = keep && !wild;
+                }
             }
             unsigned bal = __ballot_sync(0xffffffffu, keep);
             if (lane == 0)
@@ -147,30 +162,82 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 int pos = total + before + __popc(bal & ((1u << lane) - 1u));
                 surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(hb));
             }
+            if (APPROX && wild) // rare: any order will do (OR is commutative)
+                surv[ge.chunk + EVAL_UNROLL - 1 - atomicAdd(s_nwild, 1)] = make_float4(hx, hy, hr2, __uint_as_float(hb));
             total += all;
             __syncthreads();
         }
-        tile_evals += (unsigned long long)total * (unsigned)(ni * nj);
-        if (tid < EVAL_UNROLL) // non-voting padding up to a multiple of the unroll factor
-            surv[total + tid] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
-        __syncthreads();
+        const int n_wild = APPROX ? s_nwild[0] : 0;
+        tile_evals += (unsigned long long)(total + n_wild) * (unsigned)(ni * nj);
+        if (!APPROX) {
+            if (tid < EVAL_UNROLL) // non-voting padding up to a multiple of the unroll factor
+                surv[total + tid] = make_float4(0.f, 0.f, __int_as_float(0x7fc00000), 0.f);
+            __syncthreads();
+        }
 
         // ---- evaluate: lane = cell, the `split` warps of a cell group interleave the survivors
+        auto cast = [&](const uint32_t k, const uint32_t bit) {
+            if (PACK == 2)
+                smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
+            else
+                smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
+            ++my_votes;
+        };
+        auto exact = [&](const float4 hv) {
+            const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+            if ((kappa >= klo) && (kappa < khi))
+                cast((uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1), __float_as_uint(hv.w));
+        };
+        // the estimate of one (hit, cell): e and den are the exact binary32 values of the recipe (A3)
+        auto estimate = [&](const float4 hv, float &e, float &den) -> uint32_t {
+            const float a = __fmul_rn(hv.x, c_sn);
+            const float b = __fmul_rn(hv.y, c_cs);
+            const float sv = __fsub_rn(b, a);
+            e = __fsub_rn(sv, c_d0);
+            den = __fadd_rn(__fsub_rn(hv.z, __fmul_rn(c_2d0, sv)), c_d0sq);
+            return approx_bin(e, den, ab_c1, ab_c0);
+        };
+        auto settle = [&](const uint32_t t, const float e, const float den, const uint32_t bit) {
+            if (t < ab_lim) {
+                if ((t & 0xffffu) < ab_edge) { // within delta of a bin edge: the exact recipe decides
+                    const float kappa = __fdiv_rn(__fadd_rn(e, e), den);
+                    if ((kappa >= klo) && (kappa < khi))
+                        cast((uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1), bit);
+                } else {
+                    cast(t >> APPROX_FRAC_BITS, bit);
+                }
+            }
+        };
         if (warp_ok) {
-            for (int hs = set * EVAL_UNROLL; hs < total; hs += split * EVAL_UNROLL) {
+            if (APPROX) {
+                int hs = set * EVAL_UNROLL;
+                for (; hs + EVAL_UNROLL <= total; hs += split * EVAL_UNROLL) {
+                    // the four estimates first (independent chains), then the four votes
+                    float4 hv[EVAL_UNROLL];
+                    float e[EVAL_UNROLL], den[EVAL_UNROLL];
+                    uint32_t t[EVAL_UNROLL];
 #pragma unroll
-                for (int u = 0; u < EVAL_UNROLL; ++u) {
-                    const float4 hv = surv[hs + u];
-                    const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-                    if ((kappa >= klo) && (kappa < khi)) {
-                        const uint32_t k = (uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1);
-                        const uint32_t bit = __float_as_uint(hv.w);
-                        if (PACK == 2)
-                            smem_red_or(row_addr + (((k << 1) ^ swzb) & ~3u), __funnelshift_l(0u, bit, k << 4));
-                        else
-                            smem_red_or(row_addr + ((k << 2) ^ swzb), bit);
-                        ++my_votes;
+                    for (int u = 0; u < EVAL_UNROLL; ++u) {
+                        hv[u] = surv[hs + u];
+                        t[u] = estimate(hv[u], e[u], den[u]);
                     }
+#pragma unroll
+                    for (int u = 0; u < EVAL_UNROLL; ++u)
+                        settle(t[u], e[u], den[u], __float_as_uint(hv[u].w));
+                }
+                for (; hs < total; ++hs) { // the last, partial group of one set
+                    const float4 hv = surv[hs];
+                    float e, den;
+                    const uint32_t t = estimate(hv, e, den);
+                    settle(t, e, den, __float_as_uint(hv.w));
+                }
+                for (int w = set; w < n_wild; w += split)
+                    exact(surv[ge.chunk + EVAL_UNROLL - 1 - w]);
+            } else {
+                for (int hs = set * EVAL_UNROLL; hs < total; hs += split * EVAL_UNROLL) {
+#pragma unroll
+                    for (int u = 0; u < EVAL_UNROLL; ++u)
+                        exact(surv[hs + u]);
                 }
             }
         }
@@ -247,7 +314,7 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     // rows for the P x D cells only: padding lanes of the last cell group never vote
     const size_t tile_bytes = (size_t)(P * D) * cfg.n_kappa * 4 / h->g.pack, extra = 0;
     ge->tile_words = (int)(tile_bytes / 4);
-    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16;
+    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);
     // the interval test needs the slab to span well under a quarter turn
     double span = (cfg.phi_max - cfg.phi_min) * (double)(P - 1) / (double)cfg.n_phi;
@@ -264,12 +331,11 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     const int step = (D <= 32 && 32 % D == 0) ? 32 / D : 0;
     if (fit_waves && step > 0 && P % step == 0 && P - step >= step) {
         int per_sm = 0;
-        cudaError_t e = h->g.pack == 2 ? ensure_dynamic_smem((const void *)k_sweep<2>, ge->smem_bytes)
-                                       : ensure_dynamic_smem((const void *)k_sweep<1>, ge->smem_bytes);
+        const void *fn = h->g.pack == 2 ? (h->ab.ok ? (const void *)k_sweep<2, true> : (const void *)k_sweep<2, false>)
+                                        : (h->ab.ok ? (const void *)k_sweep<1, true> : (const void *)k_sweep<1, false>);
+        cudaError_t e = ensure_dynamic_smem(fn, ge->smem_bytes);
         if (e == cudaSuccess)
-            e = h->g.pack == 2
-                    ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<2>, ge->threads, ge->smem_bytes)
-                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<1>, ge->threads, ge->smem_bytes);
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ge->threads, ge->smem_bytes);
         if (e != cudaSuccess || per_sm < 1) {
             cudaGetLastError();
             return 1;
@@ -316,15 +382,16 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
     p->n_evals = &h->counters->n_evals;
+    p->ab = h->ab;
 }
 
-template <int PACK>
+template <int PACK, bool APPROX>
 static cudaError_t launch_one(const SweepParams &p, cudaStream_t st)
 {
-    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK>, p.geom.smem_bytes);
+    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK, APPROX>, p.geom.smem_bytes);
     if (e != cudaSuccess)
         return e;
-    k_sweep<PACK><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
+    k_sweep<PACK, APPROX><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -333,6 +400,8 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     SweepParams p;
     fill_params(h, &p, h->vote_geom);
     h->launches += 1;
-    return h->g.pack == 2 ? launch_one<2>(p, st) : launch_one<1>(p, st);
+    if (h->ab.ok)
+        return h->g.pack == 2 ? launch_one<2, true>(p, st) : launch_one<1, true>(p, st);
+    return h->g.pack == 2 ? launch_one<2, false>(p, st) : launch_one<1, false>(p, st);
 }
 
