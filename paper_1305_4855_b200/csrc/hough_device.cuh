@@ -110,6 +110,23 @@ __device__ __forceinline__ uint32_t smem_ld(uint32_t addr)
     return v;
 }
 
+// Order-preserving compaction across the warps of a CTA: warp_cnt[w] holds the number of items
+// warp w keeps (n_warps <= 32); every warp scans the counts with shuffles.  Returns the number
+// of items of the warps before `warp`; `all` receives the CTA's total.
+__device__ __forceinline__ int warps_before(const int *warp_cnt, int n_warps, int warp, int lane, int &all)
+{
+    const int cw = lane < n_warps ? warp_cnt[lane] : 0;
+    int incl = cw;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o)
+            incl += t;
+    }
+    all = __shfl_sync(0xffffffffu, incl, 31);
+    return __shfl_sync(0xffffffffu, incl - cw, warp);
+}
+
 // ------------------------------------------------------------------ conservative tile cull
 // Can this hit cast a vote anywhere in the tile (phi0 centres between A and B, d0 centres
 // in [dlo, dhi])?  Interval arithmetic on  2|e| <= K (e^2 + c^2),  e = s - d0,

@@ -366,13 +366,8 @@ __global__ void __launch_bounds__(32 * WARPS) k_list_sweep(const ListSweepParams
             if (lane == 0)
                 warp_cnt[warp] = __popc(bal);
             __syncthreads();
-            int before = 0, all = 0;
-#pragma unroll
-            for (int w = 0; w < WARPS; ++w) {
-                const int cw = warp_cnt[w];
-                before += (w < warp) ? cw : 0;
-                all += cw;
-            }
+            int all;
+            const int before = warps_before(warp_cnt, WARPS, warp, lane, all);
             if (keep) // a hit outside the estimate's range is staged with r2 = NaN: every estimate says "undecided"
                 surv[total + before + __popc(bal & lt_mask)] =
                     make_float4(hx, hy, (APPROX && hit_is_wild(hr2)) ? __int_as_float(0x7fc00000) : hr2,

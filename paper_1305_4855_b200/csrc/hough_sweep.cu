@@ -152,12 +152,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             if (lane == 0)
                 warp_cnt[warp] = __popc(bal);
             __syncthreads();
-            int before = 0, all = 0;
-            for (int w = 0; w < nwarps; ++w) {
-                int cw = warp_cnt[w];
-                before += (w < warp) ? cw : 0;
-                all += cw;
-            }
+            int all;
+            const int before = warps_before(warp_cnt, nwarps, warp, lane, all);
             if (keep) {
                 int pos = total + before + __popc(bal & ((1u << lane) - 1u));
                 surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(hb));
