@@ -453,10 +453,10 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
         return r
 
     rl_vote = sweep_roofline("k_sweep (vote)", "vote", evals_step / n_ev, evals_done_step / n_ev, "vote")
-    rl_list = sweep_roofline("k_list_sweep (hit lists)", "list_sweep", hits_x_peak_cells / n_ev,
-                             list_evals_done / n_ev, "list_sweep")
+    rl_list = sweep_roofline("k_peak_lists (hit lists)", "lists", hits_x_peak_cells / n_ev,
+                             list_evals_done / n_ev, "lists")
     rl_list["cells_with_reported_peaks_per_event"] = peak_cells / n_ev
-    by_stage = {"vote": rl_vote, "list_sweep": rl_list}
+    by_stage = {"vote": rl_vote, "lists": rl_list}
     # the contract's `roofline` describes the MEASURED dominant stage; the other sweep sits beside it
     primary = by_stage.get(dom, rl_vote)
     out["roofline"] = dict(primary, note=alu_note, dominant_stage_measured=dom)

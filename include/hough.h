@@ -64,6 +64,8 @@ extern "C" {
 #define HOUGH_OPT_STAGE_TIMING 2u /* record a CUDA event after every kernel (see hough_stage_times) */
 #define HOUGH_OPT_EXACT_ONLY 8u   /* evaluate every bin with the exact recipe (no fixed-point fast path with
                                      exact fallback near bin edges; results are identical either way) */
+#define HOUGH_OPT_LIST_SWEEP 16u  /* hit lists by a second sweep of all hits over all cells (the round-1 path)
+                                     instead of the peak-driven lists; results are identical either way */
 #define HOUGH_OPT_UNPACKED 4u     /* one mask per 32-bit word of the vote tile even with <= 16 layers (test hook
                                      for the tile layout used with 17..32 layers) */
 

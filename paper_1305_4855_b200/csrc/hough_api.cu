@@ -16,20 +16,42 @@ __global__ void __launch_bounds__(256) k_prep(const float *__restrict__ x, const
                                               const int32_t *__restrict__ layer, uint32_t n,
                                               uint32_t n_pad, int n_layers, float *__restrict__ hx,
                                               float *__restrict__ hy, float *__restrict__ hr2,
-                                              uint32_t *__restrict__ hbit, DevCounters *counters)
+                                              uint32_t *__restrict__ hbit, DevCounters *counters, HitIndexDev ix)
 {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
+    __shared__ uint32_t s_layer_r[2 * 33]; // the CTA's share of the per-layer radius range
+    if (threadIdx.x < 2 * 33)
+        s_layer_r[threadIdx.x] = 0u;
+    __syncthreads();
     if (i < n) {
         float xv = x[i], yv = y[i];
         float pp = __fmul_rn(xv, xv);
         float qq = __fmul_rn(yv, yv);
+        float r2 = __fadd_rn(pp, qq);
         int l = layer[i];
         bad = (l < 0) || (l >= n_layers);
         hx[i] = xv;
         hy[i] = yv;
-        hr2[i] = __fadd_rn(pp, qq);
+        hr2[i] = r2;
         hbit[i] = bad ? 0u : (1u << l);
+        // index key for the peak-driven hit lists (hough_peaklists.cu): (layer label, azimuth bin);
+        // hits whose r^2 is outside [2^-40, 2^80] (or not finite) go to pseudo-layer n_layers
+        uint32_t key = 0xffffffffu;
+        if (!bad) {
+            if (!((r2 >= 9.094947017729282e-13f) && (r2 <= 1.2089258196146292e24f))) {
+                key = (uint32_t)(n_layers * ix.NA);
+            } else {
+                const float r = sqrtf(r2);
+                const float na_scale = (float)ix.NA * 0.15915494309189535f;
+                const int ab = ((int)floorf((atan2f(yv, xv) + 3.14159265358979f) * na_scale)) & (ix.NA - 1);
+                key = (uint32_t)(l * ix.NA + ab);
+                atomicMax(&s_layer_r[2 * l], ~__float_as_uint(r));
+                atomicMax(&s_layer_r[2 * l + 1], __float_as_uint(r));
+            }
+            atomicAdd(&ix.bin_cnt[key], 1u);
+        }
+        ix.key[i] = key;
     } else if (i < n_pad) {
         hx[i] = 0.f;
         hy[i] = 0.f;
@@ -39,6 +61,9 @@ __global__ void __launch_bounds__(256) k_prep(const float *__restrict__ x, const
     unsigned b = __ballot_sync(0xffffffffu, bad);
     if ((threadIdx.x & 31) == 0 && b)
         atomicAdd(&counters->n_bad_hits, (unsigned int)__popc(b));
+    __syncthreads();
+    if (threadIdx.x < 2 * 33 && s_layer_r[threadIdx.x] != 0u)
+        atomicMax(&ix.layer_r[threadIdx.x], s_layer_r[threadIdx.x]);
 }
 
 cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
@@ -47,8 +72,12 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
     uint32_t n_pad = ((n + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
     if (n_pad == 0)
         return cudaSuccess;
+    // histogram / cursor and the per-layer radius range of the event's hit index start from zero
+    cudaError_t e = cudaMemsetAsync(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4 + 2 * 33 * 4, st);
+    if (e != cudaSuccess)
+        return e;
     k_prep<<<(n_pad + 255) / 256, 256, 0, st>>>(x, y, layer, n, n_pad, h->cfg.n_layers, h->hx, h->hy, h->hr2,
-                                                h->hbit, h->counters);
+                                                h->hbit, h->counters, h->ix);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -175,6 +204,17 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *peak_len = cv.take((size_t)c->cap_peaks * 4);
     void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
+    // hit index of the peak-driven lists: azimuth bins per layer ~ 2 x hits per layer, a power of two
+    int NA = 256;
+    while (NA < 8192 && (uint64_t)NA * (uint64_t)c->n_layers < 2ull * c->max_hits)
+        NA <<= 1;
+    const int n_keys = (c->n_layers + 1) * NA;
+    void *t_phic = cv.take((size_t)c->n_phi * 4);
+    void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 33 * 4); // histogram | per-layer radius range (one memset)
+    void *ix_start = cv.take((size_t)(n_keys + 1) * 4);
+    void *ix_key = cv.take((size_t)hp * 4);
+    void *ix_sx = cv.take((size_t)hp * 4), *ix_sy = cv.take((size_t)hp * 4), *ix_sr2 = cv.take((size_t)hp * 4);
+    void *ix_hit = cv.take((size_t)hp * 4), *ix_abin = cv.take((size_t)hp * 2);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -199,6 +239,18 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ent_sub = (uint32_t *)ent_sub;
         h->ent_hit = (uint32_t *)ent_hit;
         h->ent_idx = (uint32_t *)ent_idx;
+        h->t_phic = (float *)t_phic;
+        h->ix.NA = NA;
+        h->ix.n_keys = n_keys;
+        h->ix.bin_cnt = (uint32_t *)ix_cnt;
+        h->ix.layer_r = (uint32_t *)ix_cnt + n_keys;
+        h->ix.bin_start = (uint32_t *)ix_start;
+        h->ix.key = (uint32_t *)ix_key;
+        h->ix.sx = (float *)ix_sx;
+        h->ix.sy = (float *)ix_sy;
+        h->ix.sr2 = (float *)ix_sr2;
+        h->ix.s_hit = (uint32_t *)ix_hit;
+        h->ix.s_abin = (unsigned short *)ix_abin;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
@@ -377,10 +429,12 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     float *sn = (float *)malloc(sizeof(float) * np), *cs = (float *)malloc(sizeof(float) * np);
     float *d0c = (float *)malloc(sizeof(float) * nd), *twod0 = (float *)malloc(sizeof(float) * nd);
     float *d0sq = (float *)malloc(sizeof(float) * nd);
+    float *phf = (float *)malloc(sizeof(float) * np);
     for (int i = 0; i < np; ++i) {
         double phic = cfg->phi_min + ((double)i + 0.5) * (cfg->phi_max - cfg->phi_min) / (double)np;
         sn[i] = (float)sin(phic);
         cs[i] = (float)cos(phic);
+        phf[i] = (float)remainder(phic, 6.283185307179586); // the angle itself, in [-pi, pi] (azimuth windows)
     }
     float d0abs = 0.f;
     for (int j = 0; j < nd; ++j) {
@@ -414,6 +468,8 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     int ok = 1;
     ok &= cudaMemcpy(h->t_sn, sn, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_cs, cs, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_phic, phf, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
+    free(phf);
     ok &= cudaMemcpy(h->t_d0c, d0c, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_twod0, twod0, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_d0sq, d0sq, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
@@ -480,6 +536,8 @@ int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *l
     stage_mark(h, 0, st);
     CK(cudaMemsetAsync(h->counters, 0, 64, st));
     CK(launch_prep(h, x, y, layer, n, st));
+    if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP))
+        CK(launch_index_build(h, st));
     stage_mark(h, ST_PREP + 1, st);
     CK(launch_vote(h, st));
     stage_mark(h, ST_VOTE + 1, st);
@@ -504,11 +562,12 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
-        CK(launch_list_sweep(h, st));
+        const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) ? 1 : 0;
+        CK(sweep ? launch_list_sweep(h, st) : launch_peak_lists(h, out, st));
         stage_mark(h, ST_LIST_SWEEP + 1, st);
         CK(launch_scan_lens(h, out, st));
         stage_mark(h, ST_SCAN_LENS + 1, st);
-        CK(launch_place_lists(h, out, st));
+        CK(sweep ? launch_place_lists(h, out, st) : launch_copy_lists(h, out, st));
         stage_mark(h, ST_PLACE_LISTS + 1, st);
     }
     CK(launch_finish_counts(h, out, with_lists, st));
@@ -667,7 +726,7 @@ int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int3
 uint64_t hough_launch_count(const hough_handle *h) { return h ? h->launches : 0; }
 
 static const char *const k_stage_names[HOUGH_N_STAGES] = {
-    "prep", "vote", "peak_sweep", "scan_rows", "compact", "list_sweep", "scan_lens", "place_lists",
+    "prep", "vote", "peak_sweep", "scan_rows", "compact", "lists", "scan_lens", "place_lists",
     "finish"};
 
 const char *hough_stage_name(int stage)

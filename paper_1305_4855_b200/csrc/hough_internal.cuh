@@ -72,6 +72,20 @@ struct HitsDev {         // prepared hits, SoA, padded with non-voting entries t
     uint32_t n_pad;      // padded length (multiple of the chunk size)
 };
 
+// Per-event index of the hits by (layer label, azimuth bin) for the peak-driven hit lists
+// (hough_peaklists.cu).  Pseudo-layer n_layers holds the hits outside the index's numeric range.
+struct HitIndexDev {
+    int NA;                 // azimuth bins per layer (power of two)
+    int n_keys;             // (n_layers + 1) * NA
+    uint32_t *bin_cnt;      // [n_keys] histogram of the event (k_prep), then the scatter cursor
+    uint32_t *bin_start;    // [n_keys + 1] rank of the first hit of a key
+    uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) (zeroed per event)
+    uint32_t *key;          // [max_hits_pad] key of hit h, 0xffffffff = not indexed (bad layer)
+    float *sx, *sy, *sr2;   // [max_hits_pad] the hits in key order
+    uint32_t *s_hit;        // their original indices
+    unsigned short *s_abin; // their azimuth bins
+};
+
 // Device counters of one event (internal; copied into the caller's hough_counts).
 struct DevCounters {
     unsigned long long n_votes;
@@ -99,7 +113,8 @@ struct hough_handle {
     ListGeom list_geom;
     // workspace carve-up (device)
     uint32_t *acc;
-    float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq;
+    float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq, *t_phic;
+    HitIndexDev ix;
     float *hx, *hy, *hr2;
     uint32_t *hbit;
     float *raw_x, *raw_y;  // staging of hough_process_host's host buffers
@@ -148,6 +163,9 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
 cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
+cudaError_t launch_index_build(hough_handle *h, cudaStream_t st);
+cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st);

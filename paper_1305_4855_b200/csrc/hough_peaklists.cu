@@ -1,0 +1,569 @@
+// hough_peaklists.cu -- a7, the hit lists of the reported peaks, PEAK-DRIVEN (SURVEY.md section
+// 8(a)): "each peak is emitted with its sorted hit list" (BASELINE.json
+// north_star); hit list of a peak = the hits whose own vote at the peak's (phi0, d0) cell lands
+// in the peak's kappa bin, ascending hit index, CSR (A7).
+//
+// A second sweep of all hits over all cells repeats the whole vote to recover the 4 % of the
+// votes that land in reported peaks.  Instead the hits are indexed once per event by
+// (layer label, azimuth bin), and every peak looks only at the hits that can lie between the
+// two circles that bound its bin:
+//
+//   with n = (-sin phi0, cos phi0), a hit X at radius r and w = sin(azimuth(X) - phi0):
+//     kappa(X) >= kappa_1  <=>  2 e - kappa_1 den >= 0  <=>  w >= W(kappa_1, r)     (den = |X - P0|^2 > 0)
+//     W(kappa, r) = A / r + B r,  A = d0 (2 + kappa d0) / (2 (1 + kappa d0)),  B = kappa / (2 (1 + kappa d0))
+//   (the closed form solved for s = r w; needs 1 + kappa d0 > 0).  Over the radii [ra, rb] that
+//   the hits of one layer label really have, min W(kappa_lo) and max W(kappa_hi) are taken at the
+//   end points or at the stationary point sqrt(A / B); asin of that w-interval gives two azimuth
+//   windows (the circle meets a radius twice: phi0 + asin w and phi0 + pi - asin w).
+//
+// The windows are SUPERSETS: the bin's kappa interval is widened by a bound on the binary32
+// evaluation error of the recipe (which grows as 1 / den; hits closer than L0 to the point of
+// closest approach P0 are taken through a third, "proximity" window around P0's azimuth instead),
+// every angle by 2e-5 rad and every window by one azimuth bin on each side.  Whatever cannot be
+// bounded (1 + kappa d0 not safely positive, non-finite intermediate values, a window wider than
+// the ring) falls back to the whole layer; hits outside the index's numeric range ("wild") are
+// candidates of every peak.  Every candidate is then evaluated with the EXACT recipe
+// (hough_device.cuh eval_kappa / kappa_bin), so the lists are bit-identical to the oracle's.
+//
+// Work split: a group of 16 lanes (32 with more than 16 layers) owns one peak; lane l computes
+// the windows of layer label l if bit l is set in the peak's mask (a hit of layer l in the bin
+// sets that bit, so other layers cannot contribute); the group then walks the flattened
+// candidate list 16 (32) at a time, collects the matching hit indices in shared memory, sorts
+// them and writes them to a staging buffer (one global atomic per CTA and batch).  k_scan<LENS>
+// turns the lengths into hit_offset and k_copy_lists moves the lists to their final place.
+// Lists longer than the group's buffer are counted here and written by k_copy_lists straight
+// from the hits in index order (one warp per such peak).
+#include "hough_device.cuh"
+
+#define PL_WARPS 8
+#define PL_MAXLIST 128
+#define PL_SLOW 0xffffffffu
+#define PI_F 3.14159265358979f
+
+// ------------------------------------------------------------------ index build
+// Histogram and per-layer radius range are accumulated by k_prep (hough_api.cu); here the
+// prefix over the keys and the scatter into key order.
+// Exclusive prefix over the keys by ONE CTA: per round every thread takes IS_V uint4 of the
+// histogram (coalesced, all loads in flight together), the warps scan their uint4 sums with
+// shuffles, warp 0 scans the IS_V x 32 warp totals, and the carry moves on to the next round.
+// n_keys is a multiple of 256 (NA >= 256), so uint4 accesses never straddle the end.
+#define IS_V 4
+__global__ void __launch_bounds__(1024) k_index_scan(uint32_t *__restrict__ cnt, uint32_t *__restrict__ start,
+                                                     int n_keys)
+{
+    __shared__ uint32_t s_warp[IS_V][32];
+    __shared__ uint32_t s_carry;
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    uint32_t carry = 0;
+    for (int base = 0; base < n_keys; base += IS_V * 4096) {
+        uint4 v[IS_V];
+        uint32_t incl[IS_V], sum[IS_V];
+#pragma unroll
+        for (int q = 0; q < IS_V; ++q) {
+            const int k = base + q * 4096 + t * 4;
+            v[q] = k < n_keys ? *reinterpret_cast<const uint4 *>(cnt + k) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int q = 0; q < IS_V; ++q) {
+            sum[q] = v[q].x + v[q].y + v[q].z + v[q].w;
+            incl[q] = sum[q];
+        }
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+            for (int q = 0; q < IS_V; ++q) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl[q], o);
+                if (lane >= o)
+                    incl[q] += u;
+            }
+        }
+        if (lane == 31) {
+#pragma unroll
+            for (int q = 0; q < IS_V; ++q)
+                s_warp[q][warp] = incl[q];
+        }
+        __syncthreads();
+        if (warp == 0) { // exclusive scan of the IS_V x 32 warp totals, in key order
+            uint32_t run = carry;
+#pragma unroll
+            for (int q = 0; q < IS_V; ++q) {
+                const uint32_t w = s_warp[q][lane];
+                uint32_t wi = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xffffffffu, wi, o);
+                    if (lane >= o)
+                        wi += u;
+                }
+                s_warp[q][lane] = run + wi - w;
+                run += __shfl_sync(0xffffffffu, wi, 31);
+            }
+            if (lane == 0)
+                s_carry = run;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < IS_V; ++q) {
+            const int k = base + q * 4096 + t * 4;
+            if (k < n_keys) {
+                const uint32_t e0 = s_warp[q][warp] + incl[q] - sum[q];
+                uint4 o;
+                o.x = e0;
+                o.y = e0 + v[q].x;
+                o.z = o.y + v[q].y;
+                o.w = o.z + v[q].z;
+                *reinterpret_cast<uint4 *>(start + k) = o;
+                *reinterpret_cast<uint4 *>(cnt + k) = make_uint4(0u, 0u, 0u, 0u); // becomes the scatter cursor
+            }
+        }
+        carry = s_carry;
+        __syncthreads();
+    }
+    if (t == 0)
+        start[n_keys] = carry;
+}
+
+__global__ void __launch_bounds__(256) k_index_scatter(HitIndexDev ix, const float *__restrict__ hx,
+                                                       const float *__restrict__ hy,
+                                                       const float *__restrict__ hr2, uint32_t n)
+{
+    const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n)
+        return;
+    const uint32_t key = ix.key[h];
+    if (key == 0xffffffffu)
+        return;
+    const uint32_t rank = ix.bin_start[key] + atomicAdd(&ix.bin_cnt[key], 1u);
+    ix.sx[rank] = hx[h];
+    ix.sy[rank] = hy[h];
+    ix.sr2[rank] = hr2[h];
+    ix.s_hit[rank] = h;
+    ix.s_abin[rank] = (unsigned short)(key & (uint32_t)(ix.NA - 1));
+}
+
+cudaError_t launch_index_build(hough_handle *h, cudaStream_t st)
+{
+    if (h->n_hits == 0)
+        return cudaSuccess;
+    k_index_scan<<<1, 1024, 0, st>>>(h->ix.bin_cnt, h->ix.bin_start, h->ix.n_keys);
+    k_index_scatter<<<(h->n_hits + 255) / 256, 256, 0, st>>>(h->ix, h->hx, h->hy, h->hr2, h->n_hits);
+    h->launches += 2;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ the peak-driven list kernel
+struct PeakListParams {
+    GridDev g;
+    HitIndexDev ix;
+    const float *phic; // [n_phi] bin-centre angles
+    uint32_t n_hits;
+    const uint32_t *bin, *mask; // reported peaks (k_compact)
+    const DevCounters *counters;
+    uint32_t cap_peaks;
+    uint32_t *peak_len; // [cap_peaks] list length
+    uint32_t *peak_pos; // [cap_peaks] start of the list in ent_hit, or PL_SLOW
+    uint32_t *ent_hit;  // [ent_cap] staging
+    unsigned long long ent_cap;
+    unsigned long long *n_entries;   // staging entries handed out
+    unsigned long long *n_list_evals; // candidates evaluated
+    float dk;       // kappa bin width (binary32)
+    float edge_rel; // slack on a bin edge, in bins
+};
+
+struct PlRange { // candidates of one azimuth window: virtual ranks [q0, q0 + cnt) of the layer, bins [b0, b0 + nb)
+    uint32_t q0, cnt;
+    int b0, nb;
+};
+
+// Azimuth window [a_lo, a_hi] (radians, a_lo <= a_hi) -> bins, one extra bin on each side.
+__device__ __forceinline__ void window_bins(float a_lo, float a_hi, float na_scale, int NA, int &b0, int &nb)
+{
+    const float t0 = floorf((a_lo + PI_F) * na_scale), t1 = floorf((a_hi + PI_F) * na_scale);
+    const float span = t1 - t0 + 3.0f;
+    if (!(span < (float)NA)) { // also NaN: the whole ring
+        b0 = 0;
+        nb = NA;
+        return;
+    }
+    b0 = ((int)t0 - 1) & (NA - 1);
+    nb = (int)span;
+}
+
+template <int G> // lanes per peak
+__global__ void __launch_bounds__(32 * PL_WARPS) k_peak_lists(const PeakListParams p)
+{
+    constexpr int GPW = 32 / G;            // groups per warp
+    constexpr int GPC = PL_WARPS * GPW;    // groups (= peaks) per CTA and batch
+    __shared__ PlRange s_rng[GPC][G][3];
+    __shared__ uint32_t s_pre[GPC][G + 1]; // exclusive prefix of the lanes' candidate counts
+    __shared__ uint32_t s_list[GPC][PL_MAXLIST];
+    __shared__ uint32_t s_cnt[GPC], s_off[GPC];
+    __shared__ unsigned long long s_base;
+
+    const GridDev &g = p.g;
+    const HitIndexDev &ix = p.ix;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int grp = warp * GPW + lane / G, gl = lane % G; // group in the CTA, lane in the group
+    const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((lane / G) * G));
+    const int NA = ix.NA, nL = ix.n_keys / NA - 1;
+    const float na_scale = (float)NA * 0.15915494309189535f;
+    const uint32_t n_rep = min(p.counters->n_peaks, p.cap_peaks);
+    const int nk = g.n_kappa;
+    const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
+    const float U = 5.9604645e-08f; // 2^-24
+    unsigned long long evals = 0;
+
+    for (uint32_t batch = blockIdx.x; (unsigned long long)batch * GPC < n_rep; batch += gridDim.x) {
+        const uint32_t pk = batch * GPC + grp;
+        const bool live = pk < n_rep;
+        uint32_t lin = 0, pmask = 0;
+        if (live) {
+            lin = p.bin[pk];
+            pmask = p.mask[pk];
+        }
+        const uint32_t k = lin % (uint32_t)nk, row = lin / (uint32_t)nk;
+        const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
+        const float c_sn = g.sn[i], c_cs = g.cs[i], c_d0 = g.d0c[j], c_2d0 = g.twod0[j], c_d0sq = g.d0sq[j];
+        const float phi0 = p.phic[i], ad0 = fabsf(c_d0);
+
+        // ---- phase 1: lane gl = layer label gl: its azimuth windows
+        PlRange r0 = {0u, 0u, 0, 0}, r1 = r0, r2 = r0;
+        uint32_t lbase = 0, lcnt = 0;
+        if (live && gl < nL && ((pmask >> gl) & 1u)) {
+            lbase = ix.bin_start[gl * NA];
+            lcnt = ix.bin_start[(gl + 1) * NA] - lbase;
+        }
+        if (lcnt) {
+            // the bin's kappa interval
+            float ka = __fmaf_rn((float)k, p.dk, klo), kb = __fmaf_rn((float)(k + 1u), p.dk, klo);
+            if (k == 0u)
+                ka = fminf(ka, klo);
+            if (k + 1u == (uint32_t)nk)
+                kb = fmaxf(kb, khi);
+            const float ra = __uint_as_float(~ix.layer_r[2 * gl]) * (1.0f - 4e-6f);
+            const float rb = __uint_as_float(ix.layer_r[2 * gl + 1]) * (1.0f + 4e-6f);
+            // binary32 evaluation error of the recipe: |kappa_fp - kappa| <= errnum / den + 2 U K
+            const float Gm = 1.4143f * rb + ad0, Kp = 1.01f * g.kabs + p.dk;
+            const float errnum = 2.0f * (12.0f * U * Gm + 16.0f * U * Kp * Gm * Gm);
+            const float Lmin = fmaxf(0.0f, fmaxf(ra - ad0 * (1.0f + 1e-6f), ad0 * (1.0f - 1e-6f) - rb));
+            const float L0sq = errnum / p.dk; // den >= L0sq: the error stays below one bin
+            float D = Lmin * Lmin;
+            const bool prox = !(D >= L0sq);
+            if (prox)
+                D = L0sq;
+            const float slack = errnum / D + 2.0f * U * Kp + p.edge_rel * p.dk;
+            const float k1 = ka - slack, k2 = kb + slack;
+            const float g1 = __fmaf_rn(k1, c_d0, 1.0f), g2 = __fmaf_rn(k2, c_d0, 1.0f);
+            bool whole = !(g1 > 0.01f && g2 > 0.01f);
+            int b0 = 0, nb = 0, b1 = 0, nb1 = 0, b2 = 0, nb2 = 0;
+            if (!whole) {
+                const float A1 = c_d0 * __fmaf_rn(k1, c_d0, 2.0f) / (2.0f * g1), B1 = k1 / (2.0f * g1);
+                const float A2 = c_d0 * __fmaf_rn(k2, c_d0, 2.0f) / (2.0f * g2), B2 = k2 / (2.0f * g2);
+                float wlo = fminf(A1 / ra + B1 * ra, A1 / rb + B1 * rb);
+                float whi = fmaxf(A2 / ra + B2 * ra, A2 / rb + B2 * rb);
+                if (A1 > 0.0f && B1 > 0.0f) { // W(k1, r) has its minimum 2 sqrt(A B) at r^2 = A / B
+                    const float q = A1 / B1;
+                    if (q > ra * ra && q < rb * rb)
+                        wlo = fminf(wlo, 2.0f * sqrtf(A1 * B1) * (1.0f - 1e-6f));
+                }
+                if (A2 < 0.0f && B2 < 0.0f) { // W(k2, r) has its maximum -2 sqrt(A B) at r^2 = A / B
+                    const float q = A2 / B2;
+                    if (q > ra * ra && q < rb * rb)
+                        whi = fmaxf(whi, -2.0f * sqrtf(A2 * B2) * (1.0f - 1e-6f));
+                }
+                const float ew = 1e-5f * (1.0f + fmaxf(fabsf(wlo), fabsf(whi)));
+                wlo -= ew;
+                whi += ew;
+                if (!(fabsf(wlo) < 3.0e38f) || !(fabsf(whi) < 3.0e38f) || !(wlo <= whi)) {
+                    whole = true; // inf / NaN somewhere: no bound
+                } else if (!(wlo > 1.0f) && !(whi < -1.0f)) {
+                    const float tlo = asinf(fmaxf(wlo, -1.0f)) - 2e-5f, thi = asinf(fminf(whi, 1.0f)) + 2e-5f;
+                    window_bins(phi0 + tlo, phi0 + thi, na_scale, NA, b0, nb);
+                    window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA, b1, nb1);
+                }
+            }
+            if (!whole && prox) {
+                // hits closer than L0 to P0 (azimuth of P0 = phi0 +- pi/2): |X - P0|^2 >= 4 r |d0| sin^2(dpsi / 2)
+                const float arg = 1.01f * sqrtf(L0sq) / (2.0f * sqrtf(ra * ad0));
+                if (!(arg < 0.999f)) {
+                    whole = true;
+                } else {
+                    const float hw = 2.0f * asinf(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
+                    window_bins(psi - hw, psi + hw, na_scale, NA, b2, nb2);
+                }
+            }
+            if (whole || nb >= NA || nb1 >= NA || nb2 >= NA) {
+                b0 = 0, nb = NA, nb1 = 0, nb2 = 0;
+            }
+            // bins -> virtual ranks of the layer (the layer's hits repeated twice, so no wrap)
+            const uint32_t *bs = ix.bin_start + gl * NA;
+            auto P2 = [&](int b) -> uint32_t { return b <= NA ? bs[b] - lbase : lcnt + bs[b - NA] - lbase; };
+            if (nb) {
+                r0.q0 = P2(b0), r0.cnt = P2(b0 + nb) - r0.q0, r0.b0 = b0, r0.nb = nb;
+            }
+            if (nb1) {
+                r1.q0 = P2(b1), r1.cnt = P2(b1 + nb1) - r1.q0, r1.b0 = b1, r1.nb = nb1;
+            }
+            if (nb2) {
+                r2.q0 = P2(b2), r2.cnt = P2(b2 + nb2) - r2.q0, r2.b0 = b2, r2.nb = nb2;
+            }
+        }
+        // lane nL of the group (or lane 0 of a 32-layer detector, as a 2nd task) takes the wild hits
+        uint32_t wild_cnt = 0, wild_base = 0;
+        if (live && gl == (nL < G ? nL : 0)) {
+            wild_base = ix.bin_start[nL * NA];
+            wild_cnt = ix.bin_start[nL * NA + 1] - wild_base;
+        }
+        const uint32_t mine = r0.cnt + r1.cnt + r2.cnt + wild_cnt;
+        uint32_t incl = mine;
+#pragma unroll
+        for (int o = 1; o < G; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o, G);
+            if (gl >= o)
+                incl += v;
+        }
+        const uint32_t T = __shfl_sync(0xffffffffu, incl, G - 1, G);
+        s_rng[grp][gl][0] = r0;
+        s_rng[grp][gl][1] = r1;
+        s_rng[grp][gl][2] = r2;
+        s_pre[grp][gl] = incl - mine;
+        if (gl == G - 1)
+            s_pre[grp][G] = T;
+        if (gl == 0)
+            s_cnt[grp] = 0u;
+        __syncwarp();
+
+        // ---- phase 2: the group walks its T candidates, G at a time, with the exact recipe
+        const float c_2 = c_2d0;
+        uint32_t Tw = T; // the warp's groups loop together (warp-wide ballots inside)
+#pragma unroll
+        for (int o = G; o < 32; o <<= 1)
+            Tw = max(Tw, __shfl_xor_sync(0xffffffffu, Tw, o));
+        for (uint32_t c0 = 0; c0 < Tw; c0 += G) {
+            const uint32_t c = c0 + gl;
+            bool match = false;
+            uint32_t hit = 0;
+            if (c < T) {
+                // owner lane (= layer): last l with s_pre[l] <= c
+                int lo = 0;
+#pragma unroll
+                for (int stp = G / 2; stp > 0; stp >>= 1)
+                    if (s_pre[grp][lo + stp] <= c)
+                        lo += stp;
+                uint32_t off = c - s_pre[grp][lo];
+                const PlRange q0 = s_rng[grp][lo][0], q1 = s_rng[grp][lo][1], q2 = s_rng[grp][lo][2];
+                uint32_t rank;
+                bool take = true;
+                int ab = 0;
+                if (off < q0.cnt + q1.cnt + q2.cnt) {
+                    const uint32_t lb = ix.bin_start[lo * NA], lc = ix.bin_start[(lo + 1) * NA] - lb;
+                    int which = 0;
+                    uint32_t q = q0.q0 + off;
+                    if (off >= q0.cnt) {
+                        off -= q0.cnt;
+                        which = 1;
+                        q = q1.q0 + off;
+                        if (off >= q1.cnt) {
+                            off -= q1.cnt;
+                            which = 2;
+                            q = q2.q0 + off;
+                        }
+                    }
+                    rank = lb + (q >= lc ? q - lc : q);
+                    ab = ix.s_abin[rank];
+                    // a hit already seen through an earlier window of the same layer is skipped
+                    if (which >= 1 && (uint32_t)((ab - q0.b0) & (NA - 1)) < (uint32_t)q0.nb)
+                        take = false;
+                    if (which == 2 && (uint32_t)((ab - q1.b0) & (NA - 1)) < (uint32_t)q1.nb)
+                        take = false;
+                } else { // the wild hits
+                    rank = ix.bin_start[nL * NA] + (off - (q0.cnt + q1.cnt + q2.cnt));
+                }
+                if (take) {
+                    const float kappa = eval_kappa(ix.sx[rank], ix.sy[rank], ix.sr2[rank], c_sn, c_cs, c_d0, c_2, c_d0sq);
+                    if ((kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k) {
+                        match = true;
+                        hit = ix.s_hit[rank];
+                    }
+                }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, match) & gmask;
+            if (match) {
+                const uint32_t pos = s_cnt[grp] + (uint32_t)__popc(bal & ((1u << lane) - 1u));
+                if (pos < PL_MAXLIST)
+                    s_list[grp][pos] = hit;
+            }
+            __syncwarp();
+            if (gl == 0)
+                s_cnt[grp] += (uint32_t)__popc(bal);
+            __syncwarp();
+        }
+        if (gl == 0)
+            evals += T;
+
+        // ---- phase 3: staging space (one global atomic per CTA and batch), sort, write
+        __syncthreads();
+        if (tid == 0) {
+            uint32_t tot = 0;
+            for (int q = 0; q < GPC; ++q) {
+                const uint32_t n = s_cnt[q];
+                s_off[q] = tot;
+                tot += n <= PL_MAXLIST ? n : 0u;
+            }
+            s_base = tot ? atomicAdd(p.n_entries, (unsigned long long)tot) : 0ull;
+        }
+        __syncthreads();
+        if (live) {
+            const uint32_t n = s_cnt[grp];
+            if (n > PL_MAXLIST) { // too long for the buffer: counted here, written by k_copy_lists
+                if (gl == 0) {
+                    p.peak_len[pk] = n;
+                    p.peak_pos[pk] = PL_SLOW;
+                }
+            } else {
+                const unsigned long long base = s_base + s_off[grp];
+                const bool fits = base + n <= p.ent_cap;
+                if (gl == 0) {
+                    p.peak_len[pk] = n;
+                    p.peak_pos[pk] = fits ? (uint32_t)base : PL_SLOW;
+                }
+                if (fits)
+                    for (uint32_t a = gl; a < n; a += G) { // rank by counting: the list is short
+                        const uint32_t v = s_list[grp][a];
+                        uint32_t rk = 0;
+                        for (uint32_t b = 0; b < n; ++b)
+                            rk += s_list[grp][b] < v ? 1u : 0u;
+                        p.ent_hit[base + rk] = v;
+                    }
+            }
+        }
+        __syncthreads();
+    }
+    if (gl == 0 && evals)
+        atomicAdd(p.n_list_evals, evals);
+}
+
+// ------------------------------------------------------------------ placement
+struct ListCopyParams {
+    GridDev g;
+    const float *hx, *hy, *hr2;
+    const uint32_t *hbit;
+    uint32_t n_hits;
+    const DevCounters *counters;
+    uint32_t cap_peaks;
+    const uint32_t *bin;
+    const uint32_t *peak_len, *peak_pos, *ent_hit;
+    const unsigned long long *hit_offset;
+    uint32_t *hit_index;
+    unsigned long long cap_hits;
+};
+
+// hit_index[hit_offset[p] ..] = the staged list of peak p (half a warp per peak); a peak without
+// a staged list (PL_SLOW) is written straight from the hits in index order by a whole warp.
+__global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
+{
+    const GridDev &g = p.g;
+    const int lane = threadIdx.x & 31, hl = lane & 15;
+    const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
+    const uint32_t halves = (gridDim.x * blockDim.x) >> 4;
+    for (uint32_t pk0 = (((blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 1); pk0 < n; pk0 += halves) {
+        const uint32_t pk = pk0 + (lane >> 4);
+        uint32_t pos = 0, len = 0;
+        unsigned long long dst = 0;
+        if (pk < n) {
+            pos = p.peak_pos[pk];
+            len = p.peak_len[pk];
+            dst = p.hit_offset[pk];
+        }
+        if (pos != PL_SLOW)
+            for (uint32_t a = hl; a < len; a += 16)
+                if (dst + a < p.cap_hits)
+                    p.hit_index[dst + a] = p.ent_hit[pos + a];
+        // slow peaks of this pair, one after the other, by the whole warp
+        for (int which = 0; which < 2; ++which) {
+            const uint32_t spos = __shfl_sync(0xffffffffu, pos, which * 16);
+            const uint32_t slen = __shfl_sync(0xffffffffu, len, which * 16);
+            const uint32_t spk = pk0 + which;
+            if (spk >= n || spos != PL_SLOW || slen == 0u)
+                continue;
+            unsigned long long w = p.hit_offset[spk];
+            if (w >= p.cap_hits)
+                continue;
+            const uint32_t lin = p.bin[spk];
+            const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
+            const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
+            const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
+            for (uint32_t base = 0; base < p.n_hits; base += 32) {
+                const uint32_t hidx = base + lane;
+                bool in = false;
+                if (hidx < p.n_hits && p.hbit[hidx] != 0u) {
+                    const float kappa = eval_kappa(p.hx[hidx], p.hy[hidx], p.hr2[hidx], sn, cs, d0c, twod0, d0sq);
+                    if ((kappa >= g.klo) && (kappa < g.khi))
+                        in = (uint32_t)kappa_bin(kappa, g.klo, g.inv_dk, g.n_kappa - 1) == k;
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, in);
+                if (in) {
+                    const unsigned long long q = w + __popc(bal & ((1u << lane) - 1u));
+                    if (q < p.cap_hits)
+                        p.hit_index[q] = hidx;
+                }
+                w += __popc(bal);
+            }
+        }
+    }
+}
+
+cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    if (h->n_hits == 0) // no event (hough_set_accumulator): every list is empty, the index is not built
+        return cudaMemsetAsync(h->peak_len, 0, (size_t)h->cfg.cap_peaks * 4, st);
+    PeakListParams p;
+    p.g = h->g;
+    p.ix = h->ix;
+    p.phic = h->t_phic;
+    p.n_hits = h->n_hits;
+    p.bin = out->bin;
+    p.mask = out->mask;
+    p.counters = h->counters;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.peak_len = h->peak_len;
+    p.peak_pos = h->list_len;
+    p.ent_hit = h->ent_hit;
+    p.ent_cap = h->cfg.cap_hits;
+    p.n_entries = h->n_pairs;
+    p.n_list_evals = &h->counters->n_list_evals;
+    p.dk = (float)(((double)h->g.khi - (double)h->g.klo) / (double)h->g.n_kappa);
+    // bin-edge slack in bins: the roundings of (kappa - klo) * inv_dk and of the edges computed here
+    const double A = (double)h->g.kabs / ((double)h->g.khi - (double)h->g.klo);
+    p.edge_rel = (float)(0.01 + 4e-7 * h->g.n_kappa * (1.0 + A));
+    const int blocks = h->n_sms * 8;
+    if (h->cfg.n_layers <= 15)
+        k_peak_lists<16><<<blocks, 32 * PL_WARPS, 0, st>>>(p);
+    else
+        k_peak_lists<32><<<blocks, 32 * PL_WARPS, 0, st>>>(p);
+    h->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    ListCopyParams p;
+    p.g = h->g;
+    p.hx = h->hx;
+    p.hy = h->hy;
+    p.hr2 = h->hr2;
+    p.hbit = h->hbit;
+    p.n_hits = h->n_hits;
+    p.counters = h->counters;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.bin = out->bin;
+    p.peak_len = h->peak_len;
+    p.peak_pos = h->list_len;
+    p.ent_hit = h->ent_hit;
+    p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
+    p.hit_index = out->hit_index;
+    p.cap_hits = h->cfg.cap_hits;
+    k_copy_lists<<<h->n_sms * 16, 256, 0, st>>>(p);
+    h->launches += 1;
+    return cudaGetLastError();
+}

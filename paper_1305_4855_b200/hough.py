@@ -23,6 +23,7 @@ OPT_NO_CULL = 1
 OPT_STAGE_TIMING = 2
 OPT_UNPACKED = 4
 OPT_EXACT_ONLY = 8
+OPT_LIST_SWEEP = 16
 N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)

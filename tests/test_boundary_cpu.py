@@ -46,7 +46,7 @@ def test_strerror_and_stage_names(hough):
     assert len(texts) == 6
     names = [hough._lib.hough_stage_name(s) for s in range(hough.N_STAGES)]
     assert all(n for n in names) and len(set(names)) == hough.N_STAGES
-    assert names[0] == b"prep" and names[1] == b"vote" and b"list_sweep" in names
+    assert names[0] == b"prep" and names[1] == b"vote" and b"lists" in names
     assert hough._lib.hough_stage_name(hough.N_STAGES) is None
     assert hough._lib.hough_stage_name(-1) is None
 

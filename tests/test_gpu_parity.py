@@ -69,7 +69,7 @@ def random_hits(rng, n, n_layers=10, rmax=80.0):
     ((96, 24, 32), (32, 8), 513, 4),      # smallest row, hits = chunk + 1
     ((33, 9, 256), (4, 8), 100, 5),
 ])
-@pytest.mark.parametrize("options", [0, 1])
+@pytest.mark.parametrize("options", [0, 1, 8, 16, 24])  # default, NO_CULL, EXACT_ONLY, LIST_SWEEP, both
 def test_random_hits_small_grids(hough, oracle, shape, tile, n_hits, seed, options):
     rng = np.random.default_rng(seed)
     d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
@@ -239,6 +239,19 @@ def test_baseline_configs_full_parity(hough, oracle, name):
     x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
     ref = oracle.run(w.grid, x, y, layer)
     res = run_gpu(hough, w.grid, x, y, layer, cap_peaks=w.cap_peaks, cap_hits=w.cap_hits)
+    assert res["flags"] == 0
+    assert_same(res, ref)
+
+
+@pytest.mark.parametrize("name,options", [("displaced3d", 8), ("displaced3d", 16), ("pileup", 16 | 8)])
+def test_baseline_configs_alternative_paths(hough, oracle, name, options):
+    """The same results from the alternative code paths the options select: exact recipe only
+    (HOUGH_OPT_EXACT_ONLY: no fixed-point fast path) and hit lists by a second sweep
+    (HOUGH_OPT_LIST_SWEEP) instead of the peak-driven lists."""
+    w = synth.WORKLOADS[name]
+    x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
+    ref = oracle.run(w.grid, x, y, layer)
+    res = run_gpu(hough, w.grid, x, y, layer, cap_peaks=w.cap_peaks, cap_hits=w.cap_hits, options=options)
     assert res["flags"] == 0
     assert_same(res, ref)
 
