@@ -41,6 +41,12 @@ def lib():
         _lib.oracle_hitlists.restype = C.c_uint64
         _lib.oracle_vote_one.restype = C.c_int
         _lib.oracle_num_threads.restype = C.c_int
+        for f in ("oracle_vote_variant", "oracle_hitlists_variant", "oracle_vertex_vote",
+                  "oracle_vertex_peaks", "oracle_vertex_members"):
+            getattr(_lib, f).restype = C.c_uint64
+        _lib.oracle_fit_one.restype = C.c_int
+        _lib.oracle_fit_all.restype = None
+        _lib.oracle_select_dedup.restype = None
     return _lib
 
 
@@ -163,3 +169,173 @@ def run(grid, x, y, layer, cap_peaks=None, cap_hits=None):
     return {"acc": acc, "n_votes": n_votes, "n_bad_hits": n_bad, "peak_bin": pb,
             "peak_mask": pm, "n_peaks": n_peaks, "hit_offset": off, "hit_index": idx,
             "n_hit_entries": n_ent}
+
+
+# ---------------------------------------------------------------------------------------
+# hough_ext_oracle.c: the rows SURVEY.md 8(f) marks "next" (recipes E1..E5)
+
+MODE_CIRCLE, MODE_LINE, MODE_INTERVAL = 0, 1, 2
+
+
+class _VGrid(C.Structure):
+    _fields_ = [("x_min", C.c_double), ("x_max", C.c_double), ("y_min", C.c_double),
+                ("y_max", C.c_double), ("n_x", C.c_int32), ("n_y", C.c_int32),
+                ("V_min", C.c_int32), ("reserved", C.c_int32)]
+
+
+class _Fit(C.Structure):
+    _fields_ = [("kappa", C.c_double), ("phi0", C.c_double), ("d0", C.c_double), ("rms", C.c_double)]
+
+
+FIT_DTYPE = np.dtype([("kappa", np.float64), ("phi0", np.float64), ("d0", np.float64), ("rms", np.float64)])
+
+
+def _vg(v) -> _VGrid:
+    return _VGrid(v.x_min, v.x_max, v.y_min, v.y_max, v.n_x, v.n_y, v.V_min, 0)
+
+
+def vote_variant(grid, mode, x, y, layer):
+    """E1/E2: the vote under `mode` -> (acc[n_phi, n_d0, n_kappa], n_votes, n_bad)."""
+    x, y, layer = _hits(x, y, layer)
+    g = _g(grid)
+    acc = np.empty(grid.n_phi * grid.n_d0 * grid.n_kappa, np.uint32)
+    n_bad = C.c_uint32(0)
+    nv = lib().oracle_vote_variant(C.byref(g), C.c_int(mode), _p(x, C.c_float), _p(y, C.c_float),
+                                   _p(layer, C.c_int32), C.c_uint32(x.shape[0]), _p(acc, C.c_uint32),
+                                   C.byref(n_bad))
+    return acc.reshape(grid.n_phi, grid.n_d0, grid.n_kappa), int(nv), int(n_bad.value)
+
+
+def hitlists_variant(grid, mode, x, y, layer, peak_bin, cap_hits=None):
+    """A7 under `mode`: CSR (hit_offset, hit_index[min(total, cap)], true total)."""
+    x, y, layer = _hits(x, y, layer)
+    pb = np.ascontiguousarray(peak_bin, dtype=np.uint32)
+    g = _g(grid)
+    m = pb.shape[0]
+    off = np.zeros(m + 1, np.uint64)
+
+    def call(idx, cap):
+        return int(lib().oracle_hitlists_variant(
+            C.byref(g), C.c_int(mode), _p(x, C.c_float), _p(y, C.c_float), _p(layer, C.c_int32),
+            C.c_uint32(x.shape[0]), _p(pb, C.c_uint32), C.c_uint64(m), _p(off, C.c_uint64),
+            _p(idx, C.c_uint32), C.c_uint64(cap)))
+
+    if cap_hits is None:
+        cap_hits = call(np.empty(1, np.uint32), 0)
+    idx = np.empty(max(cap_hits, 1), np.uint32)
+    total = call(idx, cap_hits)
+    return off, idx[:min(total, cap_hits)].copy(), total
+
+
+def run_variant(grid, mode, x, y, layer, cap_peaks=None, cap_hits=None):
+    """Whole path under a vote variant (peak rule A6 unchanged)."""
+    acc, n_votes, n_bad = vote_variant(grid, mode, x, y, layer)
+    pb, pm, n_peaks = peaks(grid, acc, cap_peaks)
+    off, idx, n_ent = hitlists_variant(grid, mode, x, y, layer, pb, cap_hits)
+    return {"acc": acc, "n_votes": n_votes, "n_bad_hits": n_bad, "peak_bin": pb,
+            "peak_mask": pm, "n_peaks": n_peaks, "hit_offset": off, "hit_index": idx,
+            "n_hit_entries": n_ent}
+
+
+def vertex_tables(vgrid):
+    v = _vg(vgrid)
+    xc = np.empty(vgrid.n_x, np.float32)
+    yc = np.empty(vgrid.n_y, np.float32)
+    sc = np.empty(6, np.float32)
+    lib().oracle_vertex_tables(C.byref(v), _p(xc, C.c_float), _p(yc, C.c_float), _p(sc, C.c_float))
+    return xc, yc, sc
+
+
+def vertex_vote(grid, vgrid, peak_bin):
+    """E3 V2: (vacc uint32[n_x, n_y], votes cast)."""
+    pb = np.ascontiguousarray(peak_bin, dtype=np.uint32)
+    g, v = _g(grid), _vg(vgrid)
+    vacc = np.empty(vgrid.n_x * vgrid.n_y, np.uint32)
+    nv = lib().oracle_vertex_vote(C.byref(g), C.byref(v), _p(pb, C.c_uint32), C.c_uint64(pb.shape[0]),
+                                  _p(vacc, C.c_uint32))
+    return vacc.reshape(vgrid.n_x, vgrid.n_y), int(nv)
+
+
+def vertex_peaks(vgrid, vacc, cap=None):
+    """E3 V3: (vertex_bin[m], vertex_count[m], true n_vertices)."""
+    vacc = np.ascontiguousarray(vacc, dtype=np.uint32).reshape(-1)
+    v = _vg(vgrid)
+    if cap is None:
+        cap = vacc.shape[0]
+    vb = np.empty(max(cap, 1), np.uint32)
+    vc = np.empty(max(cap, 1), np.uint32)
+    n = int(lib().oracle_vertex_peaks(C.byref(v), _p(vacc, C.c_uint32), _p(vb, C.c_uint32),
+                                      _p(vc, C.c_uint32), C.c_uint64(cap)))
+    m = min(n, cap)
+    return vb[:m].copy(), vc[:m].copy(), n
+
+
+def vertex_members(grid, vgrid, peak_bin, vertex_bin, cap=None):
+    """E3 V4: CSR (member_offset[m+1], member_index[min(total, cap)], true total)."""
+    pb = np.ascontiguousarray(peak_bin, dtype=np.uint32)
+    vb = np.ascontiguousarray(vertex_bin, dtype=np.uint32)
+    g, v = _g(grid), _vg(vgrid)
+    off = np.zeros(vb.shape[0] + 1, np.uint64)
+
+    def call(idx, c):
+        return int(lib().oracle_vertex_members(
+            C.byref(g), C.byref(v), _p(pb, C.c_uint32), C.c_uint64(pb.shape[0]), _p(vb, C.c_uint32),
+            C.c_uint64(vb.shape[0]), _p(off, C.c_uint64), _p(idx, C.c_uint32), C.c_uint64(c)))
+
+    if cap is None:
+        cap = call(np.empty(1, np.uint32), 0)
+    idx = np.empty(max(cap, 1), np.uint32)
+    total = call(idx, cap)
+    return off, idx[:min(total, cap)].copy(), total
+
+
+def run_vertices(grid, vgrid, peak_bin, cap_vertices=None, cap_members=None):
+    vacc, nv = vertex_vote(grid, vgrid, peak_bin)
+    vb, vc, n = vertex_peaks(vgrid, vacc, cap_vertices)
+    off, idx, tot = vertex_members(grid, vgrid, peak_bin, vb, cap_members)
+    return {"vacc": vacc, "n_vertex_votes": nv, "vertex_bin": vb, "vertex_count": vc, "n_vertices": n,
+            "member_offset": off, "member_index": idx, "n_member_entries": tot}
+
+
+def fit_one(x, y, idx):
+    """E4 for one list of hit indices -> (status, kappa, phi0, d0, rms)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    idx = np.ascontiguousarray(idx, dtype=np.uint32)
+    f = _Fit()
+    st = lib().oracle_fit_one(_p(x, C.c_float), _p(y, C.c_float), _p(idx, C.c_uint32),
+                              C.c_uint32(idx.shape[0]), C.byref(f))
+    return int(st), f.kappa, f.phi0, f.d0, f.rms
+
+
+def fit_all(x, y, hit_offset, hit_index):
+    """E4 for every list of a CSR -> (fit structured array[n_peaks], status int32[n_peaks])."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    off = np.ascontiguousarray(hit_offset, dtype=np.uint64)
+    idx = np.ascontiguousarray(hit_index, dtype=np.uint32)
+    m = off.shape[0] - 1
+    fit = np.zeros(max(m, 1), FIT_DTYPE)
+    status = np.zeros(max(m, 1), np.int32)
+    if idx.shape[0] == 0:
+        idx = np.zeros(1, np.uint32)
+    lib().oracle_fit_all(_p(x, C.c_float), _p(y, C.c_float), _p(off, C.c_uint64), _p(idx, C.c_uint32),
+                         C.c_uint64(m), fit.ctypes.data_as(C.POINTER(_Fit)), _p(status, C.c_int32))
+    return fit[:m], status[:m]
+
+
+def select_dedup(hit_offset, hit_index, peak_mask, n_hits, fit, status, rms_max, min_shared):
+    """E5 -> flags uint8[n_peaks]: 0 not selected, 1 kept, 2 selected but a duplicate."""
+    off = np.ascontiguousarray(hit_offset, dtype=np.uint64)
+    idx = np.ascontiguousarray(hit_index, dtype=np.uint32)
+    pm = np.ascontiguousarray(peak_mask, dtype=np.uint32)
+    fit = np.ascontiguousarray(fit, dtype=FIT_DTYPE)
+    status = np.ascontiguousarray(status, dtype=np.int32)
+    m = off.shape[0] - 1
+    flags = np.zeros(max(m, 1), np.uint8)
+    if idx.shape[0] == 0:
+        idx = np.zeros(1, np.uint32)
+    lib().oracle_select_dedup(_p(off, C.c_uint64), _p(idx, C.c_uint32), _p(pm, C.c_uint32), C.c_uint64(m),
+                              C.c_uint32(n_hits), fit.ctypes.data_as(C.POINTER(_Fit)), _p(status, C.c_int32),
+                              C.c_double(rms_max), C.c_uint32(min_shared), flags.ctypes.data_as(C.POINTER(C.c_uint8)))
+    return flags[:m]
