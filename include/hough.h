@@ -236,6 +236,61 @@ int hough_peaks_only(hough_handle *h, const hough_peaks_out *out, void *cuda_str
 int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, int iters,
                           uint32_t *sink_dev, void *cuda_stream, uint64_t *lane_ops);
 
+/*
+ * ---- f1: the second Hough transform, over the peaks of the first (section 9:
+ * "the crossings all lie along a single sinusoidal curve in the parameter space ... that one
+ * sinusoidal curve corresponds to a point in the original x-y space ... the vertex of the
+ * displaced jet ... use the Hough transform a second time, this time applying it not to the hits
+ * in the x-y space but the crossings in the parameter space").  Recipe E3 of DESIGN.md section 8:
+ * a reported peak (i, j, k) is the point (phi0_i, d0_j) of the parameter space; the sinusoid of a
+ * vertex (xv, yv) is d0 = -xv sin(phi0) + yv cos(phi0), so the peak votes along the line it
+ * defines in the (xv, yv) plane, once per bin centre of the axis the line is less steep against
+ * (|cos phi0_i| >= |sin phi0_i|: every x centre a, yv = (d0_j + xc[a] sin)/cos; otherwise every y
+ * centre b, xv = (yc[b] cos - d0_j)/sin; binary32 round-to-nearest, unfused, in that order), adding 1
+ * to the uint32 count of bin (a, b), lin = a*n_y + b.  A bin is a vertex iff its count >= V_min
+ * and it beats its (up to 8) neighbours, ties to the lower lin (no wrap).  Every vertex is emitted
+ * in ascending lin with its count and the ascending list of the positions p (in the peak arrays)
+ * of the peaks whose own vote at the vertex's column (row for steep lines) lands in its bin.
+ */
+typedef struct hough_vertex_config {
+    double x_min, x_max;   /* x_max > x_min [cm] */
+    double y_min, y_max;   /* y_max > y_min */
+    int32_t n_x, n_y;      /* 1..2048 each */
+    int32_t V_min;         /* >= 1 */
+    uint32_t cap_vertices; /* capacity of the caller's vertex arrays (>= 1, <= 65536) */
+    uint64_t cap_members;  /* capacity of the caller's member_index array (>= 1) */
+} hough_vertex_config;
+
+typedef struct hough_vertex_counts { /* 32 bytes, same layout on host and device */
+    uint64_t n_vertex_votes;   /* votes cast into the (xv, yv) accumulator */
+    uint64_t n_member_entries; /* TRUE total length of the member lists of the reported vertices */
+    uint32_t n_vertices;       /* TRUE number of vertices (may exceed cap_vertices) */
+    uint32_t flags;            /* 1: vertices truncated, 2: member lists truncated (first cap_* kept, in order) */
+    uint64_t reserved;
+} hough_vertex_counts;
+
+typedef struct hough_vertex_out { /* all [device], caller-owned */
+    uint32_t *bin;            /* cap_vertices: lin = a*n_y + b */
+    uint32_t *count;          /* cap_vertices */
+    uint64_t *member_offset;  /* cap_vertices + 1 */
+    uint32_t *member_index;   /* cap_members: positions in the peak arrays */
+    hough_vertex_counts *counts;
+} hough_vertex_out;
+
+/* Bytes of [device] scratch hough_vertices needs (0 if vc is invalid).  Its first n_x*n_y uint32
+ * words are the (xv, yv) accumulator, lin order, valid after the call's work has completed. */
+size_t hough_vertex_workspace_bytes(const hough_vertex_config *vc);
+
+/*
+ * Enqueue the second transform over the peaks in `peaks` (the arrays hough_peaks filled for this
+ * handle's grid: only bin[] and counts->n_peaks are read, on the device, so no host
+ * synchronisation is needed between hough_peaks and this call).  `workspace`: [device], 256-byte
+ * aligned, >= hough_vertex_workspace_bytes(vc), caller-owned, used only during the call's work.
+ * Errors: HOUGH_EINVAL (NULL / bad vc), HOUGH_ENOMEM (workspace too small), HOUGH_ECUDA.
+ */
+int hough_vertices(hough_handle *h, const hough_vertex_config *vc, void *workspace, size_t workspace_bytes,
+                   const hough_peaks_out *peaks, const hough_vertex_out *out, void *cuda_stream);
+
 /* Geometry the library chose (for reporting): tile_phi, tile_d0, n_tiles, threads per CTA,
  * dynamic shared memory bytes of the vote kernel, number of SMs.  Any pointer may be NULL. */
 int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,

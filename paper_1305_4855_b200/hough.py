@@ -30,7 +30,8 @@ N_STAGES = 9
 SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
            "hough_accumulator", "hough_process_host", "hough_submit_host", "hough_collect_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
-           "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror")
+           "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror",
+           "hough_vertex_workspace_bytes", "hough_vertices")
 
 
 class HoughError(RuntimeError):
@@ -64,6 +65,20 @@ class HostOut(C.Structure):
     _fields_ = [("bin", C.c_void_p), ("mask", C.c_void_p), ("hit_offset", C.c_void_p),
                 ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
 
+
+class VertexConfig(C.Structure):
+    _fields_ = [("x_min", C.c_double), ("x_max", C.c_double), ("y_min", C.c_double), ("y_max", C.c_double),
+                ("n_x", C.c_int32), ("n_y", C.c_int32), ("V_min", C.c_int32), ("cap_vertices", C.c_uint32),
+                ("cap_members", C.c_uint64)]
+
+
+class VertexOut(C.Structure):
+    _fields_ = [("bin", C.c_void_p), ("count", C.c_void_p), ("member_offset", C.c_void_p),
+                ("member_index", C.c_void_p), ("counts", C.c_void_p)]
+
+
+VERTEX_COUNTS_DTYPE = np.dtype([("n_vertex_votes", "<u8"), ("n_member_entries", "<u8"), ("n_vertices", "<u4"),
+                                ("flags", "<u4"), ("reserved", "<u8")])
 
 COUNTS_DTYPE = np.dtype([("n_votes", "<u8"), ("n_hit_entries", "<u8"), ("n_evals", "<u8"),
                          ("n_list_evals", "<u8"), ("n_peaks", "<u4"), ("n_bad_hits", "<u4"), ("flags", "<u4"),
@@ -119,6 +134,11 @@ def _load():
     lib.hough_stage_name.argtypes = [C.c_int]
     lib.hough_strerror.restype = C.c_char_p
     lib.hough_strerror.argtypes = [C.c_int]
+    lib.hough_vertex_workspace_bytes.restype = C.c_size_t
+    lib.hough_vertex_workspace_bytes.argtypes = [C.POINTER(VertexConfig)]
+    lib.hough_vertices.restype = C.c_int
+    lib.hough_vertices.argtypes = [C.c_void_p, C.POINTER(VertexConfig), C.c_void_p, C.c_size_t,
+                                   C.POINTER(PeaksOut), C.POINTER(VertexOut), C.c_void_p]
     return lib
 
 
@@ -307,6 +327,47 @@ class Hough:
         cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
         return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
                           hb["hit_index"].numpy())
+
+    # -- f1: the second transform over the peaks (hough_vertices)
+    def vertices(self, vgrid, cap_vertices=1024, cap_members=1 << 20, stream=None):
+        """hough_vertices on the peaks of the last ``peaks`` call (device arrays of this object);
+        ``vgrid`` has the synth.VertexGrid attributes.  Enqueues only; see ``read_vertices``."""
+        key = (vgrid, int(cap_vertices), int(cap_members))
+        if getattr(self, "_vx_key", None) != key:
+            vc = VertexConfig(vgrid.x_min, vgrid.x_max, vgrid.y_min, vgrid.y_max, vgrid.n_x, vgrid.n_y,
+                              vgrid.V_min, int(cap_vertices), int(cap_members))
+            nbytes = int(_lib.hough_vertex_workspace_bytes(C.byref(vc)))
+            if nbytes == 0:
+                raise HoughError("hough_vertex_workspace_bytes: invalid configuration")
+            i32 = dict(dtype=torch.int32, device=self.device)
+            self._vx = dict(cfg=vc, nbytes=nbytes, ws=torch.empty(nbytes, dtype=torch.uint8, device=self.device),
+                            bin=torch.empty(cap_vertices, **i32), count=torch.empty(cap_vertices, **i32),
+                            member_offset=torch.empty(cap_vertices + 1, dtype=torch.int64, device=self.device),
+                            member_index=torch.empty(cap_members, **i32),
+                            counts=torch.zeros(VERTEX_COUNTS_DTYPE.itemsize // 8, dtype=torch.int64, device=self.device))
+            v = self._vx
+            v["out"] = VertexOut(v["bin"].data_ptr(), v["count"].data_ptr(), v["member_offset"].data_ptr(),
+                                 v["member_index"].data_ptr(), v["counts"].data_ptr())
+            self._vx_key = key
+        v = self._vx
+        _check(_lib.hough_vertices(self._h, C.byref(v["cfg"]), C.c_void_p(v["ws"].data_ptr()), v["nbytes"],
+                                   C.byref(self._out), C.byref(v["out"]), _stream_ptr(stream)), "hough_vertices")
+
+    def read_vertices(self):
+        """Synchronise and copy the results of the last ``vertices`` call to the host."""
+        torch.cuda.synchronize(self.device)
+        v = self._vx
+        vc = v["cfg"]
+        cnt = v["counts"].cpu().numpy().view(VERTEX_COUNTS_DTYPE)[0]
+        n_rep = min(int(cnt["n_vertices"]), int(vc.cap_vertices))
+        n_mem = min(int(cnt["n_member_entries"]), int(vc.cap_members))
+        return {"vacc": v["ws"][:4 * vc.n_x * vc.n_y].view(torch.int32).cpu().numpy().view(np.uint32).reshape(vc.n_x, vc.n_y),
+                "n_vertex_votes": int(cnt["n_vertex_votes"]), "n_vertices": int(cnt["n_vertices"]),
+                "n_member_entries": int(cnt["n_member_entries"]), "flags": int(cnt["flags"]),
+                "vertex_bin": v["bin"][:n_rep].cpu().numpy().view(np.uint32),
+                "vertex_count": v["count"][:n_rep].cpu().numpy().view(np.uint32),
+                "member_offset": v["member_offset"][:n_rep + 1].cpu().numpy().view(np.uint64),
+                "member_index": v["member_index"][:n_mem].cpu().numpy().view(np.uint32)}
 
     # -- results
     def _pack(self, cnt, b, m, off, idx):

@@ -1,0 +1,139 @@
+"""GPU parity of the rows SURVEY.md 8(f) marks "next" (f1 vertices, f2 fit + duplicates, f3 vote
+variants) against oracle/hough_ext_oracle.c, through the C ABI (include/hough.h).
+
+Index and integer results are compared bit for bit; the binary64 fit within the tolerance
+DESIGN.md section 8 derives (different libm / CUDA math library sin, cos, atan2: a few ulp,
+amplified by the cancellation in the transverse moment).
+"""
+import dataclasses
+import math
+
+import numpy as np
+import pytest
+
+from paper_1305_4855_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def hough():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1305_4855_b200 import hough as hough_mod
+    return hough_mod
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def random_hits(rng, n, n_layers=10, rmax=80.0):
+    r = rng.uniform(0.5, rmax, n)
+    phi = rng.uniform(-math.pi, math.pi, n)
+    return ((r * np.cos(phi)).astype(np.float32), (r * np.sin(phi)).astype(np.float32),
+            rng.integers(0, n_layers, n).astype(np.int32))
+
+
+def make(hough, grid, x, y, layer, cap_peaks, cap_hits, **kw):
+    h = hough.Hough(grid, max_hits=max(len(x), 1), cap_peaks=cap_peaks, cap_hits=cap_hits, **kw)
+    h.vote(dev(x.astype(np.float32)), dev(y.astype(np.float32)), dev(layer.astype(np.int32)))
+    h.peaks()
+    return h
+
+
+# ============================================================ f1: hough_vertices
+
+def assert_vertices_same(res, ref):
+    assert np.array_equal(res["vacc"], ref["vacc"])
+    assert res["n_vertex_votes"] == ref["n_vertex_votes"]
+    assert res["n_vertices"] == ref["n_vertices"]
+    assert np.array_equal(res["vertex_bin"], ref["vertex_bin"])
+    assert np.array_equal(res["vertex_count"], ref["vertex_count"])
+    assert res["n_member_entries"] == ref["n_member_entries"]
+    assert np.array_equal(res["member_offset"], ref["member_offset"])
+    assert np.array_equal(res["member_index"], ref["member_index"])
+
+
+@pytest.mark.parametrize("shape,vshape,n_hits,seed", [
+    ((64, 16, 32), (20, 12), 300, 0),      # accumulator copy in shared memory, non-square
+    ((50, 13, 64), (1, 37), 400, 1),       # a single column
+    ((96, 8, 32), (130, 100), 500, 2),     # 13 000 bins: global atomics
+    ((33, 9, 32), (257, 3), 200, 3),       # ragged blocks
+])
+def test_vertices_random_small(hough, oracle, shape, vshape, n_hits, seed):
+    rng = np.random.default_rng(seed)
+    g = synth.Grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=2)
+    vg = synth.VertexGrid(n_x=vshape[0], n_y=vshape[1], V_min=3, x_min=-5.0, x_max=7.0, y_min=-4.0, y_max=2.5)
+    x, y, layer = random_hits(rng, n_hits)
+    ref = oracle.run(g, x, y, layer)
+    assert ref["n_peaks"] > 20
+    h = make(hough, g, x, y, layer, 1 << 16, 1 << 20)
+    res = h.read()
+    assert np.array_equal(res["peak_bin"], ref["peak_bin"])
+    vref = oracle.run_vertices(g, vg, ref["peak_bin"])
+    assert vref["n_vertices"] > 0
+    for rep in range(2):  # the call is repeatable on the same handle
+        h.vertices(vg, cap_vertices=4096, cap_members=1 << 20)
+        assert_vertices_same(h.read_vertices(), vref)
+    h.close()
+
+
+def test_vertices_jets_workload(hough, oracle):
+    """The displaced-jet workload (PAPER.md:154 Fig. 7, :168 Fig. 8 in synthetic form)."""
+    g, vg = synth.JETS_GRID, synth.JETS_VGRID
+    for seed in (0, 1):
+        x, y, layer, truth = synth.generate_jet_event(synth.JETS_SPEC, seed)
+        ref = oracle.run(g, x, y, layer)
+        vref = oracle.run_vertices(g, vg, ref["peak_bin"])
+        h = make(hough, g, x, y, layer, 1 << 16, 1 << 20)
+        h.vertices(vg)
+        assert_vertices_same(h.read_vertices(), vref)
+        h.close()
+
+
+def test_vertices_truncation_and_no_peaks(hough, oracle):
+    rng = np.random.default_rng(5)
+    g = synth.Grid(n_phi=64, n_d0=16, n_kappa=32, L_min=2)
+    vg = synth.VertexGrid(n_x=24, n_y=24, V_min=2)
+    x, y, layer = random_hits(rng, 300)
+    ref = oracle.run(g, x, y, layer)
+    full = oracle.run_vertices(g, vg, ref["peak_bin"])
+    assert full["n_vertices"] > 6 and full["n_member_entries"] > 40
+    h = make(hough, g, x, y, layer, 1 << 16, 1 << 20)
+    # vertex capacity smaller than the number of vertices: the first ones in lin order, with their lists
+    cut = oracle.run_vertices(g, vg, ref["peak_bin"], cap_vertices=5)
+    h.vertices(vg, cap_vertices=5, cap_members=1 << 16)
+    res = h.read_vertices()
+    assert res["flags"] & 1 and res["n_vertices"] == full["n_vertices"]
+    assert np.array_equal(res["vertex_bin"], cut["vertex_bin"]) and np.array_equal(res["member_index"], cut["member_index"])
+    assert np.array_equal(res["member_offset"], cut["member_offset"])
+    # member capacity smaller than the total: true total reported, the first entries written
+    h.vertices(vg, cap_vertices=4096, cap_members=17)
+    res = h.read_vertices()
+    assert res["flags"] & 2 and res["n_member_entries"] == full["n_member_entries"]
+    assert np.array_equal(res["member_index"], full["member_index"][:17])
+    assert np.array_equal(res["member_offset"], full["member_offset"])
+    h.close()
+    # an event without peaks: an all-zero accumulator, no vertex, member_offset[0] = 0
+    g9 = dataclasses.replace(g, L_min=9)
+    h = make(hough, g9, x[:5], y[:5], layer[:5], 1 << 10, 1 << 12)
+    assert h.read()["n_peaks"] == 0
+    h.vertices(vg)
+    res = h.read_vertices()
+    assert res["n_vertices"] == 0 and res["n_vertex_votes"] == 0 and not res["vacc"].any()
+    assert res["member_offset"].tolist() == [0]
+    h.close()
+
+
+def test_vertices_rejects_bad_arguments(hough):
+    g = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=2)
+    x, y, layer = random_hits(np.random.default_rng(0), 50)
+    h = make(hough, g, x, y, layer, 1 << 10, 1 << 12)
+    for bad in (synth.VertexGrid(n_x=0, n_y=4, V_min=1), synth.VertexGrid(n_x=4, n_y=4, V_min=0),
+                synth.VertexGrid(n_x=4, n_y=4, V_min=1, x_min=1.0, x_max=1.0), synth.VertexGrid(n_x=4096, n_y=4, V_min=1)):
+        with pytest.raises(hough.HoughError):
+            h.vertices(bad)
+    h.close()
