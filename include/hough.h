@@ -66,6 +66,12 @@ extern "C" {
                                      exact fallback near bin edges; results are identical either way) */
 #define HOUGH_OPT_LIST_SWEEP 16u  /* hit lists by a second sweep of all hits over all cells (the round-1 path)
                                      instead of the peak-driven lists; results are identical either way */
+#define HOUGH_OPT_LINE 32u        /* f3, straight-line transform (Fig. 3; recipe E1):
+                                     the phi axis is the line's direction theta, n_d0 must be 1 and the kappa axis
+                                     is rho [cm]; a hit votes rho = -x sin(theta_i) + y cos(theta_i) */
+#define HOUGH_OPT_INTERVAL 64u    /* f3, interval voting (recipe E2): a hit sets every kappa bin
+                                     between its closed-form values at the two EDGES of phi0 bin i (d0 centre j);
+                                     n_votes counts the bins set.  Not together with HOUGH_OPT_LINE */
 #define HOUGH_OPT_UNPACKED 4u     /* one mask per 32-bit word of the vote tile even with <= 16 layers (test hook
                                      for the tile layout used with 17..32 layers) */
 

@@ -157,6 +157,10 @@ static int cfg_valid(const hough_config *c)
         return 0;
     if (!list_config_ok(c))
         return 0; // max_hits beyond what the hit-list segmentation supports
+    if ((c->options & HOUGH_OPT_LINE) && (c->options & HOUGH_OPT_INTERVAL))
+        return 0;
+    if ((c->options & HOUGH_OPT_LINE) && c->n_d0 != 1)
+        return 0; // the straight-line transform has two parameters (theta, rho)
     return 1;
 }
 
@@ -210,6 +214,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         NA <<= 1;
     const int n_keys = (c->n_layers + 1) * NA;
     void *t_phic = cv.take((size_t)c->n_phi * 4);
+    void *t_sne = cv.take((size_t)(c->n_phi + 1) * 4), *t_cse = cv.take((size_t)(c->n_phi + 1) * 4);
     void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 33 * 4); // histogram | per-layer radius range (one memset)
     void *ix_start = cv.take((size_t)(n_keys + 1) * 4);
     void *ix_key = cv.take((size_t)hp * 4);
@@ -240,6 +245,8 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ent_hit = (uint32_t *)ent_hit;
         h->ent_idx = (uint32_t *)ent_idx;
         h->t_phic = (float *)t_phic;
+        h->t_sne = (float *)t_sne;
+        h->t_cse = (float *)t_cse;
         h->ix.NA = NA;
         h->ix.n_keys = n_keys;
         h->ix.bin_cnt = (uint32_t *)ix_cnt;
@@ -436,6 +443,14 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
         cs[i] = (float)cos(phic);
         phf[i] = (float)remainder(phic, 6.283185307179586); // the angle itself, in [-pi, pi] (azimuth windows)
     }
+    // E2 (interval voting): the phi0 bin EDGES, the same way
+    float *sne = (float *)malloc(sizeof(float) * (np + 1)), *cse = (float *)malloc(sizeof(float) * (np + 1));
+    for (int i = 0; i <= np; ++i) {
+        double pe = cfg->phi_min + (double)i * (cfg->phi_max - cfg->phi_min) / (double)np;
+        sne[i] = (float)sin(pe);
+        cse[i] = (float)cos(pe);
+    }
+    h->mode = (cfg->options & HOUGH_OPT_LINE) ? VOTE_LINE : (cfg->options & HOUGH_OPT_INTERVAL) ? VOTE_INTERVAL : VOTE_CENTRE;
     float d0abs = 0.f;
     for (int j = 0; j < nd; ++j) {
         volatile float c0 = (float)(cfg->d0_min + ((double)j + 0.5) * (cfg->d0_max - cfg->d0_min) / (double)nd);
@@ -461,11 +476,19 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     g.d0_absmax = d0abs;
     g.sn = h->t_sn;
     g.cs = h->t_cs;
+    g.sne = h->t_sne;
+    g.cse = h->t_cse;
     g.d0c = h->t_d0c;
     g.twod0 = h->t_twod0;
     g.d0sq = h->t_d0sq;
     approx_bin_init(h, d0c, nd);
+    if (h->mode != VOTE_CENTRE)
+        h->ab.ok = 0; // the variants evaluate the exact recipe only
     int ok = 1;
+    ok &= cudaMemcpy(h->t_sne, sne, sizeof(float) * (np + 1), cudaMemcpyHostToDevice) == cudaSuccess;
+    ok &= cudaMemcpy(h->t_cse, cse, sizeof(float) * (np + 1), cudaMemcpyHostToDevice) == cudaSuccess;
+    free(sne);
+    free(cse);
     ok &= cudaMemcpy(h->t_sn, sn, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_cs, cs, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_phic, phf, sizeof(float) * np, cudaMemcpyHostToDevice) == cudaSuccess;
@@ -536,7 +559,7 @@ int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *l
     stage_mark(h, 0, st);
     CK(cudaMemsetAsync(h->counters, 0, 64, st));
     CK(launch_prep(h, x, y, layer, n, st));
-    if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP))
+    if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE)
         CK(launch_index_build(h, st));
     stage_mark(h, ST_PREP + 1, st);
     CK(launch_vote(h, st));
@@ -562,8 +585,10 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
     if (with_lists) {
-        const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) ? 1 : 0;
-        CK(sweep ? launch_list_sweep(h, st) : launch_peak_lists(h, out, st));
+        // the vote variants (f3) take the generic lists: one warp per peak over all hits
+        const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE ? 1 : 0;
+        CK(h->mode != VOTE_CENTRE ? launch_lists_generic(h, out, st)
+                                  : sweep ? launch_list_sweep(h, st) : launch_peak_lists(h, out, st));
         stage_mark(h, ST_LIST_SWEEP + 1, st);
         CK(launch_scan_lens(h, out, st));
         stage_mark(h, ST_SCAN_LENS + 1, st);

@@ -68,6 +68,56 @@ __device__ __forceinline__ int kappa_bin(float kappa, float klo, float inv_dk, i
     float qf = __fmul_rn(__fsub_rn(kappa, klo), inv_dk);
     return min(__float2int_rz(qf), nk_minus_1);
 }
+// ------------------------------------------------------------------ vote variants (f3)
+// SURVEY.md section 8(f) f3; recipes E1 / E2 of DESIGN.md section 8.  MODE 0: the closed form at
+// the bin centres (one bin).  MODE 1: straight-line transform, the binned quantity is
+// rho = y cos(theta) - x sin(theta) (Fig. 3).  MODE 2: interval voting, every bin
+// between the closed-form values at the two phi0 bin EDGES (snB / csB = the upper edge).
+struct CellConst {
+    float sn, cs;   // bin centre (MODE 0, 1) or lower edge (MODE 2)
+    float snB, csB; // upper edge (MODE 2)
+    float d0c, twod0, d0sq;
+};
+// bins [k0, k1] that the hit votes into at this cell; false: no vote
+template <int MODE>
+__device__ __forceinline__ bool variant_bins(float x, float y, float r2, const CellConst &c, float klo, float khi,
+                                             float inv_dk, int nkm1, int &k0, int &k1)
+{
+    if (MODE == VOTE_INTERVAL) {
+        const float ka = eval_kappa(x, y, r2, c.sn, c.cs, c.d0c, c.twod0, c.d0sq);
+        const float kb = eval_kappa(x, y, r2, c.snB, c.csB, c.d0c, c.twod0, c.d0sq);
+        if (ka != ka || kb != kb)
+            return false;
+        const float lo = ka < kb ? ka : kb, hi = ka < kb ? kb : ka;
+        if (hi < klo || lo >= khi)
+            return false;
+        k0 = (lo < klo) ? 0 : kappa_bin(lo, klo, inv_dk, nkm1);
+        k1 = (hi >= khi) ? nkm1 : kappa_bin(hi, klo, inv_dk, nkm1);
+        return true;
+    }
+    float v;
+    if (MODE == VOTE_LINE)
+        v = __fsub_rn(__fmul_rn(y, c.cs), __fmul_rn(x, c.sn));
+    else
+        v = eval_kappa(x, y, r2, c.sn, c.cs, c.d0c, c.twod0, c.d0sq);
+    if (!((v >= klo) && (v < khi)))
+        return false;
+    k0 = k1 = kappa_bin(v, klo, inv_dk, nkm1);
+    return true;
+}
+__device__ __forceinline__ CellConst cell_const(const GridDev &g, int mode, int i, int j)
+{
+    CellConst c;
+    c.sn = mode == VOTE_INTERVAL ? g.sne[i] : g.sn[i];
+    c.cs = mode == VOTE_INTERVAL ? g.cse[i] : g.cs[i];
+    c.snB = mode == VOTE_INTERVAL ? g.sne[i + 1] : 0.f;
+    c.csB = mode == VOTE_INTERVAL ? g.cse[i + 1] : 0.f;
+    c.d0c = g.d0c[j];
+    c.twod0 = g.twod0[j];
+    c.d0sq = g.d0sq[j];
+    return c;
+}
+
 // ------------------------------------------------------------------ the fast bin path
 // The exact recipe costs ~14 issue slots for the IEEE divide, the two range compares and the
 // bin.  The sweeps only need the BIN, so they first compute a 16.16 fixed-point estimate

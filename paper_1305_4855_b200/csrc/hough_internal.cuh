@@ -43,6 +43,11 @@ struct ListGeom {
     int no_phi_cull_tile, no_phi_cull_sub;
 };
 
+// vote variants (hough_handle::mode; hough_device.cuh variant_bins)
+#define VOTE_CENTRE 0
+#define VOTE_LINE 1
+#define VOTE_INTERVAL 2
+
 // Device-side constant block handed to every kernel by value.
 struct GridDev {
     int n_phi, n_d0, n_kappa;
@@ -52,6 +57,7 @@ struct GridDev {
     float kabs;          // max(|klo|, |khi|)
     float d0_absmax;     // max |d0 centre|
     const float *sn, *cs;            // [n_phi]
+    const float *sne, *cse;          // [n_phi + 1] sin / cos of the phi0 bin EDGES (interval voting)
     const float *d0c, *twod0, *d0sq; // [n_d0]
 };
 
@@ -113,7 +119,8 @@ struct hough_handle {
     ListGeom list_geom;
     // workspace carve-up (device)
     uint32_t *acc;
-    float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq, *t_phic;
+    float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq, *t_phic, *t_sne, *t_cse;
+    int mode;            // vote variant: 0 closed form at bin centres, 1 straight line, 2 interval (hough_device.cuh)
     HitIndexDev ix;
     float *hx, *hy, *hr2;
     uint32_t *hbit;
@@ -166,6 +173,7 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_index_build(hough_handle *h, cudaStream_t st);
 cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st);

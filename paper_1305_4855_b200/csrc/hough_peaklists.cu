@@ -460,6 +460,7 @@ struct ListCopyParams {
 
 // hit_index[hit_offset[p] ..] = the staged list of peak p (half a warp per peak); a peak without
 // a staged list (PL_SLOW) is written straight from the hits in index order by a whole warp.
+template <int MODE>
 __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
 {
     const GridDev &g = p.g;
@@ -492,14 +493,15 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
             const uint32_t lin = p.bin[spk];
             const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
             const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
-            const float sn = g.sn[i], cs = g.cs[i], d0c = g.d0c[j], twod0 = g.twod0[j], d0sq = g.d0sq[j];
+            const CellConst cc = cell_const(g, MODE, (int)i, (int)j);
             for (uint32_t base = 0; base < p.n_hits; base += 32) {
                 const uint32_t hidx = base + lane;
                 bool in = false;
                 if (hidx < p.n_hits && p.hbit[hidx] != 0u) {
-                    const float kappa = eval_kappa(p.hx[hidx], p.hy[hidx], p.hr2[hidx], sn, cs, d0c, twod0, d0sq);
-                    if ((kappa >= g.klo) && (kappa < g.khi))
-                        in = (uint32_t)kappa_bin(kappa, g.klo, g.inv_dk, g.n_kappa - 1) == k;
+                    int k0, k1;
+                    if (variant_bins<MODE>(p.hx[hidx], p.hy[hidx], p.hr2[hidx], cc, g.klo, g.khi, g.inv_dk,
+                                           g.n_kappa - 1, k0, k1))
+                        in = (uint32_t)k0 <= k && k <= (uint32_t)k1;
                 }
                 const unsigned bal = __ballot_sync(0xffffffffu, in);
                 if (in) {
@@ -563,7 +565,74 @@ cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
     p.hit_index = out->hit_index;
     p.cap_hits = h->cfg.cap_hits;
-    k_copy_lists<<<h->n_sms * 16, 256, 0, st>>>(p);
+    if (h->mode == VOTE_LINE)
+        k_copy_lists<VOTE_LINE><<<h->n_sms * 16, 256, 0, st>>>(p);
+    else if (h->mode == VOTE_INTERVAL)
+        k_copy_lists<VOTE_INTERVAL><<<h->n_sms * 16, 256, 0, st>>>(p);
+    else
+        k_copy_lists<VOTE_CENTRE><<<h->n_sms * 16, 256, 0, st>>>(p);
+    h->launches += 1;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ generic lists (vote variants, f3)
+// One warp per reported peak counts, over all hits, those whose vote at the peak's cell covers
+// the peak's bin; every list is then written by k_copy_lists' whole-warp path (PL_SLOW).
+template <int MODE>
+__global__ void __launch_bounds__(256) k_list_count(const ListCopyParams p, uint32_t *peak_len, uint32_t *peak_pos,
+                                                    unsigned long long *n_list_evals)
+{
+    const GridDev &g = p.g;
+    const int lane = threadIdx.x & 31;
+    const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
+        const uint32_t lin = p.bin[pk];
+        const uint32_t k = lin % (uint32_t)g.n_kappa, row = lin / (uint32_t)g.n_kappa;
+        const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
+        const CellConst cc = cell_const(g, MODE, (int)i, (int)j);
+        uint32_t cnt = 0;
+        for (uint32_t hidx = lane; hidx < p.n_hits; hidx += 32) {
+            int k0, k1;
+            if (p.hbit[hidx] != 0u && variant_bins<MODE>(p.hx[hidx], p.hy[hidx], p.hr2[hidx], cc, g.klo, g.khi,
+                                                         g.inv_dk, g.n_kappa - 1, k0, k1))
+                cnt += ((uint32_t)k0 <= k && k <= (uint32_t)k1) ? 1u : 0u;
+        }
+        for (int o = 16; o > 0; o >>= 1)
+            cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        if (lane == 0) {
+            peak_len[pk] = cnt;
+            peak_pos[pk] = PL_SLOW;
+            atomicAdd(n_list_evals, (unsigned long long)p.n_hits);
+        }
+    }
+}
+
+cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    if (h->n_hits == 0)
+        return cudaMemsetAsync(h->peak_len, 0, (size_t)h->cfg.cap_peaks * 4, st);
+    ListCopyParams p;
+    p.g = h->g;
+    p.hx = h->hx;
+    p.hy = h->hy;
+    p.hr2 = h->hr2;
+    p.hbit = h->hbit;
+    p.n_hits = h->n_hits;
+    p.counters = h->counters;
+    p.cap_peaks = h->cfg.cap_peaks;
+    p.bin = out->bin;
+    p.peak_len = p.peak_pos = p.ent_hit = nullptr;
+    p.hit_offset = nullptr;
+    p.hit_index = nullptr;
+    p.cap_hits = 0;
+    unsigned long long *ev = &h->counters->n_list_evals;
+    if (h->mode == VOTE_LINE)
+        k_list_count<VOTE_LINE><<<h->n_sms * 16, 256, 0, st>>>(p, h->peak_len, h->list_len, ev);
+    else if (h->mode == VOTE_INTERVAL)
+        k_list_count<VOTE_INTERVAL><<<h->n_sms * 16, 256, 0, st>>>(p, h->peak_len, h->list_len, ev);
+    else
+        k_list_count<VOTE_CENTRE><<<h->n_sms * 16, 256, 0, st>>>(p, h->peak_len, h->list_len, ev);
     h->launches += 1;
     return cudaGetLastError();
 }

@@ -478,7 +478,7 @@ __global__ void __launch_bounds__(256) k_sub_prefix(uint32_t *sub_len, uint32_t 
 
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
 {
-    if (h->cfg.options & HOUGH_OPT_LIST_SWEEP) { // the sweep's sub-lists -> list lengths (peak-driven lists write them directly)
+    if ((h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == 0) { // the sweep's sub-lists -> list lengths (peak-driven lists write them directly)
         const uint32_t S = (uint32_t)h->list_geom.S;
         k_sub_prefix<<<(h->cfg.cap_peaks + 255) / 256, 256, 256 * (S + 1) * 4, st>>>(
             h->list_len, h->peak_len, h->counters, h->cfg.cap_peaks, S);

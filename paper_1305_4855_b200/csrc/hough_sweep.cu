@@ -24,7 +24,8 @@ struct SweepParams {
 // APPROX: bins come from the fixed-point estimate wherever it provably equals the exact
 // recipe (hough_device.cuh approx_bin); near a bin edge, and for hits whose
 // r^2 is outside the estimate's admissible range, the exact recipe runs.
-template <int PACK, bool APPROX>
+// MODE (with APPROX = false only): the vote variant, hough_device.cuh variant_bins.
+template <int PACK, bool APPROX, int MODE>
 __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -62,12 +63,16 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const int il = c / ge.D, jl = c - il * ge.D;
     const bool cell_ok = (il < ni) && (jl < nj);
     float c_sn = 0.f, c_cs = 0.f, c_d0 = 0.f, c_2d0 = 0.f, c_d0sq = __int_as_float(0x7fc00000);
+    CellConst cc; // the same for the variants (MODE != 0); a padding lane's NaN never votes
+    cc.sn = cc.cs = cc.snB = cc.csB = cc.d0c = cc.twod0 = cc.d0sq = __int_as_float(0x7fc00000);
     if (cell_ok) {
         c_sn = g.sn[i0 + il];
         c_cs = g.cs[i0 + il];
         c_d0 = g.d0c[j0 + jl];
         c_2d0 = g.twod0[j0 + jl];
         c_d0sq = g.d0sq[j0 + jl];
+        if (MODE != VOTE_CENTRE)
+            cc = cell_const(g, MODE, i0 + il, j0 + jl);
     }
     const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
 
@@ -180,9 +185,16 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             ++my_votes;
         };
         auto exact = [&](const float4 hv) {
-            const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-            if ((kappa >= klo) && (kappa < khi))
-                cast((uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1), __float_as_uint(hv.w));
+            if (MODE == VOTE_CENTRE) {
+                const float kappa = eval_kappa(hv.x, hv.y, hv.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+                if ((kappa >= klo) && (kappa < khi))
+                    cast((uint32_t)kappa_bin(kappa, klo, inv_dk, nkm1), __float_as_uint(hv.w));
+            } else {
+                int k0, k1;
+                if (__float_as_uint(hv.w) != 0u && variant_bins<MODE>(hv.x, hv.y, hv.z, cc, klo, khi, inv_dk, nkm1, k0, k1))
+                    for (int k = k0; k <= k1; ++k)
+                        cast((uint32_t)k, __float_as_uint(hv.w));
+            }
         };
         // the estimate of one (hit, cell): e and den are the exact binary32 values of the recipe (A3)
         auto estimate = [&](const float4 hv, float &e, float &den) -> uint32_t {
@@ -293,6 +305,20 @@ static int swizzle_mask_for(int row_words)
     return m;
 }
 
+template <int PACK>
+static const void *sweep_kernel_pack(const hough_handle *h)
+{
+    if (h->mode == VOTE_LINE)
+        return (const void *)k_sweep<PACK, false, VOTE_LINE>;
+    if (h->mode == VOTE_INTERVAL)
+        return (const void *)k_sweep<PACK, false, VOTE_INTERVAL>;
+    return h->ab.ok ? (const void *)k_sweep<PACK, true, VOTE_CENTRE> : (const void *)k_sweep<PACK, false, VOTE_CENTRE>;
+}
+static const void *sweep_kernel(const hough_handle *h)
+{
+    return h->g.pack == 2 ? sweep_kernel_pack<2>(h) : sweep_kernel_pack<1>(h);
+}
+
 // Tile geometry: P x D rows of n_kappa masks, PACK masks per word, plus the staging.
 int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int split, int fit_waves)
 {
@@ -327,8 +353,7 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     const int step = (D <= 32 && 32 % D == 0) ? 32 / D : 0;
     if (fit_waves && step > 0 && P % step == 0 && P - step >= step) {
         int per_sm = 0;
-        const void *fn = h->g.pack == 2 ? (h->ab.ok ? (const void *)k_sweep<2, true> : (const void *)k_sweep<2, false>)
-                                        : (h->ab.ok ? (const void *)k_sweep<1, true> : (const void *)k_sweep<1, false>);
+        const void *fn = sweep_kernel(h);
         cudaError_t e = ensure_dynamic_smem(fn, ge->smem_bytes);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ge->threads, ge->smem_bytes);
@@ -374,21 +399,11 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->geom = ge;
     int row_words = h->g.pack == 2 ? h->g.n_kappa / 2 : h->g.n_kappa;
     p->swz_mask = swizzle_mask_for(row_words);
-    p->no_cull = (h->cfg.options & HOUGH_OPT_NO_CULL) ? 1 : 0;
+    p->no_cull = ((h->cfg.options & HOUGH_OPT_NO_CULL) || h->mode != VOTE_CENTRE) ? 1 : 0;
     p->acc = h->acc;
     p->n_votes = &h->counters->n_votes;
     p->n_evals = &h->counters->n_evals;
     p->ab = h->ab;
-}
-
-template <int PACK, bool APPROX>
-static cudaError_t launch_one(const SweepParams &p, cudaStream_t st)
-{
-    cudaError_t e = ensure_dynamic_smem((const void *)k_sweep<PACK, APPROX>, p.geom.smem_bytes);
-    if (e != cudaSuccess)
-        return e;
-    k_sweep<PACK, APPROX><<<p.geom.n_tiles, p.geom.threads, p.geom.smem_bytes, st>>>(p);
-    return cudaGetLastError();
 }
 
 cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
@@ -396,8 +411,10 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     SweepParams p;
     fill_params(h, &p, h->vote_geom);
     h->launches += 1;
-    if (h->ab.ok)
-        return h->g.pack == 2 ? launch_one<2, true>(p, st) : launch_one<1, true>(p, st);
-    return h->g.pack == 2 ? launch_one<2, false>(p, st) : launch_one<1, false>(p, st);
+    const void *fn = sweep_kernel(h);
+    cudaError_t e = ensure_dynamic_smem(fn, p.geom.smem_bytes);
+    if (e != cudaSuccess)
+        return e;
+    void *args[] = {(void *)&p};
+    return cudaLaunchKernel(fn, dim3(p.geom.n_tiles), dim3(p.geom.threads), args, p.geom.smem_bytes, st);
 }
-

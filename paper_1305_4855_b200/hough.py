@@ -24,6 +24,8 @@ OPT_STAGE_TIMING = 2
 OPT_UNPACKED = 4
 OPT_EXACT_ONLY = 8
 OPT_LIST_SWEEP = 16
+OPT_LINE = 32
+OPT_INTERVAL = 64
 N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)

@@ -137,3 +137,102 @@ def test_vertices_rejects_bad_arguments(hough):
         with pytest.raises(hough.HoughError):
             h.vertices(bad)
     h.close()
+
+
+# ============================================================ f3: vote variants
+
+def read_all(h):
+    res = h.read()
+    res["acc"] = h.accumulator_host().copy()
+    return res
+
+
+def assert_same(res, ref):
+    assert res["n_votes"] == ref["n_votes"]
+    assert res["n_bad_hits"] == ref["n_bad_hits"]
+    assert np.array_equal(res["acc"], ref["acc"])
+    assert res["n_peaks"] == ref["n_peaks"]
+    assert np.array_equal(res["peak_bin"], ref["peak_bin"])
+    assert np.array_equal(res["peak_mask"], ref["peak_mask"])
+    assert res["n_hit_entries"] == ref["n_hit_entries"]
+    assert np.array_equal(res["hit_offset"], ref["hit_offset"])
+    assert np.array_equal(res["hit_index"], ref["hit_index"])
+
+
+@pytest.mark.parametrize("n_phi,n_rho,tile,n_hits,n_layers,seed", [
+    (48, 32, 0, 300, 10, 0),
+    (200, 64, 7, 1200, 10, 1),     # ragged phi slabs, several chunks
+    (64, 96, 0, 600, 20, 2),       # more than 16 layers: unpacked tile
+])
+def test_line_transform_random(hough, oracle, n_phi, n_rho, tile, n_hits, n_layers, seed):
+    rng = np.random.default_rng(seed)
+    g = synth.Grid(n_phi=n_phi, n_d0=1, n_kappa=n_rho, L_min=3, d0_min=0.0, d0_max=0.0, kappa_min=-30.0,
+                   kappa_max=45.0, layer_radii=tuple(float(3 + 4 * l) for l in range(n_layers)))
+    x, y, layer = random_hits(rng, n_hits, n_layers=n_layers)
+    layer[::17] = n_layers + 3  # some bad layers
+    ref = oracle.run_variant(g, oracle.MODE_LINE, x, y, layer)
+    assert ref["n_peaks"] > 5
+    h = make(hough, g, x, y, layer, 1 << 16, 1 << 20, options=hough.OPT_LINE, tile_phi=tile)
+    assert_same(read_all(h), ref)
+    h.close()
+
+
+def test_line_transform_toy_detector(hough, oracle):
+    """The paper's own workload: the toy detector of PAPER.md:124 with straight tracks (Fig. 3)."""
+    g = synth.TOY_LINE_GRID
+    for spec, seed in ((synth.TOY_LINE_SPEC, 0), (synth.TOY_LINE_SPEC_5000, 1)):
+        x, y, layer, truth = synth.generate_line_event(spec, seed)
+        ref = oracle.run_variant(g, oracle.MODE_LINE, x, y, layer)
+        h = make(hough, g, x, y, layer, 1 << 16, 1 << 20, options=hough.OPT_LINE)
+        assert_same(read_all(h), ref)
+        h.close()
+
+
+def test_line_transform_needs_two_parameters(hough):
+    g = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=2)
+    with pytest.raises(hough.HoughError):
+        hough.Hough(g, 10, 10, 10, options=hough.OPT_LINE)
+    g2 = synth.Grid(n_phi=16, n_d0=1, n_kappa=32, L_min=2, d0_min=0.0, d0_max=0.0)
+    with pytest.raises(hough.HoughError):
+        hough.Hough(g2, 10, 10, 10, options=hough.OPT_LINE | hough.OPT_INTERVAL)
+
+
+@pytest.mark.parametrize("shape,tile,n_hits,n_layers,seed", [
+    ((40, 4, 64), (0, 0), 200, 10, 0),
+    ((50, 13, 64), (8, 4), 700, 10, 1),
+    ((33, 9, 256), (4, 8), 300, 24, 2),    # unpacked tile
+    ((64, 1, 128), (0, 0), 400, 10, 3),    # 2-parameter transform through the origin
+])
+def test_interval_voting_random(hough, oracle, shape, tile, n_hits, n_layers, seed):
+    rng = np.random.default_rng(seed)
+    d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
+    g = synth.Grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=4,
+                   layer_radii=tuple(float(3 + 3 * l) for l in range(n_layers)), **d0)
+    x, y, layer = random_hits(rng, n_hits, n_layers=n_layers)
+    x[5], y[5] = np.float32(np.nan), np.float32(1.0)
+    x[6], y[6] = np.float32(np.inf), np.float32(2.0)
+    x[7], y[7] = np.float32(0.0), np.float32(0.0)
+    ref = oracle.run_variant(g, oracle.MODE_INTERVAL, x, y, layer)
+    assert ref["n_peaks"] > 0 and ref["n_votes"] > 5 * n_hits
+    h = make(hough, g, x, y, layer, 1 << 18, 1 << 22, options=hough.OPT_INTERVAL, tile_phi=tile[0], tile_d0=tile[1])
+    assert_same(read_all(h), ref)
+    h.close()
+
+
+def test_interval_voting_displaced3d(hough, oracle):
+    """BASELINE.json configs[1] under interval voting (accumulator, n_votes and peaks at full size;
+    hit lists of the first 4096 peaks: the oracle's list pass is O(peaks x hits))."""
+    w = synth.WORKLOADS["displaced3d"]
+    x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
+    acc, n_votes, n_bad = oracle.vote_variant(w.grid, oracle.MODE_INTERVAL, x, y, layer)
+    pb, pm, n_peaks = oracle.peaks(w.grid, acc)
+    h = make(hough, w.grid, x, y, layer, 1 << 22, 1 << 26, options=hough.OPT_INTERVAL)
+    res = read_all(h)
+    assert res["flags"] == 0
+    assert res["n_votes"] == n_votes and np.array_equal(res["acc"], acc)
+    assert res["n_peaks"] == n_peaks and np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
+    m = min(4096, n_peaks)
+    off, idx, tot = oracle.hitlists_variant(w.grid, oracle.MODE_INTERVAL, x, y, layer, pb[:m])
+    assert np.array_equal(res["hit_offset"][:m + 1], off)
+    assert np.array_equal(res["hit_index"][:tot], idx)
+    h.close()
