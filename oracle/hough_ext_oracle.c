@@ -421,7 +421,12 @@ uint64_t oracle_vertex_members(const oracle_grid *g, const oracle_vgrid *v, cons
  *   sp = sin phi, cp = cos phi;  khat = (-sp Cxr + cp Cyr) / Crr;
  *   delta = (-mx sp + my cp) - khat mr;  D = 1 - 4 delta khat  (= 1/(1 + kappa d0)^2);
  *   kappa = 2 khat / sqrt(D);  d0 = 2 delta / (1 + sqrt(D));
- *   rms = sqrt(max(0, (sp^2 Cxx - 2 sp cp Cxy + cp^2 Cyy - khat^2 Crr) / D))   [cm].
+ *   rms = sqrt((sum eps^2 / n) / D),  eps = khat w - (-sp u + cp v)   [cm]
+ *   (eps is the residual khat r^2 - s + delta of the hit written with the centred moments; a
+ *   third pass over the list.  Algebraically sum eps^2 / n = sp^2 Cxx - 2 sp cp Cxy + cp^2 Cyy
+ *   - khat^2 Crr, but that difference of ~1e3 cm^2 terms leaves ~1e-7 relative rounding noise on
+ *   a 1e-6 cm^2 variance, which would make the selection rms <= rms_max depend on the math
+ *   library: DESIGN.md section 8, reading X6.)
  * phi is defined modulo pi; (phi + pi, -d0, -kappa) is the same circle.  The representation
  * reported is the FORWARD one: mx cp + my sp >= 0 (the hits lie ahead of the point of closest
  * approach), otherwise phi -= or += pi (into [-pi, pi)), d0 = -d0, kappa = -kappa -- exact
@@ -480,8 +485,14 @@ int oracle_fit_one(const float *x, const float *y, const uint32_t *idx, uint32_t
     const double sq = sqrt(D);
     double kappa = 2.0 * khat / sq;
     double d0 = 2.0 * delta / (1.0 + sq);
-    double var = (sp * sp * Cxx - 2.0 * sp * cp * Cxy + cp * cp * Cyy - khat * khat * Crr) / D;
-    double rms = sqrt(var > 0.0 ? var : 0.0);
+    double see = 0.0;
+    for (uint32_t q = 0; q < n; ++q) {
+        double xv = (double)x[idx[q]], yv = (double)y[idx[q]];
+        double u = xv - mx, v = yv - my, w = (xv * xv + yv * yv) - mr;
+        double eps = khat * w - (-sp * u + cp * v);
+        see += eps * eps;
+    }
+    double rms = sqrt((see / dn) / D);
     if (mx * cp + my * sp < 0.0) { /* backward representation: report the forward one */
         phi = phi >= 0.0 ? phi - ORACLE_PI : phi + ORACLE_PI;
         d0 = -d0;
