@@ -297,6 +297,71 @@ size_t hough_vertex_workspace_bytes(const hough_vertex_config *vc);
 int hough_vertices(hough_handle *h, const hough_vertex_config *vc, void *workspace, size_t workspace_bytes,
                    const hough_peaks_out *peaks, const hough_vertex_out *out, void *cuda_stream);
 
+/*
+ * ---- f2: fit of every peak's hit list, selection and removal of duplicates (section 8:
+ * "find the locations of the peaks ... perform a fit of the hits to the candidate tracks";
+ * "the track candidate collection is then cleaned to remove duplicate tracks or tracks
+ * which share a large number of hits").  Recipes E4 / E5 of DESIGN.md section 8.
+ *
+ * E4, per reported peak p with hit list H(p) (ascending hit index, the arrays hough_peaks filled), all
+ * in binary64, sums taken over the list in its order, never fused: means mx, my, mr of x, y, x^2+y^2;
+ * central moments Cxx, Cxy, Cyy, Cxr, Cyr, Crr; q1 = Crr Cxy - Cxr Cyr; q2 = Crr (Cxx - Cyy) - Cxr^2 +
+ * Cyr^2; phi = atan2(2 q1, q2)/2; khat = (-sin(phi) Cxr + cos(phi) Cyr)/Crr; delta = (-mx sin(phi) +
+ * my cos(phi)) - khat mr; D = 1 - 4 delta khat; kappa = 2 khat/sqrt(D); d0 = 2 delta/(1 + sqrt(D));
+ * rms = sqrt((sum eps^2/n)/D) with eps = khat w - (-sin(phi) u + cos(phi) v) over the centred hits;
+ * the FORWARD representation is reported (mx cos(phi) + my sin(phi) >= 0, else phi -+ pi, d0 and kappa
+ * negated -- exact sign flips, so the two mirror peaks of a track fit bit-identically).
+ * status: 0 ok; 1 fewer than 3 hits; 2 degenerate (Crr = 0, D <= 0, non-finite result); 3 the peak's
+ * list is not complete in hit_index (HOUGH_TRUNCATED_HITS cut it): not fitted.
+ * E5: p is SELECTED iff status == 0 and rms <= rms_max; a selected p is a DUPLICATE iff another selected
+ * o shares at least min_shared hits with it and is better (more layers in its mask; else smaller rms;
+ * else lower position).  flag[p] = 0 not selected, 1 selected and kept, 2 selected but a duplicate.
+ * kept[] lists the positions p with flag 1 in ascending order (the de-duplicated track collection:
+ * what a host needs to read back instead of every peak).
+ * Index results (status, flag, kept, counts) are exact given the rms values; the binary64 fit agrees
+ * with the CPU oracle to the tolerance DESIGN.md section 8 derives (the moments are bit-identical; the
+ * CUDA and host math libraries' atan2 / sin / cos differ in the last bits).
+ */
+typedef struct hough_fit_config {
+    double rms_max;      /* [cm], >= 0 (may be +inf: every status-0 fit is selected) */
+    uint32_t min_shared; /* >= 1 */
+    uint32_t reserved;   /* 0 */
+} hough_fit_config;
+
+typedef struct hough_fit_counts { /* 32 bytes, same layout on host and device */
+    uint32_t n_fitted;     /* candidates looked at = min(n_peaks, cap_peaks) */
+    uint32_t n_ok;         /* status 0 */
+    uint32_t n_selected;   /* flag 1 or 2 */
+    uint32_t n_kept;       /* flag 1 = entries of kept[] */
+    uint32_t n_duplicates; /* flag 2 */
+    uint32_t n_truncated;  /* status 3 */
+    uint64_t n_pair_tests; /* candidate pairs whose shared hits were counted (work of the duplicate rule) */
+} hough_fit_counts;
+
+typedef struct hough_fit_out { /* all [device], caller-owned, cap_peaks entries each (counts: 1) */
+    double *kappa, *phi0, *d0, *rms; /* 0 where status != 0 */
+    int32_t *status;
+    uint8_t *flag;
+    uint32_t *kept;
+    hough_fit_counts *counts;
+} hough_fit_out;
+
+/* Bytes of [device] scratch hough_fit needs for this handle (its max_hits, cap_peaks, cap_hits);
+ * 0 for a NULL handle or cap_hits >= 2^32. */
+size_t hough_fit_workspace_bytes(const hough_handle *h);
+
+/*
+ * Enqueue E4 + E5 over the peaks and hit lists in `peaks` (the arrays hough_peaks filled for the event
+ * last given to hough_vote on this handle: the hit coordinates are the handle's own device copy, so
+ * the caller's x / y may already be gone).  Everything is read on the device: no host synchronisation
+ * between hough_peaks and this call.  `workspace`: [device], 256-byte aligned, >=
+ * hough_fit_workspace_bytes(h), caller-owned, used only during the call's work.
+ * Errors: HOUGH_EINVAL (NULL / bad fc / cap_hits >= 2^32), HOUGH_ENOMEM, HOUGH_ESTATE (no hough_vote
+ * before), HOUGH_ECUDA.
+ */
+int hough_fit(hough_handle *h, const hough_fit_config *fc, void *workspace, size_t workspace_bytes,
+              const hough_peaks_out *peaks, const hough_fit_out *out, void *cuda_stream);
+
 /* Geometry the library chose (for reporting): tile_phi, tile_d0, n_tiles, threads per CTA,
  * dynamic shared memory bytes of the vote kernel, number of SMs.  Any pointer may be NULL. */
 int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,

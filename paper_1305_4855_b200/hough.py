@@ -33,7 +33,7 @@ SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote
            "hough_accumulator", "hough_process_host", "hough_submit_host", "hough_collect_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
            "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror",
-           "hough_vertex_workspace_bytes", "hough_vertices")
+           "hough_vertex_workspace_bytes", "hough_vertices", "hough_fit_workspace_bytes", "hough_fit")
 
 
 class HoughError(RuntimeError):
@@ -78,6 +78,18 @@ class VertexOut(C.Structure):
     _fields_ = [("bin", C.c_void_p), ("count", C.c_void_p), ("member_offset", C.c_void_p),
                 ("member_index", C.c_void_p), ("counts", C.c_void_p)]
 
+
+class FitConfig(C.Structure):
+    _fields_ = [("rms_max", C.c_double), ("min_shared", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class FitOut(C.Structure):
+    _fields_ = [("kappa", C.c_void_p), ("phi0", C.c_void_p), ("d0", C.c_void_p), ("rms", C.c_void_p),
+                ("status", C.c_void_p), ("flag", C.c_void_p), ("kept", C.c_void_p), ("counts", C.c_void_p)]
+
+
+FIT_COUNTS_DTYPE = np.dtype([("n_fitted", "<u4"), ("n_ok", "<u4"), ("n_selected", "<u4"), ("n_kept", "<u4"),
+                             ("n_duplicates", "<u4"), ("n_truncated", "<u4"), ("n_pair_tests", "<u8")])
 
 VERTEX_COUNTS_DTYPE = np.dtype([("n_vertex_votes", "<u8"), ("n_member_entries", "<u8"), ("n_vertices", "<u4"),
                                 ("flags", "<u4"), ("reserved", "<u8")])
@@ -141,6 +153,11 @@ def _load():
     lib.hough_vertices.restype = C.c_int
     lib.hough_vertices.argtypes = [C.c_void_p, C.POINTER(VertexConfig), C.c_void_p, C.c_size_t,
                                    C.POINTER(PeaksOut), C.POINTER(VertexOut), C.c_void_p]
+    lib.hough_fit_workspace_bytes.restype = C.c_size_t
+    lib.hough_fit_workspace_bytes.argtypes = [C.c_void_p]
+    lib.hough_fit.restype = C.c_int
+    lib.hough_fit.argtypes = [C.c_void_p, C.POINTER(FitConfig), C.c_void_p, C.c_size_t, C.POINTER(PeaksOut),
+                              C.POINTER(FitOut), C.c_void_p]
     return lib
 
 
@@ -370,6 +387,42 @@ class Hough:
                 "vertex_count": v["count"][:n_rep].cpu().numpy().view(np.uint32),
                 "member_offset": v["member_offset"][:n_rep + 1].cpu().numpy().view(np.uint64),
                 "member_index": v["member_index"][:n_mem].cpu().numpy().view(np.uint32)}
+
+    # -- f2: fit + duplicate removal (hough_fit)
+    def fit(self, rms_max, min_shared, stream=None):
+        """hough_fit on the peaks and hit lists of the last ``peaks`` call.  Enqueues only; see ``read_fit``."""
+        if getattr(self, "_fit", None) is None:
+            nbytes = int(_lib.hough_fit_workspace_bytes(self._h))
+            if nbytes == 0:
+                raise HoughError("hough_fit_workspace_bytes: cap_hits too large")
+            f64 = dict(dtype=torch.float64, device=self.device)
+            f = dict(nbytes=nbytes, ws=torch.empty(nbytes, dtype=torch.uint8, device=self.device),
+                     kappa=torch.empty(self.cap_peaks, **f64), phi0=torch.empty(self.cap_peaks, **f64),
+                     d0=torch.empty(self.cap_peaks, **f64), rms=torch.empty(self.cap_peaks, **f64),
+                     status=torch.empty(self.cap_peaks, dtype=torch.int32, device=self.device),
+                     flag=torch.empty(self.cap_peaks, dtype=torch.uint8, device=self.device),
+                     kept=torch.empty(self.cap_peaks, dtype=torch.int32, device=self.device),
+                     counts=torch.zeros(FIT_COUNTS_DTYPE.itemsize // 8, dtype=torch.int64, device=self.device))
+            f["out"] = FitOut(f["kappa"].data_ptr(), f["phi0"].data_ptr(), f["d0"].data_ptr(), f["rms"].data_ptr(),
+                              f["status"].data_ptr(), f["flag"].data_ptr(), f["kept"].data_ptr(),
+                              f["counts"].data_ptr())
+            self._fit = f
+        f = self._fit
+        fc = FitConfig(float(rms_max), int(min_shared), 0)
+        _check(_lib.hough_fit(self._h, C.byref(fc), C.c_void_p(f["ws"].data_ptr()), f["nbytes"],
+                              C.byref(self._out), C.byref(f["out"]), _stream_ptr(stream)), "hough_fit")
+
+    def read_fit(self):
+        """Synchronise and copy the results of the last ``fit`` call to the host."""
+        torch.cuda.synchronize(self.device)
+        f = self._fit
+        cnt = f["counts"].cpu().numpy().view(FIT_COUNTS_DTYPE)[0]
+        n = int(cnt["n_fitted"])
+        out = {k: int(cnt[k]) for k in FIT_COUNTS_DTYPE.names}
+        for k in ("kappa", "phi0", "d0", "rms", "status", "flag"):
+            out[k] = f[k][:n].cpu().numpy()
+        out["kept"] = f["kept"][:int(cnt["n_kept"])].cpu().numpy().view(np.uint32)
+        return out
 
     # -- results
     def _pack(self, cnt, b, m, off, idx):
