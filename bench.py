@@ -291,14 +291,21 @@ def main():
 
     # ---- e2e: host buffers in, host results out, every event (hough_process_host)
     def e2e_step():
-        # hough_submit_host / hough_collect_host: the copies of event e-1 overlap event e
+        # three events in flight: inputs of e+1 on the library's copy-in stream,
+        # e computing, results of e-1 on the copy-out stream; every event's complete results land in
+        # pinned host memory before its slot is reused
         nv = 0
         for e in range(n_ev):
             x, y, layer = pin_events[e]
-            h.submit_host(x.numpy(), y.numpy(), layer.numpy(), e & 1)
+            h.submit_host(x.numpy(), y.numpy(), layer.numpy(), e % 3)
             if e > 0:
-                nv += h.collect_host((e - 1) & 1)["n_votes"]
-        nv += h.collect_host((n_ev - 1) & 1)["n_votes"]
+                h.collect_begin((e - 1) % 3)
+            if e > 1:
+                nv += h.collect_end((e - 2) % 3)["n_votes"]
+        h.collect_begin((n_ev - 1) % 3)
+        if n_ev > 1:
+            nv += h.collect_end((n_ev - 2) % 3)["n_votes"]
+        nv += h.collect_end((n_ev - 1) % 3)["n_votes"]
         return nv
 
     def e2e_step_sync():
@@ -326,7 +333,8 @@ def main():
                   min(int(c["n_hit_entries"]), workload.cap_hits) * 4 for c in cnt))
     e2e = {"value": votes_all * args.steps / e2e_secs, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs,
-           "api": "hough_submit_host + hough_collect_host (two events in flight, copies on a second stream)"}
+           "api": "hough_submit_host + hough_collect_begin/_end (three events in flight: copy-in, compute and "
+                  "copy-out streams)"}
     if rank == 0 and world == 1:
         h.process_host(*[t.numpy() for t in pin_events[0]])  # allocates its pinned buffers
         t0 = time.perf_counter()

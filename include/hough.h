@@ -193,22 +193,34 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
                        void *cuda_stream);
 
 /*
- * The same in two halves, so that the device->host copies of one event overlap the
- * computation of the next (the paper's production model: transfers of neighbouring events
- * overlap, steady-state throughput).  `slot` is 0 or 1 and names one of
- * two in-flight events; each slot needs its own `dev` arrays (and `host` buffers).
- *   hough_submit_host   copies x, y, layer host->device on `cuda_stream`, enqueues hough_vote
- *                       + hough_peaks into `dev`, records the slot's event; returns at once.
- *   hough_collect_host  waits (on `copy_stream`) for the slot's event, copies counts, then
- *                       the filled prefixes of the peak arrays and hit lists to `host`, and
- *                       SYNCHRONISES `copy_stream` before returning.
- * Pattern:  submit(e, e&1);  if (e > 0) collect(e-1, (e-1)&1);  ...  collect(last).
- * A slot must be collected before it is submitted again.  The host arrays must be pinned
- * for the copies to overlap.  Errors as hough_process_host; HOUGH_ESTATE if the slot was
- * not submitted.
+ * The same as a pipeline, so that three things run at once (the paper's production model,
+ * "simultaneously ... processing one event, transferring data ... for the next event
+ * ... and returning the results ... for the previously processed event"; steady-state throughput).
+ * `slot` (0 .. HOUGH_MAX_SLOTS-1) names one in-flight event; each slot in use needs its own `dev`
+ * arrays and `host` buffers.
+ *   hough_submit_host    copies x, y, layer host->device on a stream of the LIBRARY's own (created at the
+ *                        first call, destroyed with the handle) into the slot's own staging arrays, so the
+ *                        inputs of event e+1 land while event e computes; makes `cuda_stream` wait for
+ *                        them; enqueues hough_vote + hough_peaks into `dev` and a 48-byte copy of the
+ *                        counters to pinned memory of the library; returns at once.
+ *   hough_collect_begin  waits ON THE HOST until the slot's computation is complete, writes host->counts,
+ *                        enqueues the copies of the filled prefixes of the peak arrays and hit lists to
+ *                        `host` on `copy_stream` and returns (no device round trip for the sizes).
+ *   hough_collect_end    waits on the host until those copies have landed; the slot is free again.
+ *   hough_collect_host   = hough_collect_begin + hough_collect_end.
+ * Patterns:  two slots:   submit(e, e&1);  if (e > 0) collect_host(e-1);  ...
+ *            three slots: submit(e, e%3);  if (e > 0) collect_begin(e-1);  if (e > 1) collect_end(e-2);  ...
+ *            (the device->host copy engine never waits for the host).
+ * A slot must be collected (end) before it is submitted again.  The host arrays must be pinned for the
+ * copies to overlap.  Errors as hough_process_host; HOUGH_ESTATE if the slot is not in the state the call
+ * needs.  One handle computes one event at a time: `cuda_stream` should be the same stream for all slots.
  */
+#define HOUGH_MAX_SLOTS 4
 int hough_submit_host(hough_handle *h, const float *x, const float *y, const int32_t *layer,
                       uint32_t n, const hough_peaks_out *dev, int32_t slot, void *cuda_stream);
+int hough_collect_begin(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host,
+                        int32_t slot, void *copy_stream);
+int hough_collect_end(hough_handle *h, int32_t slot);
 int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host,
                        int32_t slot, void *copy_stream);
 

@@ -201,7 +201,12 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *t_d0sq = cv.take((size_t)c->n_d0 * 4);
     void *hx = cv.take((size_t)hp * 4), *hy = cv.take((size_t)hp * 4), *hr2 = cv.take((size_t)hp * 4);
     void *hbit = cv.take((size_t)hp * 4);
-    void *rx = cv.take((size_t)hp * 4), *ry = cv.take((size_t)hp * 4), *rl = cv.take((size_t)hp * 4);
+    void *rx[HOUGH_MAX_SLOTS], *ry[HOUGH_MAX_SLOTS], *rl[HOUGH_MAX_SLOTS];
+    for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
+        rx[s] = cv.take((size_t)hp * 4);
+        ry[s] = cv.take((size_t)hp * 4);
+        rl[s] = cv.take((size_t)hp * 4);
+    }
     void *flags = cv.take(n_bins / 8);
     void *row_base = cv.take((n_rows + 1) * 4);
     void *list_len = cv.take(n_sub * 4);
@@ -233,9 +238,11 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->hy = (float *)hy;
         h->hr2 = (float *)hr2;
         h->hbit = (uint32_t *)hbit;
-        h->raw_x = (float *)rx;
-        h->raw_y = (float *)ry;
-        h->raw_layer = (int32_t *)rl;
+        for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
+            h->raw_x[s] = (float *)rx[s];
+            h->raw_y[s] = (float *)ry[s];
+            h->raw_layer[s] = (int32_t *)rl[s];
+        }
         h->max_hits_pad = hp;
         h->flags = (uint32_t *)flags;
         h->row_base = (uint32_t *)row_base;
@@ -527,9 +534,18 @@ void hough_destroy(hough_handle *h)
         for (int s = 0; s < HOUGH_N_STAGES + 2; ++s)
             if (h->ev[s])
                 cudaEventDestroy(h->ev[s]);
-    for (int s = 0; s < 2; ++s)
+    for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
         if (h->slot_ev[s])
             cudaEventDestroy(h->slot_ev[s]);
+        if (h->h2d_ev[s])
+            cudaEventDestroy(h->h2d_ev[s]);
+        if (h->copy_ev[s])
+            cudaEventDestroy(h->copy_ev[s]);
+    }
+    if (h->h2d_stream)
+        cudaStreamDestroy(h->h2d_stream);
+    if (h->slot_counts)
+        cudaFreeHost(h->slot_counts);
     free(h->radii);
     delete h;
 }
@@ -649,11 +665,11 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
         return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n > 0) {
-        CK(cudaMemcpyAsync(h->raw_x, x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(h->raw_y, y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(h->raw_layer, layer, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_x[0], x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_y[0], y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_layer[0], layer, (size_t)n * 4, cudaMemcpyHostToDevice, st));
     }
-    int rc = hough_vote(h, h->raw_x, h->raw_y, h->raw_layer, n, cuda_stream);
+    int rc = hough_vote(h, h->raw_x[0], h->raw_y[0], h->raw_layer[0], n, cuda_stream);
     if (rc != HOUGH_OK)
         return rc;
     rc = hough_peaks(h, dev, cuda_stream);
@@ -671,51 +687,75 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
     if (host->hit_index && ne > 0)
         CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return HOUGH_OK;
+}
+
+// Lazily created resources of the pipelined host entry points.
+static int pipeline_init(hough_handle *h)
+{
+    if (h->h2d_stream)
+        return HOUGH_OK;
+    CK(cudaStreamCreateWithFlags(&h->h2d_stream, cudaStreamNonBlocking));
+    for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
+        CK(cudaEventCreateWithFlags(&h->h2d_ev[s], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&h->slot_ev[s], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&h->copy_ev[s], cudaEventDisableTiming));
+    }
+    CK(cudaMallocHost((void **)&h->slot_counts, sizeof(hough_counts) * HOUGH_MAX_SLOTS));
     return HOUGH_OK;
 }
 
 int hough_submit_host(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
                       const hough_peaks_out *dev, int32_t slot, void *cuda_stream)
 {
-    if (!h || !dev || slot < 0 || slot > 1)
+    if (!h || !dev || slot < 0 || slot >= HOUGH_MAX_SLOTS)
         return HOUGH_EINVAL;
     if (n > h->cfg.max_hits || (n > 0 && (!x || !y || !layer)))
         return HOUGH_EINVAL;
     if (h->slot_busy[slot])
         return HOUGH_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (!h->slot_ev[slot])
-        CK(cudaEventCreateWithFlags(&h->slot_ev[slot], cudaEventDisableTiming));
+    int rc = pipeline_init(h);
+    if (rc != HOUGH_OK)
+        return rc;
+    // inputs: on the library's copy-in stream, into the slot's own staging arrays (free: the slot's
+    // previous event has been collected, so its k_prep has long read them), ahead of whatever the
+    // compute stream is still doing for the previous event
     if (n > 0) {
-        CK(cudaMemcpyAsync(h->raw_x, x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(h->raw_y, y, (size_t)n * 4, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(h->raw_layer, layer, (size_t)n * 4, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(h->raw_x[slot], x, (size_t)n * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+        CK(cudaMemcpyAsync(h->raw_y[slot], y, (size_t)n * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+        CK(cudaMemcpyAsync(h->raw_layer[slot], layer, (size_t)n * 4, cudaMemcpyHostToDevice, h->h2d_stream));
     }
-    int rc = hough_vote(h, h->raw_x, h->raw_y, h->raw_layer, n, cuda_stream);
+    CK(cudaEventRecord(h->h2d_ev[slot], h->h2d_stream));
+    CK(cudaStreamWaitEvent(st, h->h2d_ev[slot], 0));
+    rc = hough_vote(h, h->raw_x[slot], h->raw_y[slot], h->raw_layer[slot], n, cuda_stream);
     if (rc != HOUGH_OK)
         return rc;
     rc = hough_peaks(h, dev, cuda_stream);
     if (rc != HOUGH_OK)
         return rc;
+    // the 48 bytes of counters follow the computation on its own stream, so that the collecting side
+    // knows the sizes of the results without a round trip of its own
+    CK(cudaMemcpyAsync(&h->slot_counts[slot], dev->counts, sizeof(hough_counts), cudaMemcpyDeviceToHost, st));
     CK(cudaEventRecord(h->slot_ev[slot], st));
     h->slot_busy[slot] = 1;
     return HOUGH_OK;
 }
 
-int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host, int32_t slot,
-                       void *copy_stream)
+int hough_collect_begin(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host, int32_t slot,
+                        void *copy_stream)
 {
     if (!h || !dev || !host || !host->counts || !host->bin || !host->mask || !host->hit_offset || slot < 0 ||
-        slot > 1)
+        slot >= HOUGH_MAX_SLOTS)
         return HOUGH_EINVAL;
-    if (!h->slot_busy[slot])
+    if (h->slot_busy[slot] != 1)
         return HOUGH_ESTATE;
     cudaStream_t st = (cudaStream_t)copy_stream;
-    CK(cudaStreamWaitEvent(st, h->slot_ev[slot], 0));
-    CK(cudaMemcpyAsync(host->counts, dev->counts, sizeof(hough_counts), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    uint64_t np = host->counts->n_peaks < h->cfg.cap_peaks ? host->counts->n_peaks : h->cfg.cap_peaks;
-    uint64_t ne = host->counts->n_hit_entries < h->cfg.cap_hits ? host->counts->n_hit_entries : h->cfg.cap_hits;
+    CK(cudaEventSynchronize(h->slot_ev[slot]));
+    const hough_counts c = h->slot_counts[slot];
+    *host->counts = c;
+    const uint64_t np = c.n_peaks < h->cfg.cap_peaks ? c.n_peaks : h->cfg.cap_peaks;
+    const uint64_t ne = c.n_hit_entries < h->cfg.cap_hits ? c.n_hit_entries : h->cfg.cap_hits;
     if (np > 0) {
         CK(cudaMemcpyAsync(host->bin, dev->bin, np * 4, cudaMemcpyDeviceToHost, st));
         CK(cudaMemcpyAsync(host->mask, dev->mask, np * 4, cudaMemcpyDeviceToHost, st));
@@ -723,9 +763,27 @@ int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_
     CK(cudaMemcpyAsync(host->hit_offset, dev->hit_offset, (np + 1) * 8, cudaMemcpyDeviceToHost, st));
     if (host->hit_index && ne > 0)
         CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
+    CK(cudaEventRecord(h->copy_ev[slot], st));
+    h->slot_busy[slot] = 2;
+    return HOUGH_OK;
+}
+
+int hough_collect_end(hough_handle *h, int32_t slot)
+{
+    if (!h || slot < 0 || slot >= HOUGH_MAX_SLOTS)
+        return HOUGH_EINVAL;
+    if (h->slot_busy[slot] != 2)
+        return HOUGH_ESTATE;
+    CK(cudaEventSynchronize(h->copy_ev[slot]));
     h->slot_busy[slot] = 0;
     return HOUGH_OK;
+}
+
+int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_host_out *host, int32_t slot,
+                       void *copy_stream)
+{
+    const int rc = hough_collect_begin(h, dev, host, slot, copy_stream);
+    return rc != HOUGH_OK ? rc : hough_collect_end(h, slot);
 }
 
 int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,

@@ -124,8 +124,9 @@ struct hough_handle {
     HitIndexDev ix;
     float *hx, *hy, *hr2;
     uint32_t *hbit;
-    float *raw_x, *raw_y;  // staging of hough_process_host's host buffers
-    int32_t *raw_layer;
+    // staging of the host entry points' hit arrays, one set per in-flight slot
+    float *raw_x[HOUGH_MAX_SLOTS], *raw_y[HOUGH_MAX_SLOTS];
+    int32_t *raw_layer[HOUGH_MAX_SLOTS];
     uint32_t max_hits_pad;
     uint32_t *flags;      // 1 bit per bin
     uint32_t *row_base;   // [n_rows + 1] exclusive scan of peaks per (i, j) row
@@ -139,9 +140,14 @@ struct hough_handle {
     uint32_t scan_blocks_max;
     // sweep tile geometry of the peak kernel
     int pk_JW, pk_Li, pk_smem;
-    // hough_submit_host / hough_collect_host: one event per slot marks the end of the slot's work
-    cudaEvent_t slot_ev[2];
-    unsigned char slot_busy[2];
+    // hough_submit_host / hough_collect_*: three-way overlap.  The library owns one
+    // non-blocking stream for the host->device copies; per slot: h2d_ev = inputs landed, slot_ev = the
+    // slot's computation (and the copy of its counters into slot_counts) is complete, copy_ev = its
+    // results have reached the host.  slot_busy: 0 free, 1 submitted, 2 results being copied.
+    cudaStream_t h2d_stream;
+    cudaEvent_t h2d_ev[HOUGH_MAX_SLOTS], slot_ev[HOUGH_MAX_SLOTS], copy_ev[HOUGH_MAX_SLOTS];
+    unsigned char slot_busy[HOUGH_MAX_SLOTS];
+    hough_counts *slot_counts;   // pinned host memory, one block per slot
     // state
     uint32_t n_hits;
     int voted;

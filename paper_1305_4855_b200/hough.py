@@ -30,7 +30,8 @@ N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
 SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote", "hough_peaks",
-           "hough_accumulator", "hough_process_host", "hough_submit_host", "hough_collect_host", "hough_clear", "hough_peak_sweep",
+           "hough_accumulator", "hough_process_host", "hough_submit_host", "hough_collect_begin", "hough_collect_end",
+           "hough_collect_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
            "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror",
            "hough_vertex_workspace_bytes", "hough_vertices", "hough_fit_workspace_bytes", "hough_fit")
@@ -126,9 +127,12 @@ def _load():
     lib.hough_submit_host.restype = C.c_int
     lib.hough_submit_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32,
                                       C.POINTER(PeaksOut), C.c_int32, C.c_void_p]
-    lib.hough_collect_host.restype = C.c_int
-    lib.hough_collect_host.argtypes = [C.c_void_p, C.POINTER(PeaksOut), C.POINTER(HostOut), C.c_int32,
-                                       C.c_void_p]
+    for name in ("hough_collect_host", "hough_collect_begin"):
+        f = getattr(lib, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.POINTER(PeaksOut), C.POINTER(HostOut), C.c_int32, C.c_void_p]
+    lib.hough_collect_end.restype = C.c_int
+    lib.hough_collect_end.argtypes = [C.c_void_p, C.c_int32]
     for name in ("hough_clear", "hough_peak_sweep"):
         f = getattr(lib, name)
         f.restype = C.c_int
@@ -340,9 +344,19 @@ class Hough:
 
     def collect_host(self, slot):
         """hough_collect_host: results of the event submitted in `slot`, copied on a second stream."""
-        _d, hb, out, host = self._slot(slot)
-        _check(_lib.hough_collect_host(self._h, C.byref(out), C.byref(host), int(slot),
-                                       C.c_void_p(self._copy_stream.cuda_stream)), "hough_collect_host")
+        self.collect_begin(slot)
+        return self.collect_end(slot)
+
+    def collect_begin(self, slot):
+        """hough_collect_begin: wait for the slot's computation, start copying its results to the host."""
+        _d, _hb, out, host = self._slot(slot)
+        _check(_lib.hough_collect_begin(self._h, C.byref(out), C.byref(host), int(slot),
+                                        C.c_void_p(self._copy_stream.cuda_stream)), "hough_collect_begin")
+
+    def collect_end(self, slot):
+        """hough_collect_end: wait for the copies; returns numpy views of the slot's pinned host buffers."""
+        _d, hb, _out, _host = self._slot(slot)
+        _check(_lib.hough_collect_end(self._h, int(slot)), "hough_collect_end")
         cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
         return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
                           hb["hit_index"].numpy())

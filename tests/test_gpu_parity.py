@@ -5,6 +5,7 @@ only) and compares accumulator masks, vote count, peak list and CSR hit lists wi
 oracle/ on the same seeded inputs (BASELINE.json north_star: "GPU results must match the
 oracle bit-exactly (accumulator masks, peak list, hit lists)").
 """
+import dataclasses
 import math
 
 import numpy as np
@@ -383,6 +384,57 @@ def test_submit_collect_pipeline_matches_oracle(hough, oracle):
         assert np.array_equal(res["peak_mask"], ref["peak_mask"])
         assert np.array_equal(res["hit_offset"], ref["hit_offset"])
         assert np.array_equal(res["hit_index"], ref["hit_index"])
+
+
+def test_three_slot_pipeline_with_pileup_events(hough, oracle):
+    """hough_submit_host / hough_collect_begin / hough_collect_end with three events in flight (inputs
+    of e+1 on the library's copy-in stream, e computing, results of e-1 on the copy-out stream;
+    PAPER.md:128-130), on pile-up events of different sizes; the slot state machine rejects misuse."""
+    w = synth.WORKLOADS["pileup"]
+    specs = [w.event, dataclasses.replace(w.event, n_prompt=300, n_noise=900), w.event,
+             dataclasses.replace(w.event, n_prompt=0, n_displaced=0, n_noise=40), w.event]
+    evs = [synth.generate_event(sp, 11 + q)[:3] for q, sp in enumerate(specs)]
+    pins = [[torch.from_numpy(a).pin_memory() for a in e] for e in evs]
+    h = hough.Hough(w.grid, max(len(e[0]) for e in evs), w.cap_peaks, w.cap_hits)
+    got = []
+
+    def keep(r):
+        got.append({k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in r.items()})
+
+    n = len(pins)
+    for e, pe in enumerate(pins):
+        h.submit_host(pe[0].numpy(), pe[1].numpy(), pe[2].numpy(), e % 3)
+        if e == 0:
+            with pytest.raises(hough.HoughError):
+                h.submit_host(pe[0].numpy(), pe[1].numpy(), pe[2].numpy(), 0)   # slot still in flight
+            with pytest.raises(hough.HoughError):
+                h.collect_end(0)                                                 # not begun
+        if e > 0:
+            h.collect_begin((e - 1) % 3)
+        if e > 1:
+            keep(h.collect_end((e - 2) % 3))
+    h.collect_begin((n - 1) % 3)
+    keep(h.collect_end((n - 2) % 3))
+    keep(h.collect_end((n - 1) % 3))
+    with pytest.raises(hough.HoughError):
+        h.collect_begin(1)          # nothing submitted in that slot any more
+    with pytest.raises(hough.HoughError):
+        h.submit_host(pins[0][0].numpy(), pins[0][1].numpy(), pins[0][2].numpy(), 4)  # no such slot
+    h.close()
+    assert len(got) == n
+    for res, ev in zip(got, evs):
+        acc, n_votes, _ = oracle.vote(w.grid, *ev)
+        pb, pm, n_peaks = oracle.peaks(w.grid, acc)
+        assert res["n_votes"] == n_votes and res["n_peaks"] == n_peaks and res["flags"] == 0
+        assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
+        # hit lists of a sample of peaks (the oracle's list pass is O(peaks x hits))
+        rng = np.random.default_rng(1)
+        sel = np.unique(rng.integers(0, max(n_peaks, 1), 400)) if n_peaks else np.zeros(0, np.int64)
+        soff, sidx, _tot = oracle.hitlists(w.grid, *ev, pb[sel])
+        for q, pk in enumerate(sel):
+            a, b = int(res["hit_offset"][pk]), int(res["hit_offset"][pk + 1])
+            assert np.array_equal(res["hit_index"][a:b], sidx[int(soff[q]):int(soff[q + 1])]), pk
+        assert int(res["hit_offset"][-1]) == res["n_hit_entries"]
 
 
 def test_second_vote_replaces_the_event_and_peaks_can_be_repeated(hough, oracle):
