@@ -215,7 +215,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
     // hit index of the peak-driven lists: azimuth bins per layer ~ 2 x hits per layer, a power of two
     int NA = 256;
-    while (NA < 8192 && (uint64_t)NA * (uint64_t)c->n_layers < 2ull * c->max_hits)
+    while (NA < 4096 && (uint64_t)NA * (uint64_t)c->n_layers < 2ull * c->max_hits)
         NA <<= 1;
     const int n_keys = (c->n_layers + 1) * NA;
     void *t_phic = cv.take((size_t)c->n_phi * 4);
@@ -223,8 +223,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 33 * 4); // histogram | per-layer radius range (one memset)
     void *ix_start = cv.take((size_t)(n_keys + 1) * 4);
     void *ix_key = cv.take((size_t)hp * 4);
-    void *ix_sx = cv.take((size_t)hp * 4), *ix_sy = cv.take((size_t)hp * 4), *ix_sr2 = cv.take((size_t)hp * 4);
-    void *ix_hit = cv.take((size_t)hp * 4), *ix_abin = cv.take((size_t)hp * 2);
+    void *ix_rec = cv.take((size_t)hp * 16);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
     void *counters = cv.take(256 + (size_t)2 * sb * 8);
     if (h) {
@@ -260,11 +259,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ix.layer_r = (uint32_t *)ix_cnt + n_keys;
         h->ix.bin_start = (uint32_t *)ix_start;
         h->ix.key = (uint32_t *)ix_key;
-        h->ix.sx = (float *)ix_sx;
-        h->ix.sy = (float *)ix_sy;
-        h->ix.sr2 = (float *)ix_sr2;
-        h->ix.s_hit = (uint32_t *)ix_hit;
-        h->ix.s_abin = (unsigned short *)ix_abin;
+        h->ix.rec = (float4 *)ix_rec;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);

@@ -25,18 +25,19 @@
 // candidates of every peak.  Every candidate is then evaluated with the EXACT recipe
 // (hough_device.cuh eval_kappa / kappa_bin), so the lists are bit-identical to the oracle's.
 //
-// Work split: a group of 16 lanes (32 with more than 16 layers) owns one peak; lane l computes
-// the windows of layer label l if bit l is set in the peak's mask (a hit of layer l in the bin
-// sets that bit, so other layers cannot contribute); the group then walks the flattened
-// candidate list 16 (32) at a time, collects the matching hit indices in shared memory, sorts
-// them and writes them to a staging buffer (one global atomic per CTA and batch).  k_scan<LENS>
-// turns the lengths into hit_offset and k_copy_lists moves the lists to their final place.
-// Lists longer than the group's buffer are counted here and written by k_copy_lists straight
-// from the hits in index order (one warp per such peak).
+// Work split: ONE THREAD per peak.  The thread walks the layer labels set in the peak's mask (a hit
+// of layer l in the bin sets bit l, so other layers cannot contribute), computes the layer's windows,
+// evaluates their candidates and appends the matching hit indices to the peak's fixed slot of the
+// staging buffer (candidate order).  k_scan<LENS> turns the lengths into hit_offset and k_copy_lists
+// sorts every list while moving it to its final place (rank by counting inside half a warp).
+// Lists longer than a slot are only counted here and written by k_copy_lists straight from the hits
+// in index order (one warp per such peak).  (Round-2 history: a group of 16 lanes per peak with lane =
+// layer spent 55 % of its instructions on the window arithmetic at 10 of 32 lanes active, plus three
+// CTA barriers per batch: 2.8e8 warp instructions per pile-up event, 0.42 ms.)
 #include "hough_device.cuh"
 
-#define PL_WARPS 8
-#define PL_MAXLIST 128
+#define PL_THREADS 256
+#define PL_MAXSLOT 64 // entries of a staging slot (at most; hough_create sizes it from the capacities)
 #define PL_SLOW 0xffffffffu
 #define PI_F 3.14159265358979f
 
@@ -134,11 +135,7 @@ __global__ void __launch_bounds__(256) k_index_scatter(HitIndexDev ix, const flo
     if (key == 0xffffffffu)
         return;
     const uint32_t rank = ix.bin_start[key] + atomicAdd(&ix.bin_cnt[key], 1u);
-    ix.sx[rank] = hx[h];
-    ix.sy[rank] = hy[h];
-    ix.sr2[rank] = hr2[h];
-    ix.s_hit[rank] = h;
-    ix.s_abin[rank] = (unsigned short)(key & (uint32_t)(ix.NA - 1));
+    ix.rec[rank] = make_float4(hx[h], hy[h], hr2[h], __uint_as_float(((key & (uint32_t)(ix.NA - 1)) << 20) | h));
 }
 
 cudaError_t launch_index_build(hough_handle *h, cudaStream_t st)
@@ -161,10 +158,9 @@ struct PeakListParams {
     const DevCounters *counters;
     uint32_t cap_peaks;
     uint32_t *peak_len; // [cap_peaks] list length
-    uint32_t *peak_pos; // [cap_peaks] start of the list in ent_hit, or PL_SLOW
-    uint32_t *ent_hit;  // [ent_cap] staging
-    unsigned long long ent_cap;
-    unsigned long long *n_entries;   // staging entries handed out
+    uint32_t *peak_pos; // [cap_peaks] 0: the list is in the peak's slot, PL_SLOW: it is not
+    uint32_t *slots;    // [cap_peaks][slot] staging
+    uint32_t slot;
     unsigned long long *n_list_evals; // candidates evaluated
     float dk;       // kappa bin width (binary32)
     float edge_rel; // slack on a bin edge, in bins
@@ -189,257 +185,168 @@ __device__ __forceinline__ void window_bins(float a_lo, float a_hi, float na_sca
     nb = (int)span;
 }
 
-template <int G> // lanes per peak
-__global__ void __launch_bounds__(32 * PL_WARPS) k_peak_lists(const PeakListParams p)
+__global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams p)
 {
-    constexpr int GPW = 32 / G;            // groups per warp
-    constexpr int GPC = PL_WARPS * GPW;    // groups (= peaks) per CTA and batch
-    __shared__ PlRange s_rng[GPC][G][3];
-    __shared__ uint32_t s_pre[GPC][G + 1]; // exclusive prefix of the lanes' candidate counts
-    __shared__ uint32_t s_list[GPC][PL_MAXLIST];
-    __shared__ uint32_t s_cnt[GPC], s_off[GPC];
-    __shared__ unsigned long long s_base;
+    __shared__ uint32_t s_lbase[34]; // rank of the first hit of layer label l (label nL = the wild hits)
+    __shared__ float s_ra[32], s_rb[32];
 
     const GridDev &g = p.g;
     const HitIndexDev &ix = p.ix;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int grp = warp * GPW + lane / G, gl = lane % G; // group in the CTA, lane in the group
-    const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((lane / G) * G));
+    const int tid = threadIdx.x, lane = tid & 31;
     const int NA = ix.NA, nL = ix.n_keys / NA - 1;
+    if (tid <= nL)
+        s_lbase[tid] = ix.bin_start[tid * NA];
+    if (tid == nL + 1)
+        s_lbase[tid] = ix.bin_start[nL * NA + 1];
+    if (tid < nL) {
+        s_ra[tid] = __uint_as_float(~ix.layer_r[2 * tid]) * (1.0f - 4e-6f);
+        s_rb[tid] = __uint_as_float(ix.layer_r[2 * tid + 1]) * (1.0f + 4e-6f);
+    }
+    __syncthreads();
     const float na_scale = (float)NA * 0.15915494309189535f;
     const uint32_t n_rep = min(p.counters->n_peaks, p.cap_peaks);
     const int nk = g.n_kappa;
     const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
     const float U = 5.9604645e-08f; // 2^-24
+    const uint32_t pk = blockIdx.x * PL_THREADS + tid;
     unsigned long long evals = 0;
 
-    for (uint32_t batch = blockIdx.x; (unsigned long long)batch * GPC < n_rep; batch += gridDim.x) {
-        const uint32_t pk = batch * GPC + grp;
-        const bool live = pk < n_rep;
-        uint32_t lin = 0, pmask = 0;
-        if (live) {
-            lin = p.bin[pk];
-            pmask = p.mask[pk];
-        }
+    if (pk < n_rep) {
+        const uint32_t lin = p.bin[pk], pmask = p.mask[pk];
         const uint32_t k = lin % (uint32_t)nk, row = lin / (uint32_t)nk;
         const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
         const float c_sn = g.sn[i], c_cs = g.cs[i], c_d0 = g.d0c[j], c_2d0 = g.twod0[j], c_d0sq = g.d0sq[j];
         const float phi0 = p.phic[i], ad0 = fabsf(c_d0);
+        uint32_t *slot = p.slots + (size_t)pk * p.slot;
+        uint32_t cnt = 0;
+        // the bin's kappa interval
+        float ka = __fmaf_rn((float)k, p.dk, klo), kb = __fmaf_rn((float)(k + 1u), p.dk, klo);
+        if (k == 0u)
+            ka = fminf(ka, klo);
+        if (k + 1u == (uint32_t)nk)
+            kb = fmaxf(kb, khi);
+        const float Kp = 1.01f * g.kabs + p.dk;
+        auto consider = [&](const float4 r) {
+            const float kappa = eval_kappa(r.x, r.y, r.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
+            if ((kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k) {
+                if (cnt < p.slot)
+                    slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
+                ++cnt;
+            }
+        };
 
-        // ---- phase 1: lane gl = layer label gl: its azimuth windows
-        PlRange r0 = {0u, 0u, 0, 0}, r1 = r0, r2 = r0;
-        uint32_t lbase = 0, lcnt = 0;
-        if (live && gl < nL && ((pmask >> gl) & 1u)) {
-            lbase = ix.bin_start[gl * NA];
-            lcnt = ix.bin_start[(gl + 1) * NA] - lbase;
-        }
-        if (lcnt) {
-            // the bin's kappa interval
-            float ka = __fmaf_rn((float)k, p.dk, klo), kb = __fmaf_rn((float)(k + 1u), p.dk, klo);
-            if (k == 0u)
-                ka = fminf(ka, klo);
-            if (k + 1u == (uint32_t)nk)
-                kb = fmaxf(kb, khi);
-            const float ra = __uint_as_float(~ix.layer_r[2 * gl]) * (1.0f - 4e-6f);
-            const float rb = __uint_as_float(ix.layer_r[2 * gl + 1]) * (1.0f + 4e-6f);
-            // binary32 evaluation error of the recipe: |kappa_fp - kappa| <= errnum / den + 2 U K
-            const float Gm = 1.4143f * rb + ad0, Kp = 1.01f * g.kabs + p.dk;
-            const float errnum = 2.0f * (12.0f * U * Gm + 16.0f * U * Kp * Gm * Gm);
-            const float Lmin = fmaxf(0.0f, fmaxf(ra - ad0 * (1.0f + 1e-6f), ad0 * (1.0f - 1e-6f) - rb));
-            const float L0sq = errnum / p.dk; // den >= L0sq: the error stays below one bin
-            float D = Lmin * Lmin;
-            const bool prox = !(D >= L0sq);
-            if (prox)
-                D = L0sq;
-            const float slack = errnum / D + 2.0f * U * Kp + p.edge_rel * p.dk;
-            const float k1 = ka - slack, k2 = kb + slack;
-            const float g1 = __fmaf_rn(k1, c_d0, 1.0f), g2 = __fmaf_rn(k2, c_d0, 1.0f);
-            bool whole = !(g1 > 0.01f && g2 > 0.01f);
-            int b0 = 0, nb = 0, b1 = 0, nb1 = 0, b2 = 0, nb2 = 0;
-            if (!whole) {
-                const float A1 = c_d0 * __fmaf_rn(k1, c_d0, 2.0f) / (2.0f * g1), B1 = k1 / (2.0f * g1);
-                const float A2 = c_d0 * __fmaf_rn(k2, c_d0, 2.0f) / (2.0f * g2), B2 = k2 / (2.0f * g2);
-                float wlo = fminf(A1 / ra + B1 * ra, A1 / rb + B1 * rb);
-                float whi = fmaxf(A2 / ra + B2 * ra, A2 / rb + B2 * rb);
-                if (A1 > 0.0f && B1 > 0.0f) { // W(k1, r) has its minimum 2 sqrt(A B) at r^2 = A / B
-                    const float q = A1 / B1;
-                    if (q > ra * ra && q < rb * rb)
-                        wlo = fminf(wlo, 2.0f * sqrtf(A1 * B1) * (1.0f - 1e-6f));
-                }
-                if (A2 < 0.0f && B2 < 0.0f) { // W(k2, r) has its maximum -2 sqrt(A B) at r^2 = A / B
-                    const float q = A2 / B2;
-                    if (q > ra * ra && q < rb * rb)
-                        whi = fmaxf(whi, -2.0f * sqrtf(A2 * B2) * (1.0f - 1e-6f));
-                }
-                const float ew = 1e-5f * (1.0f + fmaxf(fabsf(wlo), fabsf(whi)));
-                wlo -= ew;
-                whi += ew;
-                if (!(fabsf(wlo) < 3.0e38f) || !(fabsf(whi) < 3.0e38f) || !(wlo <= whi)) {
-                    whole = true; // inf / NaN somewhere: no bound
-                } else if (!(wlo > 1.0f) && !(whi < -1.0f)) {
-                    const float tlo = asinf(fmaxf(wlo, -1.0f)) - 2e-5f, thi = asinf(fminf(whi, 1.0f)) + 2e-5f;
-                    window_bins(phi0 + tlo, phi0 + thi, na_scale, NA, b0, nb);
-                    window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA, b1, nb1);
-                }
-            }
-            if (!whole && prox) {
-                // hits closer than L0 to P0 (azimuth of P0 = phi0 +- pi/2): |X - P0|^2 >= 4 r |d0| sin^2(dpsi / 2)
-                const float arg = 1.01f * sqrtf(L0sq) / (2.0f * sqrtf(ra * ad0));
-                if (!(arg < 0.999f)) {
-                    whole = true;
-                } else {
-                    const float hw = 2.0f * asinf(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
-                    window_bins(psi - hw, psi + hw, na_scale, NA, b2, nb2);
-                }
-            }
-            if (whole || nb >= NA || nb1 >= NA || nb2 >= NA) {
-                b0 = 0, nb = NA, nb1 = 0, nb2 = 0;
-            }
-            // bins -> virtual ranks of the layer (the layer's hits repeated twice, so no wrap)
-            const uint32_t *bs = ix.bin_start + gl * NA;
-            auto P2 = [&](int b) -> uint32_t { return b <= NA ? bs[b] - lbase : lcnt + bs[b - NA] - lbase; };
-            if (nb) {
-                r0.q0 = P2(b0), r0.cnt = P2(b0 + nb) - r0.q0, r0.b0 = b0, r0.nb = nb;
-            }
-            if (nb1) {
-                r1.q0 = P2(b1), r1.cnt = P2(b1 + nb1) - r1.q0, r1.b0 = b1, r1.nb = nb1;
-            }
-            if (nb2) {
-                r2.q0 = P2(b2), r2.cnt = P2(b2 + nb2) - r2.q0, r2.b0 = b2, r2.nb = nb2;
-            }
-        }
-        // lane nL of the group (or lane 0 of a 32-layer detector, as a 2nd task) takes the wild hits
-        uint32_t wild_cnt = 0, wild_base = 0;
-        if (live && gl == (nL < G ? nL : 0)) {
-            wild_base = ix.bin_start[nL * NA];
-            wild_cnt = ix.bin_start[nL * NA + 1] - wild_base;
-        }
-        const uint32_t mine = r0.cnt + r1.cnt + r2.cnt + wild_cnt;
-        uint32_t incl = mine;
-#pragma unroll
-        for (int o = 1; o < G; o <<= 1) {
-            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o, G);
-            if (gl >= o)
-                incl += v;
-        }
-        const uint32_t T = __shfl_sync(0xffffffffu, incl, G - 1, G);
-        s_rng[grp][gl][0] = r0;
-        s_rng[grp][gl][1] = r1;
-        s_rng[grp][gl][2] = r2;
-        s_pre[grp][gl] = incl - mine;
-        if (gl == G - 1)
-            s_pre[grp][G] = T;
-        if (gl == 0)
-            s_cnt[grp] = 0u;
-        __syncwarp();
-
-        // ---- phase 2: the group walks its T candidates, G at a time, with the exact recipe
-        const float c_2 = c_2d0;
-        uint32_t Tw = T; // the warp's groups loop together (warp-wide ballots inside)
-#pragma unroll
-        for (int o = G; o < 32; o <<= 1)
-            Tw = max(Tw, __shfl_xor_sync(0xffffffffu, Tw, o));
-        for (uint32_t c0 = 0; c0 < Tw; c0 += G) {
-            const uint32_t c = c0 + gl;
-            bool match = false;
-            uint32_t hit = 0;
-            if (c < T) {
-                // owner lane (= layer): last l with s_pre[l] <= c
-                int lo = 0;
-#pragma unroll
-                for (int stp = G / 2; stp > 0; stp >>= 1)
-                    if (s_pre[grp][lo + stp] <= c)
-                        lo += stp;
-                uint32_t off = c - s_pre[grp][lo];
-                const PlRange q0 = s_rng[grp][lo][0], q1 = s_rng[grp][lo][1], q2 = s_rng[grp][lo][2];
-                uint32_t rank;
-                bool take = true;
-                int ab = 0;
-                if (off < q0.cnt + q1.cnt + q2.cnt) {
-                    const uint32_t lb = ix.bin_start[lo * NA], lc = ix.bin_start[(lo + 1) * NA] - lb;
-                    int which = 0;
-                    uint32_t q = q0.q0 + off;
-                    if (off >= q0.cnt) {
-                        off -= q0.cnt;
-                        which = 1;
-                        q = q1.q0 + off;
-                        if (off >= q1.cnt) {
-                            off -= q1.cnt;
-                            which = 2;
-                            q = q2.q0 + off;
-                        }
+        for (int l = 0; l < nL; ++l) {
+            if (!((pmask >> l) & 1u))
+                continue;
+            const uint32_t lbase = s_lbase[l], lcnt = s_lbase[l + 1] - lbase;
+            if (!lcnt)
+                continue;
+            // ---- the layer's azimuth windows
+            PlRange r0 = {0u, 0u, 0, 0}, r1 = r0, r2 = r0;
+            {
+                const float ra = s_ra[l], rb = s_rb[l];
+                // binary32 evaluation error of the recipe: |kappa_fp - kappa| <= errnum / den + 2 U K
+                const float Gm = 1.4143f * rb + ad0;
+                const float errnum = 2.0f * (12.0f * U * Gm + 16.0f * U * Kp * Gm * Gm);
+                const float Lmin = fmaxf(0.0f, fmaxf(ra - ad0 * (1.0f + 1e-6f), ad0 * (1.0f - 1e-6f) - rb));
+                const float L0sq = errnum / p.dk; // den >= L0sq: the error stays below one bin
+                float D = Lmin * Lmin;
+                const bool prox = !(D >= L0sq);
+                if (prox)
+                    D = L0sq;
+                const float slack = errnum / D + 2.0f * U * Kp + p.edge_rel * p.dk;
+                const float k1 = ka - slack, k2 = kb + slack;
+                const float g1 = __fmaf_rn(k1, c_d0, 1.0f), g2 = __fmaf_rn(k2, c_d0, 1.0f);
+                bool whole = !(g1 > 0.01f && g2 > 0.01f);
+                int b0 = 0, nb = 0, b1 = 0, nb1 = 0, b2 = 0, nb2 = 0;
+                if (!whole) {
+                    const float A1 = c_d0 * __fmaf_rn(k1, c_d0, 2.0f) / (2.0f * g1), B1 = k1 / (2.0f * g1);
+                    const float A2 = c_d0 * __fmaf_rn(k2, c_d0, 2.0f) / (2.0f * g2), B2 = k2 / (2.0f * g2);
+                    float wlo = fminf(A1 / ra + B1 * ra, A1 / rb + B1 * rb);
+                    float whi = fmaxf(A2 / ra + B2 * ra, A2 / rb + B2 * rb);
+                    if (A1 > 0.0f && B1 > 0.0f) { // W(k1, r) has its minimum 2 sqrt(A B) at r^2 = A / B
+                        const float q = A1 / B1;
+                        if (q > ra * ra && q < rb * rb)
+                            wlo = fminf(wlo, 2.0f * sqrtf(A1 * B1) * (1.0f - 1e-6f));
                     }
-                    rank = lb + (q >= lc ? q - lc : q);
-                    ab = ix.s_abin[rank];
-                    // a hit already seen through an earlier window of the same layer is skipped
-                    if (which >= 1 && (uint32_t)((ab - q0.b0) & (NA - 1)) < (uint32_t)q0.nb)
-                        take = false;
-                    if (which == 2 && (uint32_t)((ab - q1.b0) & (NA - 1)) < (uint32_t)q1.nb)
-                        take = false;
-                } else { // the wild hits
-                    rank = ix.bin_start[nL * NA] + (off - (q0.cnt + q1.cnt + q2.cnt));
-                }
-                if (take) {
-                    const float kappa = eval_kappa(ix.sx[rank], ix.sy[rank], ix.sr2[rank], c_sn, c_cs, c_d0, c_2, c_d0sq);
-                    if ((kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k) {
-                        match = true;
-                        hit = ix.s_hit[rank];
+                    if (A2 < 0.0f && B2 < 0.0f) { // W(k2, r) has its maximum -2 sqrt(A B) at r^2 = A / B
+                        const float q = A2 / B2;
+                        if (q > ra * ra && q < rb * rb)
+                            whi = fmaxf(whi, -2.0f * sqrtf(A2 * B2) * (1.0f - 1e-6f));
+                    }
+                    const float ew = 1e-5f * (1.0f + fmaxf(fabsf(wlo), fabsf(whi)));
+                    wlo -= ew;
+                    whi += ew;
+                    if (!(fabsf(wlo) < 3.0e38f) || !(fabsf(whi) < 3.0e38f) || !(wlo <= whi)) {
+                        whole = true; // inf / NaN somewhere: no bound
+                    } else if (!(wlo > 1.0f) && !(whi < -1.0f)) {
+                        const float tlo = asinf(fmaxf(wlo, -1.0f)) - 2e-5f, thi = asinf(fminf(whi, 1.0f)) + 2e-5f;
+                        window_bins(phi0 + tlo, phi0 + thi, na_scale, NA, b0, nb);
+                        window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA, b1, nb1);
                     }
                 }
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, match) & gmask;
-            if (match) {
-                const uint32_t pos = s_cnt[grp] + (uint32_t)__popc(bal & ((1u << lane) - 1u));
-                if (pos < PL_MAXLIST)
-                    s_list[grp][pos] = hit;
-            }
-            __syncwarp();
-            if (gl == 0)
-                s_cnt[grp] += (uint32_t)__popc(bal);
-            __syncwarp();
-        }
-        if (gl == 0)
-            evals += T;
-
-        // ---- phase 3: staging space (one global atomic per CTA and batch), sort, write
-        __syncthreads();
-        if (tid == 0) {
-            uint32_t tot = 0;
-            for (int q = 0; q < GPC; ++q) {
-                const uint32_t n = s_cnt[q];
-                s_off[q] = tot;
-                tot += n <= PL_MAXLIST ? n : 0u;
-            }
-            s_base = tot ? atomicAdd(p.n_entries, (unsigned long long)tot) : 0ull;
-        }
-        __syncthreads();
-        if (live) {
-            const uint32_t n = s_cnt[grp];
-            if (n > PL_MAXLIST) { // too long for the buffer: counted here, written by k_copy_lists
-                if (gl == 0) {
-                    p.peak_len[pk] = n;
-                    p.peak_pos[pk] = PL_SLOW;
-                }
-            } else {
-                const unsigned long long base = s_base + s_off[grp];
-                const bool fits = base + n <= p.ent_cap;
-                if (gl == 0) {
-                    p.peak_len[pk] = n;
-                    p.peak_pos[pk] = fits ? (uint32_t)base : PL_SLOW;
-                }
-                if (fits)
-                    for (uint32_t a = gl; a < n; a += G) { // rank by counting: the list is short
-                        const uint32_t v = s_list[grp][a];
-                        uint32_t rk = 0;
-                        for (uint32_t b = 0; b < n; ++b)
-                            rk += s_list[grp][b] < v ? 1u : 0u;
-                        p.ent_hit[base + rk] = v;
+                if (!whole && prox) {
+                    // hits closer than L0 to P0 (azimuth of P0 = phi0 +- pi/2): |X - P0|^2 >= 4 r |d0| sin^2(dpsi / 2)
+                    const float arg = 1.01f * sqrtf(L0sq) / (2.0f * sqrtf(ra * ad0));
+                    if (!(arg < 0.999f)) {
+                        whole = true;
+                    } else {
+                        const float hw = 2.0f * asinf(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
+                        window_bins(psi - hw, psi + hw, na_scale, NA, b2, nb2);
                     }
+                }
+                if (whole || nb >= NA || nb1 >= NA || nb2 >= NA) {
+                    b0 = 0, nb = NA, nb1 = 0, nb2 = 0;
+                }
+                // bins -> virtual ranks of the layer (the layer's hits repeated twice, so no wrap)
+                const uint32_t *bs = ix.bin_start + l * NA;
+                auto P2 = [&](int b) -> uint32_t { return b <= NA ? bs[b] - lbase : lcnt + bs[b - NA] - lbase; };
+                if (nb) {
+                    r0.q0 = P2(b0), r0.cnt = P2(b0 + nb) - r0.q0, r0.b0 = b0, r0.nb = nb;
+                }
+                if (nb1) {
+                    r1.q0 = P2(b1), r1.cnt = P2(b1 + nb1) - r1.q0, r1.b0 = b1, r1.nb = nb1;
+                }
+                if (nb2) {
+                    r2.q0 = P2(b2), r2.cnt = P2(b2 + nb2) - r2.q0, r2.b0 = b2, r2.nb = nb2;
+                }
             }
+            // ---- the candidates of the three windows, with the exact recipe
+            const uint32_t tot = r0.cnt + r1.cnt + r2.cnt;
+            for (uint32_t c = 0; c < tot; ++c) {
+                int which = 0;
+                uint32_t off = c, q = r0.q0 + c;
+                if (off >= r0.cnt) {
+                    off -= r0.cnt;
+                    which = 1;
+                    q = r1.q0 + off;
+                    if (off >= r1.cnt) {
+                        off -= r1.cnt;
+                        which = 2;
+                        q = r2.q0 + off;
+                    }
+                }
+                const float4 r = ix.rec[lbase + (q >= lcnt ? q - lcnt : q)];
+                const int ab = (int)(__float_as_uint(r.w) >> 20);
+                // a hit already seen through an earlier window of the same layer is skipped
+                if (which >= 1 && (uint32_t)((ab - r0.b0) & (NA - 1)) < (uint32_t)r0.nb)
+                    continue;
+                if (which == 2 && (uint32_t)((ab - r1.b0) & (NA - 1)) < (uint32_t)r1.nb)
+                    continue;
+                consider(r);
+            }
+            evals += tot;
         }
-        __syncthreads();
+        // the wild hits (outside the index's numeric range) are candidates of every peak
+        for (uint32_t rank = s_lbase[nL]; rank < s_lbase[nL + 1]; ++rank)
+            consider(ix.rec[rank]);
+        evals += s_lbase[nL + 1] - s_lbase[nL];
+        p.peak_len[pk] = cnt;
+        p.peak_pos[pk] = cnt <= p.slot ? 0u : PL_SLOW;
     }
-    if (gl == 0 && evals)
+    for (int o = 16; o > 0; o >>= 1)
+        evals += __shfl_xor_sync(0xffffffffu, evals, o);
+    if (lane == 0 && evals)
         atomicAdd(p.n_list_evals, evals);
 }
 
@@ -452,14 +359,16 @@ struct ListCopyParams {
     const DevCounters *counters;
     uint32_t cap_peaks;
     const uint32_t *bin;
-    const uint32_t *peak_len, *peak_pos, *ent_hit;
+    const uint32_t *peak_len, *peak_pos, *slots;
+    uint32_t slot;
     const unsigned long long *hit_offset;
     uint32_t *hit_index;
     unsigned long long cap_hits;
 };
 
-// hit_index[hit_offset[p] ..] = the staged list of peak p (half a warp per peak); a peak without
-// a staged list (PL_SLOW) is written straight from the hits in index order by a whole warp.
+// hit_index[hit_offset[p] ..] = the staged list of peak p in ascending hit index (half a warp per
+// peak ranks the entries by counting: hit indices are distinct); a peak without a staged list
+// (PL_SLOW) is written straight from the hits in index order by a whole warp.
 template <int MODE>
 __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
 {
@@ -476,10 +385,28 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
             len = p.peak_len[pk];
             dst = p.hit_offset[pk];
         }
-        if (pos != PL_SLOW)
-            for (uint32_t a = hl; a < len; a += 16)
-                if (dst + a < p.cap_hits)
-                    p.hit_index[dst + a] = p.ent_hit[pos + a];
+        if (pos != PL_SLOW && len > 0u) {
+            const uint32_t *src = p.slots + (size_t)pk * p.slot;
+            const unsigned hmask = 0xffffu << (lane & 16);
+            if (len <= 16u) { // one entry per lane, ranks through shuffles
+                const uint32_t v = hl < len ? src[hl] : 0xffffffffu;
+                uint32_t rk = 0;
+#pragma unroll
+                for (int b = 0; b < 16; ++b)
+                    rk += __shfl_sync(hmask, v, b, 16) < v ? 1u : 0u;
+                if (hl < len && dst + rk < p.cap_hits)
+                    p.hit_index[dst + rk] = v;
+            } else {
+                for (uint32_t a = hl; a < len; a += 16) {
+                    const uint32_t v = src[a];
+                    uint32_t rk = 0;
+                    for (uint32_t b = 0; b < len; ++b)
+                        rk += src[b] < v ? 1u : 0u;
+                    if (dst + rk < p.cap_hits)
+                        p.hit_index[dst + rk] = v;
+                }
+            }
+        }
         // slow peaks of this pair, one after the other, by the whole warp
         for (int which = 0; which < 2; ++which) {
             const uint32_t spos = __shfl_sync(0xffffffffu, pos, which * 16);
@@ -515,6 +442,14 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
     }
 }
 
+// Entries of one staging slot: the three entry arrays of the legacy list sweep (3 x cap_hits words,
+// contiguous in the workspace) shared out among cap_peaks peaks.
+static uint32_t slot_entries(const hough_handle *h)
+{
+    const unsigned long long per = 3ull * h->cfg.cap_hits / h->cfg.cap_peaks;
+    return (uint32_t)(per < PL_MAXSLOT ? per : PL_MAXSLOT);
+}
+
 cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
 {
     if (h->n_hits == 0) // no event (hough_set_accumulator): every list is empty, the index is not built
@@ -530,19 +465,15 @@ cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.cap_peaks = h->cfg.cap_peaks;
     p.peak_len = h->peak_len;
     p.peak_pos = h->list_len;
-    p.ent_hit = h->ent_hit;
-    p.ent_cap = h->cfg.cap_hits;
-    p.n_entries = h->n_pairs;
+    p.slots = h->ent_sub;
+    p.slot = slot_entries(h);
     p.n_list_evals = &h->counters->n_list_evals;
     p.dk = (float)(((double)h->g.khi - (double)h->g.klo) / (double)h->g.n_kappa);
     // bin-edge slack in bins: the roundings of (kappa - klo) * inv_dk and of the edges computed here
     const double A = (double)h->g.kabs / ((double)h->g.khi - (double)h->g.klo);
     p.edge_rel = (float)(0.01 + 4e-7 * h->g.n_kappa * (1.0 + A));
-    const int blocks = h->n_sms * 8;
-    if (h->cfg.n_layers <= 15)
-        k_peak_lists<16><<<blocks, 32 * PL_WARPS, 0, st>>>(p);
-    else
-        k_peak_lists<32><<<blocks, 32 * PL_WARPS, 0, st>>>(p);
+    const unsigned blocks = (h->cfg.cap_peaks + PL_THREADS - 1) / PL_THREADS; // CTAs beyond n_peaks return at once
+    k_peak_lists<<<blocks, PL_THREADS, 0, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -561,7 +492,8 @@ cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.bin = out->bin;
     p.peak_len = h->peak_len;
     p.peak_pos = h->list_len;
-    p.ent_hit = h->ent_hit;
+    p.slots = h->ent_sub;
+    p.slot = slot_entries(h);
     p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
     p.hit_index = out->hit_index;
     p.cap_hits = h->cfg.cap_hits;
@@ -622,7 +554,8 @@ cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cu
     p.counters = h->counters;
     p.cap_peaks = h->cfg.cap_peaks;
     p.bin = out->bin;
-    p.peak_len = p.peak_pos = p.ent_hit = nullptr;
+    p.peak_len = p.peak_pos = p.slots = nullptr;
+    p.slot = 0;
     p.hit_offset = nullptr;
     p.hit_index = nullptr;
     p.cap_hits = 0;
