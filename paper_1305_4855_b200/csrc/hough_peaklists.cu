@@ -152,6 +152,7 @@ cudaError_t launch_index_build(hough_handle *h, cudaStream_t st)
 struct PeakListParams {
     GridDev g;
     HitIndexDev ix;
+    ApproxBin ab;
     const float *phic; // [n_phi] bin-centre angles
     uint32_t n_hits;
     const uint32_t *bin, *mask; // reported peaks (k_compact)
@@ -162,33 +163,81 @@ struct PeakListParams {
     uint32_t *slots;    // [cap_peaks][slot] staging
     uint32_t slot;
     unsigned long long *n_list_evals; // candidates evaluated
-    float dk;       // kappa bin width (binary32)
-    float edge_rel; // slack on a bin edge, in bins
+    float dk, inv_dk_w; // kappa bin width (binary32) and its reciprocal (window arithmetic only)
+    float edge_rel;     // slack on a bin edge, in bins
 };
 
-struct PlRange { // candidates of one azimuth window: virtual ranks [q0, q0 + cnt) of the layer, bins [b0, b0 + nb)
-    uint32_t q0, cnt;
-    int b0, nb;
-};
+// The window arithmetic only has to produce SUPERSETS, with the margins stated below; it uses the
+// approximate division / square root units (2 ulp) and a polynomial arc sine instead of the IEEE
+// routines (a third of the instructions).  Nothing here decides a list entry: the exact recipe does.
+__device__ __forceinline__ float fast_sqrt(float x)
+{
+    float r;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+// asin on [-1, 1]: pi/2 - sqrt(1 - |x|) P7(|x|) (Abramowitz & Stegun 4.4.46, |error| <= 2e-8 in exact
+// arithmetic, < 5e-7 in binary32 with the approximate square root; the windows carry 2e-5 rad of slack)
+__device__ __forceinline__ float fast_asin(float x)
+{
+    const float a = fabsf(x);
+    float p = -0.0012624911f;
+    p = __fmaf_rn(p, a, 0.0066700901f);
+    p = __fmaf_rn(p, a, -0.0170881256f);
+    p = __fmaf_rn(p, a, 0.0308918810f);
+    p = __fmaf_rn(p, a, -0.0501743046f);
+    p = __fmaf_rn(p, a, 0.0889789874f);
+    p = __fmaf_rn(p, a, -0.2145988016f);
+    p = __fmaf_rn(p, a, 1.5707963050f);
+    const float r = 1.5707963268f - fast_sqrt(fmaxf(1.0f - a, 0.0f)) * p;
+    return copysignf(r, x);
+}
 
+struct PlWin { // an arc of azimuth bins [b, b + n) on the ring of NA bins; n = 0: absent
+    int b, n;
+};
 // Azimuth window [a_lo, a_hi] (radians, a_lo <= a_hi) -> bins, one extra bin on each side.
-__device__ __forceinline__ void window_bins(float a_lo, float a_hi, float na_scale, int NA, int &b0, int &nb)
+__device__ __forceinline__ PlWin window_bins(float a_lo, float a_hi, float na_scale, int NA)
 {
     const float t0 = floorf((a_lo + PI_F) * na_scale), t1 = floorf((a_hi + PI_F) * na_scale);
     const float span = t1 - t0 + 3.0f;
+    PlWin w;
     if (!(span < (float)NA)) { // also NaN: the whole ring
-        b0 = 0;
-        nb = NA;
-        return;
+        w.b = 0;
+        w.n = NA;
+        return w;
     }
-    b0 = ((int)t0 - 1) & (NA - 1);
-    nb = (int)span;
+    w.b = ((int)t0 - 1) & (NA - 1);
+    w.n = (int)span;
+    return w;
 }
+// If the two arcs overlap, a becomes their union and b disappears (so that no hit is a candidate twice).
+__device__ __forceinline__ void merge_windows(PlWin &a, PlWin &b, int NA)
+{
+    if (a.n == 0 || b.n == 0)
+        return;
+    const int d = (b.b - a.b) & (NA - 1), d2 = (a.b - b.b) & (NA - 1);
+    if (d < a.n) {
+        a.n = max(a.n, d + b.n);
+        b.n = 0;
+    } else if (d2 < b.n) {
+        a.b = b.b;
+        a.n = max(b.n, d2 + a.n);
+        b.n = 0;
+    }
+    if (a.n >= NA) {
+        a.b = 0;
+        a.n = NA;
+    }
+}
+
+#define PL_QCAP 23 // queued candidate ranges per thread
 
 __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams p)
 {
     __shared__ uint32_t s_lbase[34]; // rank of the first hit of layer label l (label nL = the wild hits)
-    __shared__ float s_ra[32], s_rb[32];
+    __shared__ float s_ra[32], s_rb[32], s_ira[32], s_irb[32];
+    __shared__ uint2 s_q[PL_QCAP][PL_THREADS]; // (first virtual rank, count | layer << 24)
 
     const GridDev &g = p.g;
     const HitIndexDev &ix = p.ix;
@@ -199,8 +248,12 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
     if (tid == nL + 1)
         s_lbase[tid] = ix.bin_start[nL * NA + 1];
     if (tid < nL) {
-        s_ra[tid] = __uint_as_float(~ix.layer_r[2 * tid]) * (1.0f - 4e-6f);
-        s_rb[tid] = __uint_as_float(ix.layer_r[2 * tid + 1]) * (1.0f + 4e-6f);
+        const float ra = __uint_as_float(~ix.layer_r[2 * tid]) * (1.0f - 4e-6f);
+        const float rb = __uint_as_float(ix.layer_r[2 * tid + 1]) * (1.0f + 4e-6f);
+        s_ra[tid] = ra;
+        s_rb[tid] = rb;
+        s_ira[tid] = 1.0f / ra;
+        s_irb[tid] = 1.0f / rb;
     }
     __syncthreads();
     const float na_scale = (float)NA * 0.15915494309189535f;
@@ -226,121 +279,147 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
         if (k + 1u == (uint32_t)nk)
             kb = fmaxf(kb, khi);
         const float Kp = 1.01f * g.kabs + p.dk;
-        auto consider = [&](const float4 r) {
-            const float kappa = eval_kappa(r.x, r.y, r.z, c_sn, c_cs, c_d0, c_2d0, c_d0sq);
-            if ((kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k) {
-                if (cnt < p.slot)
-                    slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
-                ++cnt;
-            }
-        };
+        const bool ab_ok = p.ab.ok != 0;
 
-        for (int l = 0; l < nL; ++l) {
-            if (!((pmask >> l) & 1u))
-                continue;
-            const uint32_t lbase = s_lbase[l], lcnt = s_lbase[l + 1] - lbase;
-            if (!lcnt)
-                continue;
-            // ---- the layer's azimuth windows
-            PlRange r0 = {0u, 0u, 0, 0}, r1 = r0, r2 = r0;
-            {
-                const float ra = s_ra[l], rb = s_rb[l];
+        int l = 0;
+        while (l <= nL) {
+            // ---- queue the candidate ranges of as many layers as fit
+            int nq = 0;
+            uint32_t tot = 0;
+            auto push = [&](uint32_t q0, uint32_t n, int layer) {
+                if (n) {
+                    s_q[nq++][tid] = make_uint2(q0, n | ((uint32_t)layer << 24));
+                    tot += n;
+                }
+            };
+            for (; l <= nL && nq + 3 <= PL_QCAP; ++l) {
+                const uint32_t lbase = s_lbase[l], lcnt = s_lbase[l + 1] - lbase;
+                if (l == nL) { // the wild hits (outside the index's numeric range): candidates of every peak
+                    push(0u, lcnt, l);
+                    continue;
+                }
+                if (!((pmask >> l) & 1u) || !lcnt)
+                    continue;
+                const float ra = s_ra[l], rb = s_rb[l], ira = s_ira[l], irb = s_irb[l];
                 // binary32 evaluation error of the recipe: |kappa_fp - kappa| <= errnum / den + 2 U K
                 const float Gm = 1.4143f * rb + ad0;
                 const float errnum = 2.0f * (12.0f * U * Gm + 16.0f * U * Kp * Gm * Gm);
                 const float Lmin = fmaxf(0.0f, fmaxf(ra - ad0 * (1.0f + 1e-6f), ad0 * (1.0f - 1e-6f) - rb));
-                const float L0sq = errnum / p.dk; // den >= L0sq: the error stays below one bin
+                const float L0sq = errnum * p.inv_dk_w * (1.0f + 1e-6f); // den >= L0sq: the error stays below one bin
                 float D = Lmin * Lmin;
                 const bool prox = !(D >= L0sq);
                 if (prox)
                     D = L0sq;
-                const float slack = errnum / D + 2.0f * U * Kp + p.edge_rel * p.dk;
+                const float slack = __fdividef(errnum, D) * (1.0f + 1e-6f) + 2.0f * U * Kp + p.edge_rel * p.dk;
                 const float k1 = ka - slack, k2 = kb + slack;
                 const float g1 = __fmaf_rn(k1, c_d0, 1.0f), g2 = __fmaf_rn(k2, c_d0, 1.0f);
                 bool whole = !(g1 > 0.01f && g2 > 0.01f);
-                int b0 = 0, nb = 0, b1 = 0, nb1 = 0, b2 = 0, nb2 = 0;
+                PlWin w0 = {0, 0}, w1 = {0, 0}, w2 = {0, 0};
                 if (!whole) {
-                    const float A1 = c_d0 * __fmaf_rn(k1, c_d0, 2.0f) / (2.0f * g1), B1 = k1 / (2.0f * g1);
-                    const float A2 = c_d0 * __fmaf_rn(k2, c_d0, 2.0f) / (2.0f * g2), B2 = k2 / (2.0f * g2);
-                    float wlo = fminf(A1 / ra + B1 * ra, A1 / rb + B1 * rb);
-                    float whi = fmaxf(A2 / ra + B2 * ra, A2 / rb + B2 * rb);
-                    if (A1 > 0.0f && B1 > 0.0f) { // W(k1, r) has its minimum 2 sqrt(A B) at r^2 = A / B
-                        const float q = A1 / B1;
-                        if (q > ra * ra && q < rb * rb)
-                            wlo = fminf(wlo, 2.0f * sqrtf(A1 * B1) * (1.0f - 1e-6f));
-                    }
-                    if (A2 < 0.0f && B2 < 0.0f) { // W(k2, r) has its maximum -2 sqrt(A B) at r^2 = A / B
-                        const float q = A2 / B2;
-                        if (q > ra * ra && q < rb * rb)
-                            whi = fmaxf(whi, -2.0f * sqrtf(A2 * B2) * (1.0f - 1e-6f));
-                    }
+                    const float h1 = __fdividef(0.5f, g1), h2 = __fdividef(0.5f, g2);
+                    const float A1 = c_d0 * __fmaf_rn(k1, c_d0, 2.0f) * h1, B1 = k1 * h1;
+                    const float A2 = c_d0 * __fmaf_rn(k2, c_d0, 2.0f) * h2, B2 = k2 * h2;
+                    float wlo = fminf(A1 * ira + B1 * ra, A1 * irb + B1 * rb);
+                    float whi = fmaxf(A2 * ira + B2 * ra, A2 * irb + B2 * rb);
+                    // W(k1, r) has its minimum 2 sqrt(A B) at r^2 = A / B (A, B > 0); the test interval is
+                    // widened so that a rounded end point cannot hide the stationary point
+                    if (A1 > 0.0f && B1 > 0.0f && A1 > 0.999f * ra * ra * B1 && A1 < 1.001f * rb * rb * B1)
+                        wlo = fminf(wlo, 2.0f * fast_sqrt(A1 * B1) * (1.0f - 2e-6f));
+                    // W(k2, r) has its maximum -2 sqrt(A B) at r^2 = A / B (A, B < 0)
+                    if (A2 < 0.0f && B2 < 0.0f && A2 < 0.999f * ra * ra * B2 && A2 > 1.001f * rb * rb * B2)
+                        whi = fmaxf(whi, -2.0f * fast_sqrt(A2 * B2) * (1.0f - 2e-6f));
                     const float ew = 1e-5f * (1.0f + fmaxf(fabsf(wlo), fabsf(whi)));
                     wlo -= ew;
                     whi += ew;
                     if (!(fabsf(wlo) < 3.0e38f) || !(fabsf(whi) < 3.0e38f) || !(wlo <= whi)) {
                         whole = true; // inf / NaN somewhere: no bound
                     } else if (!(wlo > 1.0f) && !(whi < -1.0f)) {
-                        const float tlo = asinf(fmaxf(wlo, -1.0f)) - 2e-5f, thi = asinf(fminf(whi, 1.0f)) + 2e-5f;
-                        window_bins(phi0 + tlo, phi0 + thi, na_scale, NA, b0, nb);
-                        window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA, b1, nb1);
+                        const float tlo = fast_asin(fmaxf(wlo, -1.0f)) - 2e-5f, thi = fast_asin(fminf(whi, 1.0f)) + 2e-5f;
+                        w0 = window_bins(phi0 + tlo, phi0 + thi, na_scale, NA);
+                        w1 = window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA);
                     }
                 }
                 if (!whole && prox) {
                     // hits closer than L0 to P0 (azimuth of P0 = phi0 +- pi/2): |X - P0|^2 >= 4 r |d0| sin^2(dpsi / 2)
-                    const float arg = 1.01f * sqrtf(L0sq) / (2.0f * sqrtf(ra * ad0));
+                    const float arg = 0.5051f * fast_sqrt(__fdividef(L0sq, ra * ad0));
                     if (!(arg < 0.999f)) {
                         whole = true;
                     } else {
-                        const float hw = 2.0f * asinf(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
-                        window_bins(psi - hw, psi + hw, na_scale, NA, b2, nb2);
+                        const float hw = 2.0f * fast_asin(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
+                        w2 = window_bins(psi - hw, psi + hw, na_scale, NA);
                     }
                 }
-                if (whole || nb >= NA || nb1 >= NA || nb2 >= NA) {
-                    b0 = 0, nb = NA, nb1 = 0, nb2 = 0;
+                if (!whole) { // disjoint arcs
+                    merge_windows(w0, w1, NA);
+                    if (w2.n) {
+                        merge_windows(w0, w2, NA);
+                        merge_windows(w1, w2, NA);
+                        merge_windows(w0, w1, NA);
+                    }
+                    whole = w0.n >= NA || w1.n >= NA || w2.n >= NA;
+                }
+                if (whole) {
+                    push(0u, lcnt, l);
+                    continue;
                 }
                 // bins -> virtual ranks of the layer (the layer's hits repeated twice, so no wrap)
                 const uint32_t *bs = ix.bin_start + l * NA;
                 auto P2 = [&](int b) -> uint32_t { return b <= NA ? bs[b] - lbase : lcnt + bs[b - NA] - lbase; };
-                if (nb) {
-                    r0.q0 = P2(b0), r0.cnt = P2(b0 + nb) - r0.q0, r0.b0 = b0, r0.nb = nb;
+                if (w0.n) {
+                    const uint32_t q0 = P2(w0.b);
+                    push(q0, P2(w0.b + w0.n) - q0, l);
                 }
-                if (nb1) {
-                    r1.q0 = P2(b1), r1.cnt = P2(b1 + nb1) - r1.q0, r1.b0 = b1, r1.nb = nb1;
+                if (w1.n) {
+                    const uint32_t q0 = P2(w1.b);
+                    push(q0, P2(w1.b + w1.n) - q0, l);
                 }
-                if (nb2) {
-                    r2.q0 = P2(b2), r2.cnt = P2(b2 + nb2) - r2.q0, r2.b0 = b2, r2.nb = nb2;
+                if (w2.n) {
+                    const uint32_t q0 = P2(w2.b);
+                    push(q0, P2(w2.b + w2.n) - q0, l);
                 }
             }
-            // ---- the candidates of the three windows, with the exact recipe
-            const uint32_t tot = r0.cnt + r1.cnt + r2.cnt;
-            for (uint32_t c = 0; c < tot; ++c) {
-                int which = 0;
-                uint32_t off = c, q = r0.q0 + c;
-                if (off >= r0.cnt) {
-                    off -= r0.cnt;
-                    which = 1;
-                    q = r1.q0 + off;
-                    if (off >= r1.cnt) {
-                        off -= r1.cnt;
-                        which = 2;
-                        q = r2.q0 + off;
-                    }
+            // ---- one flat loop over the queued candidates, with the exact recipe (the fixed-point
+            // estimate first where it is admissible, as in the vote: hough_device.cuh approx_bin)
+            uint32_t rem = 0, q = 0, lb = 0, lc = 0;
+            int e = 0;
+            for (uint32_t t = 0; t < tot; ++t) {
+                if (rem == 0u) {
+                    const uint2 en = s_q[e++][tid];
+                    q = en.x;
+                    rem = en.y & 0xffffffu;
+                    const int ll = (int)(en.y >> 24);
+                    lb = s_lbase[ll];
+                    lc = s_lbase[ll + 1] - lb;
                 }
-                const float4 r = ix.rec[lbase + (q >= lcnt ? q - lcnt : q)];
-                const int ab = (int)(__float_as_uint(r.w) >> 20);
-                // a hit already seen through an earlier window of the same layer is skipped
-                if (which >= 1 && (uint32_t)((ab - r0.b0) & (NA - 1)) < (uint32_t)r0.nb)
-                    continue;
-                if (which == 2 && (uint32_t)((ab - r1.b0) & (NA - 1)) < (uint32_t)r1.nb)
-                    continue;
-                consider(r);
+                const float4 r = ix.rec[lb + (q >= lc ? q - lc : q)];
+                ++q;
+                --rem;
+                const float a = __fmul_rn(r.x, c_sn);
+                const float b = __fmul_rn(r.y, c_cs);
+                const float sv = __fsub_rn(b, a);
+                const float ee = __fsub_rn(sv, c_d0);
+                const float den = __fadd_rn(__fsub_rn(r.z, __fmul_rn(c_2d0, sv)), c_d0sq);
+                bool match;
+                uint32_t tb = 0;
+                const bool fast = ab_ok && !hit_is_wild(r.z);
+                if (fast)
+                    tb = approx_bin(ee, den, p.ab.c1, p.ab.c0);
+                if (fast && !(tb < p.ab.lim)) {
+                    match = false;
+                } else if (fast && (tb & 0xffffu) >= p.ab.edge) {
+                    match = (tb >> APPROX_FRAC_BITS) == k;
+                } else {
+                    const float kappa = __fdiv_rn(__fadd_rn(ee, ee), den);
+                    match = (kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k;
+                }
+                if (match) {
+                    if (cnt < p.slot)
+                        slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
+                    ++cnt;
+                }
             }
             evals += tot;
         }
-        // the wild hits (outside the index's numeric range) are candidates of every peak
-        for (uint32_t rank = s_lbase[nL]; rank < s_lbase[nL + 1]; ++rank)
-            consider(ix.rec[rank]);
-        evals += s_lbase[nL + 1] - s_lbase[nL];
         p.peak_len[pk] = cnt;
         p.peak_pos[pk] = cnt <= p.slot ? 0u : PL_SLOW;
     }
@@ -468,7 +547,9 @@ cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.slots = h->ent_sub;
     p.slot = slot_entries(h);
     p.n_list_evals = &h->counters->n_list_evals;
+    p.ab = h->ab;
     p.dk = (float)(((double)h->g.khi - (double)h->g.klo) / (double)h->g.n_kappa);
+    p.inv_dk_w = (float)((double)h->g.n_kappa / ((double)h->g.khi - (double)h->g.klo));
     // bin-edge slack in bins: the roundings of (kappa - klo) * inv_dk and of the edges computed here
     const double A = (double)h->g.kabs / ((double)h->g.khi - (double)h->g.klo);
     p.edge_rel = (float)(0.01 + 4e-7 * h->g.n_kappa * (1.0 + A));
