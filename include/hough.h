@@ -72,6 +72,13 @@ extern "C" {
 #define HOUGH_OPT_INTERVAL 64u    /* f3, interval voting (recipe E2): a hit sets every kappa bin
                                      between its closed-form values at the two EDGES of phi0 bin i (d0 centre j);
                                      n_votes counts the bins set.  Not together with HOUGH_OPT_LINE */
+#define HOUGH_OPT_FUSED_PEAKS 128u /* a5, fused variant (north_star: "peak finding is fused on the tile"): hough_vote's
+                                     tile kernel decides the peak flags of the cells that are not on the edge of its
+                                     tile from shared memory, hough_peaks only visits the tile-edge cells
+                                     (k_peak_cells) instead of sweeping the whole accumulator.  Needs n_layers <= 16
+                                     and not HOUGH_OPT_UNPACKED.  Results are identical either way */
+#define HOUGH_OPT_CELL_PEAKS 256u /* peak flags of EVERY cell by the cell-wise kernel (k_peak_cells) instead of the
+                                     streaming sweep: cross-check and measurement of that kernel */
 #define HOUGH_OPT_UNPACKED 4u     /* one mask per 32-bit word of the vote tile even with <= 16 layers (test hook
                                      for the tile layout used with 17..32 layers) */
 

@@ -159,6 +159,8 @@ static int cfg_valid(const hough_config *c)
         return 0; // max_hits beyond what the hit-list segmentation supports
     if ((c->options & HOUGH_OPT_LINE) && (c->options & HOUGH_OPT_INTERVAL))
         return 0;
+    if ((c->options & HOUGH_OPT_FUSED_PEAKS) && (c->n_layers > 16 || (c->options & HOUGH_OPT_UNPACKED)))
+        return 0; // the fused test works on the two-masks-per-word tile
     if ((c->options & HOUGH_OPT_LINE) && c->n_d0 != 1)
         return 0; // the straight-line transform has two parameters (theta, rho)
     return 1;
@@ -589,7 +591,14 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
         return HOUGH_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CK(cudaMemsetAsync((unsigned char *)h->counters + 64, 0, 192 + (size_t)2 * h->scan_blocks_max * 8, st));
-    CK(launch_peak_sweep(h, st));
+    // a5: the streaming sweep; or, fused variant, only the cells on the vote tiles' edges (the others were
+    // flagged by hough_vote's kernel -- not after hough_set_accumulator, which leaves no such flags)
+    if ((h->cfg.options & HOUGH_OPT_FUSED_PEAKS) && h->fused_valid)
+        CK(launch_peak_cells(h, 1, st));
+    else if (h->cfg.options & HOUGH_OPT_CELL_PEAKS)
+        CK(launch_peak_cells(h, 0, st));
+    else
+        CK(launch_peak_sweep(h, st));
     stage_mark(h, ST_PEAK_SWEEP + 1, st);
     CK(launch_scan_rows(h, st));
     stage_mark(h, ST_SCAN_ROWS + 1, st);
@@ -648,6 +657,7 @@ int hough_set_accumulator(hough_handle *h, const uint32_t *acc_dev, void *cuda_s
     CK(cudaMemsetAsync(h->counters, 0, 64, (cudaStream_t)cuda_stream));
     h->n_hits = 0;
     h->voted = 1;
+    h->fused_valid = 0;
     return HOUGH_OK;
 }
 

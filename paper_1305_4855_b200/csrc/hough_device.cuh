@@ -234,3 +234,44 @@ __device__ __forceinline__ bool hit_may_vote(float x, float y, float r2, const T
     return !(gmin > rhs);
 }
 
+
+// ------------------------------------------------------------------ peak rule on popcount pairs
+// A6 on 8 consecutive kappa bins of one (phi0, d0) cell (the fused / cell-wise peak test: k_sweep's
+// epilogue and k_peak_cells).  A Strip holds popcounts as u16 pairs: word x[t] = bins 2t (low half) and
+// 2t + 1 (high half) of the 8 bins, m = the word before (only its high half, bin -1, is used), p = the
+// word after (only its low half, bin 8).  C = the cell itself, L = the bin-wise maximum over its
+// neighbour cells of LOWER linear index, H = over those of HIGHER linear index (absent bins = 0).
+// A bin is a peak iff pc >= L_min, pc > every lower-lin neighbour, pc >= every higher-lin neighbour.
+struct Strip {
+    uint32_t m, x[4], p;
+};
+__device__ __forceinline__ void strip_max(Strip &a, const Strip &b)
+{
+    a.m = __vmaxu2(a.m, b.m);
+    a.p = __vmaxu2(a.p, b.p);
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+        a.x[t] = __vmaxu2(a.x[t], b.x[t]);
+}
+__device__ __forceinline__ uint32_t peak_flags8(const Strip &C, const Strip &L, const Strip &H, uint32_t lmin2)
+{
+    const uint32_t HB = 0x80008000u, ONE = 0x00010001u;
+    uint32_t byte = 0;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        const uint32_t pC = t ? C.x[t - 1] : C.m, nC = t < 3 ? C.x[t + 1] : C.p;
+        const uint32_t pL = t ? L.x[t - 1] : L.m, nL = t < 3 ? L.x[t + 1] : L.p;
+        const uint32_t pH = t ? H.x[t - 1] : H.m, nH = t < 3 ? H.x[t + 1] : H.p;
+        // (bin - 1, bin) and (bin + 1, bin + 2) re-paired so that every half sits beside its neighbour
+        const uint32_t lfC = __byte_perm(pC, C.x[t], 0x5432), rtC = __byte_perm(C.x[t], nC, 0x5432);
+        const uint32_t lfL = __byte_perm(pL, L.x[t], 0x5432), rtL = __byte_perm(L.x[t], nL, 0x5432);
+        const uint32_t lfH = __byte_perm(pH, H.x[t], 0x5432), rtH = __byte_perm(H.x[t], nH, 0x5432);
+        const uint32_t lo = __vmaxu2(__vimax3_u16x2(lfL, L.x[t], rtL), lfC);
+        const uint32_t hi = __vimax3_u16x2(__vimax3_u16x2(lfH, H.x[t], rtH), rtC, lmin2);
+        const uint32_t thr = __vmaxu2(lo + ONE, hi);
+        const uint32_t res = (C.x[t] | HB) - thr; // bit 15 / 31: the half reaches its threshold
+        byte |= ((res >> 15) & 1u) << (2 * t);
+        byte |= (res >> 31) << (2 * t + 1);
+    }
+    return byte;
+}

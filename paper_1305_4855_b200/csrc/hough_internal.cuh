@@ -149,6 +149,7 @@ struct hough_handle {
     // state
     uint32_t n_hits;
     int voted;
+    int fused_valid;     // HOUGH_OPT_FUSED_PEAKS: the last hough_vote left the interior cells' peak flags
     uint64_t launches;
     // HOUGH_OPT_STAGE_TIMING: ev[0] = start of hough_vote, ev[s + 1] = end of stage s
     int timing;
@@ -170,6 +171,7 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
 cudaError_t launch_vote(hough_handle *h, cudaStream_t st);
 cudaError_t launch_clear(hough_handle *h, cudaStream_t st);
 cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st);
+cudaError_t launch_peak_cells(hough_handle *h, int edge_cells_only, cudaStream_t st);
 cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st);
 cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);

@@ -163,6 +163,7 @@ struct PeakListParams {
     uint32_t *slots;    // [cap_peaks][slot] staging
     uint32_t slot;
     unsigned long long *n_list_evals; // candidates evaluated
+    unsigned long long *work;         // next peak to hand out (zeroed per hough_peaks)
     float dk, inv_dk_w; // kappa bin width (binary32) and its reciprocal (window arithmetic only)
     float edge_rel;     // slack on a bin edge, in bins
 };
@@ -231,13 +232,13 @@ __device__ __forceinline__ void merge_windows(PlWin &a, PlWin &b, int NA)
     }
 }
 
-#define PL_QCAP 23 // queued candidate ranges per thread
+#define PL_QCAP 40 // queued candidate ranges per thread (first rank | count << 20)
 
 __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams p)
 {
     __shared__ uint32_t s_lbase[34]; // rank of the first hit of layer label l (label nL = the wild hits)
     __shared__ float s_ra[32], s_rb[32], s_ira[32], s_irb[32];
-    __shared__ uint2 s_q[PL_QCAP][PL_THREADS]; // (first virtual rank, count | layer << 24)
+    __shared__ uint32_t s_q[PL_QCAP][PL_THREADS];
 
     const GridDev &g = p.g;
     const HitIndexDev &ix = p.ix;
@@ -261,10 +262,20 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
     const int nk = g.n_kappa;
     const float klo = g.klo, khi = g.khi, inv_dk = g.inv_dk;
     const float U = 5.9604645e-08f; // 2^-24
-    const uint32_t pk = blockIdx.x * PL_THREADS + tid;
     unsigned long long evals = 0;
 
-    if (pk < n_rep) {
+    // the warps draw 32 peaks at a time from a global counter (lists differ in length: a static split
+    // leaves the last wave of CTAs a third empty)
+    for (;;) {
+        unsigned long long base = 0;
+        if (lane == 0)
+            base = atomicAdd(p.work, 32ull);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= n_rep)
+            break;
+        const uint32_t pk = (uint32_t)base + lane;
+        if (pk >= n_rep)
+            continue;
         const uint32_t lin = p.bin[pk], pmask = p.mask[pk];
         const uint32_t k = lin % (uint32_t)nk, row = lin / (uint32_t)nk;
         const uint32_t j = row % (uint32_t)g.n_d0, i = row / (uint32_t)g.n_d0;
@@ -281,21 +292,60 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
         const float Kp = 1.01f * g.kabs + p.dk;
         const bool ab_ok = p.ab.ok != 0;
 
+        // one candidate with the exact recipe (the fixed-point estimate first where it is admissible,
+        // as in the vote: hough_device.cuh approx_bin)
+        auto consider = [&](const float4 r) {
+            const float a = __fmul_rn(r.x, c_sn);
+            const float b = __fmul_rn(r.y, c_cs);
+            const float sv = __fsub_rn(b, a);
+            const float ee = __fsub_rn(sv, c_d0);
+            const float den = __fadd_rn(__fsub_rn(r.z, __fmul_rn(c_2d0, sv)), c_d0sq);
+            bool match;
+            uint32_t tb = 0;
+            const bool fast = ab_ok && !hit_is_wild(r.z);
+            if (fast)
+                tb = approx_bin(ee, den, p.ab.c1, p.ab.c0);
+            if (fast && !(tb < p.ab.lim)) {
+                match = false;
+            } else if (fast && (tb & 0xffffu) >= p.ab.edge) {
+                match = (tb >> APPROX_FRAC_BITS) == k;
+            } else {
+                const float kappa = __fdiv_rn(__fadd_rn(ee, ee), den);
+                match = (kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k;
+            }
+            if (match) {
+                if (cnt < p.slot)
+                    slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
+                ++cnt;
+            }
+        };
+
         int l = 0;
         while (l <= nL) {
-            // ---- queue the candidate ranges of as many layers as fit
+            // ---- queue the candidate ranges (physical ranks of the key-ordered records) of as many
+            // layers as fit; a range too long for a queue entry is walked on the spot
             int nq = 0;
-            uint32_t tot = 0;
-            auto push = [&](uint32_t q0, uint32_t n, int layer) {
-                if (n) {
-                    s_q[nq++][tid] = make_uint2(q0, n | ((uint32_t)layer << 24));
-                    tot += n;
+            auto push = [&](uint32_t rank0, uint32_t n) {
+                if (n > 4095u) {
+                    for (uint32_t c = 0; c < n; ++c)
+                        consider(ix.rec[rank0 + c]);
+                } else if (n) {
+                    s_q[nq++][tid] = rank0 | (n << 20);
                 }
+                evals += n;
             };
-            for (; l <= nL && nq + 3 <= PL_QCAP; ++l) {
+            // virtual ranks [q0, q0 + n) of a layer whose hits are thought repeated twice
+            auto push_virtual = [&](uint32_t lbase, uint32_t lcnt, uint32_t q0, uint32_t n) {
+                if (q0 >= lcnt)
+                    q0 -= lcnt;
+                const uint32_t first = min(n, lcnt - q0);
+                push(lbase + q0, first);
+                push(lbase, n - first);
+            };
+            for (; l <= nL && nq + 6 <= PL_QCAP; ++l) {
                 const uint32_t lbase = s_lbase[l], lcnt = s_lbase[l + 1] - lbase;
                 if (l == nL) { // the wild hits (outside the index's numeric range): candidates of every peak
-                    push(0u, lcnt, l);
+                    push(lbase, lcnt);
                     continue;
                 }
                 if (!((pmask >> l) & 1u) || !lcnt)
@@ -359,66 +409,52 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                     whole = w0.n >= NA || w1.n >= NA || w2.n >= NA;
                 }
                 if (whole) {
-                    push(0u, lcnt, l);
+                    push(lbase, lcnt);
                     continue;
                 }
-                // bins -> virtual ranks of the layer (the layer's hits repeated twice, so no wrap)
+                // bins -> virtual ranks of the layer (its hits repeated twice, so an arc never wraps)
                 const uint32_t *bs = ix.bin_start + l * NA;
                 auto P2 = [&](int b) -> uint32_t { return b <= NA ? bs[b] - lbase : lcnt + bs[b - NA] - lbase; };
                 if (w0.n) {
                     const uint32_t q0 = P2(w0.b);
-                    push(q0, P2(w0.b + w0.n) - q0, l);
+                    push_virtual(lbase, lcnt, q0, P2(w0.b + w0.n) - q0);
                 }
                 if (w1.n) {
                     const uint32_t q0 = P2(w1.b);
-                    push(q0, P2(w1.b + w1.n) - q0, l);
+                    push_virtual(lbase, lcnt, q0, P2(w1.b + w1.n) - q0);
                 }
                 if (w2.n) {
                     const uint32_t q0 = P2(w2.b);
-                    push(q0, P2(w2.b + w2.n) - q0, l);
+                    push_virtual(lbase, lcnt, q0, P2(w2.b + w2.n) - q0);
                 }
             }
-            // ---- one flat loop over the queued candidates, with the exact recipe (the fixed-point
-            // estimate first where it is admissible, as in the vote: hough_device.cuh approx_bin)
-            uint32_t rem = 0, q = 0, lb = 0, lc = 0;
+            // ---- one flat loop over the queued candidates; the next record is loaded before the
+            // current one is evaluated
             int e = 0;
-            for (uint32_t t = 0; t < tot; ++t) {
+            uint32_t rem = 0, rank = 0;
+            float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
+            bool have = false;
+            auto advance = [&]() {
                 if (rem == 0u) {
-                    const uint2 en = s_q[e++][tid];
-                    q = en.x;
-                    rem = en.y & 0xffffffu;
-                    const int ll = (int)(en.y >> 24);
-                    lb = s_lbase[ll];
-                    lc = s_lbase[ll + 1] - lb;
+                    if (e == nq) {
+                        have = false;
+                        return;
+                    }
+                    const uint32_t en = s_q[e++][tid];
+                    rank = en & 0xfffffu;
+                    rem = en >> 20;
                 }
-                const float4 r = ix.rec[lb + (q >= lc ? q - lc : q)];
-                ++q;
+                nxt = ix.rec[rank];
+                ++rank;
                 --rem;
-                const float a = __fmul_rn(r.x, c_sn);
-                const float b = __fmul_rn(r.y, c_cs);
-                const float sv = __fsub_rn(b, a);
-                const float ee = __fsub_rn(sv, c_d0);
-                const float den = __fadd_rn(__fsub_rn(r.z, __fmul_rn(c_2d0, sv)), c_d0sq);
-                bool match;
-                uint32_t tb = 0;
-                const bool fast = ab_ok && !hit_is_wild(r.z);
-                if (fast)
-                    tb = approx_bin(ee, den, p.ab.c1, p.ab.c0);
-                if (fast && !(tb < p.ab.lim)) {
-                    match = false;
-                } else if (fast && (tb & 0xffffu) >= p.ab.edge) {
-                    match = (tb >> APPROX_FRAC_BITS) == k;
-                } else {
-                    const float kappa = __fdiv_rn(__fadd_rn(ee, ee), den);
-                    match = (kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k;
-                }
-                if (match) {
-                    if (cnt < p.slot)
-                        slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
-                    ++cnt;
-                }
+                have = true;
+            };
+            advance();
+            while (have) {
+                const float4 r = nxt;
+                advance();
+                consider(r);
             }
-            evals += tot;
         }
         p.peak_len[pk] = cnt;
         p.peak_pos[pk] = cnt <= p.slot ? 0u : PL_SLOW;
@@ -553,8 +589,11 @@ cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     // bin-edge slack in bins: the roundings of (kappa - klo) * inv_dk and of the edges computed here
     const double A = (double)h->g.kabs / ((double)h->g.khi - (double)h->g.klo);
     p.edge_rel = (float)(0.01 + 4e-7 * h->g.n_kappa * (1.0 + A));
-    const unsigned blocks = (h->cfg.cap_peaks + PL_THREADS - 1) / PL_THREADS; // CTAs beyond n_peaks return at once
-    k_peak_lists<<<blocks, PL_THREADS, 0, st>>>(p);
+    p.work = h->n_pairs;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_peak_lists, PL_THREADS, 0) != cudaSuccess || per_sm < 1)
+        per_sm = 4;
+    k_peak_lists<<<h->n_sms * per_sm, PL_THREADS, 0, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }

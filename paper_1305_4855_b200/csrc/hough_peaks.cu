@@ -13,7 +13,7 @@
 // and >= every neighbour of higher lin.
 #include <type_traits>
 
-#include "hough_internal.cuh"
+#include "hough_device.cuh"
 
 // ------------------------------------------------------------------ clear
 __global__ void k_clear(uint4 *acc, size_t n_vec)
@@ -276,6 +276,104 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
     const int Tj = 2 * p.JW - 2;
     dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
     k_peak_sweep<2, 8><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+    h->launches += 1;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ cell-wise peak test
+// The same rule, one warp per (cell, 256-bin segment), lane = 8 bins, straight from the global
+// accumulator (9 cell rows per cell).  With HOUGH_OPT_FUSED_PEAKS it visits only the cells on the edge
+// of a vote tile -- the others were decided by k_sweep's epilogue from shared memory -- and with
+// HOUGH_OPT_CELL_PEAKS every cell (cross-check of k_peak_sweep, which reads every row once instead).
+struct CellPeakParams {
+    const uint32_t *acc;
+    unsigned char *flags;
+    int n_phi, n_d0, nk, L_min, wrap;
+    int edge_only;
+    int P, D, n_big, P_small; // vote tile geometry (SweepGeom)
+};
+
+__device__ __forceinline__ Strip strip_from_masks(const uint32_t *__restrict__ row, int k0, int nk)
+{
+    const uint4 a = *reinterpret_cast<const uint4 *>(row + k0), b = *reinterpret_cast<const uint4 *>(row + k0 + 4);
+    Strip s;
+    s.x[0] = popc_pair(a.x, a.y);
+    s.x[1] = popc_pair(a.z, a.w);
+    s.x[2] = popc_pair(b.x, b.y);
+    s.x[3] = popc_pair(b.z, b.w);
+    s.m = k0 > 0 ? ((uint32_t)__popc(row[k0 - 1]) << 16) : 0u;
+    s.p = k0 + 8 < nk ? (uint32_t)__popc(row[k0 + 8]) : 0u;
+    return s;
+}
+
+__global__ void __launch_bounds__(256) k_peak_cells(const CellPeakParams p)
+{
+    const int lane = threadIdx.x & 31;
+    const int nseg = (p.nk + 255) >> 8;
+    const uint32_t n_items = (uint32_t)p.n_phi * (uint32_t)p.n_d0 * (uint32_t)nseg;
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t lmin2 = (uint32_t)p.L_min * 0x00010001u;
+    for (uint32_t item = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; item < n_items; item += warps) {
+        const int cell = (int)(item / (uint32_t)nseg), seg = (int)(item - (uint32_t)cell * (uint32_t)nseg);
+        const int i = cell / p.n_d0, j = cell - i * p.n_d0;
+        if (p.edge_only) { // position of the cell in its vote tile (two slab heights)
+            const int big = p.n_big * p.P;
+            const int Pt = i < big ? p.P : p.P_small;
+            const int i0 = i < big ? (i / p.P) * p.P : big + ((i - big) / p.P_small) * p.P_small;
+            const int j0 = (j / p.D) * p.D;
+            const int ni = min(Pt, p.n_phi - i0), nj = min(p.D, p.n_d0 - j0);
+            const int il = i - i0, jl = j - j0;
+            if (il > 0 && il < ni - 1 && jl > 0 && jl < nj - 1)
+                continue;
+        }
+        const int k0 = seg * 256 + lane * 8;
+        if (k0 >= p.nk)
+            continue;
+        const Strip C = strip_from_masks(p.acc + (size_t)cell * p.nk, k0, p.nk);
+        Strip L, H;
+        L.m = L.p = H.m = H.p = 0u;
+#pragma unroll
+        for (int t = 0; t < 4; ++t)
+            L.x[t] = H.x[t] = 0u;
+        for (int di = -1; di <= 1; ++di) {
+            int ii = i + di;
+            if (ii < 0 || ii >= p.n_phi) {
+                if (!p.wrap)
+                    continue;
+                ii = ii < 0 ? ii + p.n_phi : ii - p.n_phi;
+            }
+            for (int dj = -1; dj <= 1; ++dj) {
+                const int jj = j + dj;
+                if ((di == 0 && dj == 0) || jj < 0 || jj >= p.n_d0)
+                    continue;
+                const int ncell = ii * p.n_d0 + jj; // the neighbour's own linear order decides the tie rule
+                const Strip S = strip_from_masks(p.acc + (size_t)ncell * p.nk, k0, p.nk);
+                if (ncell < cell)
+                    strip_max(L, S);
+                else
+                    strip_max(H, S);
+            }
+        }
+        p.flags[(size_t)cell * (size_t)(p.nk >> 3) + (size_t)(k0 >> 3)] = (unsigned char)peak_flags8(C, L, H, lmin2);
+    }
+}
+
+cudaError_t launch_peak_cells(hough_handle *h, int edge_cells_only, cudaStream_t st)
+{
+    CellPeakParams p;
+    p.acc = h->acc;
+    p.flags = reinterpret_cast<unsigned char *>(h->flags);
+    p.n_phi = h->g.n_phi;
+    p.n_d0 = h->g.n_d0;
+    p.nk = h->g.n_kappa;
+    p.L_min = h->g.L_min;
+    p.wrap = h->g.phi_wrap;
+    p.edge_only = edge_cells_only;
+    p.P = h->vote_geom.P;
+    p.D = h->vote_geom.D;
+    p.n_big = h->vote_geom.n_big;
+    p.P_small = h->vote_geom.P_small;
+    k_peak_cells<<<h->n_sms * 8, 256, 0, st>>>(p);
     h->launches += 1;
     return cudaGetLastError();
 }

@@ -19,6 +19,7 @@ struct SweepParams {
     unsigned long long *n_votes;
     unsigned long long *n_evals;
     ApproxBin ab;
+    unsigned char *fused_flags; // HOUGH_OPT_FUSED_PEAKS: peak-flag bytes of the tile's interior cells (else NULL)
 };
 
 // APPROX: bins come from the fixed-point estimate wherever it provably equals the exact
@@ -284,6 +285,70 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 *reinterpret_cast<uint4 *>(p.acc + lin) = o;
             }
         }
+        // ---- a5, fused variant (HOUGH_OPT_FUSED_PEAKS; BASELINE.json north_star: "peak finding is fused on
+        // the tile"): the cells that are not on the tile's edge have all their 26 neighbours in this
+        // tile, so their peak flags are decided here, from shared memory; the edge cells are left to
+        // k_peak_cells (hough_peaks.cu).
+        if (PACK == 2 && p.fused_flags != nullptr && ni > 2 && nj > 2) {
+            const int W = nk >> 1, G = W >> 2; // words and 16-byte groups per cell row
+            __syncthreads();                   // the write-out has read the masks
+            // in place: masks -> popcount pairs, and the row swizzle undone (logical group q, word t sits
+            // at group q ^ a, word t ^ b): groups q and q ^ a trade places, one thread does both
+            for (int idx = tid; idx < Pt * ge.D * G; idx += ge.threads) {
+                const int cc = idx / G, q = idx - cc * G;
+                const int sw = (cc & 31) & p.swz_mask, q2 = q ^ (sw >> 2);
+                if (q2 < q)
+                    continue;
+                uint4 *row = reinterpret_cast<uint4 *>(tile + (size_t)cc * W);
+                auto conv = [&](uint4 v) -> uint4 {
+                    if (sw & 1) {
+                        uint32_t t0 = v.x; v.x = v.y; v.y = t0;
+                        t0 = v.z; v.z = v.w; v.w = t0;
+                    }
+                    if (sw & 2) {
+                        uint32_t t0 = v.x; v.x = v.z; v.z = t0;
+                        t0 = v.y; v.y = v.w; v.w = t0;
+                    }
+                    v.x = (uint32_t)__popc(v.x & 0xffffu) | ((uint32_t)__popc(v.x >> 16) << 16);
+                    v.y = (uint32_t)__popc(v.y & 0xffffu) | ((uint32_t)__popc(v.y >> 16) << 16);
+                    v.z = (uint32_t)__popc(v.z & 0xffffu) | ((uint32_t)__popc(v.z >> 16) << 16);
+                    v.w = (uint32_t)__popc(v.w & 0xffffu) | ((uint32_t)__popc(v.w >> 16) << 16);
+                    return v;
+                };
+                const uint4 g1 = row[q], g2 = row[q2];
+                row[q] = conv(g2);
+                if (q2 != q)
+                    row[q2] = conv(g1);
+            }
+            __syncthreads();
+            const int nseg = (G + 31) >> 5, wj = nj - 2, n_items = (ni - 2) * wj * nseg;
+            const uint32_t lmin2 = (uint32_t)g.L_min * 0x00010001u;
+            auto load = [&](int cil, int cjl, int q) -> Strip {
+                const uint32_t *row = tile + (size_t)(cil * ge.D + cjl) * W;
+                const uint4 v = *reinterpret_cast<const uint4 *>(row + 4 * q);
+                Strip s;
+                s.x[0] = v.x, s.x[1] = v.y, s.x[2] = v.z, s.x[3] = v.w;
+                s.m = q > 0 ? row[4 * q - 1] : 0u;
+                s.p = q + 1 < G ? row[4 * q + 4] : 0u;
+                return s;
+            };
+            for (int item = warp; item < n_items; item += nwarps) {
+                const int ic = item / nseg, q = (item - ic * nseg) * 32 + lane;
+                const int cil = 1 + ic / wj, cjl = 1 + ic % wj;
+                if (q >= G)
+                    continue;
+                const Strip C = load(cil, cjl, q);
+                Strip L = load(cil - 1, cjl - 1, q), H = load(cil + 1, cjl + 1, q);
+                strip_max(L, load(cil - 1, cjl, q));
+                strip_max(L, load(cil - 1, cjl + 1, q));
+                strip_max(L, load(cil, cjl - 1, q));
+                strip_max(H, load(cil, cjl + 1, q));
+                strip_max(H, load(cil + 1, cjl - 1, q));
+                strip_max(H, load(cil + 1, cjl, q));
+                const size_t rowg = (size_t)(i0 + cil) * g.n_d0 + (j0 + cjl);
+                p.fused_flags[rowg * (size_t)(nk >> 3) + q] = (unsigned char)peak_flags8(C, L, H, lmin2);
+            }
+        }
         // ---- a8: vote count (one global atomic per warp per tile)
         for (int o = 16; o > 0; o >>= 1)
             my_votes += __shfl_xor_sync(0xffffffffu, my_votes, o);
@@ -404,6 +469,7 @@ static void fill_params(hough_handle *h, SweepParams *p, const SweepGeom &ge)
     p->n_votes = &h->counters->n_votes;
     p->n_evals = &h->counters->n_evals;
     p->ab = h->ab;
+    p->fused_flags = (h->cfg.options & HOUGH_OPT_FUSED_PEAKS) ? reinterpret_cast<unsigned char *>(h->flags) : nullptr;
 }
 
 cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
@@ -415,6 +481,7 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
     cudaError_t e = ensure_dynamic_smem(fn, p.geom.smem_bytes);
     if (e != cudaSuccess)
         return e;
+    h->fused_valid = p.fused_flags != nullptr ? 1 : 0;
     void *args[] = {(void *)&p};
     return cudaLaunchKernel(fn, dim3(p.geom.n_tiles), dim3(p.geom.threads), args, p.geom.smem_bytes, st);
 }

@@ -26,6 +26,8 @@ OPT_EXACT_ONLY = 8
 OPT_LIST_SWEEP = 16
 OPT_LINE = 32
 OPT_INTERVAL = 64
+OPT_FUSED_PEAKS = 128
+OPT_CELL_PEAKS = 256
 N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)

@@ -70,7 +70,8 @@ def random_hits(rng, n, n_layers=10, rmax=80.0):
     ((96, 24, 32), (32, 8), 513, 4),      # smallest row, hits = chunk + 1
     ((33, 9, 256), (4, 8), 100, 5),
 ])
-@pytest.mark.parametrize("options", [0, 1, 8, 16, 24])  # default, NO_CULL, EXACT_ONLY, LIST_SWEEP, both
+# default, NO_CULL, EXACT_ONLY, LIST_SWEEP, both, FUSED_PEAKS, FUSED_PEAKS | NO_CULL, CELL_PEAKS
+@pytest.mark.parametrize("options", [0, 1, 8, 16, 24, 128, 129, 256])
 def test_random_hits_small_grids(hough, oracle, shape, tile, n_hits, seed, options):
     rng = np.random.default_rng(seed)
     d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
@@ -92,6 +93,15 @@ def test_no_wrap_and_asymmetric_kappa_range(hough, oracle):
     res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
                   cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4)
     assert_same(res, ref)
+
+
+def test_fused_peaks_needs_packed_tiles(hough):
+    g = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=2, layer_radii=tuple(float(3 + l) for l in range(20)))
+    with pytest.raises(hough.HoughError):
+        hough.Hough(g, 10, 10, 10, options=hough.OPT_FUSED_PEAKS)
+    g = synth.Grid(n_phi=16, n_d0=4, n_kappa=32, L_min=2)
+    with pytest.raises(hough.HoughError):
+        hough.Hough(g, 10, 10, 10, options=hough.OPT_FUSED_PEAKS | hough.OPT_UNPACKED)
 
 
 def test_more_than_16_layers_uses_unpacked_tiles(hough, oracle):
@@ -186,7 +196,8 @@ def test_truncation_is_deterministic(hough, oracle):
     assert np.array_equal(res["hit_index"][:whole], ref["hit_index"][:whole])
 
 
-def test_peak_rule_on_handmade_accumulators(hough, oracle):
+@pytest.mark.parametrize("options", [0, 256, 128])  # streaming sweep, cell-wise kernel, (fused: falls back to the sweep)
+def test_peak_rule_on_handmade_accumulators(hough, oracle, options):
     """Plateaus, ties, edges and phi wrap, through hough_set_accumulator + hough_peaks_only."""
     rng = np.random.default_rng(16)
     for (shape, wrap, L_min, dens) in [((6, 5, 32), 1, 1, 0.5), ((6, 5, 32), 0, 2, 0.9),
@@ -203,7 +214,7 @@ def test_peak_rule_on_handmade_accumulators(hough, oracle):
             if variant == 2:
                 acc &= 0x7                           # few distinct popcounts: many ties
             pb, pm, n = oracle.peaks(grid, acc)
-            h = hough.Hough(grid, max_hits=1, cap_peaks=grid.n_bins, cap_hits=1)
+            h = hough.Hough(grid, max_hits=1, cap_peaks=grid.n_bins, cap_hits=1, options=options)
             h.set_accumulator(dev(acc.view(np.int32)))
             h.peaks(lists=False)
             res = h.read(lists=False)
@@ -244,11 +255,15 @@ def test_baseline_configs_full_parity(hough, oracle, name):
     assert_same(res, ref)
 
 
-@pytest.mark.parametrize("name,options", [("displaced3d", 8), ("displaced3d", 16), ("pileup", 16 | 8)])
+@pytest.mark.parametrize("name,options", [("displaced3d", 8), ("displaced3d", 16), ("pileup", 16 | 8),
+                                          ("prompt2d", 128), ("displaced3d", 128), ("pileup", 128),
+                                          ("displaced3d", 256), ("pileup", 256)])
 def test_baseline_configs_alternative_paths(hough, oracle, name, options):
     """The same results from the alternative code paths the options select: exact recipe only
-    (HOUGH_OPT_EXACT_ONLY: no fixed-point fast path) and hit lists by a second sweep
-    (HOUGH_OPT_LIST_SWEEP) instead of the peak-driven lists."""
+    (HOUGH_OPT_EXACT_ONLY: no fixed-point fast path), hit lists by a second sweep
+    (HOUGH_OPT_LIST_SWEEP) instead of the peak-driven lists, peak flags fused into the vote tile
+    plus the tile-edge pass (HOUGH_OPT_FUSED_PEAKS), peak flags by the cell-wise kernel
+    (HOUGH_OPT_CELL_PEAKS)."""
     w = synth.WORKLOADS[name]
     x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
     ref = oracle.run(w.grid, x, y, layer)
@@ -344,6 +359,17 @@ def test_finegrid_full_accumulator_parity(hough, oracle):
     for q, pk in enumerate(sel):
         got = idx[off[pk]:off[pk + 1]]
         assert np.array_equal(got, sidx[int(soff[q]):int(soff[q + 1])]), pk
+    # the fused peak test (two 256-bin segments per cell row here) and the cell-wise kernel give the
+    # same peaks and lists as the path just checked against the oracle
+    for opt in (hough.OPT_FUSED_PEAKS, hough.OPT_CELL_PEAKS):
+        h = hough.Hough(g, len(x), w.cap_peaks, w.cap_hits, options=opt)
+        h.vote(dev(x), dev(y), dev(layer))
+        h.peaks()
+        alt = h.read()
+        h.close()
+        assert alt["n_peaks"] == n and alt["n_votes"] == ref_votes and alt["n_hit_entries"] == res["n_hit_entries"]
+        assert np.array_equal(alt["peak_bin"], pb) and np.array_equal(alt["peak_mask"], pm)
+        assert np.array_equal(alt["hit_offset"], res["hit_offset"]) and np.array_equal(alt["hit_index"], idx)
 
 
 def test_unpacked_tile_option_with_few_layers(hough, oracle):
@@ -507,7 +533,10 @@ def test_random_configurations_share_the_process(hough, oracle):
         ref = oracle.run(grid, x, y, layer)
         tile = (0, 0) if rng.random() < 0.5 else (int(rng.integers(1, 20)),
                                                   int(rng.integers(1, min(n_d0, 12) + 1)))
+        opts = int(rng.integers(0, 2))          # NO_CULL or not
+        peaks_by = int(rng.integers(0, 3))      # streaming sweep, fused (two-masks-per-word tiles only), cell-wise
+        opts |= (128 if nl <= 16 else 0) if peaks_by == 1 else 256 if peaks_by == 2 else 0
         res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
                       cap_hits=max(ref["n_hit_entries"], 1) + 3, tile_phi=tile[0], tile_d0=tile[1],
-                      options=int(rng.integers(0, 2)))
+                      options=opts)
         assert_same(res, ref)
