@@ -510,9 +510,36 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
     if sweeps:
         out["ncu_sweeps"] = dict(sweeps, note="copied from the committed ncu capture, not measured in this run")
 
-    # HBM roofline of the accumulator sweeps, on the fine grid (512 MiB > L2)
+    # a5 variants, measured: stand-alone streaming sweep, peak test fused into the
+    # vote tile + tile-edge pass (HOUGH_OPT_FUSED_PEAKS), cell-wise kernel over every cell
+    def peak_variant(wl, evs, options, reps=3):
+        hv = hough.Hough(wl.grid, max(int(e[0].numel()) for e in evs), wl.cap_peaks, wl.cap_hits,
+                         device=local_rank, options=hough.OPT_STAGE_TIMING | options)
+        tv, tp, n = 0.0, 0.0, 0
+        for r in range(reps + 1):
+            for ev in evs:
+                hv.vote(*ev)
+                hv.peaks(lists=False)
+                if r > 0:
+                    t = hv.stage_times()
+                    tv += t["vote"]
+                    tp += t["peak_sweep"]
+                    n += 1
+        hv.close()
+        return {"vote_ms": tv / n, "peak_flags_ms": tp / n, "sum_ms": (tv + tp) / n}
+
     fine = synth.WORKLOADS["finegrid"]
     x, y, layer = [torch.from_numpy(a).to(dev) for a in synth.generate_event(fine.event, 0)[:3]]
+    variants = (("standalone_sweep", 0), ("fused_tile_plus_edge_cells", hough.OPT_FUSED_PEAKS),
+                ("cellwise_all_cells", hough.OPT_CELL_PEAKS))
+    out["peak_variants"] = {
+        workload.name: {k: peak_variant(workload, d_events[:min(n_ev, 5)], o) for k, o in variants},
+        "finegrid": {k: peak_variant(fine, [(x, y, layer)], o, reps=2) for k, o in variants},
+        "note": "per event, CUDA events around the kernels (hough_stage_times); peak_flags_ms = k_peak_sweep, "
+                "or k_peak_cells over the tile-edge cells / all cells; the fused variant's interior test "
+                "is inside vote_ms"}
+
+    # HBM roofline of the accumulator sweeps, on the fine grid (512 MiB > L2)
     hf = hough.Hough(fine.grid, len(x), fine.cap_peaks, fine.cap_hits, device=local_rank)
     hf.vote(x, y, layer)
     st = torch.cuda.current_stream()

@@ -28,7 +28,10 @@
  *     (e.g. a torch tensor) and the output arrays, and keeps them alive.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *     Calls that take a stream only ENQUEUE work and return without synchronising,
- *     unless stated otherwise.  One handle is used from one stream at a time.
+ *     unless stated otherwise.  One handle is used from one stream at a time.  The handle owns one
+ *     auxiliary stream of its own (created by hough_create): hough_vote builds the per-event hit index
+ *     of the hit lists there, beside the vote kernel, and hough_peaks makes `cuda_stream` wait for it
+ *     through events -- invisible to the caller, whose stream order is all that matters.
  *   - Every int-returning call returns HOUGH_OK (0) or a negative HOUGH_E* code; nothing
  *     throws across the boundary.  All configuration is the hough_config struct: the library
  *     reads no environment variable.  Its only process-wide state is a mutex-guarded record

@@ -434,6 +434,13 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
         h->timing = 1;
     }
     carve_workspace(cfg, (unsigned char *)workspace, h);
+    if (cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ix_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ix_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        hough_destroy(h);
+        return HOUGH_ECUDA;
+    }
 
     // A1: bin centres in fp64, one rounding to fp32
     const int np = cfg->n_phi, nd = cfg->n_d0;
@@ -541,6 +548,12 @@ void hough_destroy(hough_handle *h)
     }
     if (h->h2d_stream)
         cudaStreamDestroy(h->h2d_stream);
+    if (h->aux_stream)
+        cudaStreamDestroy(h->aux_stream);
+    if (h->ix_fork)
+        cudaEventDestroy(h->ix_fork);
+    if (h->ix_join)
+        cudaEventDestroy(h->ix_join);
     if (h->slot_counts)
         cudaFreeHost(h->slot_counts);
     free(h->radii);
@@ -569,11 +582,21 @@ int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *l
     h->n_hits = n;
     if (h->timing)
         memset(h->ev_set, 0, sizeof(h->ev_set));
+    if (h->ix_pending) { // an index build of a vote that no hough_peaks followed: k_prep resets its arrays
+        CK(cudaStreamWaitEvent(st, h->ix_join, 0));
+        h->ix_pending = 0;
+    }
     stage_mark(h, 0, st);
     CK(cudaMemsetAsync(h->counters, 0, 64, st));
     CK(launch_prep(h, x, y, layer, n, st));
-    if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE)
-        CK(launch_index_build(h, st));
+    if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE && n > 0) {
+        // beside the vote kernel, on the library's own stream (joined before the list kernel)
+        CK(cudaEventRecord(h->ix_fork, st));
+        CK(cudaStreamWaitEvent(h->aux_stream, h->ix_fork, 0));
+        CK(launch_index_build(h, h->aux_stream));
+        CK(cudaEventRecord(h->ix_join, h->aux_stream));
+        h->ix_pending = 1;
+    }
     stage_mark(h, ST_PREP + 1, st);
     CK(launch_vote(h, st));
     stage_mark(h, ST_VOTE + 1, st);
@@ -604,6 +627,10 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     stage_mark(h, ST_SCAN_ROWS + 1, st);
     CK(launch_compact(h, out, st));
     stage_mark(h, ST_COMPACT + 1, st);
+    if (h->ix_pending) {
+        CK(cudaStreamWaitEvent(st, h->ix_join, 0));
+        h->ix_pending = 0;
+    }
     if (with_lists) {
         // the vote variants (f3) take the generic lists: one warp per peak over all hits
         const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE ? 1 : 0;

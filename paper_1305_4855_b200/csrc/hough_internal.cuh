@@ -146,6 +146,11 @@ struct hough_handle {
     cudaEvent_t h2d_ev[HOUGH_MAX_SLOTS], slot_ev[HOUGH_MAX_SLOTS], copy_ev[HOUGH_MAX_SLOTS];
     unsigned char slot_busy[HOUGH_MAX_SLOTS];
     hough_counts *slot_counts;   // pinned host memory, one block per slot
+    // the hit index of the peak-driven lists is built on a stream of the library's own, beside the vote
+    // kernel (it is needed by hough_peaks only): ix_fork = hits prepared, ix_join = index built
+    cudaStream_t aux_stream;
+    cudaEvent_t ix_fork, ix_join;
+    int ix_pending;
     // state
     uint32_t n_hits;
     int voted;

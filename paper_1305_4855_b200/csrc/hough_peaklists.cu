@@ -489,44 +489,56 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
 {
     const GridDev &g = p.g;
     const int lane = threadIdx.x & 31, hl = lane & 15;
+    const unsigned hmask = 0xffffu << (lane & 16);
     const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
     const uint32_t halves = (gridDim.x * blockDim.x) >> 4;
-    for (uint32_t pk0 = (((blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 1); pk0 < n; pk0 += halves) {
-        const uint32_t pk = pk0 + (lane >> 4);
-        uint32_t pos = 0, len = 0;
-        unsigned long long dst = 0;
-        if (pk < n) {
-            pos = p.peak_pos[pk];
-            len = p.peak_len[pk];
-            dst = p.hit_offset[pk];
+    // two pairs of peaks per warp and round (A and B), so that their loads are in flight together
+    for (uint32_t pk0 = (((blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 1); pk0 < n; pk0 += 2 * halves) {
+        uint32_t pk[2], pos[2], len[2], v[2];
+        unsigned long long dst[2];
+        const uint32_t *src[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            pk[u] = pk0 + (uint32_t)u * halves + (lane >> 4);
+            pos[u] = 0, len[u] = 0, dst[u] = 0;
+            if (pk[u] < n) {
+                pos[u] = p.peak_pos[pk[u]];
+                len[u] = p.peak_len[pk[u]];
+                dst[u] = p.hit_offset[pk[u]];
+            }
+            src[u] = p.slots + (size_t)pk[u] * p.slot;
         }
-        if (pos != PL_SLOW && len > 0u) {
-            const uint32_t *src = p.slots + (size_t)pk * p.slot;
-            const unsigned hmask = 0xffffu << (lane & 16);
-            if (len <= 16u) { // one entry per lane, ranks through shuffles
-                const uint32_t v = hl < len ? src[hl] : 0xffffffffu;
+#pragma unroll
+        for (int u = 0; u < 2; ++u)
+            v[u] = (pos[u] != PL_SLOW && hl < len[u] && len[u] <= 16u) ? src[u][hl] : 0xffffffffu;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (pos[u] == PL_SLOW || len[u] == 0u)
+                continue;
+            if (len[u] <= 16u) { // one entry per lane, ranks through shuffles
                 uint32_t rk = 0;
 #pragma unroll
                 for (int b = 0; b < 16; ++b)
-                    rk += __shfl_sync(hmask, v, b, 16) < v ? 1u : 0u;
-                if (hl < len && dst + rk < p.cap_hits)
-                    p.hit_index[dst + rk] = v;
+                    rk += __shfl_sync(hmask, v[u], b, 16) < v[u] ? 1u : 0u;
+                if (hl < len[u] && dst[u] + rk < p.cap_hits)
+                    p.hit_index[dst[u] + rk] = v[u];
             } else {
-                for (uint32_t a = hl; a < len; a += 16) {
-                    const uint32_t v = src[a];
+                for (uint32_t a = hl; a < len[u]; a += 16) {
+                    const uint32_t w = src[u][a];
                     uint32_t rk = 0;
-                    for (uint32_t b = 0; b < len; ++b)
-                        rk += src[b] < v ? 1u : 0u;
-                    if (dst + rk < p.cap_hits)
-                        p.hit_index[dst + rk] = v;
+                    for (uint32_t b = 0; b < len[u]; ++b)
+                        rk += src[u][b] < w ? 1u : 0u;
+                    if (dst[u] + rk < p.cap_hits)
+                        p.hit_index[dst[u] + rk] = w;
                 }
             }
         }
-        // slow peaks of this pair, one after the other, by the whole warp
-        for (int which = 0; which < 2; ++which) {
-            const uint32_t spos = __shfl_sync(0xffffffffu, pos, which * 16);
-            const uint32_t slen = __shfl_sync(0xffffffffu, len, which * 16);
-            const uint32_t spk = pk0 + which;
+        // slow peaks of these pairs, one after the other, by the whole warp
+        for (int which = 0; which < 4; ++which) {
+            const int u = which >> 1;
+            const uint32_t spos = __shfl_sync(0xffffffffu, u ? pos[1] : pos[0], (which & 1) * 16);
+            const uint32_t slen = __shfl_sync(0xffffffffu, u ? len[1] : len[0], (which & 1) * 16);
+            const uint32_t spk = pk0 + (uint32_t)u * halves + (uint32_t)(which & 1);
             if (spk >= n || spos != PL_SLOW || slen == 0u)
                 continue;
             unsigned long long w = p.hit_offset[spk];

@@ -471,27 +471,41 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
     }
     unsigned long long texcl = wbase + incl - tsum;
 
-    if (tid == 0) {
+    if (warp == 0) {
+        // decoupled look-back by a whole warp: 32 predecessors per round (lane 0 = the nearest)
         volatile unsigned long long *status = p.status;
+        const unsigned long long VAL = (1ull << 62) - 1ull;
         unsigned long long prefix = 0;
         if (t == 0) {
-            status[0] = (2ull << 62) | agg;
+            if (lane == 0)
+                status[0] = (2ull << 62) | agg;
         } else {
-            status[t] = (1ull << 62) | agg;
+            if (lane == 0)
+                status[t] = (1ull << 62) | agg;
             long long q = (long long)t - 1;
             while (true) {
-                unsigned long long s = status[q];
-                unsigned long long flag = s >> 62;
-                if (flag == 0ull)
-                    continue; // predecessor (already scheduled: lower ticket) not there yet
-                prefix += s & ((1ull << 62) - 1ull);
-                if (flag == 2ull)
+                const long long idx = q - lane;
+                const unsigned long long sw = idx >= 0 ? status[idx] : (2ull << 62); // before block 0: prefix 0
+                const unsigned long long flag = sw >> 62;
+                const unsigned m2 = __ballot_sync(0xffffffffu, flag == 2ull);
+                const unsigned m0 = __ballot_sync(0xffffffffu, flag == 0ull);
+                const int first2 = m2 ? __ffs((int)m2) - 1 : 32;
+                const unsigned need = first2 >= 31 ? 0xffffffffu : ((1u << (first2 + 1)) - 1u);
+                if (m0 & need)
+                    continue; // a predecessor this side of the nearest inclusive prefix is not there yet
+                unsigned long long val = lane <= first2 ? (sw & VAL) : 0ull;
+                for (int o = 16; o > 0; o >>= 1)
+                    val += __shfl_xor_sync(0xffffffffu, val, o);
+                prefix += val;
+                if (first2 < 32)
                     break;
-                --q;
+                q -= 32;
             }
-            status[t] = (2ull << 62) | (prefix + agg);
+            if (lane == 0)
+                status[t] = (2ull << 62) | (prefix + agg);
         }
-        s_prefix = prefix;
+        if (lane == 0)
+            s_prefix = prefix;
     }
     __syncthreads();
     unsigned long long run = s_prefix + texcl;
