@@ -159,7 +159,8 @@ struct PeakListParams {
     const DevCounters *counters;
     uint32_t cap_peaks;
     uint32_t *peak_len; // [cap_peaks] list length
-    uint32_t *peak_pos; // [cap_peaks] 0: the list is in the peak's slot, PL_SLOW: it is not
+    uint32_t *peak_pos; // [cap_peaks] 0: the list is in the peak's slot in ascending order, PL_UNSORTED: in
+                        // candidate order, PL_SLOW: it is not there
     uint32_t *slots;    // [cap_peaks][slot] staging
     uint32_t slot;
     unsigned long long *n_list_evals; // candidates evaluated
@@ -232,7 +233,10 @@ __device__ __forceinline__ void merge_windows(PlWin &a, PlWin &b, int NA)
     }
 }
 
-#define PL_QCAP 40 // queued candidate ranges per thread (first rank | count << 20)
+#define PL_QCAP 40 // words per thread: queued candidate ranges (first rank | count << 20) from the bottom,
+                   // the list being collected from the top
+#define PL_LCAP 24 // entries of a list collected (and sorted) in shared memory; longer lists spill to the slot
+#define PL_UNSORTED 1u
 
 __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams p)
 {
@@ -291,6 +295,9 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
             kb = fmaxf(kb, khi);
         const float Kp = 1.01f * g.kabs + p.dk;
         const bool ab_ok = p.ab.ok != 0;
+        int nq = 0;         // queued ranges of the current pass
+        bool spill = false; // the list has outgrown shared memory
+        uint32_t n_sm = 0;  // its entries in shared memory when that happened
 
         // one candidate with the exact recipe (the fixed-point estimate first where it is admissible,
         // as in the vote: hough_device.cuh approx_bin)
@@ -314,8 +321,19 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                 match = (kappa >= klo) && (kappa < khi) && (uint32_t)kappa_bin(kappa, klo, inv_dk, nk - 1) == k;
             }
             if (match) {
-                if (cnt < p.slot)
-                    slot[cnt] = __float_as_uint(r.w) & 0xfffffu;
+                // collected at the top of the thread's queue words while it stays clear of the queued
+                // ranges; after that straight into the slot (candidate order: k_copy_lists sorts those)
+                const uint32_t hit = __float_as_uint(r.w) & 0xfffffu;
+                if (!spill && cnt < PL_LCAP && (uint32_t)nq + cnt < PL_QCAP) {
+                    s_q[PL_QCAP - 1 - cnt][tid] = hit;
+                } else {
+                    if (!spill) {
+                        spill = true;
+                        n_sm = cnt;
+                    }
+                    if (cnt < p.slot)
+                        slot[cnt] = hit;
+                }
                 ++cnt;
             }
         };
@@ -324,9 +342,13 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
         while (l <= nL) {
             // ---- queue the candidate ranges (physical ranks of the key-ordered records) of as many
             // layers as fit; a range too long for a queue entry is walked on the spot
-            int nq = 0;
+            nq = 0;
             auto push = [&](uint32_t rank0, uint32_t n) {
                 if (n > 4095u) {
+                    if (!spill) { // matches found now must not grow into the words the next pushes use
+                        spill = true;
+                        n_sm = cnt;
+                    }
                     for (uint32_t c = 0; c < n; ++c)
                         consider(ix.rec[rank0 + c]);
                 } else if (n) {
@@ -342,7 +364,7 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                 push(lbase + q0, first);
                 push(lbase, n - first);
             };
-            for (; l <= nL && nq + 6 <= PL_QCAP; ++l) {
+            for (; l <= nL && (uint32_t)nq + 6u + (spill ? n_sm : min(cnt, (uint32_t)PL_LCAP)) <= PL_QCAP; ++l) {
                 const uint32_t lbase = s_lbase[l], lcnt = s_lbase[l + 1] - lbase;
                 if (l == nL) { // the wild hits (outside the index's numeric range): candidates of every peak
                     push(lbase, lcnt);
@@ -456,8 +478,24 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                 consider(r);
             }
         }
+        // ---- the list: sorted here when all of it is in shared memory (insertion sort, one thread per
+        // list), then written to the peak's slot
+        auto L = [&](uint32_t c) -> uint32_t & { return s_q[PL_QCAP - 1 - c][tid]; };
+        const uint32_t in_sm = spill ? n_sm : cnt;
+        if (!spill)
+            for (uint32_t a = 1; a < cnt; ++a) {
+                const uint32_t v = L(a);
+                uint32_t b = a;
+                while (b > 0 && L(b - 1) > v) {
+                    L(b) = L(b - 1);
+                    --b;
+                }
+                L(b) = v;
+            }
+        for (uint32_t c = 0; c < in_sm && c < p.slot; ++c)
+            slot[c] = L(c);
         p.peak_len[pk] = cnt;
-        p.peak_pos[pk] = cnt <= p.slot ? 0u : PL_SLOW;
+        p.peak_pos[pk] = cnt > p.slot ? PL_SLOW : spill ? PL_UNSORTED : 0u;
     }
     for (int o = 16; o > 0; o >>= 1)
         evals += __shfl_xor_sync(0xffffffffu, evals, o);
@@ -482,8 +520,9 @@ struct ListCopyParams {
 };
 
 // hit_index[hit_offset[p] ..] = the staged list of peak p in ascending hit index (half a warp per
-// peak ranks the entries by counting: hit indices are distinct); a peak without a staged list
-// (PL_SLOW) is written straight from the hits in index order by a whole warp.
+// peak): a plain copy where k_peak_lists has sorted it, ranks by counting (hit indices are distinct)
+// where the slot is in candidate order (PL_UNSORTED); a peak without a staged list (PL_SLOW) is
+// written straight from the hits in index order by a whole warp.
 template <int MODE>
 __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
 {
@@ -510,12 +549,18 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
         }
 #pragma unroll
         for (int u = 0; u < 2; ++u)
-            v[u] = (pos[u] != PL_SLOW && hl < len[u] && len[u] <= 16u) ? src[u][hl] : 0xffffffffu;
+            v[u] = (pos[u] != PL_SLOW && hl < len[u]) ? src[u][hl] : 0xffffffffu;
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             if (pos[u] == PL_SLOW || len[u] == 0u)
                 continue;
-            if (len[u] <= 16u) { // one entry per lane, ranks through shuffles
+            if (pos[u] == 0u) { // already in ascending order (sorted by k_peak_lists): a plain copy
+                if (hl < len[u] && dst[u] + hl < p.cap_hits)
+                    p.hit_index[dst[u] + hl] = v[u];
+                for (uint32_t a = hl + 16; a < len[u]; a += 16)
+                    if (dst[u] + a < p.cap_hits)
+                        p.hit_index[dst[u] + a] = src[u][a];
+            } else if (len[u] <= 16u) { // one entry per lane, ranks through shuffles
                 uint32_t rk = 0;
 #pragma unroll
                 for (int b = 0; b < 16; ++b)
