@@ -285,8 +285,8 @@ static int choose_geometry(hough_handle *h)
 {
     const hough_config &c = h->cfg;
     const int nk = c.n_kappa;
-    const int budget = 113 * 1024;
-    const int staging = 2 * 4 * HOUGH_CHUNK * 4 + (HOUGH_CHUNK + 8) * 16 + 1024;
+    const int budget = 115 * 1024;
+    const int staging = 4 * 1536 * 4 + (1536 + 8) * 16 + 1024; // hough_sweep.cu: VOTE_CHUNK hits staged + survivors
     // vote
     {
         int cell_bytes = nk * 4 / h->g.pack;

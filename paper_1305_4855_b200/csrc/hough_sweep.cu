@@ -7,6 +7,7 @@
 #include "hough_device.cuh"
 
 #define EVAL_UNROLL 4
+#define VOTE_CHUNK 1536 // hits staged per round of bulk copies (a multiple of HOUGH_CHUNK)
 
 // ------------------------------------------------------------------ kernel parameters
 struct SweepParams {
@@ -39,15 +40,15 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     // ---- carve shared memory: tile = masks [P * D cells][nk / PACK words], then staging
     uint32_t *tile = reinterpret_cast<uint32_t *>(smem_raw);
     unsigned char *ptr = smem_raw + (size_t)ge.tile_words * 4;
-    float *stage = reinterpret_cast<float *>(ptr); // [2][4][chunk]
-    ptr += (size_t)2 * 4 * ge.chunk * 4;
+    float *stage = reinterpret_cast<float *>(ptr); // [4][chunk]
+    ptr += (size_t)4 * ge.chunk * 4;
     float4 *surv = reinterpret_cast<float4 *>(ptr); // [chunk + EVAL_UNROLL]
     ptr += (size_t)(ge.chunk + EVAL_UNROLL) * 16;
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
     int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
     ptr += 32 * 4;
-    int *s_nwild = reinterpret_cast<int *>(ptr);
+    int *s_nwild = reinterpret_cast<int *>(ptr); // [4]: survivors of even / odd chunks, wild hits of even / odd chunks
 
     // ---- which tile: the first n_big phi0 slabs are P rows high, the others P_small
     // (two heights so that the CTAs fill whole waves)
@@ -88,24 +89,27 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     tc.off = p.no_cull;
     const bool warp_ok = set < split;
 
-    const uint32_t n_chunks = p.hits.n_pad / ge.chunk;
-    const uint32_t chunk_bytes = (uint32_t)ge.chunk * 4;
+    // chunks of ge.chunk hits; the padded hit count is a multiple of HOUGH_CHUNK, so the last chunk may
+    // be shorter
+    const uint32_t n_chunks = (p.hits.n_pad + ge.chunk - 1) / ge.chunk;
 
+    if (tid < 4)
+        s_nwild[tid] = 0; // survivor / wild counters of the even and odd chunks
     if (tid == 0) {
         mbar_init(&mbar[0], 1);
-        mbar_init(&mbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    // ONE staging buffer: the survivors of a chunk are compacted out of it before the evaluation, so
+    // the next chunk's bulk copies are issued right after the cull and land under the evaluation
     auto issue = [&](uint32_t ch) {
-        float *dst = stage + (size_t)(ch & 1) * 4 * ge.chunk;
-        uint64_t *bar = &mbar[ch & 1];
-        mbar_expect_tx(bar, 4 * chunk_bytes);
-        size_t off = (size_t)ch * ge.chunk;
-        tma_load_1d(dst, p.hits.x + off, chunk_bytes, bar);
-        tma_load_1d(dst + ge.chunk, p.hits.y + off, chunk_bytes, bar);
-        tma_load_1d(dst + 2 * ge.chunk, p.hits.r2 + off, chunk_bytes, bar);
-        tma_load_1d(dst + 3 * ge.chunk, p.hits.bit + off, chunk_bytes, bar);
+        const size_t off = (size_t)ch * ge.chunk;
+        const uint32_t bytes = (uint32_t)min((size_t)ge.chunk, (size_t)p.hits.n_pad - off) * 4u;
+        mbar_expect_tx(&mbar[0], 4 * bytes);
+        tma_load_1d(stage, p.hits.x + off, bytes, &mbar[0]);
+        tma_load_1d(stage + ge.chunk, p.hits.y + off, bytes, &mbar[0]);
+        tma_load_1d(stage + 2 * ge.chunk, p.hits.r2 + off, bytes, &mbar[0]);
+        tma_load_1d(stage + 3 * ge.chunk, p.hits.bit + off, bytes, &mbar[0]);
     };
     if (tid == 0 && n_chunks > 0)
         issue(0);
@@ -128,22 +132,21 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     asm volatile("" : "+r"(row_addr), "+r"(swzb));
 
     for (uint32_t ch = 0; ch < n_chunks; ++ch) {
-        const float *st = stage + (size_t)(ch & 1) * 4 * ge.chunk;
-        mbar_wait(&mbar[ch & 1], (ch >> 1) & 1);
-        if (tid == 0 && ch + 1 < n_chunks)
-            issue(ch + 1); // the other buffer was released by the barrier ending chunk ch-1
+        const float *st = stage;
+        const int len = (int)min((size_t)ge.chunk, (size_t)p.hits.n_pad - (size_t)ch * ge.chunk);
+        mbar_wait(&mbar[0], ch & 1);
 
         // ---- cull + compaction of the survivors: ordinary hits from the front of surv, hits
-        // outside the fast path's range ("wild") from its back
-        int total = 0;
-        if (APPROX && tid == 0)
-            s_nwild[0] = 0; // (the barrier inside the loop orders it before the first use)
-        for (int base = 0; base < ge.chunk; base += ge.threads) {
+        // outside the fast path's range ("wild") from its back.  Votes commute (OR), so the order
+        // of the survivors is free: every warp reserves its places with one shared atomic (the
+        // counter of chunk ch + 1 is cleared during the evaluation of chunk ch).
+        int *s_total = s_nwild + (ch & 1), *s_wild = s_nwild + 2 + (ch & 1);
+        for (int base = 0; base < len; base += ge.threads) {
             int hidx = base + tid;
             bool keep = false, wild = false;
             float hx = 0.f, hy = 0.f, hr2 = 0.f;
             uint32_t hb = 0;
-            if (hidx < ge.chunk) {
+            if (hidx < len) {
                 hx = st[hidx];
                 hy = st[ge.chunk + hidx];
                 hr2 = st[2 * ge.chunk + hidx];
@@ -154,22 +157,25 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                     keep = keep && !wild;
                 }
             }
-            unsigned bal = __ballot_sync(0xffffffffu, keep);
-            if (lane == 0)
-                warp_cnt[warp] = __popc(bal);
-            __syncthreads();
-            int all;
-            const int before = warps_before(warp_cnt, nwarps, warp, lane, all);
-            if (keep) {
-                int pos = total + before + __popc(bal & ((1u << lane) - 1u));
-                surv[pos] = make_float4(hx, hy, hr2, __uint_as_float(hb));
-            }
-            if (APPROX && wild) // rare: any order will do (OR is commutative)
-                surv[ge.chunk + EVAL_UNROLL - 1 - atomicAdd(s_nwild, 1)] = make_float4(hx, hy, hr2, __uint_as_float(hb));
-            total += all;
-            __syncthreads();
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            int wbase = 0;
+            if (lane == 0 && bal)
+                wbase = atomicAdd(s_total, __popc(bal));
+            wbase = __shfl_sync(0xffffffffu, wbase, 0);
+            if (keep)
+                surv[wbase + __popc(bal & ((1u << lane) - 1u))] = make_float4(hx, hy, hr2, __uint_as_float(hb));
+            if (APPROX && wild) // rare
+                surv[ge.chunk + EVAL_UNROLL - 1 - atomicAdd(s_wild, 1)] = make_float4(hx, hy, hr2, __uint_as_float(hb));
         }
-        const int n_wild = APPROX ? s_nwild[0] : 0;
+        __syncthreads();
+        const int total = *s_total;
+        const int n_wild = APPROX ? *s_wild : 0;
+        if (tid == 0) {
+            s_nwild[(ch + 1) & 1] = 0;
+            s_nwild[2 + ((ch + 1) & 1)] = 0;
+            if (ch + 1 < n_chunks)
+                issue(ch + 1); // the staging buffer was released by the barrier above
+        }
         tile_evals += (unsigned long long)(total + n_wild) * (unsigned)(ni * nj);
         if (!APPROX) {
             if (tid < EVAL_UNROLL) // non-voting padding up to a multiple of the unroll factor
@@ -394,14 +400,14 @@ int sweep_geom_init(const hough_handle *h, SweepGeom *ge, int P, int D, int spli
     ge->groups = ge->cells_pad / 32;
     ge->split = split;
     ge->threads = 32 * ge->groups * split;
-    ge->chunk = HOUGH_CHUNK;
+    ge->chunk = VOTE_CHUNK;
     ge->tiles_phi = (cfg.n_phi + P - 1) / P;
     ge->tiles_d0 = (cfg.n_d0 + D - 1) / D;
     ge->n_tiles = ge->tiles_phi * ge->tiles_d0;
     // rows for the P x D cells only: padding lanes of the last cell group never vote
     const size_t tile_bytes = (size_t)(P * D) * cfg.n_kappa * 4 / h->g.pack, extra = 0;
     ge->tile_words = (int)(tile_bytes / 4);
-    size_t stage = (size_t)2 * 4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16;
+    size_t stage = (size_t)4 * ge->chunk * 4 + (size_t)(ge->chunk + EVAL_UNROLL) * 16 + 16 + 32 * 4 + 16 + 16;
     ge->smem_bytes = (int)(tile_bytes + extra + stage);
     // the interval test needs the slab to span well under a quarter turn
     double span = (cfg.phi_max - cfg.phi_min) * (double)(P - 1) / (double)cfg.n_phi;
