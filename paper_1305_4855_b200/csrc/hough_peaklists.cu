@@ -19,7 +19,8 @@
 // The windows are SUPERSETS: the bin's kappa interval is widened by a bound on the binary32
 // evaluation error of the recipe (which grows as 1 / den; hits closer than L0 to the point of
 // closest approach P0 are taken through a third, "proximity" window around P0's azimuth instead),
-// every angle by 2e-5 rad and every window by one azimuth bin on each side.  Whatever cannot be
+// and every angle by 5e-5 rad (the azimuth bins of the index come from atan2f, 2 ulp ~ 1e-6 rad, and the
+// window angles carry a few binary32 roundings of values below 2 pi).  Whatever cannot be
 // bounded (1 + kappa d0 not safely positive, non-finite intermediate values, a window wider than
 // the ring) falls back to the whole layer; hits outside the index's numeric range ("wild") are
 // candidates of every peak.  Every candidate is then evaluated with the EXACT recipe
@@ -198,18 +199,18 @@ __device__ __forceinline__ float fast_asin(float x)
 struct PlWin { // an arc of azimuth bins [b, b + n) on the ring of NA bins; n = 0: absent
     int b, n;
 };
-// Azimuth window [a_lo, a_hi] (radians, a_lo <= a_hi) -> bins, one extra bin on each side.
+// Azimuth window [a_lo, a_hi] (radians, a_lo <= a_hi, slack included) -> the bins it touches.
 __device__ __forceinline__ PlWin window_bins(float a_lo, float a_hi, float na_scale, int NA)
 {
     const float t0 = floorf((a_lo + PI_F) * na_scale), t1 = floorf((a_hi + PI_F) * na_scale);
-    const float span = t1 - t0 + 3.0f;
+    const float span = t1 - t0 + 1.0f;
     PlWin w;
     if (!(span < (float)NA)) { // also NaN: the whole ring
         w.b = 0;
         w.n = NA;
         return w;
     }
-    w.b = ((int)t0 - 1) & (NA - 1);
+    w.b = (int)t0 & (NA - 1);
     w.n = (int)span;
     return w;
 }
@@ -406,7 +407,7 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                     if (!(fabsf(wlo) < 3.0e38f) || !(fabsf(whi) < 3.0e38f) || !(wlo <= whi)) {
                         whole = true; // inf / NaN somewhere: no bound
                     } else if (!(wlo > 1.0f) && !(whi < -1.0f)) {
-                        const float tlo = fast_asin(fmaxf(wlo, -1.0f)) - 2e-5f, thi = fast_asin(fminf(whi, 1.0f)) + 2e-5f;
+                        const float tlo = fast_asin(fmaxf(wlo, -1.0f)) - 5e-5f, thi = fast_asin(fminf(whi, 1.0f)) + 5e-5f;
                         w0 = window_bins(phi0 + tlo, phi0 + thi, na_scale, NA);
                         w1 = window_bins(phi0 + PI_F - thi, phi0 + PI_F - tlo, na_scale, NA);
                     }
@@ -417,7 +418,7 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
                     if (!(arg < 0.999f)) {
                         whole = true;
                     } else {
-                        const float hw = 2.0f * fast_asin(arg) + 2e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
+                        const float hw = 2.0f * fast_asin(arg) + 5e-5f, psi = phi0 + (c_d0 >= 0.0f ? 1.5707963f : -1.5707963f);
                         w2 = window_bins(psi - hw, psi + hw, na_scale, NA);
                     }
                 }
