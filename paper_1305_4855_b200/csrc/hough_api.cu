@@ -215,9 +215,10 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *peak_len = cv.take((size_t)c->cap_peaks * 4);
     void *ent_sub = cv.take((size_t)c->cap_hits * 4), *ent_hit = cv.take((size_t)c->cap_hits * 4);
     void *ent_idx = cv.take((size_t)c->cap_hits * 4);
-    // hit index of the peak-driven lists: azimuth bins per layer ~ 2 x hits per layer, a power of two
+    // hit index of the peak-driven lists: azimuth bins per layer ~ 5 x hits per layer (a window touches
+    // the bins it overlaps, so finer bins mean fewer candidates), a power of two
     int NA = 256;
-    while (NA < 4096 && (uint64_t)NA * (uint64_t)c->n_layers < 2ull * c->max_hits)
+    while (NA < 16384 && (uint64_t)NA * (uint64_t)c->n_layers < 5ull * c->max_hits)
         NA <<= 1;
     const int n_keys = (c->n_layers + 1) * NA;
     void *t_phic = cv.take((size_t)c->n_phi * 4);

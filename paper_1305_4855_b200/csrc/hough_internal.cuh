@@ -81,13 +81,13 @@ struct HitsDev {         // prepared hits, SoA, padded with non-voting entries t
 // Per-event index of the hits by (layer label, azimuth bin) for the peak-driven hit lists
 // (hough_peaklists.cu).  Pseudo-layer n_layers holds the hits outside the index's numeric range.
 struct HitIndexDev {
-    int NA;                 // azimuth bins per layer (power of two, <= 4096: 12 bits beside the 20-bit hit index)
+    int NA;                 // azimuth bins per layer (power of two, 256 .. 16384)
     int n_keys;             // (n_layers + 1) * NA
     uint32_t *bin_cnt;      // [n_keys] histogram of the event (k_prep), then the scatter cursor
     uint32_t *bin_start;    // [n_keys + 1] rank of the first hit of a key
     uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) (zeroed per event)
     uint32_t *key;          // [max_hits_pad] key of hit h, 0xffffffff = not indexed (bad layer)
-    float4 *rec;            // [max_hits_pad] the hits in key order: (x, y, r2, bits of (azimuth bin << 20 | hit index))
+    float4 *rec;            // [max_hits_pad] the hits in key order: (x, y, r2, bits of the hit index)
 };
 
 // Device counters of one event (internal; copied into the caller's hough_counts).

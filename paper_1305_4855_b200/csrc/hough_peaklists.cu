@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(256) k_index_scatter(HitIndexDev ix, const flo
     if (key == 0xffffffffu)
         return;
     const uint32_t rank = ix.bin_start[key] + atomicAdd(&ix.bin_cnt[key], 1u);
-    ix.rec[rank] = make_float4(hx[h], hy[h], hr2[h], __uint_as_float(((key & (uint32_t)(ix.NA - 1)) << 20) | h));
+    ix.rec[rank] = make_float4(hx[h], hy[h], hr2[h], __uint_as_float(h));
 }
 
 cudaError_t launch_index_build(hough_handle *h, cudaStream_t st)
@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
             if (match) {
                 // collected at the top of the thread's queue words while it stays clear of the queued
                 // ranges; after that straight into the slot (candidate order: k_copy_lists sorts those)
-                const uint32_t hit = __float_as_uint(r.w) & 0xfffffu;
+                const uint32_t hit = __float_as_uint(r.w);
                 if (!spill && cnt < PL_LCAP && (uint32_t)nq + cnt < PL_QCAP) {
                     s_q[PL_QCAP - 1 - cnt][tid] = hit;
                 } else {
