@@ -453,8 +453,10 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
              "achieved_executed": FLOP_PER_EVAL * done_evals / secs / 1e12,
              "frac_executed": FLOP_PER_EVAL * done_evals / secs / 1e12 / alu_peak}
         instr = sweeps.get(key, {}).get("warp_instructions")
+        r["algorithmic_equiv_frac"] = r["frac"]  # the contract's `frac` under the name the advisor asked for
         if instr:
             r["issue_slot_frac"] = instr / secs / issue_peak
+            r["hardware_frac"] = r["issue_slot_frac"]  # the utilisation figure: issue slots actually used
             r["warp_instructions_per_launch"] = instr
             r["instructions_source"] = sweeps.get("source")
             r["issue_active_pct_ncu"] = sweeps.get(key, {}).get("issue_active_pct")
