@@ -329,12 +329,14 @@ def main():
         e2e_secs = float(t.item())
     assert nv_e2e == votes_step * args.steps
     h2d = sum(len(e[0]) for e in events) * 12
-    d2h = int(sum(40 + min(int(c["n_peaks"]), workload.cap_peaks) * 16 + 8 +
-                  min(int(c["n_hit_entries"]), workload.cap_hits) * 4 for c in cnt))
+    idx_bytes = 2 if max_hits <= 65536 else 4  # the lists come back as 16-bit indices when they fit (hit_index16)
+    d2h = int(sum(48 + min(int(c["n_peaks"]), workload.cap_peaks) * 16 + 8 +
+                  min(int(c["n_hit_entries"]), workload.cap_hits) * idx_bytes for c in cnt))
     e2e = {"value": votes_all * args.steps / e2e_secs, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "events_per_s": events_all * args.steps / e2e_secs,
            "api": "hough_submit_host + hough_collect_begin/_end (three events in flight: copy-in, compute and "
-                  "copy-out streams)"}
+                  "copy-out streams); complete results per event: counters, peak bins and masks, 64-bit list "
+                  "offsets, hit lists as %d-bit indices" % (8 * idx_bytes)}
     if rank == 0 and world == 1:
         h.process_host(*[t.numpy() for t in pin_events[0]])  # allocates its pinned buffers
         t0 = time.perf_counter()

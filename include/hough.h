@@ -61,6 +61,7 @@ extern "C" {
 /* hough_counts.flags */
 #define HOUGH_TRUNCATED_PEAKS 1u /* n_peaks > cap_peaks: only the first cap_peaks (in lin order) were written */
 #define HOUGH_TRUNCATED_HITS 2u  /* n_hit_entries > cap_hits: hit_index holds the first cap_hits entries */
+#define HOUGH_INDEX16 4u         /* hit_index16 was written as well (the event has <= 65536 hits) */
 
 /* hough_config.options */
 #define HOUGH_OPT_NO_CULL 1u      /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
@@ -137,6 +138,10 @@ typedef struct hough_peaks_out {
     uint64_t *hit_offset; /* [device] cap_peaks + 1 */
     uint32_t *hit_index;  /* [device] cap_hits */
     hough_counts *counts; /* [device] 1 */
+    uint16_t *hit_index16; /* [device] cap_hits, OPTIONAL (NULL: not wanted): the same entries as 16-bit values,
+                              written beside hit_index when the event has <= 65536 hits and the lists come from
+                              the default (peak-driven) path or the vote variants; counts->flags then carries
+                              HOUGH_INDEX16.  Halves the bytes a host has to read back (see hough_host_out) */
 } hough_peaks_out;
 
 /* Host mirror of hough_peaks_out for hough_process_host ([host] pointers, same capacities). */
@@ -146,6 +151,9 @@ typedef struct hough_host_out {
     uint64_t *hit_offset;
     uint32_t *hit_index; /* may be NULL: hit lists are then computed but not copied back */
     hough_counts *counts;
+    uint16_t *hit_index16; /* OPTIONAL (NULL: not wanted), cap_hits entries: when the event's counts carry
+                              HOUGH_INDEX16 the lists are copied back in this form INSTEAD of hit_index (12 MB
+                              instead of 24 MB for a config-3 event); otherwise hit_index is used as above */
 } hough_host_out;
 
 /* Bytes of device workspace hough_create needs for cfg (0 if cfg is invalid). */

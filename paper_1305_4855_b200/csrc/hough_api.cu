@@ -717,8 +717,12 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
         CK(cudaMemcpyAsync(host->mask, dev->mask, np * 4, cudaMemcpyDeviceToHost, st));
     }
     CK(cudaMemcpyAsync(host->hit_offset, dev->hit_offset, (np + 1) * 8, cudaMemcpyDeviceToHost, st));
-    if (host->hit_index && ne > 0)
+    if (host->hit_index16 && dev->hit_index16 && (host->counts->flags & HOUGH_INDEX16)) {
+        if (ne > 0)
+            CK(cudaMemcpyAsync(host->hit_index16, dev->hit_index16, ne * 2, cudaMemcpyDeviceToHost, st));
+    } else if (host->hit_index && ne > 0) {
         CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
+    }
     CK(cudaStreamSynchronize(st));
     return HOUGH_OK;
 }
@@ -794,8 +798,12 @@ int hough_collect_begin(hough_handle *h, const hough_peaks_out *dev, const hough
         CK(cudaMemcpyAsync(host->mask, dev->mask, np * 4, cudaMemcpyDeviceToHost, st));
     }
     CK(cudaMemcpyAsync(host->hit_offset, dev->hit_offset, (np + 1) * 8, cudaMemcpyDeviceToHost, st));
-    if (host->hit_index && ne > 0)
+    if (host->hit_index16 && dev->hit_index16 && (host->counts->flags & HOUGH_INDEX16)) {
+        if (ne > 0)
+            CK(cudaMemcpyAsync(host->hit_index16, dev->hit_index16, ne * 2, cudaMemcpyDeviceToHost, st));
+    } else if (host->hit_index && ne > 0) {
         CK(cudaMemcpyAsync(host->hit_index, dev->hit_index, ne * 4, cudaMemcpyDeviceToHost, st));
+    }
     CK(cudaEventRecord(h->copy_ev[slot], st));
     h->slot_busy[slot] = 2;
     return HOUGH_OK;

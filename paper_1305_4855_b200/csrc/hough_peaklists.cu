@@ -517,6 +517,7 @@ struct ListCopyParams {
     uint32_t slot;
     const unsigned long long *hit_offset;
     uint32_t *hit_index;
+    unsigned short *hit_index16; // optional 16-bit copy of the entries (NULL: not wanted)
     unsigned long long cap_hits;
 };
 
@@ -532,6 +533,11 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
     const unsigned hmask = 0xffffu << (lane & 16);
     const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
     const uint32_t halves = (gridDim.x * blockDim.x) >> 4;
+    auto put = [&](unsigned long long pos, uint32_t hit) {
+        p.hit_index[pos] = hit;
+        if (p.hit_index16)
+            p.hit_index16[pos] = (unsigned short)hit;
+    };
     // two pairs of peaks per warp and round (A and B), so that their loads are in flight together
     for (uint32_t pk0 = (((blockIdx.x * blockDim.x + threadIdx.x) >> 5) << 1); pk0 < n; pk0 += 2 * halves) {
         uint32_t pk[2], pos[2], len[2], v[2];
@@ -557,17 +563,17 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
                 continue;
             if (pos[u] == 0u) { // already in ascending order (sorted by k_peak_lists): a plain copy
                 if (hl < len[u] && dst[u] + hl < p.cap_hits)
-                    p.hit_index[dst[u] + hl] = v[u];
+                    put(dst[u] + hl, v[u]);
                 for (uint32_t a = hl + 16; a < len[u]; a += 16)
                     if (dst[u] + a < p.cap_hits)
-                        p.hit_index[dst[u] + a] = src[u][a];
+                        put(dst[u] + a, src[u][a]);
             } else if (len[u] <= 16u) { // one entry per lane, ranks through shuffles
                 uint32_t rk = 0;
 #pragma unroll
                 for (int b = 0; b < 16; ++b)
                     rk += __shfl_sync(hmask, v[u], b, 16) < v[u] ? 1u : 0u;
                 if (hl < len[u] && dst[u] + rk < p.cap_hits)
-                    p.hit_index[dst[u] + rk] = v[u];
+                    put(dst[u] + rk, v[u]);
             } else {
                 for (uint32_t a = hl; a < len[u]; a += 16) {
                     const uint32_t w = src[u][a];
@@ -575,7 +581,7 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
                     for (uint32_t b = 0; b < len[u]; ++b)
                         rk += src[u][b] < w ? 1u : 0u;
                     if (dst[u] + rk < p.cap_hits)
-                        p.hit_index[dst[u] + rk] = w;
+                        put(dst[u] + rk, w);
                 }
             }
         }
@@ -607,7 +613,7 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
                 if (in) {
                     const unsigned long long q = w + __popc(bal & ((1u << lane) - 1u));
                     if (q < p.cap_hits)
-                        p.hit_index[q] = hidx;
+                        put(q, hidx);
                 }
                 w += __popc(bal);
             }
@@ -674,6 +680,7 @@ cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.slot = slot_entries(h);
     p.hit_offset = reinterpret_cast<const unsigned long long *>(out->hit_offset);
     p.hit_index = out->hit_index;
+    p.hit_index16 = (out->hit_index16 && h->n_hits <= 65536u) ? out->hit_index16 : nullptr;
     p.cap_hits = h->cfg.cap_hits;
     if (h->mode == VOTE_LINE)
         k_copy_lists<VOTE_LINE><<<h->n_sms * 16, 256, 0, st>>>(p);
@@ -736,6 +743,7 @@ cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cu
     p.slot = 0;
     p.hit_offset = nullptr;
     p.hit_index = nullptr;
+    p.hit_index16 = nullptr;
     p.cap_hits = 0;
     unsigned long long *ev = &h->counters->n_list_evals;
     if (h->mode == VOTE_LINE)

@@ -663,7 +663,7 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
 
 // ------------------------------------------------------------------ counters out
 __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_peaks,
-                         unsigned long long cap_hits, int with_lists)
+                         unsigned long long cap_hits, int with_lists, int index16)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         hough_counts r;
@@ -678,6 +678,8 @@ __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_p
             r.flags |= HOUGH_TRUNCATED_PEAKS;
         if (r.n_hit_entries > cap_hits)
             r.flags |= HOUGH_TRUNCATED_HITS;
+        if (index16)
+            r.flags |= HOUGH_INDEX16;
         r.reserved = 0u;
         *out = r;
     }
@@ -686,7 +688,10 @@ __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_p
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,
                                  cudaStream_t st)
 {
-    k_finish<<<1, 32, 0, st>>>(h->counters, out->counts, h->cfg.cap_peaks, h->cfg.cap_hits, with_lists);
+    // the 16-bit entries are written by k_copy_lists (not by the round-1 list sweep's placement kernel)
+    const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE;
+    const int index16 = with_lists && !sweep && out->hit_index16 && h->n_hits <= 65536u;
+    k_finish<<<1, 32, 0, st>>>(h->counters, out->counts, h->cfg.cap_peaks, h->cfg.cap_hits, with_lists, index16);
     h->launches += 1;
     return cudaGetLastError();
 }

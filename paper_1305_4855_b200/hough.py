@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libhough_b200.so")
 
 HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3, -4
-TRUNCATED_PEAKS, TRUNCATED_HITS = 1, 2
+TRUNCATED_PEAKS, TRUNCATED_HITS, INDEX16 = 1, 2, 4
 OPT_NO_CULL = 1
 OPT_STAGE_TIMING = 2
 OPT_UNPACKED = 4
@@ -63,12 +63,12 @@ class Counts(C.Structure):
 
 class PeaksOut(C.Structure):
     _fields_ = [("bin", C.c_void_p), ("mask", C.c_void_p), ("hit_offset", C.c_void_p),
-                ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
+                ("hit_index", C.c_void_p), ("counts", C.c_void_p), ("hit_index16", C.c_void_p)]
 
 
 class HostOut(C.Structure):
     _fields_ = [("bin", C.c_void_p), ("mask", C.c_void_p), ("hit_offset", C.c_void_p),
-                ("hit_index", C.c_void_p), ("counts", C.c_void_p)]
+                ("hit_index", C.c_void_p), ("counts", C.c_void_p), ("hit_index16", C.c_void_p)]
 
 
 class VertexConfig(C.Structure):
@@ -312,7 +312,8 @@ class Hough:
                           hb["hit_index"].numpy() if want_lists else None)
 
     def _slot(self, slot):
-        """Device and pinned host arrays of one in-flight event (submit_host / collect_host)."""
+        """Device and pinned host arrays of one in-flight event (submit_host / collect_host).  With at
+        most 65536 hits per event the hit lists travel as 16-bit indices (hit_index16)."""
         if not hasattr(self, "_slots"):
             self._slots, self._copy_stream = {}, torch.cuda.Stream(device=self.device)
         if slot not in self._slots:
@@ -322,15 +323,22 @@ class Hough:
                      hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, device=self.device),
                      hit_index=torch.empty(self.cap_hits, **i32),
                      counts=torch.zeros(COUNTS_WORDS, dtype=torch.int64, device=self.device))
+            use16 = self.max_hits <= 65536
+            if use16:
+                d["hit_index16"] = torch.empty(self.cap_hits, dtype=torch.int16, device=self.device)
             hb = dict(bin=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
                       mask=torch.empty(self.cap_peaks, dtype=torch.int32, **pin),
                       hit_offset=torch.empty(self.cap_peaks + 1, dtype=torch.int64, **pin),
                       hit_index=torch.empty(self.cap_hits, dtype=torch.int32, **pin),
                       counts=torch.zeros(COUNTS_WORDS, dtype=torch.int64, **pin))
+            if use16:
+                hb["hit_index16"] = torch.empty(self.cap_hits, dtype=torch.int16, **pin)
             out = PeaksOut(d["bin"].data_ptr(), d["mask"].data_ptr(), d["hit_offset"].data_ptr(),
-                           d["hit_index"].data_ptr(), d["counts"].data_ptr())
+                           d["hit_index"].data_ptr(), d["counts"].data_ptr(),
+                           d["hit_index16"].data_ptr() if use16 else None)
             host = HostOut(hb["bin"].data_ptr(), hb["mask"].data_ptr(), hb["hit_offset"].data_ptr(),
-                           hb["hit_index"].data_ptr(), hb["counts"].data_ptr())
+                           hb["hit_index"].data_ptr(), hb["counts"].data_ptr(),
+                           hb["hit_index16"].data_ptr() if use16 else None)
             self._slots[slot] = (d, hb, out, host)
         return self._slots[slot]
 
@@ -360,8 +368,11 @@ class Hough:
         _d, hb, _out, _host = self._slot(slot)
         _check(_lib.hough_collect_end(self._h, int(slot)), "hough_collect_end")
         cnt = hb["counts"].numpy().view(COUNTS_DTYPE)[0]
-        return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(),
-                          hb["hit_index"].numpy())
+        if int(cnt["flags"]) & INDEX16 and "hit_index16" in hb:  # the lists came back as 16-bit indices
+            idx = hb["hit_index16"].numpy().view(np.uint16)
+        else:
+            idx = hb["hit_index"].numpy()
+        return self._pack(cnt, hb["bin"].numpy(), hb["mask"].numpy(), hb["hit_offset"].numpy(), idx)
 
     # -- f1: the second transform over the peaks (hough_vertices)
     def vertices(self, vgrid, cap_vertices=1024, cap_members=1 << 20, stream=None):
@@ -451,7 +462,7 @@ class Hough:
                "peak_bin": b[:n_rep].view(np.uint32), "peak_mask": m[:n_rep].view(np.uint32),
                "hit_offset": off[:n_rep + 1].view(np.uint64)}
         if idx is not None:
-            out["hit_index"] = idx[:n_ent].view(np.uint32)
+            out["hit_index"] = idx[:n_ent] if idx.dtype == np.uint16 else idx[:n_ent].view(np.uint32)
         return out
 
     def read_counts(self):

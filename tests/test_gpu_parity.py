@@ -403,6 +403,11 @@ def test_submit_collect_pipeline_matches_oracle(hough, oracle):
     got.append({k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in r.items()})
     with pytest.raises(hough.HoughError):
         h.collect_host(0)          # nothing submitted in that slot any more
+    # the optional 16-bit copy of the lists holds the same entries as the 32-bit array
+    d, hb, _out, _host = h._slot(0)
+    n_e = int(hb["counts"].numpy().view(hough.COUNTS_DTYPE)[0]["n_hit_entries"])
+    assert n_e > 0 and np.array_equal(d["hit_index"][:n_e].cpu().numpy().view(np.uint32),
+                                      d["hit_index16"][:n_e].cpu().numpy().view(np.uint16))
     h.close()
     for res, ref in zip(got, refs):
         assert res["n_votes"] == ref["n_votes"] and res["n_peaks"] == ref["n_peaks"]
@@ -451,7 +456,9 @@ def test_three_slot_pipeline_with_pileup_events(hough, oracle):
     for res, ev in zip(got, evs):
         acc, n_votes, _ = oracle.vote(w.grid, *ev)
         pb, pm, n_peaks = oracle.peaks(w.grid, acc)
-        assert res["n_votes"] == n_votes and res["n_peaks"] == n_peaks and res["flags"] == 0
+        # events of at most 65536 hits come back with their lists as 16-bit indices (hit_index16)
+        assert res["n_votes"] == n_votes and res["n_peaks"] == n_peaks and res["flags"] == hough.INDEX16
+        assert res["hit_index"].dtype == np.uint16
         assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
         # hit lists of a sample of peaks (the oracle's list pass is O(peaks x hits))
         rng = np.random.default_rng(1)
