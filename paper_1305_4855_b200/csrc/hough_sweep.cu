@@ -46,7 +46,6 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     ptr += (size_t)(ge.chunk + EVAL_UNROLL) * 16;
     uint64_t *mbar = reinterpret_cast<uint64_t *>(ptr);
     ptr += 16;
-    int *warp_cnt = reinterpret_cast<int *>(ptr); // [32]
     ptr += 32 * 4;
     int *s_nwild = reinterpret_cast<int *>(ptr); // [4]: survivors of even / odd chunks, wild hits of even / odd chunks
 
