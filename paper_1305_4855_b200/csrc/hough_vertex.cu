@@ -84,12 +84,19 @@ __global__ void __launch_bounds__(VX_THREADS) k_vertex_vote(const VertexParams p
             s_acc[q] = 0u;
     __syncthreads();
     const uint32_t n_rep = min(p.peak_counts->n_peaks, p.cap_peaks);
-    // a group of 8 lanes shares one peak and strides the iterated axis
+    // a group of 8 lanes shares one peak and strides the iterated axis.  The vote of a peak depends on
+    // its (phi0, d0) cell only and the peaks are in ascending lin, so the peaks of one cell are
+    // neighbours in the list: the first of them votes for all, with their number as the weight
     const uint32_t sub = threadIdx.x & 7u;
     const uint32_t grp = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, n_grp = (gridDim.x * blockDim.x) >> 3;
     unsigned int votes = 0;
     for (uint32_t pk = grp; pk < n_rep; pk += n_grp) {
         const uint32_t row = p.peak_bin[pk] / (uint32_t)p.n_kappa;
+        if (pk > 0 && p.peak_bin[pk - 1] / (uint32_t)p.n_kappa == row)
+            continue;
+        uint32_t weight = 1;
+        while (pk + weight < n_rep && p.peak_bin[pk + weight] / (uint32_t)p.n_kappa == row)
+            ++weight;
         const uint32_t j = row % (uint32_t)p.n_d0, i = row / (uint32_t)p.n_d0;
         const float sn = p.sn[i], cs = p.cs[i], d = p.d0c[j];
         const bool steep = !(fabsf(cs) >= fabsf(sn));
@@ -100,10 +107,10 @@ __global__ void __launch_bounds__(VX_THREADS) k_vertex_vote(const VertexParams p
                 continue;
             const int lin = steep ? o * p.n_y + q : q * p.n_y + o;
             if (SMEM)
-                atomicAdd(&s_acc[lin], 1u);
+                atomicAdd(&s_acc[lin], weight);
             else
-                atomicAdd(&p.vacc[lin], 1u);
-            ++votes;
+                atomicAdd(&p.vacc[lin], weight);
+            votes += weight;
         }
     }
     for (int o = 16; o > 0; o >>= 1)
