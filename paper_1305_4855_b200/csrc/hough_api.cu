@@ -21,6 +21,7 @@ __global__ void __launch_bounds__(256) k_prep(const float *__restrict__ x, const
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
     __shared__ uint32_t s_layer_r[2 * 33]; // the CTA's share of the per-layer radius range
+    pdl_trigger(); // the vote kernel may set up its tile meanwhile (it waits before it reads the hits)
     if (threadIdx.x < 2 * 33)
         s_layer_r[threadIdx.x] = 0u;
     __syncthreads();

@@ -170,6 +170,31 @@ static inline void stage_mark(hough_handle *h, int slot, cudaStream_t st)
     }
 }
 
+// Programmatic dependent launch (sm_90+): a kernel launched with launch_pdl may be scheduled while its
+// predecessor in the stream is still draining; it must call pdl_wait() before it touches anything the
+// predecessor wrote (the wait returns when the predecessor has completed and flushed), and a kernel
+// lets its successor in early with pdl_trigger().  Without the attribute both are no-ops.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+#endif
+
 // kernels' host launchers (each enqueues on `st`, returns cudaGetLastError())
 cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const int32_t *layer,
                         uint32_t n, cudaStream_t st);

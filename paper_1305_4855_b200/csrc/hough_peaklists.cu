@@ -249,6 +249,8 @@ __global__ void __launch_bounds__(PL_THREADS) k_peak_lists(const PeakListParams 
     const HitIndexDev &ix = p.ix;
     const int tid = threadIdx.x, lane = tid & 31;
     const int NA = ix.NA, nL = ix.n_keys / NA - 1;
+    pdl_wait();
+    pdl_trigger();
     if (tid <= nL)
         s_lbase[tid] = ix.bin_start[tid * NA];
     if (tid == nL + 1)
@@ -531,6 +533,8 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
     const GridDev &g = p.g;
     const int lane = threadIdx.x & 31, hl = lane & 15;
     const unsigned hmask = 0xffffu << (lane & 16);
+    pdl_wait();
+    pdl_trigger();
     const uint32_t n = min(p.counters->n_peaks, p.cap_peaks);
     const uint32_t halves = (gridDim.x * blockDim.x) >> 4;
     auto put = [&](unsigned long long pos, uint32_t hit) {
@@ -657,7 +661,7 @@ cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_peak_lists, PL_THREADS, 0) != cudaSuccess || per_sm < 1)
         per_sm = 4;
-    k_peak_lists<<<h->n_sms * per_sm, PL_THREADS, 0, st>>>(p);
+    launch_pdl(k_peak_lists, dim3(h->n_sms * per_sm), dim3(PL_THREADS), 0, st, p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -683,11 +687,11 @@ cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaS
     p.hit_index16 = (out->hit_index16 && h->n_hits <= 65536u) ? out->hit_index16 : nullptr;
     p.cap_hits = h->cfg.cap_hits;
     if (h->mode == VOTE_LINE)
-        k_copy_lists<VOTE_LINE><<<h->n_sms * 16, 256, 0, st>>>(p);
+        launch_pdl(k_copy_lists<VOTE_LINE>, dim3(h->n_sms * 16), dim3(256), 0, st, p);
     else if (h->mode == VOTE_INTERVAL)
-        k_copy_lists<VOTE_INTERVAL><<<h->n_sms * 16, 256, 0, st>>>(p);
+        launch_pdl(k_copy_lists<VOTE_INTERVAL>, dim3(h->n_sms * 16), dim3(256), 0, st, p);
     else
-        k_copy_lists<VOTE_CENTRE><<<h->n_sms * 16, 256, 0, st>>>(p);
+        launch_pdl(k_copy_lists<VOTE_CENTRE>, dim3(h->n_sms * 16), dim3(256), 0, st, p);
     h->launches += 1;
     return cudaGetLastError();
 }

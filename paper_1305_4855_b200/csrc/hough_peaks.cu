@@ -76,6 +76,8 @@ template <int PEAK_RJ, int MAXJW>
 __global__ void __launch_bounds__(32 * MAXJW, 2) k_peak_sweep(const PeakParams p)
 {
     extern __shared__ uint4 ex[]; // [2][rows][32] : m3 of every row of the current plane
+    pdl_wait();
+    pdl_trigger();
     // one warp per pair of d0 rows, 256 kappa bins wide
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr int KW = 1;
@@ -275,7 +277,7 @@ cudaError_t launch_peak_sweep(hough_handle *h, cudaStream_t st)
     p.Li = h->pk_Li;
     const int Tj = 2 * p.JW - 2;
     dim3 grid((p.nk + 255) / 256, (p.n_d0 + Tj - 1) / Tj, (p.n_phi + p.Li - 1) / p.Li);
-    k_peak_sweep<2, 8><<<grid, 32 * p.JW, h->pk_smem, st>>>(p);
+    launch_pdl(k_peak_sweep<2, 8>, grid, dim3(32 * p.JW), h->pk_smem, st, p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -413,6 +415,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
     __shared__ unsigned long long s_warp[SCAN_THREADS / 32];
     __shared__ unsigned long long s_prefix;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_wait();
+    pdl_trigger();
     if (tid == 0)
         s_ticket = atomicAdd(p.ticket, 1u);
     __syncthreads();
@@ -553,7 +557,7 @@ cudaError_t launch_scan_rows(hough_handle *h, cudaStream_t st)
     ScanParams p;
     scan_params(h, &p, nullptr, 0);
     uint32_t blocks = (p.n_rows + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS;
-    k_scan<SCAN_ROWS><<<blocks, SCAN_THREADS, 0, st>>>(p);
+    launch_pdl(k_scan<SCAN_ROWS>, dim3(blocks), dim3(SCAN_THREADS), 0, st, p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -599,7 +603,7 @@ cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaSt
     ScanParams p;
     scan_params(h, &p, out, 1);
     uint32_t blocks = (h->cfg.cap_peaks + HOUGH_SCAN_ITEMS - 1) / HOUGH_SCAN_ITEMS;
-    k_scan<SCAN_LENS><<<blocks, SCAN_THREADS, 0, st>>>(p);
+    launch_pdl(k_scan<SCAN_LENS>, dim3(blocks), dim3(SCAN_THREADS), 0, st, p);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -617,6 +621,8 @@ __global__ void __launch_bounds__(256) k_compact(const uint32_t *__restrict__ fl
     const int lane = threadIdx.x & 31;
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
     const int fw_per_row = nk >> 5;
+    pdl_wait();
+    pdl_trigger();
     for (uint32_t row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < n_rows; row += warps) {
         uint32_t gb = row_base[row];
         uint32_t cnt = row_base[row + 1] - gb;
@@ -655,8 +661,8 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
     uint32_t maxb = (uint32_t)h->n_sms * 16;
     if (blocks > maxb)
         blocks = maxb;
-    k_compact<<<blocks, 256, 0, st>>>(h->flags, h->row_base, h->acc, n_rows, h->g.n_kappa,
-                                      h->cfg.cap_peaks, out->bin, out->mask);
+    launch_pdl(k_compact, dim3(blocks), dim3(256), 0, st, (const uint32_t *)h->flags, (const uint32_t *)h->row_base,
+               (const uint32_t *)h->acc, n_rows, h->g.n_kappa, h->cfg.cap_peaks, out->bin, out->mask);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -665,6 +671,7 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
 __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_peaks,
                          unsigned long long cap_hits, int with_lists, int index16)
 {
+    pdl_wait();
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         hough_counts r;
         r.n_votes = c->n_votes;
@@ -691,7 +698,8 @@ cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, in
     // the 16-bit entries are written by k_copy_lists (not by the round-1 list sweep's placement kernel)
     const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE;
     const int index16 = with_lists && !sweep && out->hit_index16 && h->n_hits <= 65536u;
-    k_finish<<<1, 32, 0, st>>>(h->counters, out->counts, h->cfg.cap_peaks, h->cfg.cap_hits, with_lists, index16);
+    launch_pdl(k_finish, dim3(1), dim3(32), 0, st, (const DevCounters *)h->counters, out->counts, h->cfg.cap_peaks,
+               (unsigned long long)h->cfg.cap_hits, with_lists, index16);
     h->launches += 1;
     return cudaGetLastError();
 }

@@ -110,12 +110,13 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
         tma_load_1d(stage + 2 * ge.chunk, p.hits.r2 + off, bytes, &mbar[0]);
         tma_load_1d(stage + 3 * ge.chunk, p.hits.bit + off, bytes, &mbar[0]);
     };
-    if (tid == 0 && n_chunks > 0)
-        issue(0);
-
-    // ---- clear the tile (a2, shared-memory part)
+    // ---- clear the tile (a2, shared-memory part); everything up to here is independent of the hits,
+    // so it may run while the preparation kernel is still draining (programmatic dependent launch)
     for (int w = tid; w < ge.tile_words; w += ge.threads)
         tile[w] = 0u;
+    pdl_wait();
+    if (tid == 0 && n_chunks > 0)
+        issue(0);
     __syncthreads();
 
     const float ab_c1 = p.ab.c1, ab_c0 = p.ab.c0;
@@ -488,5 +489,15 @@ cudaError_t launch_vote(hough_handle *h, cudaStream_t st)
         return e;
     h->fused_valid = p.fused_flags != nullptr ? 1 : 0;
     void *args[] = {(void *)&p};
-    return cudaLaunchKernel(fn, dim3(p.geom.n_tiles), dim3(p.geom.threads), args, p.geom.smem_bytes, st);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(p.geom.n_tiles);
+    cfg.blockDim = dim3(p.geom.threads);
+    cfg.dynamicSmemBytes = (size_t)p.geom.smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelExC(&cfg, fn, args);
 }
