@@ -73,10 +73,13 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
     uint32_t n_pad = ((n + HOUGH_CHUNK - 1) / HOUGH_CHUNK) * HOUGH_CHUNK;
     if (n_pad == 0)
         return cudaSuccess;
-    // histogram / cursor and the per-layer radius range of the event's hit index start from zero
-    cudaError_t e = cudaMemsetAsync(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4 + 2 * 33 * 4, st);
-    if (e != cudaSuccess)
-        return e;
+    // the key histogram starts from zero: k_index_scan leaves it so; where no index is built (vote variants,
+    // HOUGH_OPT_LIST_SWEEP) nobody reads it, but it is cleared all the same
+    if ((h->cfg.options & HOUGH_OPT_LIST_SWEEP) || h->mode != VOTE_CENTRE) {
+        cudaError_t e = cudaMemsetAsync(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4, st);
+        if (e != cudaSuccess)
+            return e;
+    }
     k_prep<<<(n_pad + 255) / 256, 256, 0, st>>>(x, y, layer, n, n_pad, h->cfg.n_layers, h->hx, h->hy, h->hr2,
                                                 h->hbit, h->counters, h->ix);
     h->launches += 1;
@@ -226,6 +229,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     void *t_sne = cv.take((size_t)(c->n_phi + 1) * 4), *t_cse = cv.take((size_t)(c->n_phi + 1) * 4);
     void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 33 * 4); // histogram | per-layer radius range (one memset)
     void *ix_start = cv.take((size_t)(n_keys + 1) * 4);
+    void *ix_cur = cv.take((size_t)n_keys * 4);
     void *ix_key = cv.take((size_t)hp * 4);
     void *ix_rec = cv.take((size_t)hp * 16);
     // reset region: counters | tickets | status words (kept contiguous for one memset)
@@ -262,10 +266,13 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ix.bin_cnt = (uint32_t *)ix_cnt;
         h->ix.layer_r = (uint32_t *)ix_cnt + n_keys;
         h->ix.bin_start = (uint32_t *)ix_start;
+        h->ix.bin_cur = (uint32_t *)ix_cur;
         h->ix.key = (uint32_t *)ix_key;
         h->ix.rec = (float4 *)ix_rec;
         h->n_pairs = (unsigned long long *)((unsigned char *)counters + 128);
         h->counters = (DevCounters *)counters;
+        h->cnt2[0] = (DevCounters *)counters;
+        h->cnt2[1] = (DevCounters *)((unsigned char *)counters + 192);
         h->scan_ticket = (unsigned int *)((unsigned char *)counters + 64);
         h->scan_status = (unsigned long long *)((unsigned char *)counters + 256);
         h->scan_blocks_max = sb;
@@ -510,6 +517,9 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     ok &= cudaMemcpy(h->t_twod0, twod0, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_d0sq, d0sq, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemset(h->counters, 0, 256 + (size_t)2 * h->scan_blocks_max * 8) == cudaSuccess;
+    ok &= cudaMemset(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4 + 2 * 33 * 4) == cudaSuccess;
+    h->cbuf = 0;
+    h->next_clean = 1;
     free(sn);
     free(cs);
     free(d0c);
@@ -589,7 +599,12 @@ int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *l
         h->ix_pending = 0;
     }
     stage_mark(h, 0, st);
-    CK(cudaMemsetAsync(h->counters, 0, 64, st));
+    // the event's counters: the block the previous hough_peaks cleared (k_finish), else a memset
+    h->cbuf ^= 1;
+    h->counters = h->cnt2[h->cbuf];
+    if (!h->next_clean)
+        CK(cudaMemsetAsync(h->counters, 0, 64, st));
+    h->next_clean = 0;
     CK(launch_prep(h, x, y, layer, n, st));
     if (!(h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE && n > 0) {
         // beside the vote kernel, on the library's own stream (joined before the list kernel)
@@ -615,7 +630,13 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     if (!h->voted)
         return HOUGH_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    CK(cudaMemsetAsync((unsigned char *)h->counters + 64, 0, 192 + (size_t)2 * h->scan_blocks_max * 8, st));
+    // tickets, work counter and look-back words were cleared by the previous call's k_finish -- unless that
+    // call failed on the way
+    if (h->peaks_dirty)
+        CK(cudaMemsetAsync((unsigned char *)h->cnt2[0] + 64, 0, 128, st));
+    if (h->peaks_dirty)
+        CK(cudaMemsetAsync(h->scan_status, 0, (size_t)2 * h->scan_blocks_max * 8, st));
+    h->peaks_dirty = 1;
     // a5: the streaming sweep; or, fused variant, only the cells on the vote tiles' edges (the others were
     // flagged by hough_vote's kernel -- not after hough_set_accumulator, which leaves no such flags)
     if ((h->cfg.options & HOUGH_OPT_FUSED_PEAKS) && h->fused_valid)
@@ -645,6 +666,8 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
         stage_mark(h, ST_PLACE_LISTS + 1, st);
     }
     CK(launch_finish_counts(h, out, with_lists, st));
+    h->next_clean = 1;
+    h->peaks_dirty = 0;
     stage_mark(h, ST_FINISH + 1, st);
     return HOUGH_OK;
 }

@@ -83,9 +83,11 @@ struct HitsDev {         // prepared hits, SoA, padded with non-voting entries t
 struct HitIndexDev {
     int NA;                 // azimuth bins per layer (power of two, 256 .. 16384)
     int n_keys;             // (n_layers + 1) * NA
-    uint32_t *bin_cnt;      // [n_keys] histogram of the event (k_prep), then the scatter cursor
+    uint32_t *bin_cnt;      // [n_keys] histogram of the event (k_prep); k_index_scan leaves it zero for the next event
+    uint32_t *bin_cur;      // [n_keys] scatter cursor (k_index_scan: rank of the first hit of the key)
     uint32_t *bin_start;    // [n_keys + 1] rank of the first hit of a key
-    uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) (zeroed per event)
+    uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) over the handle's events so far
+                            // (zeroed by hough_create only: the windows are supersets for any wider range)
     uint32_t *key;          // [max_hits_pad] key of hit h, 0xffffffff = not indexed (bad layer)
     float4 *rec;            // [max_hits_pad] the hits in key order: (x, y, r2, bits of the hit index)
 };
@@ -134,7 +136,10 @@ struct hough_handle {
     unsigned long long *n_pairs; // entries emitted (lives in the per-hough_peaks reset region)
     unsigned long long *scan_status; // look-back words of the chained scans
     unsigned int *scan_ticket;       // [4]
-    DevCounters *counters;
+    DevCounters *counters;   // the current event's counters = cnt2[cbuf]
+    DevCounters *cnt2[2];    // two blocks: k_finish clears the one the next hough_vote will use
+    int cbuf, next_clean;
+    int peaks_dirty;         // a hough_peaks call did not get as far as its k_finish: clear its scratch by memset
     uint32_t scan_blocks_max;
     // sweep tile geometry of the peak kernel
     int pk_JW, pk_Li, pk_smem;

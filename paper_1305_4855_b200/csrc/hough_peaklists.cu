@@ -51,7 +51,7 @@
 // n_keys is a multiple of 256 (NA >= 256), so uint4 accesses never straddle the end.
 #define IS_V 4
 __global__ void __launch_bounds__(1024) k_index_scan(uint32_t *__restrict__ cnt, uint32_t *__restrict__ start,
-                                                     int n_keys)
+                                                     uint32_t *__restrict__ cur, int n_keys)
 {
     __shared__ uint32_t s_warp[IS_V][32];
     __shared__ uint32_t s_carry;
@@ -115,7 +115,8 @@ __global__ void __launch_bounds__(1024) k_index_scan(uint32_t *__restrict__ cnt,
                 o.z = o.y + v[q].y;
                 o.w = o.z + v[q].z;
                 *reinterpret_cast<uint4 *>(start + k) = o;
-                *reinterpret_cast<uint4 *>(cnt + k) = make_uint4(0u, 0u, 0u, 0u); // becomes the scatter cursor
+                *reinterpret_cast<uint4 *>(cur + k) = o;                          // the scatter cursor
+                *reinterpret_cast<uint4 *>(cnt + k) = make_uint4(0u, 0u, 0u, 0u); // clean for the next event
             }
         }
         carry = s_carry;
@@ -135,7 +136,7 @@ __global__ void __launch_bounds__(256) k_index_scatter(HitIndexDev ix, const flo
     const uint32_t key = ix.key[h];
     if (key == 0xffffffffu)
         return;
-    const uint32_t rank = ix.bin_start[key] + atomicAdd(&ix.bin_cnt[key], 1u);
+    const uint32_t rank = atomicAdd(&ix.bin_cur[key], 1u);
     ix.rec[rank] = make_float4(hx[h], hy[h], hr2[h], __uint_as_float(h));
 }
 
@@ -143,7 +144,7 @@ cudaError_t launch_index_build(hough_handle *h, cudaStream_t st)
 {
     if (h->n_hits == 0)
         return cudaSuccess;
-    k_index_scan<<<1, 1024, 0, st>>>(h->ix.bin_cnt, h->ix.bin_start, h->ix.n_keys);
+    k_index_scan<<<1, 1024, 0, st>>>(h->ix.bin_cnt, h->ix.bin_start, h->ix.bin_cur, h->ix.n_keys);
     k_index_scatter<<<(h->n_hits + 255) / 256, 256, 0, st>>>(h->ix, h->hx, h->hy, h->hr2, h->n_hits);
     h->launches += 2;
     return cudaGetLastError();

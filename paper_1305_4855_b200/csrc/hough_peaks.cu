@@ -668,10 +668,19 @@ cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStre
 }
 
 // ------------------------------------------------------------------ counters out
+// Also clears what the next calls expect clean: the other counter block (the next hough_vote's), the scan
+// tickets / work counter and the look-back words (the next hough_peaks').
 __global__ void k_finish(const DevCounters *c, hough_counts *out, uint32_t cap_peaks,
-                         unsigned long long cap_hits, int with_lists, int index16)
+                         unsigned long long cap_hits, int with_lists, int index16, uint32_t *next_counters,
+                         uint32_t *reset, uint32_t reset_words, uint32_t *status, uint32_t status_words)
 {
     pdl_wait();
+    if (threadIdx.x < 16)
+        next_counters[threadIdx.x] = 0u;
+    for (uint32_t w = threadIdx.x; w < reset_words; w += blockDim.x)
+        reset[w] = 0u;
+    for (uint32_t w = threadIdx.x; w < status_words; w += blockDim.x)
+        status[w] = 0u;
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         hough_counts r;
         r.n_votes = c->n_votes;
@@ -698,8 +707,10 @@ cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, in
     // the 16-bit entries are written by k_copy_lists (not by the round-1 list sweep's placement kernel)
     const int sweep = (h->cfg.options & HOUGH_OPT_LIST_SWEEP) && h->mode == VOTE_CENTRE;
     const int index16 = with_lists && !sweep && out->hit_index16 && h->n_hits <= 65536u;
-    launch_pdl(k_finish, dim3(1), dim3(32), 0, st, (const DevCounters *)h->counters, out->counts, h->cfg.cap_peaks,
-               (unsigned long long)h->cfg.cap_hits, with_lists, index16);
+    unsigned char *base = (unsigned char *)h->cnt2[0];
+    launch_pdl(k_finish, dim3(1), dim3(1024), 0, st, (const DevCounters *)h->counters, out->counts, h->cfg.cap_peaks,
+               (unsigned long long)h->cfg.cap_hits, with_lists, index16, (uint32_t *)h->cnt2[h->cbuf ^ 1],
+               (uint32_t *)(base + 64), 32u, (uint32_t *)h->scan_status, (uint32_t)(4 * h->scan_blocks_max));
     h->launches += 1;
     return cudaGetLastError();
 }
