@@ -19,7 +19,8 @@
 
 struct VertexParams {
     // first transform
-    int n_d0, n_kappa;
+    int n_phi, n_d0, n_kappa;
+    double d0_min, d0_max;
     const float *sn, *cs, *d0c;
     const uint32_t *peak_bin;
     const hough_counts *peak_counts;
@@ -211,7 +212,25 @@ __global__ void __launch_bounds__(VX_THREADS) k_vertex_compact(const VertexParam
     }
 }
 
-// V4: one CTA per reported vertex sweeps the reported peaks in order
+// V4: one CTA per reported vertex.  The peaks are in ascending lin = ((i * n_d0 + j) * n_kappa + k), so the
+// peaks of a (phi0, d0) cell are neighbours in the list and the cells of one phi0 row i follow each other.
+// For the vertex bin (a, b) and a row i only the cells whose d0 centre lies within the bin's image
+// d = -xv sin + yv cos can vote into it: thread = phi0 row finds that d0 interval (one d0 bin of margin on
+// each side), brackets its peaks in the list by two binary searches and evaluates the EXACT V2 vote for
+// them only; a block scan over the rows keeps the members in ascending peak position.
+__device__ __forceinline__ uint32_t vx_lower_bound(const uint32_t *__restrict__ bin, uint32_t n, uint32_t key)
+{
+    uint32_t lo = 0, hi = n; // first position with bin[pos] >= key
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (bin[mid] < key)
+            lo = mid + 1;
+        else
+            hi = mid;
+    }
+    return lo;
+}
+
 template <bool FILL>
 __global__ void __launch_bounds__(VX_THREADS) k_vertex_members(const VertexParams p)
 {
@@ -241,23 +260,61 @@ __global__ void __launch_bounds__(VX_THREADS) k_vertex_members(const VertexParam
     const uint32_t vlin = p.out_bin[m];
     const int va = (int)(vlin / (uint32_t)p.n_y), vb = (int)(vlin - (uint32_t)va * (uint32_t)p.n_y);
     const float xca = vx_centre(p.x_min, p.x_max, p.n_x, va), ycb = vx_centre(p.y_min, p.y_max, p.n_y, vb);
+    // the bin's edges and the d0 grid, in binary64
+    const double wx = (p.x_max - p.x_min) / (double)p.n_x, wy = (p.y_max - p.y_min) / (double)p.n_y;
+    const double xe0 = p.x_min + va * wx, xe1 = xe0 + wx, ye0 = p.y_min + vb * wy, ye1 = ye0 + wy;
+    const double dd0 = p.n_d0 > 1 ? (p.d0_max - p.d0_min) / (double)p.n_d0 : 1.0;
     const uint32_t n_rep = min(p.peak_counts->n_peaks, p.cap_peaks);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t total = 0;
-    for (uint32_t base = 0; base < n_rep; base += VX_THREADS) {
-        const uint32_t pk = base + threadIdx.x;
-        bool in = false;
-        if (pk < n_rep) {
-            const uint32_t row = p.peak_bin[pk] / (uint32_t)p.n_kappa;
-            const uint32_t j = row % (uint32_t)p.n_d0, i = row / (uint32_t)p.n_d0;
-            const float sn = p.sn[i], cs = p.cs[i], d = p.d0c[j];
-            const bool steep = !(fabsf(cs) >= fabsf(sn));
-            const int o = vx_vote_one(p, sn, cs, d, steep, steep ? ycb : xca);
-            in = o >= 0 && o == (steep ? va : vb);
+    for (int i0 = 0; i0 < p.n_phi; i0 += VX_THREADS) {
+        const int i = i0 + (int)threadIdx.x;
+        uint32_t p0 = 0, p1 = 0, cnt = 0;
+        float sn = 0.f, cs = 0.f;
+        bool steep = false;
+        if (i < p.n_phi) {
+            sn = p.sn[i];
+            cs = p.cs[i];
+            steep = !(fabsf(cs) >= fabsf(sn));
+            // image of the bin along the voted axis: d between these two values (either order)
+            double da, db;
+            if (!steep) { // yv = (d + xc sn) / cs in [ye0, ye1)  ->  d = yv cs - xc sn
+                da = ye0 * (double)cs - (double)xca * (double)sn;
+                db = ye1 * (double)cs - (double)xca * (double)sn;
+            } else {      // xv = (yc cs - d) / sn in [xe0, xe1)  ->  d = yc cs - xv sn
+                da = (double)ycb * (double)cs - xe0 * (double)sn;
+                db = (double)ycb * (double)cs - xe1 * (double)sn;
+            }
+            const double dlo = fmin(da, db) - dd0, dhi = fmax(da, db) + dd0;
+            int j0 = 0, j1 = p.n_d0 - 1;
+            if (p.n_d0 > 1 && dlo == dlo && dhi == dhi) { // d0 centres d0_min + (j + 0.5) dd0 inside [dlo, dhi]
+                const double t0 = floor((dlo - p.d0_min) / dd0 - 0.5), t1 = ceil((dhi - p.d0_min) / dd0 - 0.5);
+                j0 = t0 < 0.0 ? 0 : (t0 > (double)(p.n_d0 - 1) ? p.n_d0 : (int)t0);
+                j1 = t1 < 0.0 ? -1 : (t1 > (double)(p.n_d0 - 1) ? p.n_d0 - 1 : (int)t1);
+            }
+            if (j0 <= j1) {
+                const uint32_t r0 = (uint32_t)i * (uint32_t)p.n_d0 + (uint32_t)j0, r1 = (uint32_t)i * (uint32_t)p.n_d0 + (uint32_t)j1;
+                p0 = vx_lower_bound(p.peak_bin, n_rep, r0 * (uint32_t)p.n_kappa);
+                // (r1 + 1) * n_kappa may be 2^32 for the very last row: then every remaining peak is in range
+                const unsigned long long end = ((unsigned long long)r1 + 1ull) * (unsigned long long)p.n_kappa;
+                p1 = end > 0xffffffffull ? n_rep : vx_lower_bound(p.peak_bin, n_rep, (uint32_t)end);
+            }
+            for (uint32_t pk = p0; pk < p1; ++pk) {
+                const uint32_t row = p.peak_bin[pk] / (uint32_t)p.n_kappa;
+                const uint32_t j = row % (uint32_t)p.n_d0;
+                const int o = vx_vote_one(p, sn, cs, p.d0c[j], steep, steep ? ycb : xca);
+                cnt += (o >= 0 && o == (steep ? va : vb)) ? 1u : 0u;
+            }
         }
-        const unsigned bal = __ballot_sync(0xffffffffu, in);
-        if (lane == 0)
-            s_wcnt[warp] = (uint32_t)__popc(bal);
+        // ordered placement: exclusive scan of the rows' counts over the block
+        uint32_t incl = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o)
+                incl += t;
+        }
+        if (lane == 31)
+            s_wcnt[warp] = incl;
         __syncthreads();
         uint32_t before = 0, all = 0;
         for (int q = 0; q < VX_THREADS / 32; ++q) {
@@ -265,10 +322,18 @@ __global__ void __launch_bounds__(VX_THREADS) k_vertex_members(const VertexParam
             before += q < warp ? c : 0u;
             all += c;
         }
-        if (FILL && in) {
-            const unsigned long long pos = w + total + before + (uint32_t)__popc(bal & ((1u << lane) - 1u));
-            if (pos < p.cap_members)
-                p.member_index[pos] = pk;
+        if (FILL && cnt) {
+            unsigned long long pos = w + total + before + incl - cnt;
+            for (uint32_t pk = p0; pk < p1; ++pk) {
+                const uint32_t row = p.peak_bin[pk] / (uint32_t)p.n_kappa;
+                const uint32_t j = row % (uint32_t)p.n_d0;
+                const int o = vx_vote_one(p, sn, cs, p.d0c[j], steep, steep ? ycb : xca);
+                if (o >= 0 && o == (steep ? va : vb)) {
+                    if (pos < p.cap_members)
+                        p.member_index[pos] = pk;
+                    ++pos;
+                }
+            }
         }
         total += all;
         __syncthreads();
@@ -326,8 +391,11 @@ int hough_vertices(hough_handle *h, const hough_vertex_config *v, void *workspac
     const size_t n_bins = (size_t)v->n_x * v->n_y, n_blocks = (n_bins + VX_THREADS - 1) / VX_THREADS;
     unsigned char *w = (unsigned char *)workspace;
     VertexParams p;
+    p.n_phi = h->cfg.n_phi;
     p.n_d0 = h->cfg.n_d0;
     p.n_kappa = h->cfg.n_kappa;
+    p.d0_min = h->cfg.d0_min;
+    p.d0_max = h->cfg.d0_max;
     p.sn = h->t_sn;
     p.cs = h->t_cs;
     p.d0c = h->t_d0c;

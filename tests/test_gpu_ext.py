@@ -94,6 +94,26 @@ def test_vertices_jets_workload(hough, oracle):
         h.close()
 
 
+def test_vertices_over_the_peaks_of_a_pileup_event(hough, oracle):
+    """4.9e5 peaks (BASELINE.json configs[2]) into 32 x 32 and 100 x 60 vertex grids: the member lists
+    come from the d0 rows that can reach the vertex bin (binary searches in the sorted peak list)."""
+    w = synth.WORKLOADS["pileup"]
+    x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
+    acc, _nv, _nb = oracle.vote(w.grid, x, y, layer)
+    pb, _pm, n_peaks = oracle.peaks(w.grid, acc)
+    h = hough.Hough(w.grid, len(x), w.cap_peaks, w.cap_hits)
+    h.vote(dev(x), dev(y), dev(layer))
+    h.peaks(lists=False)
+    assert np.array_equal(h.read(lists=False)["peak_bin"], pb)
+    for vg, cap_v in ((synth.JETS_VGRID, 1024), (synth.VertexGrid(n_x=100, n_y=60, V_min=2500, x_min=-9.0, x_max=11.0,
+                                                                   y_min=-6.0, y_max=6.0), 4096)):
+        vref = oracle.run_vertices(w.grid, vg, pb)
+        assert vref["n_vertices"] > 10
+        h.vertices(vg, cap_vertices=cap_v, cap_members=1 << 23)
+        assert_vertices_same(h.read_vertices(), vref)
+    h.close()
+
+
 def test_vertices_truncation_and_no_peaks(hough, oracle):
     rng = np.random.default_rng(5)
     g = synth.Grid(n_phi=64, n_d0=16, n_kappa=32, L_min=2)
