@@ -137,3 +137,41 @@ def test_two_ranks_shard_events_and_reduce(tmp_path):
     assert total_ms == 15.0                              # max over ranks
     assert votes == float(sum(1000 + s for s in range(6)))
     assert evals == 600.0 and events == 6.0
+
+
+def test_binding_structs_have_the_layout_of_the_header(hough, tmp_path):
+    """The ctypes structures of the binding against sizeof / offsetof of include/hough.h as gcc sees it
+    (a field added on one side only would shift every pointer after it)."""
+    import subprocess
+    structs = {
+        "hough_config": (hough.Config, ["n_layers", "layer_radius_cm", "phi_min", "kappa_max", "n_phi", "L_min",
+                                        "max_hits", "cap_peaks", "cap_hits", "tile_phi", "options", "device"]),
+        "hough_counts": (hough.Counts, ["n_votes", "n_hit_entries", "n_evals", "n_list_evals", "n_peaks",
+                                        "n_bad_hits", "flags"]),
+        "hough_peaks_out": (hough.PeaksOut, ["bin", "mask", "hit_offset", "hit_index", "counts", "hit_index16"]),
+        "hough_host_out": (hough.HostOut, ["bin", "mask", "hit_offset", "hit_index", "counts", "hit_index16"]),
+        "hough_vertex_config": (hough.VertexConfig, ["x_min", "y_max", "n_x", "V_min", "cap_vertices", "cap_members"]),
+        "hough_vertex_out": (hough.VertexOut, ["bin", "count", "member_offset", "member_index", "counts"]),
+        "hough_fit_config": (hough.FitConfig, ["rms_max", "min_shared", "reserved"]),
+        "hough_fit_out": (hough.FitOut, ["kappa", "phi0", "d0", "rms", "status", "flag", "kept", "counts"]),
+    }
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "hough.h"', 'int main(void) {']
+    for name, (_cls, fields) in structs.items():
+        lines.append('printf("%s %%zu\\n", sizeof(%s));' % (name, name))
+        for f in fields:
+            lines.append('printf("%s.%s %%zu\\n", offsetof(%s, %s));' % (name, f, name, f))
+    lines.append('printf("hough_vertex_counts %zu\\n", sizeof(hough_vertex_counts));')
+    lines.append('printf("hough_fit_counts %zu\\n", sizeof(hough_fit_counts));')
+    lines += ['return 0; }']
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    out = dict(l.split() for l in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    for name, (cls, fields) in structs.items():
+        assert int(out[name]) == C.sizeof(cls), name
+        for f in fields:
+            assert int(out["%s.%s" % (name, f)]) == getattr(cls, f).offset, (name, f)
+    assert int(out["hough_counts"]) == hough.COUNTS_DTYPE.itemsize == 48
+    assert int(out["hough_vertex_counts"]) == hough.VERTEX_COUNTS_DTYPE.itemsize
+    assert int(out["hough_fit_counts"]) == hough.FIT_COUNTS_DTYPE.itemsize
