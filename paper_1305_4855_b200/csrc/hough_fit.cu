@@ -164,24 +164,22 @@ __global__ void __launch_bounds__(FIT_THREADS) k_fit(const FitParams p)
         p.counts->n_fitted = n_rep;
 }
 
-// exclusive scan of inv_start[0 .. n_hits) in place, total at [n_hits]; copy into the fill cursor
+// exclusive scan of inv_start[0 .. n_hits) in place, total at [n_hits]; copy into the fill cursor.
+// One CTA; warp w owns the contiguous chunk [w * per, (w + 1) * per) and walks it 32 items at a time
+// (coalesced), first for its sum, then -- after the scan of the 32 warp sums -- for the prefixes.
 __global__ void __launch_bounds__(1024) k_inv_scan(const FitParams p)
 {
     __shared__ uint32_t s_warp[32];
-    const uint32_t n = p.n_hits, per = (n + 1023u) / 1024u;
-    const uint32_t b0 = min(threadIdx.x * per, n), b1 = min(b0 + per, n);
-    uint32_t sum = 0;
-    for (uint32_t q = b0; q < b1; ++q)
-        sum += p.inv_start[q];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t inc = sum;
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o)
-            inc += t;
-    }
-    if (lane == 31)
-        s_warp[warp] = inc;
+    const uint32_t n = p.n_hits, per = ((n + 1023u) / 1024u) * 32u;
+    const uint32_t b0 = min((uint32_t)warp * per, n), b1 = min(b0 + per, n);
+    uint32_t sum = 0;
+    for (uint32_t q = b0 + lane; q < b1; q += 32)
+        sum += p.inv_start[q];
+    for (int o = 16; o > 0; o >>= 1)
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if (lane == 0)
+        s_warp[warp] = sum;
     __syncthreads();
     if (warp == 0) {
         uint32_t w = s_warp[lane];
@@ -190,15 +188,24 @@ __global__ void __launch_bounds__(1024) k_inv_scan(const FitParams p)
             if (lane >= o)
                 w += t;
         }
-        s_warp[lane] = w;
+        s_warp[lane] = w; // inclusive over the warps
     }
     __syncthreads();
-    uint32_t run = inc - sum + (warp > 0 ? s_warp[warp - 1] : 0u);
-    for (uint32_t q = b0; q < b1; ++q) {
-        const uint32_t v = p.inv_start[q];
-        p.inv_start[q] = run;
-        p.inv_cur[q] = run;
-        run += v;
+    uint32_t run = warp > 0 ? s_warp[warp - 1] : 0u;
+    for (uint32_t q0 = b0; q0 < b1; q0 += 32) {
+        const uint32_t q = q0 + lane;
+        const uint32_t v = q < b1 ? p.inv_start[q] : 0u;
+        uint32_t incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o)
+                incl += t;
+        }
+        if (q < b1) {
+            p.inv_start[q] = run + incl - v;
+            p.inv_cur[q] = run + incl - v;
+        }
+        run += __shfl_sync(0xffffffffu, incl, 31);
     }
     if (threadIdx.x == 1023)
         p.inv_start[n] = s_warp[31];
@@ -231,9 +238,13 @@ __global__ void __launch_bounds__(FIT_THREADS) k_dedup(const FitParams p)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t n_warps = gridDim.x * (FIT_THREADS / 32);
     unsigned long long tests = 0;
-    for (uint32_t c = blockIdx.x * (FIT_THREADS / 32) + warp; c < n_rep; c += n_warps) {
-        if (!p.flag[c])
-            continue;
+    // a warp looks at 32 candidates at a time (one coalesced read of their flags) and takes the selected
+    // ones among them one after the other
+    for (uint32_t c32 = (blockIdx.x * (FIT_THREADS / 32) + warp) * 32u; c32 < n_rep; c32 += n_warps * 32u) {
+      unsigned todo = __ballot_sync(0xffffffffu, c32 + lane < n_rep && p.flag[c32 + lane] != 0);
+      while (todo) {
+        const uint32_t c = c32 + (uint32_t)(__ffs((int)todo) - 1);
+        todo &= todo - 1;
         const unsigned long long o0 = p.hit_offset[c];
         const uint32_t np = (uint32_t)(p.hit_offset[c + 1] - o0);
         const uint32_t *A = p.hit_index + o0;
@@ -295,6 +306,7 @@ __global__ void __launch_bounds__(FIT_THREADS) k_dedup(const FitParams p)
         }
         if (dup && lane == 0)
             p.flag[c] = 2;
+      }
     }
     for (int o = 16; o > 0; o >>= 1)
         tests += __shfl_xor_sync(0xffffffffu, tests, o);
