@@ -514,6 +514,35 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
     if sweeps:
         out["ncu_sweeps"] = dict(sweeps, note="copied from the committed ncu capture, not measured in this run")
 
+    # the rows after the hot path, on the same events: f2 fit + duplicate removal, f1 second
+    # transform over the peaks; device times per event, CUDA events around the C-ABI calls
+    hx = hough.Hough(g, max(len(e[0]) for e in d_events), workload.cap_peaks, workload.cap_hits, device=local_rank)
+    st0 = torch.cuda.current_stream()
+    t_fit, t_vx, n_x, kept, nvx = 0.0, 0.0, 0, 0, 0
+    for r in range(2):
+        for ev in d_events[:min(n_ev, 5)]:
+            hx.vote(*ev)
+            hx.peaks()
+            ea, eb, ec = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            ea.record(st0)
+            hx.fit(0.01, 3)
+            eb.record(st0)
+            hx.vertices(synth.JETS_VGRID)
+            ec.record(st0)
+            ec.synchronize()
+            if r > 0:
+                t_fit += ea.elapsed_time(eb)
+                t_vx += eb.elapsed_time(ec)
+                n_x += 1
+                kept += hx.read_fit()["n_kept"]
+                nvx += hx.read_vertices()["n_vertices"]
+    hx.close()
+    out["next_rows"] = {"hough_fit_ms_per_event": t_fit / n_x, "hough_vertices_ms_per_event": t_vx / n_x,
+                        "tracks_kept_per_event": kept / n_x, "vertices_per_event": nvx / n_x,
+                        "note": "f2: circle fit of every peak's list, selection at rms <= 100 um, duplicates sharing "
+                                ">= 3 hits removed; f1: second transform of all reported peaks into a 32 x 32 vertex "
+                                "grid (parity against the oracle in tests/test_gpu_ext.py)"}
+
     # a5 variants, measured: stand-alone streaming sweep, peak test fused into the
     # vote tile + tile-edge pass (HOUGH_OPT_FUSED_PEAKS), cell-wise kernel over every cell
     def peak_variant(wl, evs, options, reps=3):
