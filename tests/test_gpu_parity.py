@@ -547,3 +547,63 @@ def test_random_configurations_share_the_process(hough, oracle):
                       cap_hits=max(ref["n_hit_entries"], 1) + 3, tile_phi=tile[0], tile_d0=tile[1],
                       options=opts)
         assert_same(res, ref)
+
+
+def test_call_patterns_on_one_handle(hough, oracle):
+    """Two long-lived handles (default and HOUGH_OPT_LIST_SWEEP) through 80 events of random sizes and
+    call patterns -- vote twice, peaks twice, peaks without lists then with, a hand-made accumulator in
+    between, the host entry point -- every result against the oracle.  The library keeps its per-event
+    scratch clean without memsets (counters double-buffered, k_finish prepares the next calls): this
+    is the test of that bookkeeping."""
+    rng = np.random.default_rng(77)
+    g = synth.Grid(n_phi=96, n_d0=12, n_kappa=64, L_min=4)
+    handles = [hough.Hough(g, 4000, g.n_bins // 2 + 1, 1 << 22),
+               hough.Hough(g, 4000, g.n_bins // 2 + 1, 1 << 22, options=hough.OPT_LIST_SWEEP)]
+
+    def event():
+        n = int(rng.choice([0, 1, 50, 700, 2500, 4000]))
+        r, ph = rng.uniform(0.5, 80, n), rng.uniform(-math.pi, math.pi, n)
+        return ((r * np.cos(ph)).astype(np.float32), (r * np.sin(ph)).astype(np.float32),
+                rng.integers(-1, 11, n).astype(np.int32))
+
+    for it in range(80):
+        h = handles[0] if rng.random() < 0.7 else handles[1]
+        x, y, layer = event()
+        ref = oracle.run(g, x, y, layer)
+        pat = int(rng.integers(0, 6))
+        if pat == 0:      # a second vote replaces the first
+            xa, ya, la = event()
+            h.vote(dev(xa), dev(ya), dev(la))
+            h.vote(dev(x), dev(y), dev(layer))
+            h.peaks()
+        elif pat == 1:    # peaks twice
+            h.vote(dev(x), dev(y), dev(layer))
+            h.peaks()
+            h.peaks()
+        elif pat == 2:    # without lists, then with
+            h.vote(dev(x), dev(y), dev(layer))
+            h.peaks(lists=False)
+            h.peaks()
+        elif pat == 3:    # a hand-made accumulator in between
+            acc = rng.integers(0, 1 << 10, g.n_bins, dtype=np.uint32)
+            h.set_accumulator(dev(acc.view(np.int32)))
+            h.peaks(lists=False)
+            pb, _pm, npk = oracle.peaks(g, acc)
+            r0 = h.read(lists=False)
+            assert r0["n_peaks"] == npk and r0["n_votes"] == 0 and np.array_equal(r0["peak_bin"], pb), it
+            h.vote(dev(x), dev(y), dev(layer))
+            h.peaks()
+        elif pat == 4:    # host entry point
+            res = h.process_host(x, y, layer)
+            res = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in res.items()}
+            res["acc"] = ref["acc"]
+            assert_same(res, ref)
+            continue
+        else:
+            h.vote(dev(x), dev(y), dev(layer))
+            h.peaks()
+        res = h.read()
+        res["acc"] = h.accumulator_host()
+        assert_same(res, ref)
+    for h in handles:
+        h.close()
