@@ -543,6 +543,31 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
                                 ">= 3 hits removed; f1: second transform of all reported peaks into a 32 x 32 vertex "
                                 "grid (parity against the oracle in tests/test_gpu_ext.py)"}
 
+    # f4, second half (SURVEY.md 8(f) "multi-event"): two handles on two streams, events
+    # alternating between them, so that the small latency-bound kernels of one event run beside the
+    # issue-bound vote of the other.  Not the headline (BASELINE.json configs[3] is one stream, back to back).
+    h2 = [hough.Hough(g, max(len(e[0]) for e in d_events), workload.cap_peaks, workload.cap_hits, device=local_rank)
+          for _ in range(2)]
+    s2 = [torch.cuda.Stream(device=dev) for _ in range(2)]
+
+    def two_stream_pass():
+        for e in range(n_ev):
+            h2[e & 1].vote(*d_events[e], stream=s2[e & 1])
+            h2[e & 1].peaks(stream=s2[e & 1])
+
+    two_stream_pass()
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    for _ in range(3):
+        two_stream_pass()
+    torch.cuda.synchronize(dev)
+    dt2 = time.perf_counter() - t0
+    for hh in h2:
+        hh.close()
+    out["two_handles_two_streams"] = {"events_per_s": 3 * n_ev / dt2, "ms_per_event": dt2 / (3 * n_ev) * 1e3,
+                                      "note": "device-resident, wall clock over 3 passes with a device synchronise on "
+                                              "both sides; each handle has its own workspace and output arrays"}
+
     # a5 variants, measured: stand-alone streaming sweep, peak test fused into the
     # vote tile + tile-edge pass (HOUGH_OPT_FUSED_PEAKS), cell-wise kernel over every cell
     def peak_variant(wl, evs, options, reps=3):
