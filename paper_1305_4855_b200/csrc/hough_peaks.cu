@@ -609,47 +609,54 @@ cudaError_t launch_scan_lens(hough_handle *h, const hough_peaks_out *out, cudaSt
 }
 
 // ------------------------------------------------------------------ compaction (a6)
-// One warp per accumulator row: ballot-free popcount prefix over the row's flag words,
-// each lane expands the set bits of its word.  Records land in ascending lin because
-// row_base is the exclusive scan of the rows in lin order.
+// G lanes per accumulator row (G = the power of two that holds the row's flag words, at most 32), so a
+// warp works on 32 / G rows at a time and their loads are in flight together: popcount prefix over the
+// row's flag words inside the lane group, each lane expands the set bits of its word.  Records land in
+// ascending lin because row_base is the exclusive scan of the rows in lin order.
+template <int G>
 __global__ void __launch_bounds__(256) k_compact(const uint32_t *__restrict__ flags,
                                                  const uint32_t *__restrict__ row_base,
                                                  const uint32_t *__restrict__ acc, uint32_t n_rows,
                                                  int nk, uint32_t cap_peaks, uint32_t *__restrict__ bin,
                                                  uint32_t *__restrict__ mask)
 {
-    const int lane = threadIdx.x & 31;
+    constexpr int R = 32 / G; // rows per warp and round
+    const int lane = threadIdx.x & 31, sl = lane % G, slot = lane / G;
     const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
     const int fw_per_row = nk >> 5;
     pdl_wait();
     pdl_trigger();
-    for (uint32_t row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < n_rows; row += warps) {
-        uint32_t gb = row_base[row];
-        uint32_t cnt = row_base[row + 1] - gb;
-        if (cnt == 0u || gb >= cap_peaks)
-            continue;
+    for (uint32_t row0 = ((blockIdx.x * blockDim.x + threadIdx.x) >> 5) * R; row0 < n_rows; row0 += warps * R) {
+        const uint32_t row = row0 + (uint32_t)slot;
+        uint32_t gb = 0, cnt = 0;
+        if (row < n_rows) {
+            gb = row_base[row];
+            cnt = row_base[row + 1] - gb;
+        }
+        const bool live = cnt != 0u && gb < cap_peaks;
         const uint32_t *fw = flags + (size_t)row * fw_per_row;
         uint32_t rank0 = gb;
-        for (int wb = 0; wb < fw_per_row; wb += 32) {
-            uint32_t f = (wb + lane < fw_per_row) ? fw[wb + lane] : 0u;
+        for (int wb = 0; wb < fw_per_row; wb += G) { // one round unless a row has more than 32 flag words
+            uint32_t f = (live && wb + sl < fw_per_row) ? fw[wb + sl] : 0u;
             uint32_t pc = __popc(f), incl = pc;
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o)
+#pragma unroll
+            for (int o = 1; o < G; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o, G);
+                if (sl >= o)
                     incl += t;
             }
             uint32_t rank = rank0 + incl - pc;
             while (f) {
-                int b = __ffs(f) - 1;
+                const int b = __ffs(f) - 1;
                 f &= f - 1;
                 if (rank < cap_peaks) {
-                    uint32_t lin = row * (uint32_t)nk + (uint32_t)(((wb + lane) << 5) + b);
+                    const uint32_t lin = row * (uint32_t)nk + (uint32_t)(((wb + sl) << 5) + b);
                     bin[rank] = lin;
                     mask[rank] = acc[lin];
                 }
                 ++rank;
             }
-            rank0 += __shfl_sync(0xffffffffu, incl, 31);
+            rank0 += __shfl_sync(0xffffffffu, incl, G - 1, G);
         }
     }
 }
@@ -657,12 +664,27 @@ __global__ void __launch_bounds__(256) k_compact(const uint32_t *__restrict__ fl
 cudaError_t launch_compact(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
 {
     uint32_t n_rows = (uint32_t)h->g.n_phi * (uint32_t)h->g.n_d0;
-    uint32_t blocks = (n_rows + 7) / 8;
+    const int fwr = h->g.n_kappa >> 5, lanes = fwr <= 2 ? 2 : fwr <= 4 ? 4 : fwr <= 8 ? 8 : fwr <= 16 ? 16 : 32;
+    uint32_t blocks = (n_rows + 8 * (32 / lanes) - 1) / (8 * (32 / lanes));
     uint32_t maxb = (uint32_t)h->n_sms * 16;
     if (blocks > maxb)
         blocks = maxb;
-    launch_pdl(k_compact, dim3(blocks), dim3(256), 0, st, (const uint32_t *)h->flags, (const uint32_t *)h->row_base,
-               (const uint32_t *)h->acc, n_rows, h->g.n_kappa, h->cfg.cap_peaks, out->bin, out->mask);
+    const int fw = h->g.n_kappa >> 5;
+    const uint32_t *fl = h->flags, *rb = h->row_base, *ac = h->acc;
+#define COMPACT(G)                                                                                          \
+    launch_pdl(k_compact<G>, dim3(blocks), dim3(256), 0, st, fl, rb, ac, n_rows, h->g.n_kappa, h->cfg.cap_peaks, \
+               out->bin, out->mask)
+    if (fw <= 2)
+        COMPACT(2);
+    else if (fw <= 4)
+        COMPACT(4);
+    else if (fw <= 8)
+        COMPACT(8);
+    else if (fw <= 16)
+        COMPACT(16);
+    else
+        COMPACT(32);
+#undef COMPACT
     h->launches += 1;
     return cudaGetLastError();
 }
