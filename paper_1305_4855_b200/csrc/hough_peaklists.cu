@@ -590,7 +590,9 @@ __global__ void __launch_bounds__(256) k_copy_lists(const ListCopyParams p)
                 }
             }
         }
-        // slow peaks of these pairs, one after the other, by the whole warp
+        // slow peaks of these pairs (rare), one after the other, by the whole warp
+        if (!__any_sync(0xffffffffu, (pos[0] == PL_SLOW && len[0] != 0u) || (pos[1] == PL_SLOW && len[1] != 0u)))
+            continue;
         for (int which = 0; which < 4; ++which) {
             const int u = which >> 1;
             const uint32_t spos = __shfl_sync(0xffffffffu, u ? pos[1] : pos[0], (which & 1) * 16);
