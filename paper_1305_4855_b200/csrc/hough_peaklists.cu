@@ -26,15 +26,18 @@
 // candidates of every peak.  Every candidate is then evaluated with the EXACT recipe
 // (hough_device.cuh eval_kappa / kappa_bin), so the lists are bit-identical to the oracle's.
 //
-// Work split: ONE THREAD per peak.  The thread walks the layer labels set in the peak's mask (a hit
-// of layer l in the bin sets bit l, so other layers cannot contribute), computes the layer's windows,
-// evaluates their candidates and appends the matching hit indices to the peak's fixed slot of the
-// staging buffer (candidate order).  k_scan<LENS> turns the lengths into hit_offset and k_copy_lists
-// sorts every list while moving it to its final place (rank by counting inside half a warp).
-// Lists longer than a slot are only counted here and written by k_copy_lists straight from the hits
-// in index order (one warp per such peak).  (Round-2 history: a group of 16 lanes per peak with lane =
-// layer spent 55 % of its instructions on the window arithmetic at 10 of 32 lanes active, plus three
-// CTA barriers per batch: 2.8e8 warp instructions per pile-up event, 0.42 ms.)
+// Work split: ONE THREAD per peak; the warps draw 32 peaks at a time from a global counter.  The thread
+// walks the layer labels set in the peak's mask (a hit of layer l in the bin sets bit l, so other
+// layers cannot contribute), queues the candidate ranges of their windows in its 40 words of shared
+// memory, evaluates all queued candidates in one flat loop and collects the matching hit indices at
+// the top of the same words; it sorts them (insertion sort) and writes them to the peak's fixed slot
+// of the staging buffer.  A list that outgrows shared memory spills to the slot in candidate order
+// (PL_UNSORTED); one that outgrows the slot is only counted (PL_SLOW).  k_scan<LENS> turns the lengths
+// into hit_offset and k_copy_lists moves the lists to their final place: a plain copy for sorted
+// slots, ranks by counting for unsorted ones, and straight from the hits in index order (one warp per
+// peak) for the rest.  (Round-2 history: a group of 16 lanes per peak with lane = layer spent 55 % of
+// its instructions on the window arithmetic at 10 of 32 lanes active, plus three CTA barriers per
+// batch: 2.8e8 warp instructions per pile-up event, 0.42 ms; now 1.2e8 and 0.17 ms.)
 #include "hough_device.cuh"
 
 #define PL_THREADS 256
