@@ -179,8 +179,8 @@ void hough_destroy(hough_handle *h);
  * hit preparation (r^2, layer bit), per-tile hit staging, shared-memory tile voting,
  * tile write-out and the vote count are enqueued on the stream.  n = 0 is legal (all-zero
  * accumulator).  Hits with a layer outside [0, n_layers) or non-finite coordinates cast no vote.
- * The hit arrays must stay valid until the stream has passed this call's work AND the
- * following hough_peaks (the hit lists re-read them).
+ * The hit arrays must stay valid until the stream has passed this call's work (the first kernel
+ * copies them into the workspace; everything after it, hit lists and hough_fit included, reads that copy).
  * Errors: HOUGH_EINVAL (NULL handle, n > max_hits, NULL arrays with n > 0), HOUGH_ECUDA.
  */
 int hough_vote(hough_handle *h, const float *x, const float *y, const int32_t *layer, uint32_t n,
