@@ -392,6 +392,52 @@ size_t hough_fit_workspace_bytes(const hough_handle *h);
 int hough_fit(hough_handle *h, const hough_fit_config *fc, void *workspace, size_t workspace_bytes,
               const hough_peaks_out *peaks, const hough_fit_out *out, void *cuda_stream);
 
+/*
+ * ---- Peaks of an accumulator for callers that cannot allocate device memory.
+ *
+ * Everything above needs a handle, and a handle needs a workspace somebody got from cudaMalloc.  Some
+ * users of a trigger library cannot call it: a plug-in inside a host framework that owns the whole
+ * device-memory budget and only lends out input and output buffers; an event loop with real-time
+ * constraints, where cudaMalloc / cudaFree are banned because they synchronise the whole device and
+ * stall the events in flight on other streams; a thin C / Fortran client that is handed device
+ * pointers and links no allocator.  This one call serves them.  It takes NO handle and NO workspace:
+ * the scratch its scan needs (a ticket and one look-back word per 2048 bins, 65 792 bytes in all) is a
+ * fixed array inside the library's own device code, so every GPU that loads libhough_b200.so holds
+ * those 64 KiB from the moment the module is loaded until the process exits.  The call itself never
+ * runs cudaMalloc, cudaFree or any library routine that allocates.
+ *
+ * The operation is the peak rule ("local maxima of the accumulator are the track
+ * candidates"; PAPER.md:128 peak detection resident in GPU memory; north_star: popcount >= L_min and a
+ * local maximum of the 3x3x3 neighbourhood, ties to the lower linear index; rule A6 of DESIGN.md
+ * section 2) followed by the ordered compaction (A7 without the hit lists), i.e. what
+ * hough_set_accumulator + hough_peaks_only compute, in one kernel launch:
+ *   acc      [device] n_phi*n_d0*n_kappa uint32 masks, lin = (i*n_d0 + j)*n_kappa + k, read-only;
+ *   bin,mask [device] cap_peaks entries each: the peaks in ascending lin and their masks; with more
+ *            than cap_peaks peaks the first cap_peaks (in lin order) are written;
+ *   n_peaks  [device] one uint32: the TRUE number of peaks (may exceed cap_peaks);
+ *   n_kappa  any value >= 1 (no multiple-of-32 rule here); L_min 1..32; phi_wrap 1 needs n_phi >= 3.
+ * All pointers are the caller's and must stay valid until the stream has passed the call's work.  The
+ * call acts on the CURRENT device of the calling thread (cudaSetDevice), which must be the one the
+ * pointers live on; it enqueues one 0-fill of the scratch and one kernel on `cuda_stream` and returns
+ * without synchronising.
+ *
+ * Limits and rules that follow from the fixed array:
+ *   - n_phi*n_d0*n_kappa <= HOUGH_NOALLOC_MAX_BINS (the 1024 x 64 x 256 grid of BASELINE.json configs
+ *     2-4); a larger grid is refused with HOUGH_ENOMEM before anything is enqueued;
+ *   - all calls on one GPU share the one array, from every thread and every stream.  Each call clears
+ *     the part it uses first (the array keeps the previous call's contents), so calls in stream order
+ *     are fine, but two calls whose work OVERLAPS on the same GPU race on it and return garbage or
+ *     never finish: issue them on one stream, or order the streams with events;
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, which
+ *     may load the module); make that first call before starting any stream capture.
+ * Errors: HOUGH_EINVAL (NULL pointer, cap_peaks = 0, bad sizes / L_min / phi_wrap), HOUGH_ENOMEM (grid
+ * beyond HOUGH_NOALLOC_MAX_BINS), HOUGH_ECUDA (no device, or a runtime call failed).
+ */
+#define HOUGH_NOALLOC_MAX_BINS (1u << 24)
+int hough_peaks_noalloc(const uint32_t *acc, int32_t n_phi, int32_t n_d0, int32_t n_kappa, int32_t L_min,
+                        int32_t phi_wrap, uint32_t *bin, uint32_t *mask, uint32_t cap_peaks, uint32_t *n_peaks,
+                        void *cuda_stream);
+
 /* Geometry the library chose (for reporting): tile_phi, tile_d0, n_tiles, threads per CTA,
  * dynamic shared memory bytes of the vote kernel, number of SMs.  Any pointer may be NULL. */
 int hough_query(const hough_handle *h, int32_t *tile_phi, int32_t *tile_d0, int32_t *n_tiles,

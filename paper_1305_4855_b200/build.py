@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhough_b200.so")
 SOURCES = ["hough_api.cu", "hough_sweep.cu", "hough_lists.cu", "hough_peaklists.cu", "hough_peaks.cu", "hough_vertex.cu",
-           "hough_fit.cu", "hough_microbench.cu"]
+           "hough_fit.cu", "hough_microbench.cu", "hough_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "hough_internal.cuh"), os.path.join(CSRC, "hough_device.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "hough.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

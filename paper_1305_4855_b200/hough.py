@@ -36,7 +36,8 @@ SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote
            "hough_collect_host", "hough_clear", "hough_peak_sweep",
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
            "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror",
-           "hough_vertex_workspace_bytes", "hough_vertices", "hough_fit_workspace_bytes", "hough_fit")
+           "hough_vertex_workspace_bytes", "hough_vertices", "hough_fit_workspace_bytes", "hough_fit",
+           "hough_peaks_noalloc")
 
 
 class HoughError(RuntimeError):
@@ -164,6 +165,9 @@ def _load():
     lib.hough_fit.restype = C.c_int
     lib.hough_fit.argtypes = [C.c_void_p, C.POINTER(FitConfig), C.c_void_p, C.c_size_t, C.POINTER(PeaksOut),
                               C.POINTER(FitOut), C.c_void_p]
+    lib.hough_peaks_noalloc.restype = C.c_int
+    lib.hough_peaks_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                        C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p]
     return lib
 
 
@@ -500,6 +504,27 @@ class Hough:
         if n < 0:
             _check(n, "hough_stage_times")
         return {_lib.hough_stage_name(s).decode(): float(ms[s]) for s in range(n)}
+
+
+NOALLOC_MAX_BINS = 1 << 24
+
+
+def peaks_noalloc(acc, n_phi, n_d0, n_kappa, L_min, phi_wrap, peak_bin, peak_mask, n_peaks, stream=None):
+    """hough_peaks_noalloc: peaks of the accumulator ``acc`` (int32 CUDA tensor of n_phi*n_d0*n_kappa
+    masks) into the caller's ``peak_bin`` / ``peak_mask`` (int32, equal capacity) and ``n_peaks``
+    (int32, one element), for callers that may not allocate device memory: the call takes no handle
+    and no workspace, its scratch is a fixed array inside the library (at most NOALLOC_MAX_BINS bins;
+    calls that overlap on one GPU race on it).  Every tensor here is the caller's; this wrapper
+    allocates nothing either.  Enqueues on ``stream`` and returns."""
+    for t in (acc, peak_bin, peak_mask, n_peaks):
+        assert t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.device == acc.device
+    assert acc.numel() == n_phi * n_d0 * n_kappa and peak_mask.numel() == peak_bin.numel() and n_peaks.numel() == 1
+    with torch.cuda.device(acc.device):   # the call acts on the thread's current device
+        _check(_lib.hough_peaks_noalloc(C.c_void_p(acc.data_ptr()), int(n_phi), int(n_d0), int(n_kappa), int(L_min),
+                                        int(phi_wrap), C.c_void_p(peak_bin.data_ptr()),
+                                        C.c_void_p(peak_mask.data_ptr()), int(peak_bin.numel()),
+                                        C.c_void_p(n_peaks.data_ptr()), _stream_ptr(stream)),
+               "hough_peaks_noalloc")
 
 
 def microbench_smem(mode, threads=1024, ctas_per_sm=2, iters=4096, device=0, reps=5):
