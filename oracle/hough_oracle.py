@@ -39,6 +39,7 @@ def lib():
         _lib.oracle_vote_cells.restype = C.c_uint64
         _lib.oracle_peaks.restype = C.c_uint64
         _lib.oracle_hitlists.restype = C.c_uint64
+        _lib.oracle_hitlists_cells.restype = C.c_uint64
         _lib.oracle_vote_one.restype = C.c_int
         _lib.oracle_num_threads.restype = C.c_int
         for f in ("oracle_vote_variant", "oracle_hitlists_variant", "oracle_vertex_vote",
@@ -130,22 +131,25 @@ def peaks(grid, acc, cap=None):
     return pb[:m].copy(), pm[:m].copy(), n
 
 
-def hitlists(grid, x, y, layer, peak_bin, cap_hits=None):
-    """A7: CSR (hit_offset uint64[m+1], hit_index uint32[min(total, cap)], true total)."""
+def hitlists(grid, x, y, layer, peak_bin, cap_hits=None, by_cell=False):
+    """A7: CSR (hit_offset uint64[m+1], hit_index uint32[min(total, cap)], true total).
+    by_cell: the same lists from oracle_hitlists_cells (one vote pass over the cells that hold a
+    peak instead of one pass per peak: the only form that finishes on a pile-up event)."""
     x, y, layer = _hits(x, y, layer)
+    fn = lib().oracle_hitlists_cells if by_cell else lib().oracle_hitlists
     pb = np.ascontiguousarray(peak_bin, dtype=np.uint32)
     g = _g(grid)
     m = pb.shape[0]
     off = np.zeros(m + 1, np.uint64)
     if cap_hits is None:
         # first call sizes the output (cap 0 writes nothing), second fills it
-        total = int(lib().oracle_hitlists(C.byref(g), _p(x, C.c_float), _p(y, C.c_float),
+        total = int(fn(C.byref(g), _p(x, C.c_float), _p(y, C.c_float),
                                           _p(layer, C.c_int32), C.c_uint32(x.shape[0]),
                                           _p(pb, C.c_uint32), C.c_uint64(m), _p(off, C.c_uint64),
                                           _p(np.empty(1, np.uint32), C.c_uint32), C.c_uint64(0)))
         cap_hits = total
     idx = np.empty(max(cap_hits, 1), np.uint32)
-    total = int(lib().oracle_hitlists(C.byref(g), _p(x, C.c_float), _p(y, C.c_float),
+    total = int(fn(C.byref(g), _p(x, C.c_float), _p(y, C.c_float),
                                       _p(layer, C.c_int32), C.c_uint32(x.shape[0]),
                                       _p(pb, C.c_uint32), C.c_uint64(m), _p(off, C.c_uint64),
                                       _p(idx, C.c_uint32), C.c_uint64(cap_hits)))
@@ -161,11 +165,16 @@ def vote_one(grid, x, y, i, j):
     return float(kap.value), int(k)
 
 
-def run(grid, x, y, layer, cap_peaks=None, cap_hits=None):
+def hitlists_cells(grid, x, y, layer, peak_bin, cap_hits=None):
+    """A7 walked cell by cell (oracle_hitlists_cells); same outputs as hitlists."""
+    return hitlists(grid, x, y, layer, peak_bin, cap_hits, by_cell=True)
+
+
+def run(grid, x, y, layer, cap_peaks=None, cap_hits=None, by_cell=False):
     """Whole path A1-A7 for one event; dict of outputs in the C-ABI's layout."""
     acc, n_votes, n_bad = vote(grid, x, y, layer)
     pb, pm, n_peaks = peaks(grid, acc, cap_peaks)
-    off, idx, n_ent = hitlists(grid, x, y, layer, pb, cap_hits)
+    off, idx, n_ent = hitlists(grid, x, y, layer, pb, cap_hits, by_cell=by_cell)
     return {"acc": acc, "n_votes": n_votes, "n_bad_hits": n_bad, "peak_bin": pb,
             "peak_mask": pm, "n_peaks": n_peaks, "hit_offset": off, "hit_index": idx,
             "n_hit_entries": n_ent}

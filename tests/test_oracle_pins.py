@@ -416,6 +416,46 @@ def test_hit_list_invariants_and_whole_pipeline_brute_force(oracle):
     assert np.array_equal(off3, off2)
 
 
+def test_cellwise_hit_lists_equal_the_peakwise_ones(oracle):
+    """oracle_hitlists_cells (one vote pass over the cells that hold a peak) against oracle_hitlists (one
+    pass per peak), whose own pins are above: equal CSR on random grids with bad / non-finite hits, on the
+    prompt2d and displaced3d events, with a cap that cuts a list, on the peak subsets a truncated GPU run
+    reports, with no peaks and no hits; and its total over EVERY non-empty bin is the vote count."""
+    rng = np.random.default_rng(12)
+    cases = []
+    for shape, n in [((16, 4, 8), 50), ((9, 1, 32), 200), ((24, 7, 64), 900), ((5, 3, 16), 1)]:
+        d0 = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
+        grid = tiny_grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=2, **d0)
+        x, y, layer = random_hits(rng, n)
+        if n >= 50:
+            layer[::17] = 12                                    # bad layers cast no vote
+            x[3], y[5] = np.nan, np.inf
+        cases.append((grid, x, y, layer))
+    for name, seed in (("prompt2d", 0), ("displaced3d", 1)):
+        w = synth.WORKLOADS[name]
+        cases.append((w.grid,) + tuple(synth.generate_event(w.event, seed)[:3]))
+    for grid, x, y, layer in cases:
+        acc, n_votes, _ = oracle.vote(grid, x, y, layer)
+        pb, _pm, n_peaks = oracle.peaks(grid, acc)
+        for bins in (pb, pb[: len(pb) // 2], pb[1::3], pb[:0]):
+            off1, idx1, tot1 = oracle.hitlists(grid, x, y, layer, bins)
+            off2, idx2, tot2 = oracle.hitlists_cells(grid, x, y, layer, bins)
+            assert tot1 == tot2 and np.array_equal(off1, off2) and np.array_equal(idx1, idx2)
+        if len(pb) > 2:
+            offf, idxf, totf = oracle.hitlists(grid, x, y, layer, pb)
+            cap = int(offf[len(pb) // 2]) + 1                   # cuts inside a list
+            offc, idxc, totc = oracle.hitlists_cells(grid, x, y, layer, pb, cap_hits=cap)
+            assert totc == totf and np.array_equal(offc, offf) and np.array_equal(idxc, idxf[:cap])
+        if grid.n_bins <= 1 << 16:
+            allbins = np.nonzero(acc.reshape(-1))[0].astype(np.uint32)
+            _off, idx, tot = oracle.hitlists_cells(grid, x, y, layer, allbins)
+            assert tot == n_votes == len(idx)
+    g = cases[0][0]
+    z = np.zeros(0, np.float32)
+    off, idx, tot = oracle.hitlists_cells(g, z, z, np.zeros(0, np.int32), np.array([3, 40], np.uint32))
+    assert tot == 0 and off.tolist() == [0, 0, 0] and len(idx) == 0
+
+
 def test_oracle_is_deterministic_and_thread_count_independent(oracle):
     """OR of masks is order independent (the race remark of PAPER.md:126)."""
     w = synth.WORKLOADS["prompt2d"]
