@@ -152,8 +152,9 @@ typedef struct hough_host_out {
     uint32_t *hit_index; /* may be NULL: hit lists are then computed but not copied back */
     hough_counts *counts;
     uint16_t *hit_index16; /* OPTIONAL (NULL: not wanted), cap_hits entries: when the event's counts carry
-                              HOUGH_INDEX16 the lists are copied back in this form INSTEAD of hit_index (12 MB
-                              instead of 24 MB for a config-3 event); otherwise hit_index is used as above */
+                              HOUGH_INDEX16 the lists are copied back in this form INSTEAD of hit_index (halves the
+                              bytes of the lists: a config-3 event returns 19.7 MB instead of 31.8 MB in all);
+                              otherwise hit_index is used as above */
 } hough_host_out;
 
 /* Bytes of device workspace hough_create needs for cfg (0 if cfg is invalid). */
@@ -205,6 +206,8 @@ const uint32_t *hough_accumulator(const hough_handle *h);
  * hough_peaks), copies counts, the peak arrays and (if host->hit_index != NULL) the hit
  * lists back to `host`, and SYNCHRONISES the stream before returning.  Only the filled
  * prefixes are copied back (a second small synchronisation on counts is used for that).
+ * It stages the hits where slot 0 of the pipeline below stages its own, so it is refused with
+ * HOUGH_ESTATE while an event submitted in slot 0 has not been collected.
  */
 int hough_process_host(hough_handle *h, const float *x, const float *y, const int32_t *layer,
                        uint32_t n, const hough_peaks_out *dev, const hough_host_out *host,
@@ -229,6 +232,8 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
  * Patterns:  two slots:   submit(e, e&1);  if (e > 0) collect_host(e-1);  ...
  *            three slots: submit(e, e%3);  if (e > 0) collect_begin(e-1);  if (e > 1) collect_end(e-2);  ...
  *            (the device->host copy engine never waits for the host).
+ * The pipeline's stream, events and pinned counters are created by the first hough_submit_host, all or nothing:
+ * if that fails (HOUGH_ECUDA) nothing is kept and the next call starts over.
  * A slot must be collected (end) before it is submitted again.  The host arrays must be pinned for the
  * copies to overlap.  Errors as hough_process_host; HOUGH_ESTATE if the slot is not in the state the call
  * needs.  One handle computes one event at a time: `cuda_stream` should be the same stream for all slots.

@@ -16,14 +16,18 @@ __global__ void __launch_bounds__(256) k_prep(const float *__restrict__ x, const
                                               const int32_t *__restrict__ layer, uint32_t n,
                                               uint32_t n_pad, int n_layers, float *__restrict__ hx,
                                               float *__restrict__ hy, float *__restrict__ hr2,
-                                              uint32_t *__restrict__ hbit, DevCounters *counters, HitIndexDev ix)
+                                              uint32_t *__restrict__ hbit, DevCounters *counters, HitIndexDev ix,
+                                              uint32_t *__restrict__ layer_r_next)
 {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     bool bad = false;
     __shared__ uint32_t s_layer_r[2 * 33]; // the CTA's share of the per-layer radius range
     pdl_trigger(); // the vote kernel may set up its tile meanwhile (it waits before it reads the hits)
-    if (threadIdx.x < 2 * 33)
+    if (threadIdx.x < 2 * 33) {
         s_layer_r[threadIdx.x] = 0u;
+        if (blockIdx.x == 0)
+            layer_r_next[threadIdx.x] = 0u; // the range is per event: the next event's block starts empty
+    }
     __syncthreads();
     if (i < n) {
         float xv = x[i], yv = y[i];
@@ -80,8 +84,12 @@ cudaError_t launch_prep(hough_handle *h, const float *x, const float *y, const i
         if (e != cudaSuccess)
             return e;
     }
+    // per-layer radius range of THIS event: the two blocks alternate, k_prep fills one and empties the other
+    // (both start empty: hough_create).  The previous event's list kernel has read its block by now (stream order).
+    h->rbuf ^= 1;
+    h->ix.layer_r = h->layer_r2[h->rbuf];
     k_prep<<<(n_pad + 255) / 256, 256, 0, st>>>(x, y, layer, n, n_pad, h->cfg.n_layers, h->hx, h->hy, h->hr2,
-                                                h->hbit, h->counters, h->ix);
+                                                h->hbit, h->counters, h->ix, h->layer_r2[h->rbuf ^ 1]);
     h->launches += 1;
     return cudaGetLastError();
 }
@@ -227,7 +235,7 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
     const int n_keys = (c->n_layers + 1) * NA;
     void *t_phic = cv.take((size_t)c->n_phi * 4);
     void *t_sne = cv.take((size_t)(c->n_phi + 1) * 4), *t_cse = cv.take((size_t)(c->n_phi + 1) * 4);
-    void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 33 * 4); // histogram | per-layer radius range (one memset)
+    void *ix_cnt = cv.take((size_t)n_keys * 4 + 2 * 2 * 33 * 4); // histogram | two blocks of per-layer radius range (one memset)
     void *ix_start = cv.take((size_t)(n_keys + 1) * 4);
     void *ix_cur = cv.take((size_t)n_keys * 4);
     void *ix_key = cv.take((size_t)hp * 4);
@@ -264,7 +272,10 @@ static size_t carve_workspace(const hough_config *c, unsigned char *base, hough_
         h->ix.NA = NA;
         h->ix.n_keys = n_keys;
         h->ix.bin_cnt = (uint32_t *)ix_cnt;
-        h->ix.layer_r = (uint32_t *)ix_cnt + n_keys;
+        h->layer_r2[0] = (uint32_t *)ix_cnt + n_keys;
+        h->layer_r2[1] = h->layer_r2[0] + 2 * 33;
+        h->ix.layer_r = h->layer_r2[0];
+        h->rbuf = 0;
         h->ix.bin_start = (uint32_t *)ix_start;
         h->ix.bin_cur = (uint32_t *)ix_cur;
         h->ix.key = (uint32_t *)ix_key;
@@ -517,7 +528,7 @@ int hough_create(const hough_config *cfg, void *workspace, size_t workspace_byte
     ok &= cudaMemcpy(h->t_twod0, twod0, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemcpy(h->t_d0sq, d0sq, sizeof(float) * nd, cudaMemcpyHostToDevice) == cudaSuccess;
     ok &= cudaMemset(h->counters, 0, 256 + (size_t)2 * h->scan_blocks_max * 8) == cudaSuccess;
-    ok &= cudaMemset(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4 + 2 * 33 * 4) == cudaSuccess;
+    ok &= cudaMemset(h->ix.bin_cnt, 0, (size_t)h->ix.n_keys * 4 + 2 * 2 * 33 * 4) == cudaSuccess;
     h->cbuf = 0;
     h->next_clean = 1;
     free(sn);
@@ -720,6 +731,8 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
         return HOUGH_EINVAL;
     if (n > h->cfg.max_hits || (n > 0 && (!x || !y || !layer)))
         return HOUGH_EINVAL;
+    if (h->slot_busy[0]) // this call stages its hits where pipeline slot 0 does
+        return HOUGH_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n > 0) {
         CK(cudaMemcpyAsync(h->raw_x[0], x, (size_t)n * 4, cudaMemcpyHostToDevice, st));
@@ -752,17 +765,45 @@ int hough_process_host(hough_handle *h, const float *x, const float *y, const in
 }
 
 // Lazily created resources of the pipelined host entry points.
+// All or nothing: `pipeline_ready` is set only when every resource exists; a failure on the way
+// releases what was created, so that the next call starts over instead of using half of them.
+static void pipeline_release(hough_handle *h)
+{
+    for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
+        if (h->slot_ev[s])
+            cudaEventDestroy(h->slot_ev[s]);
+        if (h->h2d_ev[s])
+            cudaEventDestroy(h->h2d_ev[s]);
+        if (h->copy_ev[s])
+            cudaEventDestroy(h->copy_ev[s]);
+        h->slot_ev[s] = h->h2d_ev[s] = h->copy_ev[s] = nullptr;
+    }
+    if (h->h2d_stream)
+        cudaStreamDestroy(h->h2d_stream);
+    h->h2d_stream = nullptr;
+    if (h->slot_counts)
+        cudaFreeHost(h->slot_counts);
+    h->slot_counts = nullptr;
+    h->pipeline_ready = 0;
+}
+
 static int pipeline_init(hough_handle *h)
 {
-    if (h->h2d_stream)
+    if (h->pipeline_ready)
         return HOUGH_OK;
-    CK(cudaStreamCreateWithFlags(&h->h2d_stream, cudaStreamNonBlocking));
-    for (int s = 0; s < HOUGH_MAX_SLOTS; ++s) {
-        CK(cudaEventCreateWithFlags(&h->h2d_ev[s], cudaEventDisableTiming));
-        CK(cudaEventCreateWithFlags(&h->slot_ev[s], cudaEventDisableTiming));
-        CK(cudaEventCreateWithFlags(&h->copy_ev[s], cudaEventDisableTiming));
+    bool ok = cudaStreamCreateWithFlags(&h->h2d_stream, cudaStreamNonBlocking) == cudaSuccess;
+    for (int s = 0; ok && s < HOUGH_MAX_SLOTS; ++s) {
+        ok = ok && cudaEventCreateWithFlags(&h->h2d_ev[s], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&h->slot_ev[s], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&h->copy_ev[s], cudaEventDisableTiming) == cudaSuccess;
     }
-    CK(cudaMallocHost((void **)&h->slot_counts, sizeof(hough_counts) * HOUGH_MAX_SLOTS));
+    ok = ok && cudaMallocHost((void **)&h->slot_counts, sizeof(hough_counts) * HOUGH_MAX_SLOTS) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        pipeline_release(h);
+        return HOUGH_ECUDA;
+    }
+    h->pipeline_ready = 1;
     return HOUGH_OK;
 }
 

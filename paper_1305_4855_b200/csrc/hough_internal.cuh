@@ -86,8 +86,8 @@ struct HitIndexDev {
     uint32_t *bin_cnt;      // [n_keys] histogram of the event (k_prep); k_index_scan leaves it zero for the next event
     uint32_t *bin_cur;      // [n_keys] scatter cursor (k_index_scan: rank of the first hit of the key)
     uint32_t *bin_start;    // [n_keys + 1] rank of the first hit of a key
-    uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) over the handle's events so far
-                            // (zeroed by hough_create only: the windows are supersets for any wider range)
+    uint32_t *layer_r;      // [2 * 33] per layer: max of ~bits(r) and max of bits(r) over the hits of THIS event
+                            // (one of hough_handle::layer_r2's two blocks; k_prep fills it and empties the other)
     uint32_t *key;          // [max_hits_pad] key of hit h, 0xffffffff = not indexed (bad layer)
     float4 *rec;            // [max_hits_pad] the hits in key order: (x, y, r2, bits of the hit index)
 };
@@ -122,6 +122,8 @@ struct hough_handle {
     float *t_sn, *t_cs, *t_d0c, *t_twod0, *t_d0sq, *t_phic, *t_sne, *t_cse;
     int mode;            // vote variant: 0 closed form at bin centres, 1 straight line, 2 interval (hough_device.cuh)
     HitIndexDev ix;
+    uint32_t *layer_r2[2]; // the two alternating blocks behind ix.layer_r
+    int rbuf;              // the block of the current event
     float *hx, *hy, *hr2;
     uint32_t *hbit;
     // staging of the host entry points' hit arrays, one set per in-flight slot
@@ -148,6 +150,7 @@ struct hough_handle {
     // slot's computation (and the copy of its counters into slot_counts) is complete, copy_ev = its
     // results have reached the host.  slot_busy: 0 free, 1 submitted, 2 results being copied.
     cudaStream_t h2d_stream;
+    int pipeline_ready;          // every resource of the pipeline exists (pipeline_init is all or nothing)
     cudaEvent_t h2d_ev[HOUGH_MAX_SLOTS], slot_ev[HOUGH_MAX_SLOTS], copy_ev[HOUGH_MAX_SLOTS];
     unsigned char slot_busy[HOUGH_MAX_SLOTS];
     hough_counts *slot_counts;   // pinned host memory, one block per slot

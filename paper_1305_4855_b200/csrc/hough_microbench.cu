@@ -1,6 +1,8 @@
 // hough_microbench.cu -- shared-memory atomic micro-benchmark that DEFINES the
 // "shared-atomic roofline" the vote kernel is reported against (SURVEY.md section 8(d),
 // BASELINE.json north_star "% of smem-atomic roofline").  Not part of the hot path.
+#include <atomic>
+
 #include "hough_internal.cuh"
 
 #define MB_WORDS 8192 // 32 KB table per CTA
@@ -46,14 +48,29 @@ int hough_microbench_smem(int device, int mode, int threads, int ctas_per_sm, in
     if (mode < 0 || mode > 2 || threads < 32 || threads > 1024 || (threads & 31) || ctas_per_sm < 1 ||
         iters < 1 || !sink_dev)
         return HOUGH_EINVAL;
-    int ndev = 0, sms = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+    // The caller times this call with events recorded around it, so after the first call on a device nothing
+    // but the launch may sit between them: the SM count is looked up once per device and remembered.
+    static std::atomic<int> sm_count[64];
+    if (device < 0 || device >= 64)
+        return HOUGH_ECUDA;
+    int sms = sm_count[device].load(std::memory_order_relaxed);
+    if (sms == 0) {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) {
+            cudaGetLastError();
+            return HOUGH_ECUDA;
+        }
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || sms < 1) {
+            cudaGetLastError();
+            return HOUGH_ECUDA;
+        }
+        sm_count[device].store(sms, std::memory_order_relaxed);
+    }
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || (cur != device && cudaSetDevice(device) != cudaSuccess)) {
         cudaGetLastError();
         return HOUGH_ECUDA;
     }
-    if (cudaSetDevice(device) != cudaSuccess ||
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
-        return HOUGH_ECUDA;
     int blocks = sms * ctas_per_sm;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (mode == 0)

@@ -428,6 +428,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
             if (KIND == SCAN_ROWS) {
                 p.row_base[0] = 0u;
                 p.counters->n_peaks = 0u;
+                p.counters->n_list_evals = 0ull;
             } else {
                 p.hit_offset[0] = 0ull;
                 p.counters->n_hit_entries = 0ull;
@@ -527,6 +528,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const ScanParams p)
                 if (KIND == SCAN_ROWS) {
                     p.row_base[n] = (uint32_t)run;
                     p.counters->n_peaks = (unsigned int)run;
+                    // hough_peaks may be repeated on one vote: the list stage that follows counts from zero
+                    p.counters->n_list_evals = 0ull;
                 } else {
                     p.hit_offset[n] = run;
                     p.counters->n_hit_entries = run;

@@ -1,8 +1,9 @@
 // hough_sweep.cu -- the tiled vote sweep of the hits over the (phi0, d0) cells: a3 vote into a
 // shared-memory tile with shared atomic OR, a4 coalesced write-out, a8 vote count
 // (DESIGN.md 4.1).  Hits are staged by TMA 1-D bulk copies of the
-// SoA arrays into shared memory (double buffered), culled per tile by the conservative
-// interval test and evaluated with the exact fp32 recipe of BASELINE.json north_star's
+// SoA arrays into ONE shared-memory staging buffer (the survivors of a chunk are compacted out of it
+// before they are evaluated, so the next chunk's copies land under the evaluation), culled per tile by
+// the conservative interval test and evaluated with the exact fp32 recipe of BASELINE.json north_star's
 // closed form (hough_device.cuh).
 #include "hough_device.cuh"
 
@@ -122,6 +123,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
     const float ab_c1 = p.ab.c1, ab_c0 = p.ab.c0;
     const uint32_t ab_lim = p.ab.lim, ab_edge = p.ab.edge;
     unsigned int my_votes = 0;
+    unsigned long long votes_wide = 0; // vote variants: my_votes is folded in after every hit (a whole-row fill is
+                                       // up to 16384 votes, so 32 bits could wrap on very large events)
     unsigned long long tile_evals = 0; // thread 0: surviving hits x owned cells
     const int nkm1 = nk - 1;
     // byte address of this cell's row in the tile and its word swizzle (in bytes)
@@ -201,6 +204,8 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
                 if (__float_as_uint(hv.w) != 0u && variant_bins<MODE>(hv.x, hv.y, hv.z, cc, klo, khi, inv_dk, nkm1, k0, k1))
                     for (int k = k0; k <= k1; ++k)
                         cast((uint32_t)k, __float_as_uint(hv.w));
+                votes_wide += my_votes;
+                my_votes = 0;
             }
         };
         // the estimate of one (hit, cell): e and den are the exact binary32 values of the recipe (A3)
@@ -356,10 +361,11 @@ __global__ void __launch_bounds__(1024, 1) k_sweep(const SweepParams p)
             }
         }
         // ---- a8: vote count (one global atomic per warp per tile)
+        unsigned long long warp_votes = votes_wide + my_votes;
         for (int o = 16; o > 0; o >>= 1)
-            my_votes += __shfl_xor_sync(0xffffffffu, my_votes, o);
-        if (lane == 0 && my_votes)
-            atomicAdd(p.n_votes, (unsigned long long)my_votes);
+            warp_votes += __shfl_xor_sync(0xffffffffu, warp_votes, o);
+        if (lane == 0 && warp_votes)
+            atomicAdd(p.n_votes, warp_votes);
         if (tid == 0 && tile_evals)
             atomicAdd(p.n_evals, tile_evals);
     }

@@ -286,8 +286,8 @@ def test_process_host_matches_device_path(hough, oracle):
 def test_batch_all_100_events_back_to_back_on_one_handle(hough, oracle):
     """BASELINE.json configs[3]: 100 events shaped like "pileup" (seeds 0..99), one handle, one
     stream, each with its own accumulator.  EVERY seed: whole accumulator, n_votes, n_bad_hits,
-    peak list and masks against the oracle; the CSR hit lists for every tenth seed (the oracle's
-    O(n_peaks x n_hits) list passes cost ~10 s per event, its vote + peaks ~1 s)."""
+    peak list and masks, and the whole CSR (hit_offset, hit_index, n_hit_entries) against the oracle
+    ("CSR hit lists equal ... config 4: all 100 seeds")."""
     w = synth.WORKLOADS["batch100"]
     assert w.seeds == tuple(range(100))
     h = hough.Hough(w.grid, 20000, w.cap_peaks, w.cap_hits)
@@ -298,16 +298,16 @@ def test_batch_all_100_events_back_to_back_on_one_handle(hough, oracle):
         res = h.read()
         res["acc"] = h.accumulator_host()
         assert res["flags"] == 0, seed
-        with_lists = seed % 10 == 0
-        if with_lists:
-            ref = oracle.run(w.grid, x, y, layer)
-        else:
-            acc, n_votes, n_bad = oracle.vote(w.grid, x, y, layer)
-            pb, pm, n_peaks = oracle.peaks(w.grid, acc)
-            ref = {"acc": acc, "n_votes": n_votes, "n_bad_hits": n_bad, "peak_bin": pb,
-                   "peak_mask": pm, "n_peaks": n_peaks}
+        # the whole CSR of every seed: the oracle's lists walked cell by cell (one vote pass); on seed 0 the
+        # peak-by-peak oracle (O(n_peaks x n_hits), minutes) confirms the cell-wise one at this size
+        ref = oracle.run(w.grid, x, y, layer, cap_hits=w.cap_hits, by_cell=True)
+        assert ref["n_hit_entries"] <= w.cap_hits
+        if seed == 0:
+            off1, idx1, tot1 = oracle.hitlists(w.grid, x, y, layer, ref["peak_bin"])
+            assert tot1 == ref["n_hit_entries"]
+            assert np.array_equal(off1, ref["hit_offset"]) and np.array_equal(idx1, ref["hit_index"])
         res["acc"] = res["acc"].reshape(ref["acc"].shape)
-        assert_same(res, ref, lists=with_lists)
+        assert_same(res, ref)
         # CSR consistency for every seed: n_hit_entries = sum of list lengths, OR of the
         # listed hits' layer bits = the peak's mask
         off = res["hit_offset"].astype(np.int64)
@@ -321,12 +321,12 @@ def test_finegrid_full_accumulator_parity(hough, oracle):
     """BASELINE.json configs[4] at full size (134M bins, ~62k hits), in bench.py's launch
     configuration: the WHOLE 512 MiB accumulator, n_votes and n_bad_hits against the oracle's
     vote (1.6e10 evaluations: tens of seconds on the host cores); the whole peak list and masks
-    against the oracle's peak rule on the ORACLE's accumulator.  Only the oracle's hit-list
-    passes (O(n_peaks x n_hits) = 3.6e6 x 6.2e4 x 2) are infeasible at this size, so the CSR
-    lists are compared for 3000 sampled peaks plus the first and last 50, and checked for
-    every peak by properties that hold at any size: offsets strictly increasing, ascending
-    hit indices inside each list, n_hit_entries = sum of the lengths, OR of the listed hits'
-    layer bits = the peak's mask."""
+    against the oracle's peak rule on the ORACLE's accumulator; the whole CSR (every list of the
+    ~3.6e6 peaks and n_hit_entries) against the oracle's cell-wise hit lists, which the
+    peak-by-peak oracle (O(n_peaks x n_hits), infeasible in full here) confirms on 3000 sampled
+    peaks plus the first and last 50.  Also the properties that hold at any size: offsets
+    strictly increasing, ascending hit indices inside each list, OR of the listed hits' layer
+    bits = the peak's mask."""
     w = synth.WORKLOADS["finegrid"]
     g = w.grid
     x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
@@ -353,12 +353,17 @@ def test_finegrid_full_accumulator_parity(hough, oracle):
     assert np.all(np.diff(idx.astype(np.int64))[inner[1:]] > 0)   # ascending inside each list
     bits = (np.uint32(1) << layer[idx].astype(np.uint32)).astype(np.uint32)
     assert np.array_equal(np.bitwise_or.reduceat(bits, off[:-1]), pm)
+    # every list of every peak, and the total, against the oracle's cell-wise lists (one more vote pass) ...
+    coff, cidx, ctot = oracle.hitlists_cells(g, x, y, layer, pb, cap_hits=w.cap_hits)
+    assert ctot == res["n_hit_entries"] <= w.cap_hits
+    assert np.array_equal(res["hit_offset"], coff) and np.array_equal(idx, cidx)
+    # ... which the peak-by-peak oracle confirms on a sample at this size
     rng = np.random.default_rng(5)
     sel = np.unique(np.concatenate([rng.integers(0, n, 3000), np.arange(50), np.arange(n - 50, n)]))
     soff, sidx, _tot = oracle.hitlists(g, x, y, layer, pb[sel])
     for q, pk in enumerate(sel):
-        got = idx[off[pk]:off[pk + 1]]
-        assert np.array_equal(got, sidx[int(soff[q]):int(soff[q + 1])]), pk
+        assert np.array_equal(cidx[int(coff[pk]):int(coff[pk + 1])], sidx[int(soff[q]):int(soff[q + 1])]), pk
+    del coff, cidx
     # the fused peak test (two 256-bin segments per cell row here) and the cell-wise kernel give the
     # same peaks and lists as the path just checked against the oracle
     for opt in (hough.OPT_FUSED_PEAKS, hough.OPT_CELL_PEAKS):
@@ -440,6 +445,8 @@ def test_three_slot_pipeline_with_pileup_events(hough, oracle):
                 h.submit_host(pe[0].numpy(), pe[1].numpy(), pe[2].numpy(), 0)   # slot still in flight
             with pytest.raises(hough.HoughError):
                 h.collect_end(0)                                                 # not begun
+            with pytest.raises(hough.HoughError):
+                h.process_host(pe[0].numpy(), pe[1].numpy(), pe[2].numpy())      # would reuse slot 0's staging
         if e > 0:
             h.collect_begin((e - 1) % 3)
         if e > 1:
@@ -460,14 +467,10 @@ def test_three_slot_pipeline_with_pileup_events(hough, oracle):
         assert res["n_votes"] == n_votes and res["n_peaks"] == n_peaks and res["flags"] == hough.INDEX16
         assert res["hit_index"].dtype == np.uint16
         assert np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
-        # hit lists of a sample of peaks (the oracle's list pass is O(peaks x hits))
-        rng = np.random.default_rng(1)
-        sel = np.unique(rng.integers(0, max(n_peaks, 1), 400)) if n_peaks else np.zeros(0, np.int64)
-        soff, sidx, _tot = oracle.hitlists(w.grid, *ev, pb[sel])
-        for q, pk in enumerate(sel):
-            a, b = int(res["hit_offset"][pk]), int(res["hit_offset"][pk + 1])
-            assert np.array_equal(res["hit_index"][a:b], sidx[int(soff[q]):int(soff[q + 1])]), pk
-        assert int(res["hit_offset"][-1]) == res["n_hit_entries"]
+        # every hit list (the oracle's cell-wise pass)
+        coff, cidx, ctot = oracle.hitlists_cells(w.grid, *ev, pb, cap_hits=w.cap_hits)
+        assert res["n_hit_entries"] == ctot <= w.cap_hits
+        assert np.array_equal(res["hit_offset"], coff) and np.array_equal(res["hit_index"], cidx)
 
 
 def test_second_vote_replaces_the_event_and_peaks_can_be_repeated(hough, oracle):
@@ -481,11 +484,50 @@ def test_second_vote_replaces_the_event_and_peaks_can_be_repeated(hough, oracle)
     h = hough.Hough(grid, 900, grid.n_bins // 2 + 1, ref["n_hit_entries"] + 1000)
     h.vote(dev(xa), dev(ya), dev(la))
     h.vote(dev(xb), dev(yb), dev(lb))
+    evals = []
     for _ in range(2):
         h.peaks()
         res = h.read()
         res["acc"] = h.accumulator_host().copy()
         assert_same(res, ref)
+        evals.append(res["n_list_evals"])
+    h.close()
+    assert evals[0] > 0 and evals[1] == evals[0]      # the work counter of the list stage is per call
+
+
+def test_an_outlier_radius_does_not_widen_the_list_windows_of_later_events(hough, oracle):
+    """The per-layer radius range behind the peak-driven lists' azimuth windows belongs to ONE event: after
+    an event with a far-away hit in a valid layer (and after an empty event, which runs no hit preparation),
+    an ordinary event costs the list stage exactly what it costs a fresh handle."""
+    w = synth.WORKLOADS["displaced3d"]
+    x, y, layer, _ = synth.generate_event(w.event, 5)
+    ref = oracle.run(w.grid, x, y, layer)
+
+    def run(h, xs, ys, ls):
+        h.vote(dev(xs), dev(ys), dev(ls))
+        h.peaks()
+        r = h.read()
+        r["acc"] = h.accumulator_host().copy()
+        return r
+
+    fresh = hough.Hough(w.grid, len(x) + 10, w.cap_peaks, w.cap_hits)
+    base = run(fresh, x, y, layer)
+    fresh.close()
+    assert_same(base, ref)
+    xo, yo, lo = x.copy(), y.copy(), layer.copy()
+    xo[:10], yo[:10] = 1.0e6, -3.0e5                   # finite, indexed (r^2 < 2^80), far outside the detector
+    lo[:10] = np.arange(10, dtype=np.int32)            # one in every layer
+    z = np.zeros(0, np.float32)
+    h = hough.Hough(w.grid, len(x) + 10, w.cap_peaks, w.cap_hits)
+    for pattern in ("outlier", "outlier+empty", "two outliers"):
+        assert_same(run(h, xo, yo, lo), oracle.run(w.grid, xo, yo, lo))
+        if pattern == "outlier+empty":
+            assert run(h, z, z, np.zeros(0, np.int32))["n_peaks"] == 0
+        if pattern == "two outliers":
+            run(h, xo, yo, lo)
+        after = run(h, x, y, layer)
+        assert_same(after, ref)
+        assert after["n_list_evals"] == base["n_list_evals"], pattern
     h.close()
 
 
