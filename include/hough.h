@@ -62,6 +62,8 @@ extern "C" {
 #define HOUGH_TRUNCATED_PEAKS 1u /* n_peaks > cap_peaks: only the first cap_peaks (in lin order) were written */
 #define HOUGH_TRUNCATED_HITS 2u  /* n_hit_entries > cap_hits: hit_index holds the first cap_hits entries */
 #define HOUGH_INDEX16 4u         /* hit_index16 was written as well (the event has <= 65536 hits) */
+#define HOUGH_LIST_MISMATCH 8u   /* set by the list check (HOUGH_OPT_CHECK_LISTS / hough_check_lists): some peak's hit
+                                    list is not ascending or the OR of its hits' layer bits is not the peak's mask */
 
 /* hough_config.options */
 #define HOUGH_OPT_NO_CULL 1u      /* evaluate every (hit, cell): the unpruned sweep (for measurements/tests) */
@@ -83,6 +85,9 @@ extern "C" {
                                      and not HOUGH_OPT_UNPACKED.  Results are identical either way */
 #define HOUGH_OPT_CELL_PEAKS 256u /* peak flags of EVERY cell by the cell-wise kernel (k_peak_cells) instead of the
                                      streaming sweep: cross-check and measurement of that kernel */
+#define HOUGH_OPT_CHECK_LISTS 512u /* run hough_check_lists at the end of every hough_peaks (a safety net for the
+                                     peak-driven lists, whose candidate windows are supersets by derivation: a hit
+                                     missing from a list shows up as HOUGH_LIST_MISMATCH instead of silently) */
 #define HOUGH_OPT_UNPACKED 4u     /* one mask per 32-bit word of the vote tile even with <= 16 layers (test hook
                                      for the tile layout used with 17..32 layers) */
 
@@ -256,6 +261,17 @@ int hough_collect_host(hough_handle *h, const hough_peaks_out *dev, const hough_
  */
 int hough_clear(hough_handle *h, void *cuda_stream);
 int hough_peak_sweep(hough_handle *h, void *cuda_stream);
+
+/*
+ * Device-side invariant of the hit lists in `out` (as hough_peaks of the event last voted on this handle
+ * left them): every complete list (one that ends within cap_hits) is strictly ascending, holds valid hit
+ * indices, and the OR of its hits' layer bits equals the peak's mask -- which is what "each peak is emitted
+ * with its sorted hit list" (north_star) implies, since the mask IS the OR of the votes of exactly those
+ * hits.  A violation ORs HOUGH_LIST_MISMATCH into out->counts->flags (on the device, after hough_peaks has
+ * written the counters).  One kernel, one warp per peak; costs about as much as reading the lists once.
+ * Errors: HOUGH_EINVAL, HOUGH_ESTATE (no hough_vote before), HOUGH_ECUDA.
+ */
+int hough_check_lists(hough_handle *h, const hough_peaks_out *out, void *cuda_stream);
 
 /* Overwrite the accumulator from a [device] array of n_bins masks (test hook for the peak
  * rule: lets a test run hough_peak_sweep / hough_peaks_only on a hand-made accumulator). */

@@ -232,6 +232,77 @@ uint64_t oracle_hitlists_variant(const oracle_grid *g, int mode, const float *x,
     return w;
 }
 
+/*
+ * The same lists, walked cell by cell (the analogue of oracle_hitlists_cells in hough_oracle.c): peaks in
+ * ascending lin, so the peaks of one (i, j) cell are consecutive; for every such run one pass over the hits,
+ * variant_bins once per hit, and the hit joins every peak of the run whose bin lies in [k0, k1].  The
+ * (peak, hit) pairs wait in a buffer until all lengths, hence the offsets, are known.  Pinned against
+ * oracle_hitlists_variant (tests/test_ext_oracle_pins.py).
+ */
+uint64_t oracle_hitlists_variant_cells(const oracle_grid *g, int mode, const float *x, const float *y,
+                                       const int32_t *layer, uint32_t n, const uint32_t *peak_bin, uint64_t n_peaks,
+                                       uint64_t *hit_offset, uint32_t *hit_index, uint64_t cap_hits)
+{
+    const int np = g->n_phi, nd = g->n_d0, nk = g->n_kappa;
+    tables_t t;
+    tables_make(g, &t);
+    float *sne = malloc(sizeof(float) * (np + 1)), *cse = malloc(sizeof(float) * (np + 1));
+    edge_tables(g, sne, cse);
+    float *r2 = malloc(sizeof(float) * (n ? n : 1));
+    uint32_t *bit = malloc(sizeof(uint32_t) * (n ? n : 1));
+    uint32_t n_bad;
+    hit_prep(g, x, y, layer, n, r2, bit, &n_bad);
+    uint64_t *len = calloc(n_peaks + 1, sizeof(uint64_t));
+    uint64_t a = 0;
+    /* pairs of all runs, run after run, in (run, h, peak) order */
+    uint64_t cap_pairs = 1024, n_pairs = 0;
+    uint64_t *pair_peak = malloc(sizeof(uint64_t) * cap_pairs);
+    uint32_t *pair_hit = malloc(sizeof(uint32_t) * cap_pairs);
+    while (a < n_peaks) {
+        uint64_t b = a + 1;
+        while (b < n_peaks && peak_bin[b] / (uint32_t)nk == peak_bin[a] / (uint32_t)nk)
+            ++b;
+        const uint32_t cell = peak_bin[a] / (uint32_t)nk;
+        const int j = (int)(cell % (uint32_t)nd), i = (int)(cell / (uint32_t)nd);
+        for (uint32_t h = 0; h < n; ++h) {
+            int k0, k1;
+            if (!bit[h] || !variant_bins(mode, x[h], y[h], r2[h], &t, sne, cse, i, j, nk, &k0, &k1))
+                continue;
+            for (uint64_t p = a; p < b; ++p) {
+                const int k = (int)(peak_bin[p] % (uint32_t)nk);
+                if (k < k0 || k > k1)
+                    continue;
+                if (n_pairs == cap_pairs) {
+                    cap_pairs *= 2;
+                    pair_peak = realloc(pair_peak, sizeof(uint64_t) * cap_pairs);
+                    pair_hit = realloc(pair_hit, sizeof(uint32_t) * cap_pairs);
+                }
+                pair_peak[n_pairs] = p;
+                pair_hit[n_pairs] = h;
+                ++n_pairs;
+                ++len[p];
+            }
+        }
+        a = b;
+    }
+    uint64_t total = 0;
+    for (uint64_t p = 0; p < n_peaks; ++p) {
+        hit_offset[p] = total;
+        total += len[p];
+        len[p] = hit_offset[p]; /* becomes the write position */
+    }
+    hit_offset[n_peaks] = total;
+    for (uint64_t c = 0; c < n_pairs; ++c) { /* a peak's pairs come in ascending h */
+        const uint64_t w = len[pair_peak[c]]++;
+        if (w < cap_hits)
+            hit_index[w] = pair_hit[c];
+    }
+    free(len); free(pair_peak); free(pair_hit);
+    free(sne); free(cse); free(r2); free(bit);
+    tables_free(&t);
+    return total;
+}
+
 /* ======================================================================================
  * E3 -- f1, the SECOND Hough transform, over the peaks of the first ("the
  * crossings all lie along a single sinusoidal curve in the parameter space ... that one

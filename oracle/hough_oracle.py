@@ -42,7 +42,7 @@ def lib():
         _lib.oracle_hitlists_cells.restype = C.c_uint64
         _lib.oracle_vote_one.restype = C.c_int
         _lib.oracle_num_threads.restype = C.c_int
-        for f in ("oracle_vote_variant", "oracle_hitlists_variant", "oracle_vertex_vote",
+        for f in ("oracle_vote_variant", "oracle_hitlists_variant", "oracle_hitlists_variant_cells", "oracle_vertex_vote",
                   "oracle_vertex_peaks", "oracle_vertex_members"):
             getattr(_lib, f).restype = C.c_uint64
         _lib.oracle_fit_one.restype = C.c_int
@@ -215,8 +215,11 @@ def vote_variant(grid, mode, x, y, layer):
     return acc.reshape(grid.n_phi, grid.n_d0, grid.n_kappa), int(nv), int(n_bad.value)
 
 
-def hitlists_variant(grid, mode, x, y, layer, peak_bin, cap_hits=None):
-    """A7 under `mode`: CSR (hit_offset, hit_index[min(total, cap)], true total)."""
+def hitlists_variant(grid, mode, x, y, layer, peak_bin, cap_hits=None, by_cell=False):
+    """A7 under `mode`: CSR (hit_offset, hit_index[min(total, cap)], true total).
+    by_cell: the same lists from oracle_hitlists_variant_cells (one pass over the hits per cell that
+    holds a peak instead of one per peak)."""
+    fn = lib().oracle_hitlists_variant_cells if by_cell else lib().oracle_hitlists_variant
     x, y, layer = _hits(x, y, layer)
     pb = np.ascontiguousarray(peak_bin, dtype=np.uint32)
     g = _g(grid)
@@ -224,7 +227,7 @@ def hitlists_variant(grid, mode, x, y, layer, peak_bin, cap_hits=None):
     off = np.zeros(m + 1, np.uint64)
 
     def call(idx, cap):
-        return int(lib().oracle_hitlists_variant(
+        return int(fn(
             C.byref(g), C.c_int(mode), _p(x, C.c_float), _p(y, C.c_float), _p(layer, C.c_int32),
             C.c_uint32(x.shape[0]), _p(pb, C.c_uint32), C.c_uint64(m), _p(off, C.c_uint64),
             _p(idx, C.c_uint32), C.c_uint64(cap)))

@@ -680,6 +680,18 @@ static int peaks_common(hough_handle *h, const hough_peaks_out *out, void *cuda_
     h->next_clean = 1;
     h->peaks_dirty = 0;
     stage_mark(h, ST_FINISH + 1, st);
+    if (with_lists && (h->cfg.options & HOUGH_OPT_CHECK_LISTS))
+        CK(launch_check_lists(h, out, st)); // after k_finish: it ORs into the counters the caller reads
+    return HOUGH_OK;
+}
+
+int hough_check_lists(hough_handle *h, const hough_peaks_out *out, void *cuda_stream)
+{
+    if (!h || !out || !out->mask || !out->counts || !out->hit_offset || !out->hit_index)
+        return HOUGH_EINVAL;
+    if (!h->voted)
+        return HOUGH_ESTATE;
+    CK(launch_check_lists(h, out, (cudaStream_t)cuda_stream));
     return HOUGH_OK;
 }
 

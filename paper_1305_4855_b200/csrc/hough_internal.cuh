@@ -217,6 +217,7 @@ cudaError_t launch_list_sweep(hough_handle *h, cudaStream_t st);
 cudaError_t launch_index_build(hough_handle *h, cudaStream_t st);
 cudaError_t launch_peak_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_copy_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
+cudaError_t launch_check_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_place_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st);
 cudaError_t launch_finish_counts(hough_handle *h, const hough_peaks_out *out, int with_lists,

@@ -765,3 +765,55 @@ cudaError_t launch_lists_generic(hough_handle *h, const hough_peaks_out *out, cu
     h->launches += 1;
     return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------ list check (HOUGH_OPT_CHECK_LISTS)
+// One warp per reported peak: its list, as written to the caller's arrays, is strictly ascending, names
+// real hits, and the OR of their layer bits is the peak's mask.  Reads only final outputs, so it serves
+// every list path (peak-driven, list sweep, vote variants).
+__global__ void __launch_bounds__(256) k_check_lists(const hough_counts *counts_in, hough_counts *counts_out,
+                                                     uint32_t cap_peaks, unsigned long long cap_hits,
+                                                     const uint32_t *__restrict__ mask,
+                                                     const unsigned long long *__restrict__ hit_offset,
+                                                     const uint32_t *__restrict__ hit_index,
+                                                     const uint32_t *__restrict__ hbit, uint32_t n_hits)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t n = min(counts_in->n_peaks, cap_peaks);
+    const uint32_t warps = (gridDim.x * blockDim.x) >> 5;
+    bool bad = false;
+    for (uint32_t pk = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; pk < n; pk += warps) {
+        const unsigned long long a = hit_offset[pk], b = hit_offset[pk + 1];
+        if (b < a) {
+            bad = true;
+            continue;
+        }
+        if (b > cap_hits) // cut by the capacity: not a complete list
+            continue;
+        uint32_t m = 0;
+        for (unsigned long long q = a + lane; q < b; q += 32) {
+            const uint32_t hit = hit_index[q];
+            if (hit >= n_hits || (q > a && hit_index[q - 1] >= hit))
+                bad = true;
+            else
+                m |= hbit[hit];
+        }
+        for (int o = 16; o > 0; o >>= 1)
+            m |= __shfl_xor_sync(0xffffffffu, m, o);
+        if (m != mask[pk])
+            bad = true;
+    }
+    if (__any_sync(0xffffffffu, bad) && lane == 0)
+        atomicOr(&counts_out->flags, HOUGH_LIST_MISMATCH);
+}
+
+cudaError_t launch_check_lists(hough_handle *h, const hough_peaks_out *out, cudaStream_t st)
+{
+    if (h->n_hits == 0) // no event behind the accumulator (hough_set_accumulator): the lists are empty by design
+        return cudaSuccess;
+    k_check_lists<<<h->n_sms * 8, 256, 0, st>>>(out->counts, out->counts, h->cfg.cap_peaks,
+                                                (unsigned long long)h->cfg.cap_hits, out->mask,
+                                                reinterpret_cast<const unsigned long long *>(out->hit_offset),
+                                                out->hit_index, h->hbit, h->n_hits);
+    h->launches += 1;
+    return cudaGetLastError();
+}

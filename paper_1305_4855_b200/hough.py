@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libhough_b200.so")
 
 HOUGH_OK, HOUGH_EINVAL, HOUGH_ENOMEM, HOUGH_ECUDA, HOUGH_ESTATE = 0, -1, -2, -3, -4
-TRUNCATED_PEAKS, TRUNCATED_HITS, INDEX16 = 1, 2, 4
+TRUNCATED_PEAKS, TRUNCATED_HITS, INDEX16, LIST_MISMATCH = 1, 2, 4, 8
 OPT_NO_CULL = 1
 OPT_STAGE_TIMING = 2
 OPT_UNPACKED = 4
@@ -28,6 +28,7 @@ OPT_LINE = 32
 OPT_INTERVAL = 64
 OPT_FUSED_PEAKS = 128
 OPT_CELL_PEAKS = 256
+OPT_CHECK_LISTS = 512
 N_STAGES = 9
 
 # every symbol include/hough.h declares (checked by the CPU test-suite)
@@ -37,7 +38,7 @@ SYMBOLS = ("hough_workspace_bytes", "hough_create", "hough_destroy", "hough_vote
            "hough_set_accumulator", "hough_peaks_only", "hough_microbench_smem", "hough_query",
            "hough_launch_count", "hough_stage_times", "hough_stage_name", "hough_strerror",
            "hough_vertex_workspace_bytes", "hough_vertices", "hough_fit_workspace_bytes", "hough_fit",
-           "hough_peaks_noalloc")
+           "hough_peaks_noalloc", "hough_check_lists")
 
 
 class HoughError(RuntimeError):
@@ -118,7 +119,7 @@ def _load():
     lib.hough_destroy.argtypes = [C.c_void_p]
     lib.hough_vote.restype = C.c_int
     lib.hough_vote.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
-    for name in ("hough_peaks", "hough_peaks_only"):
+    for name in ("hough_peaks", "hough_peaks_only", "hough_check_lists"):
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [C.c_void_p, C.POINTER(PeaksOut), C.c_void_p]
@@ -272,6 +273,11 @@ class Hough:
             out = PeaksOut(self._out.bin, self._out.mask, self._out.hit_offset, self._out.hit_index,
                            counts_out.data_ptr())
         _check(f(self._h, C.byref(out), _stream_ptr(stream)), "hough_peaks")
+
+    def check_lists(self, stream=None):
+        """hough_check_lists on this object's device arrays: a violated list invariant sets LIST_MISMATCH
+        in the counters' flags (see ``read``)."""
+        _check(_lib.hough_check_lists(self._h, C.byref(self._out), _stream_ptr(stream)), "hough_check_lists")
 
     def clear(self, stream=None):
         _check(_lib.hough_clear(self._h, _stream_ptr(stream)), "hough_clear")

@@ -105,6 +105,40 @@ def test_variant_mode0_is_the_base_oracle(oracle):
     assert np.array_equal(o0, o1) and np.array_equal(i0, i1) and t0 == t1
 
 
+def test_cellwise_variant_hit_lists_equal_the_peakwise_ones(oracle):
+    """oracle_hitlists_variant_cells against oracle_hitlists_variant (pinned above and below) in all three
+    modes: random grids with bad and non-finite hits, whole peak lists, subsets, a cap that cuts a list,
+    every non-empty bin (total = n_votes), no peaks."""
+    rng = np.random.default_rng(40)
+    for mode in (oracle.MODE_CIRCLE, oracle.MODE_LINE, oracle.MODE_INTERVAL):
+        for shape, n in [((16, 4, 32), 120), ((24, 1, 64), 300), ((7, 3, 32), 2)]:
+            if mode == oracle.MODE_LINE and shape[1] != 1:
+                continue
+            kw = dict(d0_min=0.0, d0_max=0.0) if shape[1] == 1 else {}
+            if mode == oracle.MODE_LINE:
+                kw.update(kappa_min=-90.0, kappa_max=90.0)
+            g = synth.Grid(n_phi=shape[0], n_d0=shape[1], n_kappa=shape[2], L_min=2, **kw)
+            x, y, layer = random_hits(rng, n)
+            if n > 10:
+                layer[::13] = -1
+                x[1], y[2] = np.nan, np.inf
+            acc, n_votes, _ = oracle.vote_variant(g, mode, x, y, layer)
+            pb, _pm, _n = oracle.peaks(g, acc)
+            allbins = np.nonzero(acc.reshape(-1))[0].astype(np.uint32)
+            for bins in (pb, pb[1::2], allbins, pb[:0]):
+                o1, i1, t1 = oracle.hitlists_variant(g, mode, x, y, layer, bins)
+                o2, i2, t2 = oracle.hitlists_variant(g, mode, x, y, layer, bins, by_cell=True)
+                assert t1 == t2 and np.array_equal(o1, o2) and np.array_equal(i1, i2)
+            assert t1 == 0
+            o1, i1, t1 = oracle.hitlists_variant(g, mode, x, y, layer, allbins)
+            assert t1 == n_votes
+            if len(pb) > 2:
+                cap = int(oracle.hitlists_variant(g, mode, x, y, layer, pb)[0][len(pb) // 2]) + 1
+                o3, i3, t3 = oracle.hitlists_variant(g, mode, x, y, layer, pb, cap_hits=cap, by_cell=True)
+                of, idf, tf = oracle.hitlists_variant(g, mode, x, y, layer, pb)
+                assert t3 == tf and np.array_equal(o3, of) and np.array_equal(i3, idf[:cap])
+
+
 # ============================================================ E2: interval voting
 
 def test_interval_vote_covers_the_curvatures_met_inside_the_phi0_bin(oracle):

@@ -240,8 +240,9 @@ def test_interval_voting_random(hough, oracle, shape, tile, n_hits, n_layers, se
 
 
 def test_interval_voting_displaced3d(hough, oracle):
-    """BASELINE.json configs[1] under interval voting (accumulator, n_votes and peaks at full size;
-    hit lists of the first 4096 peaks: the oracle's list pass is O(peaks x hits))."""
+    """BASELINE.json configs[1] under interval voting, everything at full size: accumulator, n_votes, peaks
+    and the whole CSR (the oracle's cell-wise lists; its peak-by-peak pass, O(peaks x hits), confirms them
+    on the first 4096 peaks)."""
     w = synth.WORKLOADS["displaced3d"]
     x, y, layer, _ = synth.generate_event(w.event, w.seeds[0])
     acc, n_votes, n_bad = oracle.vote_variant(w.grid, oracle.MODE_INTERVAL, x, y, layer)
@@ -251,10 +252,13 @@ def test_interval_voting_displaced3d(hough, oracle):
     assert res["flags"] == 0
     assert res["n_votes"] == n_votes and np.array_equal(res["acc"], acc)
     assert res["n_peaks"] == n_peaks and np.array_equal(res["peak_bin"], pb) and np.array_equal(res["peak_mask"], pm)
+    coff, cidx, ctot = oracle.hitlists_variant(w.grid, oracle.MODE_INTERVAL, x, y, layer, pb, cap_hits=1 << 26,
+                                               by_cell=True)
+    assert res["n_hit_entries"] == ctot <= 1 << 26
+    assert np.array_equal(res["hit_offset"], coff) and np.array_equal(res["hit_index"], cidx)
     m = min(4096, n_peaks)
     off, idx, tot = oracle.hitlists_variant(w.grid, oracle.MODE_INTERVAL, x, y, layer, pb[:m])
-    assert np.array_equal(res["hit_offset"][:m + 1], off)
-    assert np.array_equal(res["hit_index"][:tot], idx)
+    assert np.array_equal(coff[:m + 1], off) and np.array_equal(cidx[:tot], idx)
     h.close()
 
 
@@ -343,10 +347,14 @@ def test_fit_everything_selected_on_a_pileup_event(hough, oracle):
     w = synth.WORKLOADS["pileup"]
     x, y, layer, _ = synth.generate_event(w.event, 1)
     h = make(hough, w.grid, x, y, layer, w.cap_peaks, w.cap_hits)
-    res = h.read()
+    res = read_all(h)
+    # the oracle's fit below is fed with lists that are the ORACLE's too: the whole event is compared first
+    ref = oracle.run(w.grid, x, y, layer, cap_hits=w.cap_hits, by_cell=True)
+    res["acc"] = res["acc"].reshape(ref["acc"].shape)
+    assert_same(res, ref)
     h.fit(0.1, 5)
     g = h.read_fit()
-    assert_fit_same(hough, oracle, res, x, y, g, 0.1, 5)
+    assert_fit_same(hough, oracle, ref, x, y, g, 0.1, 5)
     assert g["n_selected"] == res["n_peaks"] and g["n_pair_tests"] > 10**8
     h.close()
 

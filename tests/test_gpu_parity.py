@@ -42,6 +42,7 @@ def run_gpu(hough, grid, x, y, layer, cap_peaks, cap_hits, **kw):
 
 
 def assert_same(res, ref, lists=True):
+    assert not (res.get("flags", 0) & 8)             # HOUGH_LIST_MISMATCH (only ever set under OPT_CHECK_LISTS)
     assert res["n_votes"] == ref["n_votes"]
     assert res["n_bad_hits"] == ref["n_bad_hits"]
     assert np.array_equal(res["acc"], ref["acc"])
@@ -148,7 +149,7 @@ def test_bad_layers_and_non_finite_hits(hough, oracle):
     assert solo["n_votes"] > 0
     for opt in (0, 1):
         res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
-                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4, options=opt)
+                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=8, tile_d0=4, options=opt | hough.OPT_CHECK_LISTS)
         assert_same(res, ref)
     res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
                   cap_hits=ref["n_hit_entries"] + 1)
@@ -173,7 +174,7 @@ def test_hits_at_the_point_of_closest_approach(hough, oracle):
     ref = oracle.run(grid, x, y, layer)
     for opt in (0, 1):
         res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
-                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=4, tile_d0=2, options=opt)
+                      cap_hits=ref["n_hit_entries"] + 1, tile_phi=4, tile_d0=2, options=opt | hough.OPT_CHECK_LISTS)
         assert_same(res, ref)
 
 
@@ -531,6 +532,62 @@ def test_an_outlier_radius_does_not_widen_the_list_windows_of_later_events(hough
     h.close()
 
 
+def test_list_check_passes_on_real_lists_and_catches_tampering(hough, oracle):
+    """hough_check_lists / HOUGH_OPT_CHECK_LISTS: clean on the lists of displaced3d and pile-up events (all
+    three list paths), and HOUGH_LIST_MISMATCH once a list is tampered with: an entry replaced by a hit of
+    another layer (the OR of the bits no longer gives the mask), two entries swapped (not ascending), an
+    index beyond the event.  A capacity-cut list is not judged."""
+    MIS = hough.LIST_MISMATCH
+    for name, options in (("displaced3d", 0), ("displaced3d", hough.OPT_LIST_SWEEP), ("displaced3d", hough.OPT_INTERVAL),
+                          ("pileup", 0)):
+        w = synth.WORKLOADS[name]
+        x, y, layer, _ = synth.generate_event(w.event, 4)
+        cap_p, cap_h = (1 << 22, 1 << 26) if options == hough.OPT_INTERVAL else (w.cap_peaks, w.cap_hits)
+        h = hough.Hough(w.grid, len(x), cap_p, cap_h, options=options | hough.OPT_CHECK_LISTS)
+        h.vote(dev(x), dev(y), dev(layer))
+        h.peaks()
+        res = h.read()
+        assert res["n_peaks"] > 0 and res["flags"] & ~hough.INDEX16 == 0, (name, options)
+        h.check_lists()                                  # the explicit call agrees
+        assert h.read_counts()["flags"] & MIS == 0
+        if options:
+            h.close()
+            continue
+        off = res["hit_offset"].astype(np.int64)
+        lens = np.diff(off)
+        p = int(np.argmax(lens >= 3))                    # a peak with at least three hits
+        a = int(off[p])
+        orig = h.hit_index[a:a + 3].clone()
+
+        def tampered(values):
+            h.peaks()                                    # fresh lists and a fresh flags word
+            h.hit_index[a:a + len(values)] = torch.tensor(values, dtype=torch.int32, device=h.device)
+            h.check_lists()
+            flag = int(h.read_counts()["flags"]) & MIS
+            h.hit_index[a:a + 3] = orig
+            return flag
+
+        o = [int(v) for v in orig.cpu().numpy()]
+        assert tampered(o) == 0
+        assert tampered([o[1], o[0]]) == MIS             # not ascending
+        assert tampered([o[0], o[0]]) == MIS             # a repeated hit
+        assert tampered([len(x) + 5]) == MIS             # no such hit
+        # a later hit of a layer the mask does not have, in the third place: the OR gains a bit
+        missing = [l for l in range(10) if not (int(res["peak_mask"][p]) >> l) & 1]
+        cand = [hh for hh in range(o[1] + 1, len(x)) if layer[hh] in missing]
+        if cand:
+            assert tampered([o[0], o[1], cand[0]]) == MIS
+        h.close()
+    # a list cut by cap_hits is skipped, the complete ones before it are still judged
+    w = synth.WORKLOADS["displaced3d"]
+    x, y, layer, _ = synth.generate_event(w.event, 4)
+    h = hough.Hough(w.grid, len(x), w.cap_peaks, 100, options=hough.OPT_CHECK_LISTS)
+    h.vote(dev(x), dev(y), dev(layer))
+    h.peaks()
+    assert h.read()["flags"] == hough.TRUNCATED_HITS
+    h.close()
+
+
 def test_many_kappa_bins_and_single_cell_tiles(hough, oracle):
     """n_kappa = 2048 (a cell row of 4 KB: few cells per tile) and the 1 x 1 tile override."""
     rng = np.random.default_rng(22)
@@ -546,7 +603,7 @@ def test_many_kappa_bins_and_single_cell_tiles(hough, oracle):
     x, y, layer = random_hits(rng, 300)
     ref = oracle.run(grid, x, y, layer)
     res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
-                  cap_hits=ref["n_hit_entries"] + 1)
+                  cap_hits=ref["n_hit_entries"] + 1, options=hough.OPT_CHECK_LISTS)
     assert_same(res, ref)
 
 
@@ -585,6 +642,7 @@ def test_random_configurations_share_the_process(hough, oracle):
         opts = int(rng.integers(0, 2))          # NO_CULL or not
         peaks_by = int(rng.integers(0, 3))      # streaming sweep, fused (two-masks-per-word tiles only), cell-wise
         opts |= (128 if nl <= 16 else 0) if peaks_by == 1 else 256 if peaks_by == 2 else 0
+        opts |= hough.OPT_CHECK_LISTS             # the device-side list invariant rides along
         res = run_gpu(hough, grid, x, y, layer, cap_peaks=grid.n_bins // 2 + 1,
                       cap_hits=max(ref["n_hit_entries"], 1) + 3, tile_phi=tile[0], tile_d0=tile[1],
                       options=opts)
