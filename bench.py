@@ -7,8 +7,9 @@ workload: BASELINE.json configs[3], 100 independent pile-up events (seeds 0..99)
 with its own accumulator, back to back on one stream.  `value` is in-range votes cast per
 second over all ranks (inputs resident in HBM); `events_per_s` and `evaluations_per_s`
 (n * n_phi * n_d0 per event, the paper-level work) are reported beside it.  `e2e` is the
-same metric through hough_process_host: pinned HOST buffers in, results copied back to
-the host, every event.
+same metric through hough_submit_host + hough_collect_begin/_end (three events in flight):
+pinned HOST buffers in, complete results copied back to the host, every event.
+`per_config` gives events/s and votes/s of every BASELINE.json event shape.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload batch100|pileup|...]
     python bench.py --impl reference ...   # the CPU oracle, as it stands, on the host cores
@@ -136,6 +137,21 @@ def ncu_profile():
         return json.load(f)
 
 
+KERNEL_SOURCES = ("hough_sweep.cu", "hough_peaklists.cu", "hough_device.cuh", "hough_internal.cuh")
+
+
+def kernel_source_digest():
+    """SHA-256 over the sources of the two sweep kernels.  profiles/ncu_traffic.json stores the digest of
+    the tree its ncu counts were captured on; a different digest here means those counts (and every
+    fraction derived from them) describe other code, and the line says `stale`."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1305_4855_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
 def input_digest(event):
     """SHA-256 over x, y, layer of one generated event (inputs are seeded and
     reproducible; the digest lets two runs prove they measured the same hits)."""
@@ -206,7 +222,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the stage-time, sweep-roofline and micro-benchmark legs")
+    ap.add_argument("--kernel-digest", action="store_true",
+                    help="print the digest of the sweep kernels' sources (see profiles/) and exit")
     args = ap.parse_args()
+    if args.kernel_digest:
+        print(kernel_source_digest())
+        return
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -431,15 +452,20 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
     issue_peak = n_sms * 4 * peaks_info["sm_max_mhz"] * 1e6          # warp instructions / s
     prof = ncu_profile()
     sweeps = prof.get("_sweeps", {})
+    digest = kernel_source_digest()
+    stale = sweeps.get("source_sha256") != digest  # the committed ncu counts were taken on other kernel sources
+    out["kernel_source_sha256"] = digest
     alu_note = ("bound = plain fp32 ALU issue (no dense contraction, 0 HBM bytes per evaluation); "
                 "algorithmic fp32 ops = 15 per closed-form evaluation (DESIGN.md 5.1) x the evaluations the "
                 "method defines for this launch; peak = SMs x 128 fp32 lanes x sm_max_mhz without FMA (the "
                 "recipe forbids contraction); " + peaks_info["source"] + ". `frac` follows the contract "
                 "(algorithmic work / time / peak) and can exceed 1 because the conservative cull proves most "
                 "evaluations cannot vote and skips them; `frac_executed` counts only evaluations actually "
-                "run; `issue_slot_frac` = warp instructions per launch (committed ncu capture, see "
-                "`instructions_source`) / live CUDA-event time / (SMs x 4 schedulers x sm_max_mhz) is the "
-                "hardware utilisation and the number that shows headroom.")
+                "run.  `frac` is the issue-slot fraction: warp instructions per launch (committed ncu capture, "
+                "see `instructions_source`; `stale` is true when the kernel sources have changed since) / live "
+                "CUDA-event time / (SMs x 4 schedulers x sm_max_mhz): the ceiling SURVEY.md 8(d) names for "
+                "these kernels; `achieved`, `peak` and `algorithmic_equiv_frac` keep the algorithmic fp32 "
+                "figure (which can exceed 1 because the conservative cull skips evaluations).")
 
     def sweep_roofline(kernel, stage, alg_evals, done_evals, key):
         secs = per_event[stage] * 1e-3
@@ -455,13 +481,21 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
              "achieved_executed": FLOP_PER_EVAL * done_evals / secs / 1e12,
              "frac_executed": FLOP_PER_EVAL * done_evals / secs / 1e12 / alu_peak}
         instr = sweeps.get(key, {}).get("warp_instructions")
-        r["algorithmic_equiv_frac"] = r["frac"]  # the contract's `frac` under the name the advisor asked for
+        r["algorithmic_equiv_frac"] = r["frac"]  # algorithmic fp32 work / time / ALU peak (can exceed 1: the cull)
         if instr:
+            # the ceiling of these kernels is the issue slots: `frac` is the share of them
+            # in use = warp instructions per launch (committed ncu capture) / live time / issue peak
             r["issue_slot_frac"] = instr / secs / issue_peak
-            r["hardware_frac"] = r["issue_slot_frac"]  # the utilisation figure: issue slots actually used
+            r["algorithmic_achieved_tflops"], r["alu_peak_tflops"] = r["achieved"], r["peak"]
+            r["achieved"], r["peak"], r["unit"] = instr / secs, issue_peak, "warp-inst/s"
+            r["frac"] = r["hardware_frac"] = r["issue_slot_frac"]
+            r["frac_is"] = "issue slots used: warp instructions / time / (SMs x 4 schedulers x clock)"
             r["warp_instructions_per_launch"] = instr
             r["instructions_source"] = sweeps.get("source")
             r["issue_active_pct_ncu"] = sweeps.get(key, {}).get("issue_active_pct")
+            r["stale"] = stale
+        else:
+            r["frac_is"] = "algorithmic fp32 work / time / ALU peak (no ncu instruction count committed)"
         return r
 
     rl_vote = sweep_roofline("k_sweep (vote)", "vote", evals_step / n_ev, evals_done_step / n_ev, "vote")
@@ -567,6 +601,57 @@ def extras(args, hough, torch, workload, d_events, n_ev, dev, local_rank, peaks_
     out["two_handles_two_streams"] = {"events_per_s": 3 * n_ev / dt2, "ms_per_event": dt2 / (3 * n_ev) * 1e3,
                                       "note": "device-resident, wall clock over 3 passes with a device synchronise on "
                                               "both sides; each handle has its own workspace and output arrays"}
+
+    # every BASELINE.json event shape (north_star: "throughput on the synthetic event shapes ... as votes/s and
+    # events/s"): device-resident, back to back on one stream (CUDA events), and one at a time through
+    # hough_process_host with host buffers (wall clock)
+    def shape_rate(wl, n_events, reps):
+        evs_h = [synth.generate_event(wl.event, sd)[:3] for sd in range(n_events)]
+        evs_d = [tuple(torch.from_numpy(a).to(dev) for a in e) for e in evs_h]
+        hs = hough.Hough(wl.grid, max(len(e[0]) for e in evs_h), wl.cap_peaks, wl.cap_hits, device=local_rank)
+        cs = torch.zeros(n_events, hough.COUNTS_WORDS, dtype=torch.int64, device=dev)
+        stq = torch.cuda.current_stream()
+
+        def one_pass():
+            for q, ev in enumerate(evs_d):
+                hs.vote(*ev)
+                hs.peaks(counts_out=cs[q])
+
+        one_pass()
+        torch.cuda.synchronize(dev)
+        c = cs.cpu().numpy().view(hough.COUNTS_DTYPE).reshape(n_events)
+        assert int(c["flags"].max()) == 0
+        ms = []
+        for _ in range(reps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stq)
+            one_pass()
+            e1.record(stq)
+            e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        secs = float(np.median(ms)) * 1e-3
+        hs.process_host(*evs_h[0])
+        t0 = time.perf_counter()
+        for ev in evs_h:
+            hs.process_host(*ev)
+        dt_host = time.perf_counter() - t0
+        hs.close()
+        votes = int(c["n_votes"].sum())
+        return {"events_per_s": n_events / secs, "votes_per_s": votes / secs, "ms_per_event": secs / n_events * 1e3,
+                "hits_per_event": int(np.mean([len(e[0]) for e in evs_h])),
+                "peaks_per_event": float(c["n_peaks"].mean()),
+                "e2e_one_at_a_time_events_per_s": n_events / dt_host, "events_timed": n_events, "passes": reps}
+
+    out["per_config"] = {name: shape_rate(synth.WORKLOADS[name], n, r)
+                         for name, n, r in (("prompt2d", 100, 5), ("displaced3d", 100, 5), ("pileup", 10, 5),
+                                            ("finegrid", 2, 3))}
+    out["per_config"]["batch100"] = "the headline of this line (value, events_per_s, e2e)" \
+        if workload.name == "batch100" else None
+    out["per_config"]["note"] = ("seeds 0..n-1 of each shape, one handle, one stream, back to back, median of the "
+                                 "passes, 512 MiB L2 flush before each pass; e2e_one_at_a_time = hough_process_host "
+                                 "(pageable numpy inputs, full results back, synchronous): the small shapes are bound "
+                                 "by the 11-launch chain and host latency, not by arithmetic")
 
     # a5 variants, measured: stand-alone streaming sweep, peak test fused into the
     # vote tile + tile-edge pass (HOUGH_OPT_FUSED_PEAKS), cell-wise kernel over every cell
